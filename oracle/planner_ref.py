@@ -1,0 +1,79 @@
+"""Reference greedy contraction-order planner — ORACLE-SIDE (test infrastructure).
+
+The paper delegates ordering to CoTenGra; BASELINE.json's north_star
+asks for a greedy planner whose plan is bit-identical between the library and this
+reference.  Rules P1-P6 of DESIGN.md, all integer-valued:
+
+P1 leaves are subcircuits 0..m-1; the node created at step t (0-based) has id m+t.
+P2 candidates: all unordered pairs of live nodes sharing >= 1 cut; if none exist but
+   more than one node is live (disconnected network) the single candidate is the pair
+   of the two smallest live ids (outer product).
+P3 cost exponent e(a,b) = 2*|E_a u E_b| in states mode (cost 4^{#inner+#outer},
+   P:407-412); + o_a + o_b in distribution mode (open output bits carried, reading G10).
+P4 choose min e; tie -> fewer resulting open cuts |E_a xor E_b|; tie -> smaller min(id);
+   tie -> smaller max(id).
+P5 lhs = smaller id; all shared cuts are contracted together as one merged bond
+   (P:318-319), digits in ascending cut id.
+P6 K_max = max_t |E_a u E_b|; per-step log2 cost = e.
+
+Serialisation (little-endian int32): 'TQCP', version 1, mode (0 states, 1 distribution),
+n, m, K, then per step: lhs, rhs, #inner, #outer_lhs, #outer_rhs, log2cost, inner ids...,
+outer_lhs ids..., outer_rhs ids... (each ascending); then K_max.
+"""
+from __future__ import annotations
+
+import struct
+
+MODE_STATES, MODE_DISTRIBUTION = 0, 1
+
+
+def plan(net, mode: int = MODE_STATES):
+    m = net.m
+    open_cuts = {s: frozenset(net.sub_cuts[s]) for s in range(m)}
+    obits = {s: net.o(s) for s in range(m)}
+    steps = []
+    t = 0
+    while len(open_cuts) > 1:
+        live = sorted(open_cuts)
+        best = None
+        for i, a in enumerate(live):
+            for b in live[i + 1:]:
+                if not (open_cuts[a] & open_cuts[b]):
+                    continue
+                e = 2 * len(open_cuts[a] | open_cuts[b])
+                if mode == MODE_DISTRIBUTION:
+                    e += obits[a] + obits[b]
+                key = (e, len(open_cuts[a] ^ open_cuts[b]), a, b)
+                if best is None or key < best:
+                    best = key
+        if best is None:
+            a, b = live[0], live[1]
+            e = 2 * len(open_cuts[a] | open_cuts[b])
+            if mode == MODE_DISTRIBUTION:
+                e += obits[a] + obits[b]
+            best = (e, len(open_cuts[a] ^ open_cuts[b]), a, b)
+        e, _r, a, b = best
+        inner = sorted(open_cuts[a] & open_cuts[b])
+        outer_a = sorted(open_cuts[a] - open_cuts[b])
+        outer_b = sorted(open_cuts[b] - open_cuts[a])
+        steps.append(dict(lhs=a, rhs=b, inner=inner, outer_lhs=outer_a, outer_rhs=outer_b, log2cost=e))
+        new = m + t
+        open_cuts[new] = open_cuts[a] ^ open_cuts[b]
+        obits[new] = obits[a] + obits[b]
+        del open_cuts[a], open_cuts[b]
+        t += 1
+    kmax = max([len(s["inner"]) + len(s["outer_lhs"]) + len(s["outer_rhs"]) for s in steps], default=0)
+    return dict(mode=mode, n=net.n_qubits, m=m, K=net.K, steps=steps, kmax=kmax)
+
+
+def serialize(p) -> bytes:
+    words = [p["mode"], p["n"], p["m"], p["K"]]
+    for s in p["steps"]:
+        words += [s["lhs"], s["rhs"], len(s["inner"]), len(s["outer_lhs"]), len(s["outer_rhs"]), s["log2cost"]]
+        words += s["inner"] + s["outer_lhs"] + s["outer_rhs"]
+    words.append(p["kmax"])
+    return b"TQCP" + struct.pack("<i", 1) + struct.pack(f"<{len(words)}i", *words)
+
+
+def step_pairs(p):
+    return [(s["lhs"], s["rhs"]) for s in p["steps"]]

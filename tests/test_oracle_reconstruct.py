@@ -1,0 +1,195 @@
+"""Pins for oracle/reconstruct.py, oracle/direct_sum.c and oracle/planner_ref.py — CPU only.
+
+Pi-1 rank-one closed form, Pi-2 m=2 == library GEMM, Pi-3 chain == matrix chain,
+Pi-4 brute-force einsum, Pi-5 slicing identity, Pi-6 distribution
+sum, the paper's printed multiplication counts (144 / 768).
+"""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import planner_ref as P, reconstruct as R
+from oracle.direct_sum_c import direct_sum_c
+from tqc_inputs import configs, random_states, random_tensors, rank_one_tensors
+from tqc_inputs.network import Network
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _golden(name):
+    out = {}
+    for line in open(os.path.join(GOLDEN, name)):
+        if line.strip() and not line.startswith("#"):
+            k, *v = line.split()
+            out[k] = [int(x) for x in v]
+    return out
+
+
+def _fig5_network():
+    # e1: 1-2, e2: 2-3, e3: 2-4, e4: 3-4 (0-based subcircuits 0..3, cuts 0..3)
+    return Network(4, [(0, 1), (1, 2), (1, 3), (2, 3)], [[0], [0, 1, 2], [1, 3], [2, 3]], [[0], [1], [2], [3]])
+
+
+def test_paper_multiplication_counts():
+    g = _golden("fig5_counts.txt")
+    net = _fig5_network()
+    costs, kmax = R.multiplication_counts(net, [(0, 1), (4, 2), (5, 3)])       # ((1,2),3),4
+    assert costs == g["steps_paper_order"] and sum(costs) == g["total_paper_order"][0]
+    assert kmax == g["kmax_paper_order"][0]
+    assert 4 ** net.K * (net.m - 1) == g["prior_method"][0]
+    costs, _ = R.multiplication_counts(net, [(2, 3), (4, 1), (5, 0)])          # ((3,4),2),1
+    assert costs == g["steps_alt_order"] and sum(costs) == g["total_alt_order"][0]
+    assert g["prior_method"][0] / g["total_paper_order"][0] > 5                # "more than fivefold"
+
+
+def test_m2_is_a_gemm():
+    """Pi-2: two subcircuits => P = 2^{-K} A^T B, a library matmul."""
+    net = Network(5, [(0, 1), (1, 0), (0, 1)], [[0, 1, 2], [0, 1, 2]], [[0, 1], [2, 3, 4]])
+    T = random_tensors(net, 5)
+    want = (T[0].astype(np.float64).T @ T[1].astype(np.float64)).reshape(-1) / 8.0
+    bits = R.full_distribution_bits(5)
+    assert np.allclose(R.direct_sum(net, T, bits), want, rtol=1e-13)
+    assert np.allclose(direct_sum_c(net, T, bits)[0], want, rtol=1e-13)
+    # axis order matters: permuting B's incident-cut order permutes its rows
+    net2 = Network(5, net.cuts, [[0, 1, 2], [2, 0, 1]], net.sub_qubits)
+    Bp = T[1].reshape(4, 4, 4, 8).transpose(2, 0, 1, 3).reshape(64, 8)         # axes (e2, e0, e1)
+    assert np.allclose(R.direct_sum(net2, [T[0], Bp], bits), want, rtol=1e-13)
+    assert np.allclose(direct_sum_c(net2, [T[0], Bp], bits)[0], want, rtol=1e-13)
+
+
+def test_chain_is_a_matrix_chain():
+    """Pi-3: A - B - C chain (config 3's shape) => 2^{-K} v_A^T W_B v_C."""
+    net = Network(3, [(0, 1), (1, 0), (1, 2), (2, 1)], [[0, 1], [0, 1, 2, 3], [2, 3]], [[0], [1], [2]])
+    T = [t.astype(np.float64) for t in random_tensors(net, 6)]
+    bits = R.full_distribution_bits(3)
+    want = np.zeros(8)
+    for i, (a, b, c) in enumerate(bits):
+        W = T[1][:, b].reshape(16, 16)
+        want[i] = T[0][:, a] @ W @ T[2][:, c] / 16.0
+    for got in (R.direct_sum(net, T, bits), direct_sum_c(net, T, bits)[0], R.bucket_elimination(net, T, bits)):
+        assert np.allclose(got, want, rtol=1e-12)
+
+
+def _einsum_brute_force(net, tensors, bits):
+    """One einsum over explicit axes, per state."""
+    out = np.zeros(bits.shape[0])
+    keys = R.keys_from_bits(net, bits)
+    for b in range(bits.shape[0]):
+        args = []
+        for s in range(net.m):
+            v = np.asarray(tensors[s], dtype=np.float64)[:, keys[b, s]].reshape((4,) * net.c(s))
+            args += [v, list(net.sub_cuts[s])]
+        out[b] = np.einsum(*args, []) / 2.0 ** net.K
+    return out
+
+
+@pytest.mark.parametrize("seed", range(10))
+def test_all_oracle_tiers_agree_on_tiny_networks(seed):
+    """Pi-4 + order invariance."""
+    m = 2 + seed % 4
+    net = configs.random_network(m, (m - 1) + seed % 3, 50 + seed, o_lo=0, o_hi=2,
+                                 connected=(seed % 5 != 4))
+    if net.n_qubits == 0:
+        net = configs.random_network(m, m, 50 + seed, o_lo=1, o_hi=2)
+    T = random_tensors(net, 60 + seed)
+    bits = random_states(net.n_qubits, 20, 70 + seed)
+    want = _einsum_brute_force(net, T, bits)
+    scale = np.abs(want).max()
+    assert np.abs(R.direct_sum(net, T, bits) - want).max() <= 1e-12 * scale
+    assert np.abs(direct_sum_c(net, T, bits)[0] - want).max() <= 1e-12 * scale
+    assert np.abs(R.bucket_elimination(net, T, bits) - want).max() <= 1e-12 * scale
+    assert np.abs(R.bucket_elimination(net, T, bits, order=list(range(net.K))[::-1]) - want).max() <= 1e-12 * scale
+    for mode in (P.MODE_STATES, P.MODE_DISTRIBUTION):
+        steps = P.step_pairs(P.plan(net, mode))
+        assert np.abs(R.pairwise_contract(net, T, bits, steps) - want).max() <= 1e-12 * scale
+
+
+@pytest.mark.parametrize("seed", range(4))
+def test_rank_one_closed_form(seed):
+    """Pi-1 against the literal sum (small K) and bucket elimination (K too large for 4^K)."""
+    net = configs.random_network(4, 6, 80 + seed, o_lo=1, o_hi=3)
+    T, g, a = rank_one_tensors(net, 90 + seed)
+    bits = random_states(net.n_qubits, 16, 95 + seed)
+    want = R.rank_one_closed_form(net, g, a, bits)
+    assert np.allclose(R.direct_sum(net, T, bits), want, rtol=1e-13)
+    assert np.allclose(direct_sum_c(net, T, bits)[0], want, rtol=1e-13)
+    big = configs.random_network(12, 22, 180 + seed, o_lo=1, o_hi=2)
+    T, g, a = rank_one_tensors(big, 190 + seed)
+    bits = random_states(big.n_qubits, 8, 195 + seed)
+    assert np.allclose(R.bucket_elimination(big, T, bits), R.rank_one_closed_form(big, g, a, bits), rtol=1e-12)
+
+
+def test_slicing_identity():
+    """Pi-5: fixing one cut to each of its 4 bases and summing reproduces the network (Fig. 6)."""
+    net = configs.random_network(4, 5, 123, o_lo=1, o_hi=2)
+    T = random_tensors(net, 124)
+    bits = random_states(net.n_qubits, 12, 125)
+    want = R.direct_sum(net, T, bits)
+    e = 2
+    total = np.zeros_like(want)
+    keep = [x for x in range(net.K) if x != e]
+    relabel = {x: i for i, x in enumerate(keep)}
+    for basis in range(4):
+        Ts, sub_cuts = [], []
+        for s in range(net.m):
+            t = np.asarray(T[s], dtype=np.float64)
+            if e in net.sub_cuts[s]:
+                ax = net.sub_cuts[s].index(e)
+                t4 = t.reshape((4,) * net.c(s) + (-1,))
+                t = np.take(t4, basis, axis=ax).reshape(4 ** (net.c(s) - 1), -1)
+            Ts.append(t)
+            sub_cuts.append([relabel[x] for x in net.sub_cuts[s] if x != e])
+        sliced = Network(net.n_qubits, [net.cuts[x] for x in keep], sub_cuts, net.sub_qubits)
+        total += R.direct_sum(sliced, Ts, bits) / 2.0          # the removed cut's 1/2
+    assert np.allclose(total, want, rtol=1e-12)
+
+
+def test_distribution_sum():
+    """Pi-6: sum_x p(x) = 2^{-K} contract(sum_{x_s} T_s)."""
+    net = configs.random_network(4, 5, 223, o_lo=1, o_hi=2)
+    T = random_tensors(net, 224)
+    p = R.direct_sum(net, T, R.full_distribution_bits(net.n_qubits))
+    marg = Network(0, net.cuts, net.sub_cuts, [[] for _ in range(net.m)])
+    Tm = [np.asarray(t, dtype=np.float64).sum(axis=1, keepdims=True) for t in T]
+    tot = R.direct_sum(marg, Tm, np.zeros((1, 0), dtype=np.uint8))[0]
+    assert np.isclose(p.sum(), tot, rtol=1e-12)
+
+
+def test_c_direct_sum_on_cfg4_shape_prefix():
+    """The C odometer at config-4 size (K = 14) on 2 states against bucket elimination."""
+    net = configs.cfg4_network()
+    assert (net.m, net.K, net.n_qubits) == (8, 14, 64)
+    T = random_tensors(net, 1)
+    bits = random_states(64, 2, 2)
+    a, _ = direct_sum_c(net, T, bits)
+    b = R.bucket_elimination(net, T, bits)
+    assert np.allclose(a, b, rtol=1e-12)
+
+
+def test_reference_planner_fixtures():
+    net = _fig5_network()
+    p = P.plan(net)
+    costs, kmax = R.multiplication_counts(net, P.step_pairs(p))
+    assert sum(costs) <= 144 and kmax <= 3 and p["kmax"] == kmax          # greedy is no worse than Fig. 5's order
+    assert sum(costs) <= net.m * 4 ** kmax                                 # Eq. 2 bound
+    assert [2 ** s["log2cost"] for s in p["steps"]] == costs
+    # m = 2  =>  K_max = |E|
+    net2 = Network(2, [(0, 1)] * 3, [[0, 1, 2], [0, 1, 2]], [[0], [1]])
+    assert P.plan(net2)["kmax"] == 3
+    # m > 3 connected => K_max < |E|
+    for seed in range(5):
+        big = configs.random_network(6, 9, 300 + seed, o_lo=1, o_hi=1)
+        assert P.plan(big)["kmax"] < big.K
+    # determinism and serialisation
+    assert P.serialize(P.plan(net)) == P.serialize(P.plan(net))
+    assert P.serialize(p)[:4] == b"TQCP"
+
+
+def test_cfg5_network_shape_and_rank_one():
+    net = configs.cfg5_network()
+    assert net.m == 52 and net.n_qubits == 196
+    assert sum(net.o(s) for s in range(52)) == 196
+    assert all(2 <= net.o(s) <= 4 for s in range(52))
+    p = P.plan(net)
+    assert len(p["steps"]) == 51
