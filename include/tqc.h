@@ -1,0 +1,150 @@
+/* tqc.h — C ABI of the B200-native TensorQC reconstruction library (libtqc.so).
+ *
+ * What the library computes (arXiv 2502.03445, "TensorQC"; PAPER.md = /root/reference/PAPER.md):
+ *
+ *     p(x) = 2^{-K} * sum_{k in {I,X,Y,Z}^K}  prod_{s=1..m}  T_s[ idx_s(k), x_s ]
+ *
+ * i.e. Eq. 1 with the factor 1/2 per cut the printed equation omits
+ * (reading G1), evaluated not as the 4^K-term sum but as a tensor-network
+ * contraction of the subcircuit output tensors over their 4-valued cut-edge bonds
+ * (section 3.2-3.3): m-1 pairwise contractions, parallel cuts merged
+ * into one bond, any order giving the same value (lines 343-348, 397-399).
+ *
+ * Conventions (readings G4-G6):
+ *   - Basis index order I=0, X=1, Y=2, Z=3.
+ *   - Subcircuit tensor T_s is [4^{c_s}][2^{o_s}] row-major fp32 (trailing output axis); the
+ *     first listed incident cut of s is the most significant base-4 digit of the row index.
+ *   - x_s packs the output qubits of s in their listed order, first = MSB.
+ *   - A distribution index is i = sum_q x_q 2^{n-1-q} (qubit 0 = MSB).
+ *   - A batch state is ceil(n/64) uint64 words; qubit q is bit (q % 64) of word (q / 64).
+ *
+ * Every call returns 0 on success or a negative tqc_status; tqc_last_error() gives a
+ * thread-local message.  No exception crosses the boundary.  Pointers are marked HOST or
+ * DEVICE.  The library never synchronises the caller's stream inside the contract calls and
+ * never allocates there: persistent device state (re-laid-out tensors) is allocated in
+ * tqc_load_subcircuit_tensors, scratch comes from the caller's workspace.
+ * There is no CPU fallback: without a CUDA device the compute calls fail with TQC_E_CUDA.
+ */
+#ifndef TQC_H
+#define TQC_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    TQC_OK = 0,
+    TQC_E_ARG = -1,        /* null pointer, out-of-range id, inconsistent description */
+    TQC_E_SHAPE = -2,      /* n_elems does not match 4^{c_s} * 2^{o_s} */
+    TQC_E_STATE = -3,      /* a tensor has not been loaded / wrong mode for this call */
+    TQC_E_INFEASIBLE = -4, /* partitioning caps cannot be met */
+    TQC_E_WORKSPACE = -5,  /* workspace too small (see tqc_plan_workspace_bytes) */
+    TQC_E_TOO_LARGE = -6,  /* a dimension exceeds what the library indexes */
+    TQC_E_CUDA = -7,       /* CUDA runtime error (message has the CUDA string) */
+    TQC_E_PARSE = -8       /* circuit text could not be parsed */
+} tqc_status;
+
+enum { TQC_MODE_STATES = 0, TQC_MODE_DISTRIBUTION = 1 };
+
+/* Kernel class chosen per plan step (integer thresholds):
+ * SIMT_TILE  register-tiled fp32 FFMA contraction (any shape);
+ * DOT        final reduction: no outer cuts left, one dot product over the merged bond per state;
+ * TCGEN05    3xTF32 tcgen05.mma / TMEM / TMA contraction for steps with large outer dimensions. */
+enum { TQC_KERNEL_SIMT_TILE = 0, TQC_KERNEL_DOT = 1, TQC_KERNEL_TCGEN05 = 2 };
+/* How a node of the contraction tree is evaluated. */
+enum { TQC_NODE_LEAF = 0, TQC_NODE_TABLE = 1, TQC_NODE_BATCH = 2 };
+
+typedef struct tqc_plan tqc_plan_t;
+
+/* Cut network (cut set E, subcircuits C_1..C_m, E_i subset of E).
+ * All arrays HOST, caller-owned, copied by tqc_plan. */
+typedef struct {
+    int32_t n_qubits;               /* n */
+    int32_t m;                      /* subcircuits */
+    int32_t K;                      /* wire cuts |E| */
+    const int32_t *cut_up;          /* [K] subcircuit holding the upstream (measured) end of cut e */
+    const int32_t *cut_down;        /* [K] subcircuit holding the downstream (initialised) end */
+    const int32_t *sub_cut_ofs;     /* [m+1] offsets into sub_cuts */
+    const int32_t *sub_cuts;        /* incident cut ids of s in the AXIS ORDER of the caller's T_s */
+    const int32_t *sub_qubit_ofs;   /* [m+1] offsets into sub_qubits */
+    const int32_t *sub_qubits;      /* output qubits of s, first = MSB of x_s; every qubit exactly once */
+} tqc_network_desc;
+
+typedef struct {
+    int32_t mode;                   /* TQC_MODE_STATES or TQC_MODE_DISTRIBUTION */
+    int32_t n_order_steps;          /* 0: greedy planner (rules P1-P6); else m-1 explicit steps */
+    const int32_t *order;           /* HOST [2*n_order_steps] (lhs, rhs) node ids; leaves 0..m-1, step t creates m+t */
+    int32_t restarts;               /* >0: seeded randomised-greedy restarts, best total cost kept (not bit-pinned) */
+    uint64_t seed;
+    int64_t batch_hint;             /* states mode: expected n_states per call (0 = 2^20).  A node that carries at most
+                                       log2(batch_hint) - 2 output bits is evaluated once per KEY (a table) instead of
+                                       once per state.  Any n_states is still legal at contract time. */
+    int32_t table_log2_floats_max;  /* 0 = default 24: cap on log2(entries) of such a table */
+    int32_t use_tcgen05;            /* 0 = default (on where a step qualifies), -1 = never (fp32 FFMA everywhere) */
+} tqc_plan_opts;
+
+/* ---- planning (host only; no CUDA call) -------------------------------------------------
+ * tqc_plan: network description -> contraction order (section 3.5.1;
+ * the paper delegates this to CoTenGra, this library ships a deterministic greedy planner)
+ * + device layouts + kernel class per step.  *out is library-owned until tqc_plan_destroy. */
+int tqc_plan(const tqc_network_desc *net, const tqc_plan_opts *opts, tqc_plan_t **out);
+void tqc_plan_destroy(tqc_plan_t *plan);
+
+int tqc_plan_mode(const tqc_plan_t *plan);
+int tqc_plan_num_qubits(const tqc_plan_t *plan);
+int tqc_plan_num_subcircuits(const tqc_plan_t *plan);
+int tqc_plan_num_cuts(const tqc_plan_t *plan);
+int tqc_plan_num_steps(const tqc_plan_t *plan);
+int tqc_plan_kmax(const tqc_plan_t *plan);                       /* max_t |E_a u E_b| */
+int tqc_plan_tensor_shape(const tqc_plan_t *plan, int s, int *c_s, int *o_s);
+/* step i: operands, #inner, #outer_lhs, #outer_rhs, log2 of its multiplication count
+ * (4^{#inner+#outer}; + open output bits in distribution mode), kernel class */
+int tqc_plan_step(const tqc_plan_t *plan, int i, int *lhs, int *rhs, int *n_inner,
+                  int *n_outer_lhs, int *n_outer_rhs, int *log2cost, int *kernel_class);
+/* node v (leaves 0..m-1, then one per step): kind (TQC_NODE_*), carried output bits, open cuts */
+int tqc_plan_node(const tqc_plan_t *plan, int v, int *kind, int *n_bits, int *n_open);
+/* log2 of the total multiplication count sum_t 2^{log2cost_t} (per state in states mode) */
+double tqc_plan_cost_log2(const tqc_plan_t *plan);
+/* Serialised plan (little-endian int32 words, format in DESIGN.md "Plan blob"): the object
+ * compared byte-for-byte with the reference planner.  Call with buf = NULL to get *len. */
+int tqc_plan_serialize(const tqc_plan_t *plan, void *buf /*HOST*/, size_t *len);
+/* Workspace bytes that let tqc_contract_states process n_states in ONE chunk (a smaller
+ * workspace is legal down to tqc_plan_workspace_min_bytes: the batch is then chunked), or
+ * that tqc_contract_distribution needs for the given prefix_bits (pass n_states = 0). */
+size_t tqc_plan_workspace_bytes(const tqc_plan_t *plan, size_t n_states, int prefix_bits);
+size_t tqc_plan_workspace_min_bytes(const tqc_plan_t *plan);
+
+/* ---- a1: load + re-layout (the subcircuit output as a tensor) ----
+ * data: [4^{c_s}][2^{o_s}] row-major fp32, HOST (on_device = 0) or DEVICE (on_device = 1).
+ * The library copies it into its own device buffer, state-major [2^{o_s}][4^{c_s}] with the
+ * bond digits permuted for the plan and multiplied by the exact 2^{-d_s} (sum_s d_s = K);
+ * the caller may free `data` once `stream` has completed.  Reloading replaces the tensor. */
+int tqc_load_subcircuit_tensors(tqc_plan_t *plan, int s, const float *data, size_t n_elems,
+                                int on_device, void *stream /* cudaStream_t */);
+
+/* ---- a2-a5: states mode ------------------------------------------------------------------
+ * out_dev[b] = p(x_b) for b < n_states.  states_dev: DEVICE [n_states][ceil(n/64)] uint64.
+ * Asynchronous on `stream`; workspace_dev DEVICE, caller-owned, 256-byte aligned. */
+int tqc_contract_states(tqc_plan_t *plan, const uint64_t *states_dev, size_t n_states,
+                        float *out_dev, void *workspace_dev, size_t workspace_bytes, void *stream);
+
+/* ---- a6: distribution mode ---------------------------------------------------------------
+ * out_dev[i] = p(x) for the 2^{n-prefix_bits} bitstrings whose first prefix_bits qubits equal
+ * prefix_value (qubit 0 = MSB of prefix_value's prefix_bits-bit field), i enumerating the
+ * remaining qubits, lowest-numbered remaining qubit = MSB.  Plan must be MODE_DISTRIBUTION. */
+int tqc_contract_distribution(tqc_plan_t *plan, uint64_t prefix_value, int prefix_bits,
+                              float *out_dev, void *workspace_dev, size_t workspace_bytes, void *stream);
+
+/* number of kernels the library has launched so far on behalf of this plan (for bench.py) */
+uint64_t tqc_plan_launch_count(const tqc_plan_t *plan);
+
+const char *tqc_last_error(void);
+const char *tqc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TQC_H */

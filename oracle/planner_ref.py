@@ -8,10 +8,14 @@ P1 leaves are subcircuits 0..m-1; the node created at step t (0-based) has id m+
 P2 candidates: all unordered pairs of live nodes sharing >= 1 cut; if none exist but
    more than one node is live (disconnected network) the single candidate is the pair
    of the two smallest live ids (outer product).
-P3 cost exponent e(a,b) = 2*|E_a u E_b| in states mode (cost 4^{#inner+#outer},
-   P:407-412); + o_a + o_b in distribution mode (open output bits carried, reading G10).
-P4 choose min e; tie -> fewer resulting open cuts |E_a xor E_b|; tie -> smaller min(id);
-   tie -> smaller max(id).
+P3 two exact integers per candidate.  Cost exponent e(a,b) = 2*|E_a u E_b| in states mode
+   (a step costs 4^{#inner+#outer} multiplications); + o_a + o_b in distribution
+   mode (open output bits carried, reading G10).  Memory score
+   sigma(a,b) = size(result) - size(a) - size(b), size(v) = 2^{w_v} 4^{|E_v|}, w_v = 0 in
+   states mode and the carried output bits in distribution mode: the greedy objective of the
+   order-search library the paper used (CoTenGra), which keeps the frontier of a 2-D
+   network small where a pure min-cost rule grows one large tensor (reading P3).
+P4 choose min sigma; tie -> smaller e; tie -> smaller min(id); tie -> smaller max(id).
 P5 lhs = smaller id; all shared cuts are contracted together as one merged bond
    (P:318-319), digits in ascending cut id.
 P6 K_max = max_t |E_a u E_b|; per-step log2 cost = e.
@@ -25,6 +29,13 @@ from __future__ import annotations
 import struct
 
 MODE_STATES, MODE_DISTRIBUTION = 0, 1
+
+
+def _sigma(open_cuts, obits, a, b, mode):
+    wa = obits[a] if mode == MODE_DISTRIBUTION else 0
+    wb = obits[b] if mode == MODE_DISTRIBUTION else 0
+    r = len(open_cuts[a] ^ open_cuts[b])
+    return (1 << (wa + wb + 2 * r)) - (1 << (wa + 2 * len(open_cuts[a]))) - (1 << (wb + 2 * len(open_cuts[b])))
 
 
 def plan(net, mode: int = MODE_STATES):
@@ -43,7 +54,7 @@ def plan(net, mode: int = MODE_STATES):
                 e = 2 * len(open_cuts[a] | open_cuts[b])
                 if mode == MODE_DISTRIBUTION:
                     e += obits[a] + obits[b]
-                key = (e, len(open_cuts[a] ^ open_cuts[b]), a, b)
+                key = (_sigma(open_cuts, obits, a, b, mode), e, a, b)
                 if best is None or key < best:
                     best = key
         if best is None:
@@ -51,8 +62,8 @@ def plan(net, mode: int = MODE_STATES):
             e = 2 * len(open_cuts[a] | open_cuts[b])
             if mode == MODE_DISTRIBUTION:
                 e += obits[a] + obits[b]
-            best = (e, len(open_cuts[a] ^ open_cuts[b]), a, b)
-        e, _r, a, b = best
+            best = (0, e, a, b)
+        _sig, e, a, b = best
         inner = sorted(open_cuts[a] & open_cuts[b])
         outer_a = sorted(open_cuts[a] - open_cuts[b])
         outer_b = sorted(open_cuts[b] - open_cuts[a])

@@ -1,0 +1,9 @@
+"""B200-native TensorQC reconstruction hot path (arXiv 2502.03445): thin Python binding over the
+C-ABI library libtqc.so (include/tqc.h).  Argument marshalling only; every step of the path runs
+in the CUDA kernels under csrc/.  There is no CPU fallback: without the built library the import
+of `binding` fails, and without a CUDA device the compute calls return TQC_E_CUDA."""
+from .binding import (MODE_DISTRIBUTION, MODE_STATES, Plan, TqcError, lib_path, tqc_contract_distribution,
+                      tqc_contract_states, tqc_load_subcircuit_tensors, tqc_plan, version)
+
+__all__ = ["MODE_STATES", "MODE_DISTRIBUTION", "Plan", "TqcError", "tqc_plan", "tqc_load_subcircuit_tensors",
+           "tqc_contract_states", "tqc_contract_distribution", "version", "lib_path"]

@@ -1,0 +1,240 @@
+// SIMT kernels of the reconstruction hot path (sm_100a).  PAPER.md section 3.2 (lines 321-330):
+// a pairwise contraction multiplies two tensors and sums over their shared (merged) bond;
+// section 3.3 (lines 407-412): it costs 4^{#inner + #outer} multiplications per state.
+#pragma once
+#include <cuda_runtime.h>
+#include "device_args.h"
+
+namespace tqc {
+
+// ---------------------------------------------------------------------------------------------
+// a1  load / re-layout:  dst[x][j] = scale * src[row_of(j)][x]
+// 32x32 shared-memory transpose: reads run along x (contiguous in the caller's layout), writes
+// along j (contiguous in the state-major device layout).
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) relayout_kernel(const RelayoutArgs a) {
+    __shared__ float tile[32][33];
+    const long long rows = 1ll << a.lgRows, cols = 1ll << a.lgCols;
+    const long long tiles_x = (cols + 31) / 32;
+    const long long bx = blockIdx.x % tiles_x, bj = blockIdx.x / tiles_x;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const long long x = bx * 32 + tx;
+    for (int jj = ty; jj < 32; jj += 8) {
+        const long long j = bj * 32 + jj;
+        if (j < rows && x < cols) {
+            const unsigned long long row = bitmap_apply(a.row_of, (unsigned long long)j);
+            tile[jj][tx] = a.src[row * cols + x];
+        }
+    }
+    __syncthreads();
+    const long long j = bj * 32 + tx;
+    for (int xx = ty; xx < 32; xx += 8) {
+        const long long xo = bx * 32 + xx;
+        if (j < rows && xo < cols) a.dst[xo * rows + j] = a.scale * tile[tx][xx];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a2  key extraction:  keys[slot][r] = bits of state r at the slot's qubits, first listed = MSB
+// (readings G4, G5: qubit q is bit q%64 of word q/64).
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) key_kernel(const KeyArgs a) {
+    const int slot = blockIdx.y;
+    const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= a.R) return;
+    const uint64_t *w = a.states + r * a.words;
+    uint32_t key = 0;
+    for (int p = a.slot_ofs[slot]; p < a.slot_ofs[slot + 1]; ++p) {
+        const int q = a.slot_qubits[p];
+        key = (key << 1) | (uint32_t)((w[q >> 6] >> (q & 63)) & 1ull);
+    }
+    a.keys[slot * a.cap + r] = key;
+}
+
+// ---------------------------------------------------------------------------------------------
+// a3 + a4  contraction step, register-tiled fp32 FFMA.
+//   C[rowC][outA(i') | outB(j')] = sum_k A[i', k] * B[j', k]
+// Both operands are K-major (the merged bond is the contiguous axis).  The gather of a3 is the
+// operand addressing: a row of a LEAF/TABLE operand is selected by the state's key.
+// One block: RPB rows x (TI x TJ) outputs; each thread an MI x MJ micro-tile; the bond is
+// consumed in slabs of TK staged through shared memory as [k][i] so the inner loop reads
+// float4s that are broadcast (A) or contiguous (B) across a warp.
+// ---------------------------------------------------------------------------------------------
+template <int MI, int MJ>
+__global__ void __launch_bounds__(256) step_tile_kernel(const StepArgs a) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int TI = a.TI, TJ = a.TJ, TK = a.TK, RPB = a.RPB;
+    const int TIp = TI + (MI == 4 ? 4 : 1), TJp = TJ + (MJ == 4 ? 4 : 1);
+    unsigned long long *rowA = reinterpret_cast<unsigned long long *>(smem_raw);     // [RPB*TI] float offsets
+    unsigned long long *rowB = rowA + RPB * TI;                                       // [RPB*TJ]
+    float *As = reinterpret_cast<float *>(rowB + RPB * TJ);                           // [RPB][TK][TIp]
+    float *Bs = As + RPB * TK * TIp;                                                  // [RPB][TK][TJp]
+
+    const long long bid = blockIdx.x;
+    const int tjb = (int)(bid % a.tiles_j);
+    const int tib = (int)((bid / a.tiles_j) % a.tiles_i);
+    const long long rg = bid / ((long long)a.tiles_j * a.tiles_i);
+    const int nti = TI / MI, ntj = TJ / MJ, tpr = nti * ntj;
+    const int tid = threadIdx.x;
+    const int row_l = tid / tpr, within = tid % tpr;
+    const int ti = within / ntj, tj = within % ntj;
+    const long long K = 1ll << a.lgK;
+    const long long M = 1ll << a.lgM, N = 1ll << a.lgN;
+
+    // operand row offsets (in floats) of every (row, i) and (row, j) this block touches
+    for (int e = tid; e < RPB * TI; e += 256) {
+        const int rl = e / TI, i = e % TI;
+        const long long r = rg * RPB + rl;
+        unsigned long long off = ~0ull;
+        if (r < a.R) {
+            const unsigned long long ip = (unsigned long long)tib * TI + i;
+            if (a.A.use_map) off = (bitmap_apply(a.A.in_map, ip) | a.A.in_or) << a.lgK;
+            else {
+                const unsigned long long row = a.A.keys ? (unsigned long long)a.A.keys[r] : (unsigned long long)r;
+                off = ((row << a.lgM) + ip) << a.lgK;
+            }
+        }
+        rowA[e] = off;
+    }
+    for (int e = tid; e < RPB * TJ; e += 256) {
+        const int rl = e / TJ, j = e % TJ;
+        const long long r = rg * RPB + rl;
+        unsigned long long off = ~0ull;
+        if (r < a.R) {
+            const unsigned long long jp = (unsigned long long)tjb * TJ + j;
+            if (a.B.use_map) off = (bitmap_apply(a.B.in_map, jp) | a.B.in_or) << a.lgK;
+            else {
+                const unsigned long long row = a.B.keys ? (unsigned long long)a.B.keys[r] : (unsigned long long)r;
+                off = ((row << a.lgN) + jp) << a.lgK;
+            }
+        }
+        rowB[e] = off;
+    }
+    __syncthreads();
+
+    float acc[MI][MJ];
+#pragma unroll
+    for (int x = 0; x < MI; ++x)
+#pragma unroll
+        for (int y = 0; y < MJ; ++y) acc[x][y] = 0.f;
+
+    for (long long k0 = 0; k0 < K; k0 += TK) {
+        if (TK >= 4) {
+            const int kq = TK / 4;
+            for (int e = tid; e < RPB * TI * kq; e += 256) {
+                const int k4 = e % kq, ri = e / kq;                 // ri = rl * TI + i
+                const unsigned long long off = rowA[ri];
+                float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (off != ~0ull) v = __ldg(reinterpret_cast<const float4 *>(a.A.base + off + k0) + k4);
+                float *dst = As + ((ri / TI) * TK + k4 * 4) * TIp + (ri % TI);
+                dst[0] = v.x; dst[TIp] = v.y; dst[2 * TIp] = v.z; dst[3 * TIp] = v.w;
+            }
+            for (int e = tid; e < RPB * TJ * kq; e += 256) {
+                const int k4 = e % kq, rj = e / kq;
+                const unsigned long long off = rowB[rj];
+                float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (off != ~0ull) v = __ldg(reinterpret_cast<const float4 *>(a.B.base + off + k0) + k4);
+                float *dst = Bs + ((rj / TJ) * TK + k4 * 4) * TJp + (rj % TJ);
+                dst[0] = v.x; dst[TJp] = v.y; dst[2 * TJp] = v.z; dst[3 * TJp] = v.w;
+            }
+        } else {
+            for (int e = tid; e < RPB * TI * TK; e += 256) {
+                const int k = e % TK, ri = e / TK;
+                const unsigned long long off = rowA[ri];
+                As[((ri / TI) * TK + k) * TIp + (ri % TI)] = (off != ~0ull) ? __ldg(a.A.base + off + k0 + k) : 0.f;
+            }
+            for (int e = tid; e < RPB * TJ * TK; e += 256) {
+                const int k = e % TK, rj = e / TK;
+                const unsigned long long off = rowB[rj];
+                Bs[((rj / TJ) * TK + k) * TJp + (rj % TJ)] = (off != ~0ull) ? __ldg(a.B.base + off + k0 + k) : 0.f;
+            }
+        }
+        __syncthreads();
+        if (row_l < RPB) {
+            const float *ap = As + row_l * TK * TIp + ti * MI;
+            const float *bp = Bs + row_l * TK * TJp + tj * MJ;
+#pragma unroll 4
+            for (int k = 0; k < TK; ++k) {
+                float av[MI], bv[MJ];
+                if (MI == 4) { const float4 t = *reinterpret_cast<const float4 *>(ap + k * TIp); av[0] = t.x; av[1] = t.y; av[2] = t.z; av[3] = t.w; }
+                else av[0] = ap[k * TIp];
+                if (MJ == 4) { const float4 t = *reinterpret_cast<const float4 *>(bp + k * TJp); bv[0] = t.x; bv[1] = t.y; bv[2] = t.z; bv[3] = t.w; }
+                else bv[0] = bp[k * TJp];
+#pragma unroll
+                for (int x = 0; x < MI; ++x)
+#pragma unroll
+                    for (int y = 0; y < MJ; ++y) acc[x][y] = fmaf(av[x], bv[y], acc[x][y]);
+            }
+        }
+        __syncthreads();
+    }
+
+    const long long r = rg * RPB + row_l;
+    if (row_l >= RPB || r >= a.R) return;
+    const unsigned long long i0 = (unsigned long long)tib * TI + ti * MI;
+    const unsigned long long j0 = (unsigned long long)tjb * TJ + tj * MJ;
+    if (i0 >= (unsigned long long)M || j0 >= (unsigned long long)N) return;
+    float *crow = a.C + r * a.c_row_stride;
+    unsigned long long ob[MJ];
+#pragma unroll
+    for (int y = 0; y < MJ; ++y) ob[y] = bitmap_apply(a.outB, j0 + y);
+#pragma unroll
+    for (int x = 0; x < MI; ++x) {
+        const unsigned long long oa = bitmap_apply(a.outA, i0 + x);
+        if (MJ == 4 && a.vec_store) {
+            *reinterpret_cast<float4 *>(crow + (oa | ob[0])) = make_float4(acc[x][0], acc[x][1], acc[x][2], acc[x][3]);
+        } else {
+#pragma unroll
+            for (int y = 0; y < MJ; ++y) crow[oa | ob[y]] = acc[x][y];
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a5  final reduction: no outer cut is left, out[r] = sum_k A_r[k] * B_r[k] over the last merged
+// bond (the 2^{-K} of reading G1 is already folded into the leaves as 2^{-d_s}, reading G2).
+// G lanes per row (G = min(32, K/4), float4 loads), shuffle tree inside the group.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) dot_kernel(const DotArgs a) {
+    const long long K = 1ll << a.lgK;
+    int G = (int)(K / 4);
+    if (G > 32) G = 32;
+    if (G < 1) G = 1;
+    const int rows_per_warp = 32 / G;
+    const int lane = threadIdx.x & 31;
+    const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const long long r = warp * rows_per_warp + lane / G;
+    const int g = lane % G;
+    float s = 0.f;
+    if (r < a.R) {
+        const unsigned long long ra = a.keysA ? (unsigned long long)a.keysA[r] : (unsigned long long)r;
+        const unsigned long long rb = a.keysB ? (unsigned long long)a.keysB[r] : (unsigned long long)r;
+        const float *pa = a.A + (ra << a.lgK), *pb = a.B + (rb << a.lgK);
+        if (K >= 4) {
+            const float4 *qa = reinterpret_cast<const float4 *>(pa), *qb = reinterpret_cast<const float4 *>(pb);
+            float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
+            for (long long k = g; k < K / 4; k += G) {
+                const float4 x = __ldg(qa + k), y = __ldg(qb + k);
+                s0 = fmaf(x.x, y.x, s0); s1 = fmaf(x.y, y.y, s1); s2 = fmaf(x.z, y.z, s2); s3 = fmaf(x.w, y.w, s3);
+            }
+            s = (s0 + s1) + (s2 + s3);
+        } else {
+            for (long long k = 0; k < K; ++k) s = fmaf(pa[k], pb[k], s);
+        }
+    }
+    for (int d = G >> 1; d > 0; d >>= 1) s += __shfl_down_sync(0xffffffffu, s, d, G);
+    if (r < a.R && g == 0) a.out[r] = s;
+}
+
+// ---------------------------------------------------------------------------------------------
+// root is a LEAF or a TABLE: out[...] = table[row]   (m = 1 / K = 0, or a network so small that
+// the whole distribution is one table)
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) gather_kernel(const GatherArgs a) {
+    const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= a.R) return;
+    if (a.keys) a.out[r] = a.table[a.keys[r]];
+    else a.out[bitmap_apply(a.out_map, (unsigned long long)r)] = a.table[bitmap_apply(a.map, (unsigned long long)r) | a.map_or];
+}
+
+}  // namespace tqc

@@ -1,0 +1,588 @@
+// C ABI of libtqc.so (include/tqc.h): plan handle, tensor load, states / distribution contraction.
+// Host launch logic only; the arithmetic is in kernels_simt.cuh / kernels_tc.cuh.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/tqc.h"
+#include "device_args.h"
+#include "kernels_simt.cuh"
+#include "plan.hpp"
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const std::string &msg) {
+    g_err = msg;
+    return code;
+}
+
+#define TQC_CUDA(expr)                                                                         \
+    do {                                                                                       \
+        cudaError_t e__ = (expr);                                                              \
+        if (e__ != cudaSuccess)                                                                \
+            return fail(TQC_E_CUDA, std::string(#expr) + ": " + cudaGetErrorString(e__));      \
+    } while (0)
+
+// ---- BitMap construction -------------------------------------------------------------------
+struct BitPairs {
+    std::vector<std::pair<int, int>> p;   // (src bit, dst bit)
+    void add(int src, int dst) { p.emplace_back(src, dst); }
+    void add_run(int src, int dst, int len) { for (int i = 0; i < len; ++i) add(src + i, dst + i); }
+    bool build(BitMap &m) const {
+        std::vector<std::pair<int, int>> q = p;
+        std::sort(q.begin(), q.end());
+        m.n = 0;
+        for (size_t i = 0; i < q.size();) {
+            size_t j = i + 1;
+            while (j < q.size() && q[j].first == q[j - 1].first + 1 && q[j].second == q[j - 1].second + 1) ++j;
+            if (m.n >= TQC_MAXSEG) return false;
+            m.src[m.n] = (uint8_t)q[i].first; m.dst[m.n] = (uint8_t)q[i].second; m.len[m.n] = (uint8_t)(j - i);
+            ++m.n;
+            i = j;
+        }
+        return true;
+    }
+};
+
+int index_of(const std::vector<int> &v, int x) {
+    for (size_t i = 0; i < v.size(); ++i) if (v[i] == x) return (int)i;
+    return -1;
+}
+
+}  // namespace
+
+struct tqc_plan {
+    tqc::HostPlan hp;
+    int use_tcgen05 = 0;
+    std::vector<float *> d_leaf;
+    std::vector<char> loaded;
+    int32_t *d_slot_ofs = nullptr, *d_slot_qubits = nullptr;
+    float *d_staging = nullptr;
+    size_t staging_elems = 0;
+    uint64_t launches = 0;
+    bool attrs_set = false;
+};
+
+namespace {
+
+using tqc::HostPlan;
+using tqc::Node;
+using tqc::Step;
+
+constexpr int kMaxDynSmem = 200 * 1024;
+
+template <int MI, int MJ>
+int launch_tile_t(const StepArgs &a, size_t smem, long long blocks, cudaStream_t st) {
+    static bool attr = false;
+    if (!attr) {
+        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tile_kernel<MI, MJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
+        attr = true;
+    }
+    tqc::step_tile_kernel<MI, MJ><<<(unsigned)blocks, 256, smem, st>>>(a);
+    TQC_CUDA(cudaGetLastError());
+    return 0;
+}
+
+// Tile choice for the FFMA kernel: TI x TJ outputs per row, RPB rows per 256-thread block.
+int launch_tile(tqc_plan_t *pl, StepArgs &a, cudaStream_t st) {
+    const int MI = a.lgM >= 2 ? 4 : 1, MJ = a.lgN >= 2 ? 4 : 1;
+    const long long M = 1ll << a.lgM, N = 1ll << a.lgN, K = 1ll << a.lgK;
+    long long TI = MI == 4 ? std::min<long long>(M, 64) : M;
+    long long capJ = 256ll * MJ * MI / TI;                 // threads per row-tile <= 256
+    long long TJ = MJ == 4 ? std::min<long long>(std::min<long long>(N, capJ), 256) : N;
+    if (MI == 4 && MJ == 4 && TJ < 64 && TI == 64 && M > 64) TI = std::min<long long>(M, std::min<long long>(256, 4096 / TJ));
+    const long long tpr = (TI / MI) * (TJ / MJ);
+    const long long RPB = std::max<long long>(1, 256 / tpr);
+    long long TK = std::min<long long>(K, 16);
+    const long long TIp = TI + (MI == 4 ? 4 : 1), TJp = TJ + (MJ == 4 ? 4 : 1);
+    auto smem_of = [&](long long tk) { return (size_t)(8 * RPB * (TI + TJ) + 4 * RPB * tk * (TIp + TJp)); };
+    while (TK > 1 && smem_of(TK) > (size_t)96 * 1024) TK /= 2;
+    if (smem_of(TK) > (size_t)kMaxDynSmem) return fail(TQC_E_TOO_LARGE, "internal: tile does not fit shared memory");
+    a.TI = (int)TI; a.TJ = (int)TJ; a.TK = (int)TK; a.RPB = (int)RPB;
+    a.tiles_i = (int)(M / TI); a.tiles_j = (int)(N / TJ);
+    a.vec_store = (MJ == 4 && a.outB.n >= 1 && a.outB.src[0] == 0 && a.outB.dst[0] == 0 && a.outB.len[0] >= 2) ? 1 : 0;
+    const long long rgroups = (a.R + RPB - 1) / RPB;
+    const long long blocks = (long long)a.tiles_i * a.tiles_j * rgroups;
+    if (blocks <= 0 || blocks > 0x7fffffffll) return fail(TQC_E_TOO_LARGE, "step needs more than 2^31 thread blocks");
+    int rc;
+    if (MI == 4 && MJ == 4) rc = launch_tile_t<4, 4>(a, smem_of(TK), blocks, st);
+    else if (MI == 4) rc = launch_tile_t<4, 1>(a, smem_of(TK), blocks, st);
+    else if (MJ == 4) rc = launch_tile_t<1, 4>(a, smem_of(TK), blocks, st);
+    else rc = launch_tile_t<1, 1>(a, smem_of(TK), blocks, st);
+    if (rc == 0) pl->launches++;
+    return rc;
+}
+
+// digits of an operand's outer index (most significant first) -> bit positions inside C's row
+void add_digit_scatter(BitPairs &bp, const std::vector<int> &outer, const std::vector<int> &c_layout) {
+    const int no = (int)outer.size(), nc = (int)c_layout.size();
+    for (int x = 0; x < no; ++x) {
+        const int p = no - 1 - x;                                // digit position from the LSB side
+        const int y = index_of(c_layout, outer[x]);
+        const int pos = nc - 1 - y;
+        bp.add_run(2 * p, 2 * pos, 2);
+    }
+}
+
+// ---- cross mode (TABLE outputs; distribution mode and states-mode tables) --------------------
+struct CrossCtx {
+    int prefix_bits = 0;
+    uint64_t prefix_value = 0;
+    const std::vector<int> *free_bits = nullptr;      // per node (distribution) or null (all bits free)
+    const std::vector<int64_t> *offsets = nullptr;    // per node float offsets (distribution)
+    float *ws = nullptr;                               // base of table storage
+    float *out = nullptr;                              // distribution root target
+};
+
+std::vector<int> free_qubits(const Node &v, int prefix_bits) {
+    std::vector<int> f;
+    for (int q : v.qubits) if (q >= prefix_bits) f.push_back(q);
+    return f;
+}
+
+int build_cross_operand(tqc_plan_t *pl, const CrossCtx &cx, int v, const std::vector<int> &outer, OperandArgs &o,
+                        int &lg_rows) {
+    const HostPlan &hp = pl->hp;
+    const Node &nd = hp.nodes[v];
+    const std::vector<int> fq = free_qubits(nd, cx.prefix_bits);
+    const int nd_bits = 2 * (int)outer.size();
+    lg_rows = (int)fq.size() + nd_bits;
+    o.keys = nullptr; o.in_or = 0; o.use_map = 0; o.in_map.n = 0;
+    if (v < hp.m) {
+        o.base = pl->d_leaf[v];
+        if (fq.size() != nd.qubits.size()) {
+            BitPairs bp;
+            bp.add_run(0, 0, nd_bits);
+            const int nq = (int)nd.qubits.size(), nf = (int)fq.size();
+            unsigned long long fixed = 0;
+            int t = 0;
+            for (int pq = 0; pq < nq; ++pq) {
+                const int q = nd.qubits[pq];
+                const int keybit = nq - 1 - pq;
+                if (q >= cx.prefix_bits) { bp.add(nd_bits + (nf - 1 - t), nd_bits + keybit); ++t; }
+                else if ((cx.prefix_value >> (cx.prefix_bits - 1 - q)) & 1ull) fixed |= 1ull << (nd_bits + keybit);
+            }
+            if (!bp.build(o.in_map)) return fail(TQC_E_TOO_LARGE, "bit map needs too many segments");
+            o.in_or = fixed;
+            o.use_map = 1;
+        }
+    } else {
+        const int64_t off = cx.offsets ? (*cx.offsets)[v] : nd.table_offset;
+        o.base = cx.ws + off;
+    }
+    return 0;
+}
+
+int launch_cross_step(tqc_plan_t *pl, const CrossCtx &cx, int t, cudaStream_t st) {
+    const HostPlan &hp = pl->hp;
+    const Step &s = hp.steps[t];
+    const int vc = hp.m + t;
+    const Node &A = hp.nodes[s.lhs], &B = hp.nodes[s.rhs], &C = hp.nodes[vc];
+    StepArgs a;
+    memset(&a, 0, sizeof(a));
+    int rc;
+    if ((rc = build_cross_operand(pl, cx, s.lhs, s.outer_lhs, a.A, a.lgM))) return rc;
+    if ((rc = build_cross_operand(pl, cx, s.rhs, s.outer_rhs, a.B, a.lgN))) return rc;
+    a.lgK = 2 * (int)s.inner.size();
+    a.R = 1;
+    a.c_row_stride = 0;
+    const std::vector<int> fa = free_qubits(A, cx.prefix_bits), fb = free_qubits(B, cx.prefix_bits);
+    const bool dist_root = cx.out != nullptr && vc == hp.root();
+    const int cdig = 2 * (int)C.layout.size();
+    BitPairs pa, pb;
+    add_digit_scatter(pa, s.outer_lhs, C.layout);
+    add_digit_scatter(pb, s.outer_rhs, C.layout);
+    const int na = 2 * (int)s.outer_lhs.size(), nb = 2 * (int)s.outer_rhs.size();
+    if (dist_root) {
+        // product-order row bits -> global bit order: free qubits ascending, lowest id = MSB (G4)
+        std::vector<int> all = fa;
+        all.insert(all.end(), fb.begin(), fb.end());
+        auto dst_of = [&](int q) { int c = 0; for (int x : all) if (x > q) ++c; return c; };
+        for (size_t i = 0; i < fa.size(); ++i) pa.add(na + (int)(fa.size() - 1 - i), dst_of(fa[i]));
+        for (size_t i = 0; i < fb.size(); ++i) pb.add(nb + (int)(fb.size() - 1 - i), dst_of(fb[i]));
+        a.C = cx.out;
+    } else {
+        pa.add_run(na, cdig + (int)fb.size(), (int)fa.size());
+        pb.add_run(nb, cdig, (int)fb.size());
+        const int64_t off = cx.offsets ? (*cx.offsets)[vc] : C.table_offset;
+        a.C = cx.ws + off;
+    }
+    if (!pa.build(a.outA) || !pb.build(a.outB)) return fail(TQC_E_TOO_LARGE, "bit map needs too many segments");
+    return launch_tile(pl, a, st);
+}
+
+// ---- batch mode (one row per state of the chunk) ---------------------------------------------
+struct BatchCtx {
+    float *tables = nullptr;     // states-mode table region
+    uint32_t *keys = nullptr;    // [n_slots][cap]
+    float *batch = nullptr;      // BATCH intermediates: node block at ws_offset * cap
+    long long cap = 0;
+    int R = 0;
+    float *out = nullptr;        // out + chunk_start
+};
+
+void batch_operand(tqc_plan_t *pl, const BatchCtx &bx, int v, const float *&base, const uint32_t *&keys) {
+    const HostPlan &hp = pl->hp;
+    const Node &nd = hp.nodes[v];
+    if (nd.kind == tqc::NODE_BATCH) { base = bx.batch + nd.ws_offset * bx.cap; keys = nullptr; }
+    else {
+        base = v < hp.m ? pl->d_leaf[v] : bx.tables + nd.table_offset;
+        keys = bx.keys + (long long)nd.key_slot * bx.cap;
+    }
+}
+
+int launch_batch_step(tqc_plan_t *pl, const BatchCtx &bx, int t, cudaStream_t st) {
+    const HostPlan &hp = pl->hp;
+    const Step &s = hp.steps[t];
+    const int vc = hp.m + t;
+    const Node &C = hp.nodes[vc];
+    const int lgM = 2 * (int)s.outer_lhs.size(), lgN = 2 * (int)s.outer_rhs.size(), lgK = 2 * (int)s.inner.size();
+    float *cbase = (vc == hp.root()) ? bx.out : bx.batch + C.ws_offset * bx.cap;
+    if (lgM == 0 && lgN == 0) {
+        DotArgs d;
+        memset(&d, 0, sizeof(d));
+        batch_operand(pl, bx, s.lhs, d.A, d.keysA);
+        batch_operand(pl, bx, s.rhs, d.B, d.keysB);
+        d.out = cbase; d.lgK = lgK; d.R = bx.R;
+        long long G = std::min<long long>(32, std::max<long long>(1, (1ll << lgK) / 4));
+        const long long rows_per_block = (32 / G) * 8;
+        const long long blocks = (bx.R + rows_per_block - 1) / rows_per_block;
+        tqc::dot_kernel<<<(unsigned)blocks, 256, 0, st>>>(d);
+        TQC_CUDA(cudaGetLastError());
+        pl->launches++;
+        return 0;
+    }
+    StepArgs a;
+    memset(&a, 0, sizeof(a));
+    batch_operand(pl, bx, s.lhs, a.A.base, a.A.keys);
+    batch_operand(pl, bx, s.rhs, a.B.base, a.B.keys);
+    a.lgM = lgM; a.lgN = lgN; a.lgK = lgK;
+    a.R = bx.R;
+    a.C = cbase;
+    a.c_row_stride = 1ll << (2 * (int)C.open.size());
+    BitPairs pa, pb;
+    add_digit_scatter(pa, s.outer_lhs, C.layout);
+    add_digit_scatter(pb, s.outer_rhs, C.layout);
+    if (!pa.build(a.outA) || !pb.build(a.outB)) return fail(TQC_E_TOO_LARGE, "bit map needs too many segments");
+    return launch_tile(pl, a, st);
+}
+
+int ensure_meta(tqc_plan_t *pl) {
+    if (pl->d_slot_ofs || pl->hp.mode != TQC_MODE_STATES || pl->hp.n_key_slots == 0) return 0;
+    const HostPlan &hp = pl->hp;
+    std::vector<int32_t> ofs(hp.n_key_slots + 1, 0), qs;
+    for (int slot = 0; slot < hp.n_key_slots; ++slot) {
+        for (const Node &nd : hp.nodes)
+            if (nd.key_slot == slot) for (int q : nd.qubits) qs.push_back(q);
+        ofs[slot + 1] = (int32_t)qs.size();
+    }
+    TQC_CUDA(cudaMalloc(&pl->d_slot_ofs, ofs.size() * sizeof(int32_t)));
+    TQC_CUDA(cudaMalloc(&pl->d_slot_qubits, std::max<size_t>(1, qs.size()) * sizeof(int32_t)));
+    TQC_CUDA(cudaMemcpy(pl->d_slot_ofs, ofs.data(), ofs.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
+    if (!qs.empty()) TQC_CUDA(cudaMemcpy(pl->d_slot_qubits, qs.data(), qs.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
+    return 0;
+}
+
+size_t align256(size_t v) { return (v + 255) / 256 * 256; }
+
+// states-mode workspace: [tables][keys: n_slots x cap u32][batch: ws_floats_per_state x cap]
+size_t states_fixed_bytes(const HostPlan &hp) { return align256((size_t)hp.table_floats * 4); }
+size_t states_bytes_per_state(const HostPlan &hp) { return (size_t)hp.n_key_slots * 4 + (size_t)hp.ws_floats_per_state * 4; }
+
+}  // namespace
+
+extern "C" {
+
+const char *tqc_last_error(void) { return g_err.c_str(); }
+const char *tqc_version(void) { return "tqc-b200 0.1 (sm_100a)"; }
+
+int tqc_plan(const tqc_network_desc *net, const tqc_plan_opts *opts, tqc_plan_t **out) {
+    if (!net || !out) return fail(TQC_E_ARG, "null argument");
+    tqc::PlanOptions po;
+    int use_tc = 0;
+    if (opts) {
+        po.mode = opts->mode;
+        po.restarts = opts->restarts;
+        po.seed = opts->seed;
+        po.batch_hint = opts->batch_hint;
+        po.table_log2_floats_max = opts->table_log2_floats_max;
+        use_tc = opts->use_tcgen05;
+        if (opts->n_order_steps > 0) {
+            if (!opts->order) return fail(TQC_E_ARG, "n_order_steps > 0 but order is null");
+            for (int i = 0; i < opts->n_order_steps; ++i) po.order.emplace_back(opts->order[2 * i], opts->order[2 * i + 1]);
+        }
+    }
+    tqc_plan_t *pl = new tqc_plan_t();
+    std::string err;
+    const int rc = tqc::build_plan(net->n_qubits, net->m, net->K, net->cut_up, net->cut_down, net->sub_cut_ofs,
+                                   net->sub_cuts, net->sub_qubit_ofs, net->sub_qubits, po, pl->hp, err);
+    if (rc != 0) { delete pl; return fail(rc, err); }
+    pl->use_tcgen05 = use_tc;
+    pl->d_leaf.assign(pl->hp.m, nullptr);
+    pl->loaded.assign(pl->hp.m, 0);
+    for (int t = 0; t < pl->hp.m - 1; ++t) {
+        Step &s = pl->hp.steps[t];
+        s.kernel_class = (s.outer_lhs.empty() && s.outer_rhs.empty() && pl->hp.nodes[pl->hp.m + t].kind == tqc::NODE_BATCH)
+                             ? TQC_KERNEL_DOT : TQC_KERNEL_SIMT_TILE;
+    }
+    *out = pl;
+    return 0;
+}
+
+void tqc_plan_destroy(tqc_plan_t *pl) {
+    if (!pl) return;
+    for (float *p : pl->d_leaf) if (p) cudaFree(p);
+    if (pl->d_slot_ofs) cudaFree(pl->d_slot_ofs);
+    if (pl->d_slot_qubits) cudaFree(pl->d_slot_qubits);
+    if (pl->d_staging) cudaFree(pl->d_staging);
+    delete pl;
+}
+
+int tqc_plan_mode(const tqc_plan_t *pl) { return pl ? pl->hp.mode : TQC_E_ARG; }
+int tqc_plan_num_qubits(const tqc_plan_t *pl) { return pl ? pl->hp.n : TQC_E_ARG; }
+int tqc_plan_num_subcircuits(const tqc_plan_t *pl) { return pl ? pl->hp.m : TQC_E_ARG; }
+int tqc_plan_num_cuts(const tqc_plan_t *pl) { return pl ? pl->hp.K : TQC_E_ARG; }
+int tqc_plan_num_steps(const tqc_plan_t *pl) { return pl ? (int)pl->hp.steps.size() : TQC_E_ARG; }
+int tqc_plan_kmax(const tqc_plan_t *pl) { return pl ? pl->hp.kmax : TQC_E_ARG; }
+
+int tqc_plan_tensor_shape(const tqc_plan_t *pl, int s, int *c_s, int *o_s) {
+    if (!pl || s < 0 || s >= pl->hp.m) return fail(TQC_E_ARG, "bad plan or subcircuit id");
+    if (c_s) *c_s = pl->hp.c(s);
+    if (o_s) *o_s = pl->hp.o(s);
+    return 0;
+}
+
+int tqc_plan_step(const tqc_plan_t *pl, int i, int *lhs, int *rhs, int *n_inner, int *n_outer_lhs, int *n_outer_rhs,
+                  int *log2cost, int *kernel_class) {
+    if (!pl || i < 0 || i >= (int)pl->hp.steps.size()) return fail(TQC_E_ARG, "bad plan or step id");
+    const Step &s = pl->hp.steps[i];
+    if (lhs) *lhs = s.lhs;
+    if (rhs) *rhs = s.rhs;
+    if (n_inner) *n_inner = (int)s.inner.size();
+    if (n_outer_lhs) *n_outer_lhs = (int)s.outer_lhs.size();
+    if (n_outer_rhs) *n_outer_rhs = (int)s.outer_rhs.size();
+    if (log2cost) *log2cost = s.log2cost;
+    if (kernel_class) *kernel_class = s.kernel_class;
+    return 0;
+}
+
+int tqc_plan_node(const tqc_plan_t *pl, int v, int *kind, int *n_bits, int *n_open) {
+    if (!pl || v < 0 || v >= (int)pl->hp.nodes.size()) return fail(TQC_E_ARG, "bad plan or node id");
+    const Node &nd = pl->hp.nodes[v];
+    if (kind) *kind = nd.kind;
+    if (n_bits) *n_bits = (int)nd.qubits.size();
+    if (n_open) *n_open = (int)nd.open.size();
+    return 0;
+}
+
+double tqc_plan_cost_log2(const tqc_plan_t *pl) { return pl ? tqc::cost_log2(pl->hp) : -1.0; }
+
+int tqc_plan_serialize(const tqc_plan_t *pl, void *buf, size_t *len) {
+    if (!pl || !len) return fail(TQC_E_ARG, "null argument");
+    const std::vector<int32_t> w = tqc::serialize_words(pl->hp);
+    const size_t need = 8 + w.size() * 4;
+    if (!buf) { *len = need; return 0; }
+    if (*len < need) { *len = need; return fail(TQC_E_ARG, "buffer too small"); }
+    unsigned char *b = (unsigned char *)buf;
+    memcpy(b, "TQCP", 4);
+    const int32_t version = 1;
+    memcpy(b + 4, &version, 4);
+    memcpy(b + 8, w.data(), w.size() * 4);
+    *len = need;
+    return 0;
+}
+
+size_t tqc_plan_workspace_min_bytes(const tqc_plan_t *pl) {
+    if (!pl) return 0;
+    if (pl->hp.mode == TQC_MODE_STATES) return states_fixed_bytes(pl->hp) + align256(states_bytes_per_state(pl->hp) * 64) + 256;
+    return tqc_plan_workspace_bytes(pl, 0, 0);
+}
+
+size_t tqc_plan_workspace_bytes(const tqc_plan_t *pl, size_t n_states, int prefix_bits) {
+    if (!pl) return 0;
+    const HostPlan &hp = pl->hp;
+    if (hp.mode == TQC_MODE_STATES) {
+        const size_t cap = (std::max<size_t>(n_states, 1) + 63) / 64 * 64;
+        return states_fixed_bytes(hp) + align256(states_bytes_per_state(hp) * cap) + 256;
+    }
+    std::vector<int> fb;
+    std::vector<int64_t> off;
+    const int64_t floats = tqc::distribution_layout(hp, std::max(0, std::min(prefix_bits, hp.n)), fb, off);
+    return align256((size_t)floats * 4) + 256;
+}
+
+int tqc_load_subcircuit_tensors(tqc_plan_t *pl, int s, const float *data, size_t n_elems, int on_device, void *stream) {
+    if (!pl || !data) return fail(TQC_E_ARG, "null argument");
+    HostPlan &hp = pl->hp;
+    if (s < 0 || s >= hp.m) return fail(TQC_E_ARG, "subcircuit id out of range");
+    const int c = hp.c(s), o = hp.o(s);
+    const size_t need = (size_t)1 << (2 * c + o);
+    if (n_elems != need) return fail(TQC_E_SHAPE, "n_elems must be 4^c_s * 2^o_s = " + std::to_string(need));
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = ensure_meta(pl);
+    if (rc) return rc;
+    if (!pl->d_leaf[s]) TQC_CUDA(cudaMalloc(&pl->d_leaf[s], need * sizeof(float)));
+    const float *src = data;
+    if (!on_device) {
+        if (pl->staging_elems < need) {
+            if (pl->d_staging) { TQC_CUDA(cudaStreamSynchronize(st)); TQC_CUDA(cudaFree(pl->d_staging)); pl->d_staging = nullptr; }
+            TQC_CUDA(cudaMalloc(&pl->d_staging, need * sizeof(float)));
+            pl->staging_elems = need;
+        }
+        TQC_CUDA(cudaMemcpyAsync(pl->d_staging, data, need * sizeof(float), cudaMemcpyHostToDevice, st));
+        src = pl->d_staging;
+    }
+    RelayoutArgs a;
+    memset(&a, 0, sizeof(a));
+    a.src = src; a.dst = pl->d_leaf[s];
+    a.lgRows = 2 * c; a.lgCols = o;
+    a.scale = std::ldexp(1.0f, -hp.d[s]);
+    // device digit x (most significant first) holds cut layout[x]; the caller's digit order is sub_cuts[s]
+    const Node &leaf = hp.nodes[s];
+    std::vector<int> layout = leaf.layout;
+    if (layout.empty()) layout = leaf.open;               // m == 1 has no consumer: keep ascending order
+    BitPairs bp;
+    for (int x = 0; x < c; ++x) {
+        const int y = index_of(hp.sub_cuts[s], layout[x]);
+        bp.add_run(2 * (c - 1 - x), 2 * (c - 1 - y), 2);
+    }
+    if (!bp.build(a.row_of)) return fail(TQC_E_TOO_LARGE, "bit map needs too many segments");
+    const long long tiles = (((1ll << o) + 31) / 32) * (((1ll << (2 * c)) + 31) / 32);
+    tqc::relayout_kernel<<<(unsigned)tiles, 256, 0, st>>>(a);
+    TQC_CUDA(cudaGetLastError());
+    pl->launches++;
+    pl->loaded[s] = 1;
+    return 0;
+}
+
+int tqc_contract_states(tqc_plan_t *pl, const uint64_t *states_dev, size_t n_states, float *out_dev, void *workspace_dev,
+                        size_t workspace_bytes, void *stream) {
+    if (!pl) return fail(TQC_E_ARG, "null plan");
+    HostPlan &hp = pl->hp;
+    if (hp.mode != TQC_MODE_STATES) return fail(TQC_E_STATE, "plan was built for distribution mode");
+    for (int s = 0; s < hp.m; ++s) if (!pl->loaded[s]) return fail(TQC_E_STATE, "tensor of subcircuit " + std::to_string(s) + " not loaded");
+    if (n_states == 0) return 0;
+    if (!states_dev || !out_dev) return fail(TQC_E_ARG, "null states/out pointer");
+    if (n_states > (size_t)0x7fffffff) return fail(TQC_E_TOO_LARGE, "more than 2^31-1 states in one call");
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t fixed = states_fixed_bytes(hp), per = states_bytes_per_state(hp);
+    if ((fixed + per > 0) && !workspace_dev) return fail(TQC_E_WORKSPACE, "workspace is null");
+    if (((uintptr_t)workspace_dev & 255) != 0) return fail(TQC_E_ARG, "workspace must be 256-byte aligned");
+    long long cap;
+    if (per == 0) cap = (long long)((n_states + 63) / 64 * 64);
+    else {
+        if (workspace_bytes < fixed + 256) return fail(TQC_E_WORKSPACE, "workspace smaller than tqc_plan_workspace_min_bytes");
+        cap = (long long)((workspace_bytes - fixed - 256) / per) / 64 * 64;
+        cap = std::min<long long>(cap, (long long)((n_states + 63) / 64 * 64));
+        if (cap < 64) return fail(TQC_E_WORKSPACE, "workspace smaller than tqc_plan_workspace_min_bytes");
+    }
+    char *ws = (char *)workspace_dev;
+    float *tables = (float *)ws;
+    uint32_t *keys = (uint32_t *)(ws + fixed);
+    float *batch = (float *)(ws + fixed + align256((size_t)hp.n_key_slots * 4 * (size_t)cap));
+    // the alignment pad of the key region is covered by the +256 of tqc_plan_workspace_bytes
+    int rc;
+    // phase T: nodes evaluated once per key (tables), independent of the batch
+    CrossCtx cx;
+    cx.ws = tables;
+    for (int t = 0; t < hp.m - 1; ++t)
+        if (hp.nodes[hp.m + t].kind == tqc::NODE_TABLE && (rc = launch_cross_step(pl, cx, t, st))) return rc;
+    // phase B: chunks of states
+    const int words = (hp.n + 63) / 64;
+    const Node &root = hp.nodes[hp.root()];
+    for (size_t lo = 0; lo < n_states; lo += (size_t)cap) {
+        BatchCtx bx;
+        bx.tables = tables; bx.keys = keys; bx.batch = batch; bx.cap = cap;
+        bx.R = (int)std::min<size_t>((size_t)cap, n_states - lo);
+        bx.out = out_dev + lo;
+        if (hp.n_key_slots > 0) {
+            KeyArgs ka;
+            ka.states = states_dev + lo * (size_t)std::max(words, 0);
+            ka.keys = keys; ka.slot_ofs = pl->d_slot_ofs; ka.slot_qubits = pl->d_slot_qubits;
+            ka.words = words; ka.R = bx.R; ka.cap = cap;
+            dim3 grid((unsigned)((bx.R + 255) / 256), (unsigned)hp.n_key_slots);
+            tqc::key_kernel<<<grid, 256, 0, st>>>(ka);
+            TQC_CUDA(cudaGetLastError());
+            pl->launches++;
+        }
+        for (int t = 0; t < hp.m - 1; ++t)
+            if (hp.nodes[hp.m + t].kind == tqc::NODE_BATCH && (rc = launch_batch_step(pl, bx, t, st))) return rc;
+        if (root.kind != tqc::NODE_BATCH) {
+            GatherArgs g;
+            memset(&g, 0, sizeof(g));
+            g.table = hp.m == 1 ? pl->d_leaf[0] : tables + root.table_offset;
+            g.keys = keys + (long long)root.key_slot * cap;
+            g.out = bx.out; g.R = bx.R;
+            tqc::gather_kernel<<<(unsigned)((bx.R + 255) / 256), 256, 0, st>>>(g);
+            TQC_CUDA(cudaGetLastError());
+            pl->launches++;
+        }
+    }
+    return 0;
+}
+
+int tqc_contract_distribution(tqc_plan_t *pl, uint64_t prefix_value, int prefix_bits, float *out_dev, void *workspace_dev,
+                              size_t workspace_bytes, void *stream) {
+    if (!pl) return fail(TQC_E_ARG, "null plan");
+    HostPlan &hp = pl->hp;
+    if (hp.mode != TQC_MODE_DISTRIBUTION) return fail(TQC_E_STATE, "plan was built for states mode");
+    for (int s = 0; s < hp.m; ++s) if (!pl->loaded[s]) return fail(TQC_E_STATE, "tensor of subcircuit " + std::to_string(s) + " not loaded");
+    if (prefix_bits < 0 || prefix_bits > hp.n || prefix_bits > 64) return fail(TQC_E_ARG, "prefix_bits out of range");
+    if (prefix_bits < 64 && (prefix_value >> prefix_bits) != 0) return fail(TQC_E_ARG, "prefix_value has more than prefix_bits bits");
+    if (hp.n - prefix_bits > 34) return fail(TQC_E_TOO_LARGE, "more than 2^34 outputs; raise prefix_bits");
+    if (!out_dev) return fail(TQC_E_ARG, "null out pointer");
+    cudaStream_t st = (cudaStream_t)stream;
+    std::vector<int> fb;
+    std::vector<int64_t> off;
+    const int64_t floats = tqc::distribution_layout(hp, prefix_bits, fb, off);
+    if (floats > 0) {
+        if (!workspace_dev || workspace_bytes < (size_t)floats * 4) return fail(TQC_E_WORKSPACE, "workspace smaller than tqc_plan_workspace_bytes");
+        if (((uintptr_t)workspace_dev & 255) != 0) return fail(TQC_E_ARG, "workspace must be 256-byte aligned");
+    }
+    CrossCtx cx;
+    cx.prefix_bits = prefix_bits; cx.prefix_value = prefix_value;
+    cx.free_bits = &fb; cx.offsets = &off;
+    cx.ws = (float *)workspace_dev; cx.out = out_dev;
+    int rc;
+    for (int t = 0; t < hp.m - 1; ++t)
+        if ((rc = launch_cross_step(pl, cx, t, st))) return rc;
+    if (hp.m == 1) {
+        // K = 0: p(x) = T_0[x] (reading G15), permuted from the listed qubit order to global bit order
+        const Node &leaf = hp.nodes[0];
+        GatherArgs g;
+        memset(&g, 0, sizeof(g));
+        const std::vector<int> fq = free_qubits(leaf, prefix_bits);
+        const int nq = (int)leaf.qubits.size(), nf = (int)fq.size();
+        BitPairs in, om;
+        unsigned long long fixed = 0;
+        int t = 0;
+        for (int pq = 0; pq < nq; ++pq) {
+            const int q = leaf.qubits[pq];
+            if (q >= prefix_bits) {
+                int dst = 0;
+                for (int x : fq) if (x > q) ++dst;
+                in.add(nf - 1 - t, nq - 1 - pq);
+                om.add(nf - 1 - t, dst);
+                ++t;
+            } else if ((prefix_value >> (prefix_bits - 1 - q)) & 1ull) fixed |= 1ull << (nq - 1 - pq);
+        }
+        if (!in.build(g.map) || !om.build(g.out_map)) return fail(TQC_E_TOO_LARGE, "bit map needs too many segments");
+        g.map_or = fixed;
+        g.table = pl->d_leaf[0]; g.keys = nullptr; g.out = out_dev; g.R = 1ll << nf;
+        tqc::gather_kernel<<<(unsigned)((g.R + 255) / 256), 256, 0, st>>>(g);
+        TQC_CUDA(cudaGetLastError());
+        pl->launches++;
+    }
+    return 0;
+}
+
+uint64_t tqc_plan_launch_count(const tqc_plan_t *pl) { return pl ? pl->launches : 0; }
+
+}  // extern "C"
