@@ -1,0 +1,249 @@
+"""ctypes binding of libtqc.so (include/tqc.h).  Argument marshalling only.
+
+The four entry points carry the C names: tqc_plan, tqc_load_subcircuit_tensors,
+tqc_contract_states, tqc_contract_distribution.  Device buffers are torch tensors whose
+data_ptr() is passed through; the stream is torch's current CUDA stream.  There is no CPU
+fallback: if libtqc.so has not been built the import raises, and a compute call without a
+CUDA device raises TqcError(TQC_E_CUDA).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import POINTER, byref, c_char_p, c_double, c_int, c_int32, c_int64, c_size_t, c_uint64, c_void_p
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libtqc.so")
+
+MODE_STATES, MODE_DISTRIBUTION = 0, 1
+KERNEL_SIMT_TILE, KERNEL_DOT, KERNEL_TCGEN05 = 0, 1, 2
+NODE_LEAF, NODE_TABLE, NODE_BATCH = 0, 1, 2
+
+STATUS_NAMES = {0: "TQC_OK", -1: "TQC_E_ARG", -2: "TQC_E_SHAPE", -3: "TQC_E_STATE", -4: "TQC_E_INFEASIBLE",
+                -5: "TQC_E_WORKSPACE", -6: "TQC_E_TOO_LARGE", -7: "TQC_E_CUDA", -8: "TQC_E_PARSE"}
+
+# every symbol include/tqc.h declares (tests check that the library exports each one)
+EXPORTED = ["tqc_plan", "tqc_plan_destroy", "tqc_plan_mode", "tqc_plan_num_qubits", "tqc_plan_num_subcircuits",
+            "tqc_plan_num_cuts", "tqc_plan_num_steps", "tqc_plan_kmax", "tqc_plan_tensor_shape", "tqc_plan_step",
+            "tqc_plan_node", "tqc_plan_cost_log2", "tqc_plan_serialize", "tqc_plan_workspace_bytes",
+            "tqc_plan_workspace_min_bytes", "tqc_load_subcircuit_tensors", "tqc_contract_states",
+            "tqc_contract_distribution", "tqc_plan_launch_count", "tqc_last_error", "tqc_version"]
+
+
+class TqcError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"{STATUS_NAMES.get(code, code)}: {msg}")
+        self.code = code
+
+
+class _NetworkDesc(ctypes.Structure):
+    _fields_ = [("n_qubits", c_int32), ("m", c_int32), ("K", c_int32),
+                ("cut_up", POINTER(c_int32)), ("cut_down", POINTER(c_int32)),
+                ("sub_cut_ofs", POINTER(c_int32)), ("sub_cuts", POINTER(c_int32)),
+                ("sub_qubit_ofs", POINTER(c_int32)), ("sub_qubits", POINTER(c_int32))]
+
+
+class _PlanOpts(ctypes.Structure):
+    _fields_ = [("mode", c_int32), ("n_order_steps", c_int32), ("order", POINTER(c_int32)),
+                ("restarts", c_int32), ("seed", c_uint64), ("batch_hint", c_int64),
+                ("table_log2_floats_max", c_int32), ("use_tcgen05", c_int32)]
+
+
+def lib_path() -> str:
+    return _LIB_PATH
+
+
+def _load() -> ctypes.CDLL:
+    if not os.path.exists(_LIB_PATH):
+        raise ImportError(f"{_LIB_PATH} is missing: build it with `python -m paper_2502_03445_b200.build` "
+                          "(there is no CPU fallback)")
+    lib = ctypes.CDLL(_LIB_PATH)
+    lib.tqc_last_error.restype = c_char_p
+    lib.tqc_version.restype = c_char_p
+    lib.tqc_plan.argtypes = [POINTER(_NetworkDesc), POINTER(_PlanOpts), POINTER(c_void_p)]
+    lib.tqc_plan_destroy.argtypes = [c_void_p]
+    lib.tqc_plan_destroy.restype = None
+    for name in ("tqc_plan_mode", "tqc_plan_num_qubits", "tqc_plan_num_subcircuits", "tqc_plan_num_cuts",
+                 "tqc_plan_num_steps", "tqc_plan_kmax"):
+        getattr(lib, name).argtypes = [c_void_p]
+    lib.tqc_plan_tensor_shape.argtypes = [c_void_p, c_int, POINTER(c_int), POINTER(c_int)]
+    lib.tqc_plan_step.argtypes = [c_void_p, c_int] + [POINTER(c_int)] * 7
+    lib.tqc_plan_node.argtypes = [c_void_p, c_int] + [POINTER(c_int)] * 3
+    lib.tqc_plan_cost_log2.argtypes = [c_void_p]
+    lib.tqc_plan_cost_log2.restype = c_double
+    lib.tqc_plan_serialize.argtypes = [c_void_p, c_void_p, POINTER(c_size_t)]
+    lib.tqc_plan_workspace_bytes.argtypes = [c_void_p, c_size_t, c_int]
+    lib.tqc_plan_workspace_bytes.restype = c_size_t
+    lib.tqc_plan_workspace_min_bytes.argtypes = [c_void_p]
+    lib.tqc_plan_workspace_min_bytes.restype = c_size_t
+    lib.tqc_load_subcircuit_tensors.argtypes = [c_void_p, c_int, c_void_p, c_size_t, c_int, c_void_p]
+    lib.tqc_contract_states.argtypes = [c_void_p, c_void_p, c_size_t, c_void_p, c_void_p, c_size_t, c_void_p]
+    lib.tqc_contract_distribution.argtypes = [c_void_p, c_uint64, c_int, c_void_p, c_void_p, c_size_t, c_void_p]
+    lib.tqc_plan_launch_count.argtypes = [c_void_p]
+    lib.tqc_plan_launch_count.restype = c_uint64
+    return lib
+
+
+_lib = _load()
+
+
+def _check(rc: int) -> None:
+    if rc != 0:
+        raise TqcError(rc, _lib.tqc_last_error().decode())
+
+
+def version() -> str:
+    return _lib.tqc_version().decode()
+
+
+def _i32(values):
+    arr = np.ascontiguousarray(np.asarray(list(values), dtype=np.int32))
+    if arr.size == 0:
+        arr = np.zeros(1, dtype=np.int32)
+    return arr, arr.ctypes.data_as(POINTER(c_int32))
+
+
+def _stream_ptr(stream) -> int:
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream)
+
+
+class Plan:
+    """Owner of a tqc_plan_t handle (plan + the library's device copies of the tensors)."""
+
+    def __init__(self, handle: int):
+        self._h = c_void_p(handle)
+
+    def close(self) -> None:
+        if self._h:
+            _lib.tqc_plan_destroy(self._h)
+            self._h = c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- queries --------------------------------------------------------------------------
+    @property
+    def mode(self) -> int: return _lib.tqc_plan_mode(self._h)
+    @property
+    def n_qubits(self) -> int: return _lib.tqc_plan_num_qubits(self._h)
+    @property
+    def m(self) -> int: return _lib.tqc_plan_num_subcircuits(self._h)
+    @property
+    def K(self) -> int: return _lib.tqc_plan_num_cuts(self._h)
+    @property
+    def num_steps(self) -> int: return _lib.tqc_plan_num_steps(self._h)
+    @property
+    def kmax(self) -> int: return _lib.tqc_plan_kmax(self._h)
+    @property
+    def cost_log2(self) -> float: return _lib.tqc_plan_cost_log2(self._h)
+    @property
+    def launch_count(self) -> int: return int(_lib.tqc_plan_launch_count(self._h))
+
+    def tensor_shape(self, s: int):
+        c, o = c_int(), c_int()
+        _check(_lib.tqc_plan_tensor_shape(self._h, s, byref(c), byref(o)))
+        return c.value, o.value
+
+    def step(self, i: int) -> dict:
+        v = [c_int() for _ in range(7)]
+        _check(_lib.tqc_plan_step(self._h, i, *[byref(x) for x in v]))
+        names = ("lhs", "rhs", "n_inner", "n_outer_lhs", "n_outer_rhs", "log2cost", "kernel_class")
+        return {k: x.value for k, x in zip(names, v)}
+
+    def node(self, v: int) -> dict:
+        out = [c_int() for _ in range(3)]
+        _check(_lib.tqc_plan_node(self._h, v, *[byref(x) for x in out]))
+        return {k: x.value for k, x in zip(("kind", "n_bits", "n_open"), out)}
+
+    def steps(self):
+        return [self.step(i) for i in range(self.num_steps)]
+
+    def serialize(self) -> bytes:
+        n = c_size_t(0)
+        _check(_lib.tqc_plan_serialize(self._h, None, byref(n)))
+        buf = ctypes.create_string_buffer(n.value)
+        _check(_lib.tqc_plan_serialize(self._h, buf, byref(n)))
+        return buf.raw[:n.value]
+
+    def workspace_bytes(self, n_states: int = 0, prefix_bits: int = 0) -> int:
+        return int(_lib.tqc_plan_workspace_bytes(self._h, n_states, prefix_bits))
+
+    def workspace_min_bytes(self) -> int:
+        return int(_lib.tqc_plan_workspace_min_bytes(self._h))
+
+
+def tqc_plan(net, mode: int = MODE_STATES, order=None, restarts: int = 0, seed: int = 0, batch_hint: int = 0,
+             table_log2_floats_max: int = 0, use_tcgen05: int = 0) -> Plan:
+    """net: any object with n_qubits, cuts [(up, down)], sub_cuts [[cut ids]], sub_qubits [[qubit ids]]
+    (e.g. tqc_inputs.Network).  order: optional list of m-1 (lhs, rhs) node-id pairs."""
+    m = len(net.sub_cuts)
+    up, up_p = _i32(c[0] for c in net.cuts)
+    down, down_p = _i32(c[1] for c in net.cuts)
+    cofs, cofs_p = _i32(np.concatenate([[0], np.cumsum([len(x) for x in net.sub_cuts])]))
+    cflat, cflat_p = _i32(e for x in net.sub_cuts for e in x)
+    qofs, qofs_p = _i32(np.concatenate([[0], np.cumsum([len(x) for x in net.sub_qubits])]))
+    qflat, qflat_p = _i32(q for x in net.sub_qubits for q in x)
+    desc = _NetworkDesc(net.n_qubits, m, len(net.cuts), up_p, down_p, cofs_p, cflat_p, qofs_p, qflat_p)
+    oflat, oflat_p = _i32(v for ab in (order or []) for v in ab)
+    opts = _PlanOpts(mode, len(order) if order else 0, oflat_p, restarts, seed, batch_hint,
+                     table_log2_floats_max, use_tcgen05)
+    h = c_void_p()
+    _check(_lib.tqc_plan(byref(desc), byref(opts), byref(h)))
+    return Plan(h.value)
+
+
+def tqc_load_subcircuit_tensors(plan: Plan, s: int, data, stream=None) -> None:
+    """data: [4^{c_s}][2^{o_s}] fp32 — a numpy array / CPU torch tensor (HOST) or a CUDA torch tensor (DEVICE)."""
+    import torch
+    if isinstance(data, torch.Tensor):
+        t = data.contiguous()
+        if t.dtype != torch.float32:
+            raise TypeError("subcircuit tensors must be float32")
+        _check(_lib.tqc_load_subcircuit_tensors(plan._h, s, t.data_ptr(), t.numel(), 1 if t.is_cuda else 0,
+                                                _stream_ptr(stream)))
+        if not t.is_cuda:
+            torch.cuda.current_stream().synchronize()      # pageable host source: keep it alive until copied
+        return
+    a = np.ascontiguousarray(data)
+    if a.dtype != np.float32:
+        raise TypeError("subcircuit tensors must be float32")
+    _check(_lib.tqc_load_subcircuit_tensors(plan._h, s, a.ctypes.data, a.size, 0, _stream_ptr(stream)))
+    torch.cuda.current_stream().synchronize()
+
+
+def tqc_contract_states(plan: Plan, states, out=None, workspace=None, stream=None):
+    """states: CUDA int64/uint64 tensor [B, ceil(n/64)] (reading G5).  Returns out (CUDA fp32 [B])."""
+    import torch
+    if not states.is_cuda or states.element_size() != 8:
+        raise TypeError("states must be a CUDA tensor of 64-bit words")
+    states = states.contiguous()
+    B = states.shape[0]
+    if out is None:
+        out = torch.empty(B, dtype=torch.float32, device=states.device)
+    if workspace is None:
+        workspace = torch.empty(plan.workspace_bytes(B), dtype=torch.uint8, device=states.device)
+    _check(_lib.tqc_contract_states(plan._h, states.data_ptr(), B, out.data_ptr(), workspace.data_ptr(),
+                                    workspace.numel() * workspace.element_size(), _stream_ptr(stream)))
+    return out
+
+
+def tqc_contract_distribution(plan: Plan, prefix_value: int = 0, prefix_bits: int = 0, out=None, workspace=None,
+                              stream=None, device="cuda"):
+    """Returns out (CUDA fp32 [2^{n - prefix_bits}]), qubit 0 = MSB (reading G4)."""
+    import torch
+    n = plan.n_qubits
+    if out is None:
+        out = torch.empty(1 << max(0, n - prefix_bits), dtype=torch.float32, device=device)
+    if workspace is None:
+        workspace = torch.empty(max(256, plan.workspace_bytes(0, prefix_bits)), dtype=torch.uint8, device=device)
+    _check(_lib.tqc_contract_distribution(plan._h, prefix_value, prefix_bits, out.data_ptr(), workspace.data_ptr(),
+                                          workspace.numel() * workspace.element_size(), _stream_ptr(stream)))
+    return out
