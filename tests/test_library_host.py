@@ -1,0 +1,114 @@
+"""Host-side tests of libtqc.so — CPU only, no compute call.
+
+* the library loads and exports every symbol include/tqc.h declares;
+* the C++ planner's serialised plan is byte-identical to the oracle-side reference planner
+  (rules P1-P6) on the fixtures, on random networks and on configs 3-5 —
+  north_star: "bit-identical in the chosen contraction plan";
+* the paper's printed multiplication counts through the library (144 / 132 / 768-bound);
+* argument validation and error codes.
+"""
+import ctypes
+import re
+import os
+
+import numpy as np
+import pytest
+
+import paper_2502_03445_b200 as tqc
+from paper_2502_03445_b200 import binding
+from oracle import planner_ref as P
+from tqc_inputs import configs
+from tqc_inputs.network import Network
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _fig5_network():
+    return Network(4, [(0, 1), (1, 2), (1, 3), (2, 3)], [[0], [0, 1, 2], [1, 3], [2, 3]], [[0], [1], [2], [3]])
+
+
+def test_library_exports_every_declared_symbol():
+    header = open(os.path.join(ROOT, "include", "tqc.h")).read()
+    declared = set(re.findall(r"\b(tqc_[a-z0-9_]+)\s*\(", header))
+    declared -= {"tqc_status"}
+    assert declared == set(binding.EXPORTED), declared ^ set(binding.EXPORTED)
+    lib = ctypes.CDLL(tqc.lib_path())
+    for name in declared:
+        assert hasattr(lib, name), name
+    assert "sm_100a" in tqc.version()
+
+
+def test_fig5_costs_through_the_library():
+    net = _fig5_network()
+    p = tqc.tqc_plan(net, order=[(0, 1), (4, 2), (5, 3)])                  # the paper's order ((1,2),3),4
+    assert [2 ** s["log2cost"] for s in p.steps()] == [64, 64, 16] and p.kmax == 3
+    assert abs(2 ** p.cost_log2 - 144) < 1e-9
+    p = tqc.tqc_plan(net, order=[(2, 3), (4, 1), (5, 0)])                  # ((3,4),2),1
+    assert [2 ** s["log2cost"] for s in p.steps()] == [64, 64, 4]
+    g = tqc.tqc_plan(net)
+    assert 2 ** g.cost_log2 <= 144 + 1e-9 < 768                            # never worse than Fig. 5
+    assert 2 ** g.cost_log2 <= net.m * 4 ** g.kmax                         # Eq. 2
+
+
+@pytest.mark.parametrize("mode", [tqc.MODE_STATES, tqc.MODE_DISTRIBUTION])
+def test_plan_is_bit_identical_to_reference_planner(mode):
+    nets = [_fig5_network(), configs.cfg4_network()]
+    if mode == tqc.MODE_STATES:
+        nets.append(configs.cfg5_network())
+    for seed in range(40):
+        m = 2 + seed % 7
+        nets.append(configs.random_network(m, m + seed % 5, 1000 + seed, connected=(seed % 4 != 0)))
+    for net in nets:
+        got = tqc.tqc_plan(net, mode).serialize()
+        want = P.serialize(P.plan(net, mode))
+        assert got == want, net.name
+
+
+def test_plan_queries_and_shapes():
+    net = configs.cfg4_network()
+    p = tqc.tqc_plan(net)
+    assert (p.n_qubits, p.m, p.K, p.num_steps, p.mode) == (64, 8, 14, 7, tqc.MODE_STATES)
+    for s in range(net.m):
+        assert p.tensor_shape(s) == (net.c(s), net.o(s))
+    ref = P.plan(net)
+    for i, st in enumerate(p.steps()):
+        r = ref["steps"][i]
+        assert (st["lhs"], st["rhs"], st["n_inner"], st["log2cost"]) == (r["lhs"], r["rhs"], len(r["inner"]), r["log2cost"])
+    assert p.workspace_bytes(1 << 18) >= p.workspace_min_bytes() > 0
+    assert p.node(2 * net.m - 2)["n_open"] == 0
+    assert p.launch_count == 0
+
+
+def test_degenerate_networks_plan():
+    one = Network(3, [], [[]], [[2, 0, 1]])                                # K = 0, m = 1 (reading G15)
+    p = tqc.tqc_plan(one, tqc.MODE_DISTRIBUTION)
+    assert (p.m, p.K, p.num_steps, p.kmax) == (1, 0, 0, 0)
+    disc = Network(2, [], [[], []], [[0], [1]])                            # disconnected: outer product
+    p = tqc.tqc_plan(disc)
+    assert p.num_steps == 1 and p.step(0)["n_inner"] == 0
+    empty_out = Network(1, [(0, 1)], [[0], [0]], [[0], []])                # o_s = 0 allowed
+    assert tqc.tqc_plan(empty_out).tensor_shape(1) == (1, 0)
+
+
+def test_argument_errors():
+    bad = Network(2, [(0, 0)], [[0], [0]], [[0], [1]])                     # cut with both ends in one subcircuit
+    with pytest.raises(tqc.TqcError) as e:
+        tqc.tqc_plan(bad)
+    assert e.value.code == -1
+    missing_q = Network(3, [(0, 1)], [[0], [0]], [[0], [1]])               # qubit 2 unowned
+    with pytest.raises(tqc.TqcError):
+        tqc.tqc_plan(missing_q)
+    net = _fig5_network()
+    with pytest.raises(tqc.TqcError):
+        tqc.tqc_plan(net, order=[(0, 1), (0, 2), (5, 3)])                  # reuses a dead node
+    with pytest.raises(tqc.TqcError):
+        tqc.tqc_plan(net, mode=7)
+
+
+def test_restarts_never_worse_and_deterministic():
+    net = configs.cfg5_network()
+    base = tqc.tqc_plan(net)
+    a = tqc.tqc_plan(net, restarts=16, seed=7)
+    b = tqc.tqc_plan(net, restarts=16, seed=7)
+    assert a.serialize() == b.serialize()
+    assert a.cost_log2 <= base.cost_log2 + 1e-9
