@@ -72,37 +72,51 @@ def _einsum(operands, out_labels):
     args = []
     for (v, lab) in operands:
         args += [v, [remap.setdefault(l, len(remap)) for l in lab]]
-    return np.einsum(*args, [remap[l] for l in out_labels])
+    return np.einsum(*args, [remap[l] for l in out_labels], optimize=len(operands) == 2)
 
 
-def _elimination_order(net):
-    """Greedy min-size order over cut ids (unrelated to the library's pairwise plan)."""
-    groups = [set(es) for es in net.sub_cuts]
-    remaining = set(range(net.K))
-    order = []
-    while remaining:
-        best = None
-        for e in sorted(remaining):
+def _elimination_order(net, trials: int = 0, seed: int = 0):
+    """Order over cut ids for O8 (unrelated to the library's pairwise plan).  trials = 0: greedy
+    min-size (eliminate the cut whose bucket product has the fewest labels, ties by cut id).
+    trials > 0: the same greedy with seeded Gumbel noise on the score, repeated `trials` times;
+    the order with the smallest total cost sum_e 4^{|labels of bucket e|} is kept.  Every
+    elimination order yields the same value; only time and memory change."""
+    def one_pass(rng, noise):
+        groups = [set(es) for es in net.sub_cuts]
+        remaining = set(range(net.K))
+        order, cost = [], 0
+        while remaining:
+            best = None
+            for e in sorted(remaining):
+                touched = [g for g in groups if e in g]
+                size = len(set().union(*touched)) - 1
+                score = size + (noise * rng.gumbel() if noise > 0 else 0.0)
+                if best is None or score < best[0]:
+                    best = (score, e, size)
+            e = best[1]
+            cost += 4 ** (best[2] + 1)
             touched = [g for g in groups if e in g]
-            size = len(set().union(*touched)) - 1
-            if best is None or size < best[0]:
-                best = (size, e)
-        e = best[1]
-        touched = [g for g in groups if e in g]
-        merged = set().union(*touched) - {e}
-        groups = [g for g in groups if e not in g] + [merged]
-        remaining.discard(e)
-        order.append(e)
-    return order
+            merged = set().union(*touched) - {e}
+            groups = [g for g in groups if e not in g] + [merged]
+            remaining.discard(e)
+            order.append(e)
+        return cost, order
+    best_cost, best_order = one_pass(None, 0.0)
+    rng = np.random.default_rng(seed)
+    for t in range(trials):
+        cost, order = one_pass(rng, 0.3 + 0.1 * (t % 8))
+        if cost < best_cost:
+            best_cost, best_order = cost, order
+    return best_order
 
 
-def bucket_elimination(net, tensors, bits: np.ndarray, order=None, chunk: int = 64) -> np.ndarray:
+def bucket_elimination(net, tensors, bits: np.ndarray, order=None, chunk: int = 64, order_trials: int = 0) -> np.ndarray:
     """O8: sum out one cut index at a time (variable elimination).  For cut e, multiply
     all current factors that carry e and sum over e; factors are float64 arrays with a
     leading batch axis.  Any elimination order gives the same value."""
     K, m = net.K, net.m
     if order is None:
-        order = _elimination_order(net)
+        order = _elimination_order(net, trials=order_trials)
     keys = keys_from_bits(net, bits)
     T = [np.asarray(t, dtype=np.float64) for t in tensors]
     out = np.zeros(bits.shape[0], dtype=np.float64)

@@ -1,0 +1,123 @@
+"""GPU parity on the five BASELINE.json configs (which oracle tier checks which).
+
+cfg1, cfg2: full distribution vs the UNCUT float64 statevector (O7) — the paper's correctness claim.
+cfg3: all 2^16 states vs the direct sum (O6, C odometer).
+cfg4: 2^18-state batch in the bench launch configuration; a 1k-state subset vs O6 (sample sized by time).
+cfg5: rank-one closed form (Pi-1) at full network size; a small subset vs bucket elimination (O8).
+"""
+import numpy as np
+import pytest
+import torch
+
+import paper_2502_03445_b200 as tqc
+from oracle import cutting, reconstruct as R, statevector as sv
+from oracle.direct_sum_c import direct_sum_c
+from tqc_inputs import configs, pack_states, random_states, random_tensors, rank_one_tensors, seed_for
+from tqc_inputs.seeds import STREAM_STATES, STREAM_SUBSET, STREAM_TENSORS
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-5
+
+
+def _loaded_plan(net, tensors, mode, **kw):
+    plan = tqc.tqc_plan(net, mode, **kw)
+    for s, t in enumerate(tensors):
+        tqc.tqc_load_subcircuit_tensors(plan, s, np.ascontiguousarray(t, dtype=np.float32))
+    return plan
+
+
+def _states_dev(bits):
+    return torch.from_numpy(pack_states(bits).view(np.int64)).cuda()
+
+
+def _run_states(plan, bits, max_ws=None):
+    st = _states_dev(bits)
+    need = plan.workspace_bytes(bits.shape[0])
+    if max_ws is not None:
+        need = max(plan.workspace_min_bytes(), min(need, max_ws))
+    ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+    out = tqc.tqc_contract_states(plan, st, workspace=ws)
+    torch.cuda.synchronize()
+    return out.cpu().numpy().astype(np.float64)
+
+
+def test_cfg1_distribution_vs_uncut_statevector():
+    circ = configs.cfg1_circuit()
+    net, T64, _ = cutting.tensors_from_circuit(circ)
+    T = [t.astype(np.float32) for t in T64]
+    plan = _loaded_plan(net, T, tqc.MODE_DISTRIBUTION)
+    got = tqc.tqc_contract_distribution(plan).cpu().numpy().astype(np.float64)
+    want = sv.uncut_probabilities(8, circ.gates)
+    assert got.shape == (256,)
+    assert np.abs(got - want).max() <= TOL * want.max()
+    assert abs(got.sum() - 1.0) < 1e-5
+    # and against the direct sum on the SAME fp32 tensors
+    assert np.abs(got - R.direct_sum(net, T, R.full_distribution_bits(8))).max() <= TOL * want.max()
+
+
+def test_cfg2_distribution_vs_uncut_statevector():
+    circ = configs.cfg2_circuit()
+    net, T64, _ = cutting.tensors_from_circuit(circ)
+    T = [t.astype(np.float32) for t in T64]
+    plan = _loaded_plan(net, T, tqc.MODE_DISTRIBUTION)
+    got = tqc.tqc_contract_distribution(plan).cpu().numpy().astype(np.float64)
+    want = sv.uncut_probabilities(20, circ.gates)
+    assert got.shape == (1 << 20,)
+    assert np.abs(got - want).max() <= TOL * want.max(), (np.abs(got - want).max(), want.max())
+    assert abs(got.sum() - 1.0) < 1e-4
+    # output-bit slicing: prefix chunks tile the same vector
+    for pv in (0, 5):
+        chunk = tqc.tqc_contract_distribution(plan, pv, 3).cpu().numpy().astype(np.float64)
+        lo = pv << 17
+        assert np.abs(chunk - want[lo:lo + (1 << 17)]).max() <= TOL * want.max()
+
+
+def test_cfg3_all_states_vs_direct_sum():
+    circ = configs.cfg3_circuit()
+    net, T64, _ = cutting.tensors_from_circuit(circ)
+    T = [t.astype(np.float32) for t in T64]
+    bits = random_states(30, configs.BATCH[3], seed_for(3, STREAM_STATES))
+    plan = _loaded_plan(net, T, tqc.MODE_STATES, batch_hint=configs.BATCH[3])
+    got = _run_states(plan, bits)
+    want, _ = direct_sum_c(net, T, bits)
+    assert np.abs(got - want).max() <= TOL * want.max(), (np.abs(got - want).max(), want.max())
+    assert (got >= -TOL * want.max()).all()
+
+
+def test_cfg4_full_batch_subset_vs_direct_sum():
+    net = configs.cfg4_network()
+    T = random_tensors(net, seed_for(4, STREAM_TENSORS))
+    B = configs.BATCH[4]
+    bits = random_states(64, B, seed_for(4, STREAM_STATES))
+    plan = _loaded_plan(net, T, tqc.MODE_STATES, batch_hint=B)
+    got = _run_states(plan, bits)                              # the launch configuration bench.py times
+    assert np.isfinite(got).all() and (got > 0).all()
+    idx = np.random.default_rng(seed_for(4, STREAM_SUBSET)).choice(B, size=1000, replace=False)
+    n_check = 64                                               # 4^14 * 1.33 multiplies each: sized to seconds
+    want, _ = direct_sum_c(net, T, bits[idx[:n_check]])
+    assert np.abs(got[idx[:n_check]] - want).max() <= TOL * want.max()
+    # the rest of the subset through the independent bucket-elimination tier (O8)
+    want8 = R.bucket_elimination(net, T, bits[idx])
+    assert np.abs(got[idx] - want8).max() <= TOL * want8.max()
+    # rank-one closed form on the whole batch (Pi-1): every state checked
+    T1, g, a = rank_one_tensors(net, 44)
+    plan1 = _loaded_plan(net, T1, tqc.MODE_STATES, batch_hint=B)
+    got1 = _run_states(plan1, bits)
+    want1 = R.rank_one_closed_form(net, g, a, bits)
+    assert np.abs(got1 - want1).max() <= TOL * want1.max()
+
+
+def test_cfg5_rank_one_and_bucket_elimination_subset():
+    net = configs.cfg5_network()
+    n_rank1, n_be = 256, 2
+    bits = random_states(196, configs.BATCH[5], seed_for(5, STREAM_STATES))[:n_rank1]
+    T1, g, a = rank_one_tensors(net, 55)
+    plan1 = _loaded_plan(net, T1, tqc.MODE_STATES, batch_hint=configs.BATCH[5])
+    got1 = _run_states(plan1, bits, max_ws=8 << 30)
+    want1 = R.rank_one_closed_form(net, g, a, bits)
+    assert np.abs(got1 - want1).max() <= TOL * want1.max(), (np.abs(got1 - want1).max(), want1.max())
+    T = random_tensors(net, seed_for(5, STREAM_TENSORS))
+    plan = _loaded_plan(net, T, tqc.MODE_STATES, batch_hint=configs.BATCH[5])
+    got = _run_states(plan, bits[:n_be], max_ws=8 << 30)
+    want = R.bucket_elimination(net, T, bits[:n_be], chunk=1, order_trials=64)
+    assert np.abs(got - want).max() <= TOL * want.max(), (got, want)
