@@ -1,0 +1,446 @@
+"""bench.py — states/s of the reconstruction hot path on B200 (one JSON line on rank 0).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4|cfg5|cfg3|cfg2] [--impl reference]
+
+A step is ONE pass of the whole hot path (a2 key extraction, a3 gather, a4 pairwise
+contractions, a5 final reduction — or a6 for a distribution workload) over one batch of
+seeded synthetic input, through the C ABI (include/tqc.h).  `value` = states / s with the batch
+resident in HBM; `e2e` = the same through tqc_contract_*_host with pinned HOST buffers (H2D of
+the states and D2H of the probabilities inside the timed region).  Multi-GPU (torchrun): the
+path shards over independent states; every rank holds the tensors and
+contracts its own seeded batch, no collective on the data path ("scaling": "weak").
+
+`--impl reference` times the CPU oracle (oracle/, float64 direct sum / bucket elimination) on a
+bounded sample of the same workload; the `cpu_baseline` leg of the default arm does the same
+once.  These two legs are the only places this file touches oracle/.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "reconstructed output-state probabilities/sec"
+UNIT = "states/s"
+SM_COUNT = 148                  # B200 (B200_PROFILING.md)
+FP32_LANES_PER_SM = 128
+NOMINAL_TF32_OVER_BF16 = 1.1 / 2.25   # nominal dense peaks (B200_PROFILING.md table)
+
+
+def measured_peaks() -> dict:
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        p["source"] = "measured"
+        return p
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "sm_max_mhz": 1965.0,
+            "source": "fallback"}
+
+
+# ---------------------------------------------------------------------------------------------
+# workloads: the BASELINE.json configs as seeded synthetic inputs (tqc_inputs/, DESIGN.md recipe)
+# ---------------------------------------------------------------------------------------------
+def make_workload(name: str, batch: int | None = None):
+    from tqc_inputs import configs, random_tensors, seed_for
+    from tqc_inputs.network import Network
+    from tqc_inputs.seeds import STREAM_TENSORS
+    if name == "cfg4":
+        net, cfg = configs.cfg4_network(), 4
+    elif name == "cfg5":
+        net, cfg = configs.cfg5_network(), 5
+    elif name == "cfg3":
+        # network shape of cfg3 (30-qubit ansatz, K = 6, tensors (3,10) (6,9) (3,11)); for timing the tensor VALUES
+        # are seeded random (the statevector-simulated ones are oracle output and are used by the parity tests)
+        net = Network(30, [(0, 1), (1, 0), (0, 1), (1, 2), (2, 1), (1, 2)], [[0, 1, 2], [0, 1, 2, 3, 4, 5], [3, 4, 5]],
+                      [list(range(0, 10)), list(range(10, 19)), list(range(19, 30))], name="cfg3-shape")
+        net.validate()
+        cfg = 3
+    elif name == "cfg2":
+        # the cut network the seeded cfg2 circuit yields (20 qubits, 3 subcircuits, K = 5; tests/test_gpu_configs.py
+        # derives it from the circuit), distribution mode, random values for timing
+        net = Network(20, [(0, 1), (1, 2), (0, 2), (0, 2), (1, 2)], [[0, 2, 3], [0, 1, 4], [1, 2, 3, 4]],
+                      [[0, 7, 10], [1, 2, 3, 11, 13, 17, 18, 19], [4, 5, 6, 8, 9, 12, 14, 15, 16]], name="cfg2-shape")
+        net.validate()
+        cfg = 2
+    else:
+        raise SystemExit(f"unknown workload {name}")
+    B = batch if batch else configs.BATCH[cfg]
+    tensors = random_tensors(net, seed_for(cfg, STREAM_TENSORS))
+    return {"name": name, "cfg": cfg, "net": net, "tensors": tensors, "mode": configs.MODE[cfg], "B": int(B),
+            "full_B": configs.BATCH[cfg]}
+
+
+def workload_states(wl, rank: int) -> np.ndarray:
+    """(B, n) bits, uniform over {0,1}^n, seeded per rank (rank 0 = the config's own seed)."""
+    from tqc_inputs import random_states, seed_for
+    from tqc_inputs.seeds import STREAM_STATES
+    full = random_states(wl["net"].n_qubits, wl["B"], seed_for(wl["cfg"], STREAM_STATES, bump=rank))
+    return full
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 100 ms while the timed regions run."""
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.tmp = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(index)], stdout=self.tmp, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.proc = None
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        self.tmp.flush()
+        self.tmp.seek(0)
+        sm, smax, power, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for line in self.tmp.read().splitlines():
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); smax.append(float(parts[1])); power.append(float(parts[2]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, parts[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        self.tmp.close()
+        os.unlink(self.tmp.name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        # samples under load: the upper half of the clock readings (idle samples sit at the floor clock)
+        load = sorted(sm)[len(sm) // 2:]
+        return {"sm_mhz": float(np.median(load)), "sm_max_mhz": float(max(smax)), "samples": len(sm),
+                "power_w_max": float(max(power)), "reasons": sorted(reasons)}
+
+
+# ---------------------------------------------------------------------------------------------
+# algorithmic work of one plan step
+# ---------------------------------------------------------------------------------------------
+def step_work(plan, t: int, B: int, mode_states: bool):
+    """(flop, bytes) one launch of plan step t must do.  flop = 2 x the paper's multiplication count
+    4^{#inner+#outer} x rows; bytes = compulsory operand reads + result write, fp32."""
+    NODE_BATCH = 2
+    st = plan.step(t)
+    m = plan.m
+    c_node = plan.node(m + t)
+    if mode_states:
+        rows = B if c_node["kind"] == NODE_BATCH else (1 << c_node["n_bits"])
+        flop = 2.0 * (2.0 ** st["log2cost"]) * rows
+    else:
+        rows = 1 << c_node["n_bits"]
+        flop = 2.0 * (2.0 ** st["log2cost"])
+    nbytes = 4.0 * rows * (4.0 ** c_node["n_open"])
+    for v in (st["lhs"], st["rhs"]):
+        nd = plan.node(v)
+        distinct = min(rows, 1 << nd["n_bits"]) if nd["kind"] != NODE_BATCH else rows
+        nbytes += 4.0 * distinct * (4.0 ** nd["n_open"])
+    return flop, nbytes
+
+
+def roofline_for(plan, tag: int, avg_ms: float, B: int, mode_states: bool, peaks: dict, traffic):
+    """Roofline object for the dominant launch (tag = plan step index)."""
+    if tag < 0 or avg_ms <= 0:
+        return {"bound": "hbm", "achieved": None, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": None,
+                "traffic": traffic, "kernel": {-1: "key_kernel", -2: "gather_kernel"}.get(tag, "?")}
+    flop, nbytes = step_work(plan, tag, B, mode_states)
+    kclass = plan.step(tag)["kernel_class"]
+    alu_peak = SM_COUNT * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12        # TFLOP/s fp32 FFMA
+    tf32_peak = peaks["bf16_tflops"] * NOMINAL_TF32_OVER_BF16
+    t_hbm = nbytes / (peaks["hbm_gbs"] * 1e9)
+    sec = avg_ms * 1e-3
+    name = {0: "step_tile_kernel (fp32 FFMA)", 1: "dot_kernel", 2: "step_tc_kernel (3xTF32 tcgen05)"}.get(kclass, "?")
+    if kclass == 2:
+        t_cmp, peak, unit, bound = 3.0 * flop / (tf32_peak * 1e12), tf32_peak, "TFLOP/s", "tensor"
+        achieved = 3.0 * flop / sec / 1e12            # issued tensor flops: 3 TF32 MMAs per fp32-accurate product
+    else:
+        t_cmp, peak, unit, bound = flop / (alu_peak * 1e12), alu_peak, "TFLOP/s", "alu"
+        achieved = flop / sec / 1e12
+    if t_hbm > t_cmp:
+        bound, peak, unit, achieved = "hbm", peaks["hbm_gbs"], "GB/s", nbytes / sec / 1e9
+    return {"bound": bound, "achieved": achieved, "peak": peak, "unit": unit, "frac": achieved / peak,
+            "traffic": traffic, "kernel": name, "plan_step": tag, "algorithmic_flop": flop, "algorithmic_bytes": nbytes,
+            "avg_launch_ms": avg_ms, "peak_source": peaks["source"] +
+            (" hbm copy" if bound == "hbm" else " sm_max_mhz x 148 SMs x 128 lanes x 2" if bound == "alu"
+             else " bf16 x nominal tf32/bf16 ratio")}
+
+
+def committed_traffic(workload: str, tag: int):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture
+    (profiles/traffic.json, written by hand from the capture named there), else None."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    if not os.path.exists(path):
+        return None
+    with open(path) as f:
+        table = json.load(f)
+    return table.get(workload, {}).get(str(tag))
+
+
+# ---------------------------------------------------------------------------------------------
+# the GPU arm
+# ---------------------------------------------------------------------------------------------
+def run_ours(args) -> None:
+    import torch
+    import torch.distributed as dist
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the library has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    import paper_2502_03445_b200 as tqc      # fails loudly if libtqc.so is missing
+
+    peaks = measured_peaks()
+    wl = make_workload(args.workload, args.batch)
+    net, B = wl["net"], wl["B"]
+    states_mode = wl["mode"] == "states"
+    plan = tqc.tqc_plan(net, tqc.MODE_STATES if states_mode else tqc.MODE_DISTRIBUTION, batch_hint=B,
+                        restarts=args.restarts, seed=args.plan_seed)
+    for s, t in enumerate(wl["tensors"]):
+        tqc.tqc_load_subcircuit_tensors(plan, s, t)
+    n_out = B if states_mode else (1 << net.n_qubits)
+
+    from tqc_inputs import pack_states
+    if states_mode:
+        packed = pack_states(workload_states(wl, rank)).view(np.int64)
+        states_host = torch.from_numpy(packed).pin_memory()
+        states_dev = states_host.to(dev)
+        ws_bytes = min(plan.workspace_bytes_host(B), max(args.max_workspace_gb << 30,
+                                                          plan.workspace_min_bytes() + (B * (packed.shape[1] * 8 + 4)) + 4096))
+    else:
+        states_host = states_dev = None
+        ws_bytes = plan.workspace_bytes_host(0, 0)
+    workspace = torch.empty(max(ws_bytes, 256), dtype=torch.uint8, device=dev)
+    out_dev = torch.empty(n_out, dtype=torch.float32, device=dev)
+    out_host = torch.empty(n_out, dtype=torch.float32).pin_memory()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def step_device():
+        if states_mode:
+            tqc.tqc_contract_states(plan, states_dev, out=out_dev, workspace=workspace, stream=stream)
+        else:
+            tqc.tqc_contract_distribution(plan, out=out_dev, workspace=workspace, stream=stream)
+
+    def step_host():
+        if states_mode:
+            tqc.tqc_contract_states_host(plan, states_host, out_host, workspace, stream=stream)
+        else:
+            tqc.tqc_contract_distribution_host(plan, out_host, workspace, stream=stream)
+
+    def timed(fn, steps, warmup):
+        for _ in range(warmup):
+            flush.zero_()
+            fn()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        l0 = plan.launch_count
+        for a, b in evs:
+            flush.zero_()                      # L2 flush between timed iterations (outside the event pair)
+            a.record(stream)
+            fn()
+            b.record(stream)
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        ms = sum(a.elapsed_time(b) for a, b in evs)
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item()), plan.launch_count - l0
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    total_ms, launches = timed(step_device, args.steps, args.warmup)
+    e2e_ms, _ = timed(step_host, args.steps, args.warmup)
+
+    # per-launch times of the same step, CUDA events on the launching stream inside the library
+    plan.profile_enable(True)
+    per_tag: dict = {}
+    for _ in range(args.steps):
+        flush.zero_()
+        step_device()
+        for tag, ms in plan.profile_read():
+            acc = per_tag.setdefault(tag, [0.0, 0])
+            acc[0] += ms
+            acc[1] += 1
+    plan.profile_enable(False)
+    torch.cuda.synchronize()
+    clocks = sampler.stop() if sampler else None
+
+    ms_per_step = total_ms / args.steps
+    value = world * n_out / (ms_per_step * 1e-3)
+    e2e_value = world * n_out / (e2e_ms / args.steps * 1e-3)
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    dom = max(per_tag.items(), key=lambda kv: kv[1][0])
+    dom_tag, (dom_total, dom_n) = dom
+    launches_per_step = dom_n / args.steps
+    rows_B = B / launches_per_step if states_mode else B          # a chunked batch runs the step once per chunk
+    roof = roofline_for(plan, dom_tag, dom_total / dom_n, int(rows_B), states_mode, peaks,
+                        committed_traffic(wl["name"], dom_tag))
+    step_ms_sum = sum(v[0] for v in per_tag.values()) / args.steps
+    roof["share_of_step"] = (dom_total / args.steps) / step_ms_sum if step_ms_sum > 0 else None
+    kernels = {str(tag): {"ms_per_step": v[0] / args.steps, "launches_per_step": v[1] / args.steps}
+               for tag, v in sorted(per_tag.items())}
+
+    words = (net.n_qubits + 63) // 64
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": workload_description(wl, plan), "states_per_step_per_gpu": n_out,
+                   "parallelism": f"states sharded over {world} GPU(s), tensors replicated, no collective",
+                   "l2": "flushed between timed iterations (256 MB write)", "plan_cost_log2_per_state": plan.cost_log2,
+                   "kmax": plan.kmax, "workspace_gb": ws_bytes / 2 ** 30},
+        "e2e": {"value": e2e_value, "unit": UNIT,
+                "h2d_bytes_per_step": int(B * words * 8) if states_mode else 0, "d2h_bytes_per_step": int(n_out * 4)},
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+        "roofline": roof,
+        "kernels_ms": kernels,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(wl, args.cpu_seconds)
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def workload_description(wl, plan) -> str:
+    net = wl["net"]
+    what = {2: "cfg2: 20-qubit QAOA cut network (3 subcircuits, K=5), full 2^20 distribution",
+            3: "cfg3: 30-qubit ansatz cut network (3 subcircuits, K=6)",
+            4: "cfg4: 64-qubit 8x8-grid cut network (8 subcircuits of 8 output qubits, K=14)",
+            5: "cfg5: 196-qubit 14x14-grid cut network (52 subcircuits, c_s in 5..8)"}[wl["cfg"]]
+    s = f"{what}; n={net.n_qubits} m={net.m} K={net.K}; seeded U[0,1) fp32 tensors"
+    if wl["mode"] == "states":
+        s += f"; batch of {wl['B']} uniform bitstrings"
+        if wl["B"] != wl["full_B"]:
+            s += f" (prefix of {wl['B']} of {wl['full_B']} states, SURVEY 8d-5)"
+    return s
+
+
+# ---------------------------------------------------------------------------------------------
+# the CPU oracle legs (the only code here that touches oracle/)
+# ---------------------------------------------------------------------------------------------
+def oracle_sample_rate(wl, seconds: float, rank: int = 0):
+    """Times the oracle AS IT STANDS on a bounded sample of the workload's states: the float64 direct sum over all
+    4^K cut assignments (oracle/direct_sum.c, OpenMP over states) while 4^K is feasible, else the float64 bucket
+    elimination (oracle/reconstruct.py, numpy).  Returns (states/s, cores, sample description)."""
+    from oracle import reconstruct as R
+    from oracle.direct_sum_c import direct_sum_c
+    net = wl["net"]
+    cores = os.cpu_count() or 1
+    if wl["mode"] == "states":
+        bits_all = workload_states(wl, rank)
+    else:
+        idx = np.random.default_rng(1).choice(1 << net.n_qubits, size=min(1 << net.n_qubits, 1 << 16), replace=False)
+        bits_all = ((idx[:, None] >> (net.n_qubits - 1 - np.arange(net.n_qubits))[None, :]) & 1).astype(np.uint8)
+    T = wl["tensors"]
+    if net.K <= 16:
+        probe = min(len(bits_all), max(cores, 8))
+        t0 = time.perf_counter()
+        _, used = direct_sum_c(net, T, bits_all[:probe])
+        dt = max(time.perf_counter() - t0, 1e-6)
+        n = int(min(len(bits_all), max(probe, probe * seconds / dt)))
+        t0 = time.perf_counter()
+        _, used = direct_sum_c(net, T, bits_all[:n])
+        dt = time.perf_counter() - t0
+        return n / dt, used, f"direct sum over 4^{net.K} cut assignments (C, OpenMP), first {n} states of the batch, {dt:.1f} s"
+    order = R._elimination_order(net, trials=16)
+    n, t0 = 0, time.perf_counter()
+    while n < len(bits_all) and (n == 0 or time.perf_counter() - t0 < seconds):
+        R.bucket_elimination(net, T, bits_all[n:n + 1], order=order, chunk=1)
+        n += 1
+    dt = time.perf_counter() - t0
+    return n / dt, cores, (f"bucket elimination (numpy float64, 4^K infeasible at K={net.K}), first {n} state(s) of the "
+                           f"batch, {dt:.1f} s; cores = host threads available to numpy")
+
+
+def cpu_baseline(wl, seconds: float) -> dict:
+    rate, cores, sample = oracle_sample_rate(wl, seconds)
+    return {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+
+
+def run_reference(args) -> None:
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    wl = make_workload(args.workload, args.batch)
+    per_step = max(2.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    rates, info = [], None
+    for i in range(args.warmup + args.steps):
+        rate, cores, sample = oracle_sample_rate(wl, per_step)
+        if i >= args.warmup:
+            rates.append(rate)
+        info = (cores, sample)
+    value = float(np.mean(rates))
+    n_out = wl["B"] if wl["mode"] == "states" else (1 << wl["net"].n_qubits)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT,
+            "n_gpus": int(os.environ.get("WORLD_SIZE", "1")), "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * n_out / value, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_description(wl, None), "states_per_step_per_gpu": n_out,
+                       "note": "CPU oracle on rank 0 only; ms_per_step extrapolated from the sampled rate"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": info[0], "kind": "oracle", "sample": info[1]},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main() -> None:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg4", choices=["cfg2", "cfg3", "cfg4", "cfg5"])
+    ap.add_argument("--batch", type=int, default=0, help="states per step per GPU (0: the config's own batch)")
+    ap.add_argument("--restarts", type=int, default=0, help="planner restarts (0: deterministic greedy)")
+    ap.add_argument("--plan-seed", type=int, default=0)
+    ap.add_argument("--max-workspace-gb", type=int, default=64)
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

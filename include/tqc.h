@@ -138,8 +138,31 @@ int tqc_contract_states(tqc_plan_t *plan, const uint64_t *states_dev, size_t n_s
 int tqc_contract_distribution(tqc_plan_t *plan, uint64_t prefix_value, int prefix_bits,
                               float *out_dev, void *workspace_dev, size_t workspace_bytes, void *stream);
 
-/* number of kernels the library has launched so far on behalf of this plan (for bench.py) */
+/* ---- the same two calls with HOST buffers (end-to-end form; "reconstruct
+ * 1 million arbitrary quantum states" handed over by the host program) -----------------------
+ * states_host / out_host: HOST (pinned memory makes the copies asynchronous).  The library
+ * stages them inside the caller's DEVICE workspace, which must hold
+ * tqc_plan_workspace_bytes_host(plan, n_states, prefix_bits) bytes for a single chunk (states
+ * mode accepts less, down to staging + tqc_plan_workspace_min_bytes).  Order on `stream`:
+ * H2D copy of the states, the contraction kernels, D2H copy of the result; the caller
+ * synchronises `stream` before reading out_host. */
+size_t tqc_plan_workspace_bytes_host(const tqc_plan_t *plan, size_t n_states, int prefix_bits);
+int tqc_contract_states_host(tqc_plan_t *plan, const uint64_t *states_host, size_t n_states,
+                             float *out_host, void *workspace_dev, size_t workspace_bytes, void *stream);
+int tqc_contract_distribution_host(tqc_plan_t *plan, uint64_t prefix_value, int prefix_bits,
+                                   float *out_host, void *workspace_dev, size_t workspace_bytes,
+                                   void *stream);
+
+/* ---- measurement hooks (bench.py) --------------------------------------------------------------
+ * tqc_plan_launch_count: kernels launched so far on behalf of this plan.
+ * tqc_plan_profile_enable(plan, 1): every later contract call records one CUDA event on the
+ * caller's stream before each of its kernel launches and one at its end.
+ * tqc_plan_profile_read: waits for the last profiled call and returns, per launch in launch
+ * order, its tag (plan step index t >= 0; -1 key extraction; -2 root gather) and the time to the
+ * next event in ms.  Call with tags = NULL to get the count in *n.  HOST arrays. */
 uint64_t tqc_plan_launch_count(const tqc_plan_t *plan);
+int tqc_plan_profile_enable(tqc_plan_t *plan, int on);
+int tqc_plan_profile_read(tqc_plan_t *plan, int32_t *tags, float *ms, size_t *n);
 
 const char *tqc_last_error(void);
 const char *tqc_version(void);

@@ -83,6 +83,12 @@ def _load() -> ctypes.CDLL:
     lib.tqc_contract_distribution.argtypes = [c_void_p, c_uint64, c_int, c_void_p, c_void_p, c_size_t, c_void_p]
     lib.tqc_plan_launch_count.argtypes = [c_void_p]
     lib.tqc_plan_launch_count.restype = c_uint64
+    lib.tqc_plan_workspace_bytes_host.argtypes = [c_void_p, c_size_t, c_int]
+    lib.tqc_plan_workspace_bytes_host.restype = c_size_t
+    lib.tqc_contract_states_host.argtypes = [c_void_p, c_void_p, c_size_t, c_void_p, c_void_p, c_size_t, c_void_p]
+    lib.tqc_contract_distribution_host.argtypes = [c_void_p, c_uint64, c_int, c_void_p, c_void_p, c_size_t, c_void_p]
+    lib.tqc_plan_profile_enable.argtypes = [c_void_p, c_int]
+    lib.tqc_plan_profile_read.argtypes = [c_void_p, c_void_p, c_void_p, POINTER(c_size_t)]
     return lib
 
 
@@ -179,6 +185,21 @@ class Plan:
     def workspace_min_bytes(self) -> int:
         return int(_lib.tqc_plan_workspace_min_bytes(self._h))
 
+    def workspace_bytes_host(self, n_states: int = 0, prefix_bits: int = 0) -> int:
+        return int(_lib.tqc_plan_workspace_bytes_host(self._h, n_states, prefix_bits))
+
+    def profile_enable(self, on: bool = True) -> None:
+        _check(_lib.tqc_plan_profile_enable(self._h, 1 if on else 0))
+
+    def profile_read(self):
+        """[(tag, ms)] per launch of the last profiled contract call (waits for it)."""
+        n = c_size_t(0)
+        _check(_lib.tqc_plan_profile_read(self._h, None, None, byref(n)))
+        tags = np.zeros(max(1, n.value), dtype=np.int32)
+        ms = np.zeros(max(1, n.value), dtype=np.float32)
+        _check(_lib.tqc_plan_profile_read(self._h, tags.ctypes.data, ms.ctypes.data, byref(n)))
+        return [(int(tags[i]), float(ms[i])) for i in range(n.value)]
+
 
 def tqc_plan(net, mode: int = MODE_STATES, order=None, restarts: int = 0, seed: int = 0, batch_hint: int = 0,
              table_log2_floats_max: int = 0, use_tcgen05: int = 0) -> Plan:
@@ -247,3 +268,25 @@ def tqc_contract_distribution(plan: Plan, prefix_value: int = 0, prefix_bits: in
     _check(_lib.tqc_contract_distribution(plan._h, prefix_value, prefix_bits, out.data_ptr(), workspace.data_ptr(),
                                           workspace.numel() * workspace.element_size(), _stream_ptr(stream)))
     return out
+
+
+def tqc_contract_states_host(plan: Plan, states_host, out_host, workspace, stream=None):
+    """End-to-end form: states_host CPU (pinned) 64-bit tensor [B, ceil(n/64)], out_host CPU (pinned) fp32 [B];
+    workspace a CUDA uint8 tensor of plan.workspace_bytes_host(B).  Asynchronous on the stream."""
+    if states_host.is_cuda or out_host.is_cuda or states_host.element_size() != 8:
+        raise TypeError("states_host/out_host must be CPU tensors (64-bit words / float32)")
+    B = states_host.shape[0]
+    _check(_lib.tqc_contract_states_host(plan._h, states_host.data_ptr(), B, out_host.data_ptr(), workspace.data_ptr(),
+                                         workspace.numel() * workspace.element_size(), _stream_ptr(stream)))
+    return out_host
+
+
+def tqc_contract_distribution_host(plan: Plan, out_host, workspace, prefix_value: int = 0, prefix_bits: int = 0,
+                                   stream=None):
+    """End-to-end form of tqc_contract_distribution: the result lands in out_host (CPU, pinned, fp32)."""
+    if out_host.is_cuda:
+        raise TypeError("out_host must be a CPU tensor")
+    _check(_lib.tqc_contract_distribution_host(plan._h, prefix_value, prefix_bits, out_host.data_ptr(),
+                                               workspace.data_ptr(), workspace.numel() * workspace.element_size(),
+                                               _stream_ptr(stream)))
+    return out_host

@@ -68,6 +68,11 @@ struct tqc_plan {
     size_t staging_elems = 0;
     uint64_t launches = 0;
     bool attrs_set = false;
+    // optional per-launch timing (tqc_plan_profile_*): one event before each launch + one at the end
+    bool profile = false;
+    std::vector<cudaEvent_t> ev_pool;
+    std::vector<int> ev_tags;          // tag of the launch that follows event i (same length as used events - 1)
+    size_t ev_used = 0;
 };
 
 namespace {
@@ -77,6 +82,31 @@ using tqc::Node;
 using tqc::Step;
 
 constexpr int kMaxDynSmem = 200 * 1024;
+
+// Tags of profiled launches: step index t >= 0, or one of these.
+enum { TAG_KEYS = -1, TAG_GATHER = -2, TAG_RELAYOUT = -3 };
+
+int prof_event(tqc_plan_t *pl, cudaStream_t st) {
+    if (pl->ev_used == pl->ev_pool.size()) {
+        cudaEvent_t e;
+        TQC_CUDA(cudaEventCreate(&e));
+        pl->ev_pool.push_back(e);
+    }
+    TQC_CUDA(cudaEventRecord(pl->ev_pool[pl->ev_used++], st));
+    return 0;
+}
+// called right before every kernel launch
+int note_launch(tqc_plan_t *pl, int tag, cudaStream_t st) {
+    pl->launches++;
+    if (!pl->profile) return 0;
+    pl->ev_tags.push_back(tag);
+    return prof_event(pl, st);
+}
+int prof_begin(tqc_plan_t *pl) {
+    if (pl->profile) { pl->ev_used = 0; pl->ev_tags.clear(); }
+    return 0;
+}
+int prof_close(tqc_plan_t *pl, cudaStream_t st) { return pl->profile ? prof_event(pl, st) : 0; }
 
 template <int MI, int MJ>
 int launch_tile_t(const StepArgs &a, size_t smem, long long blocks, cudaStream_t st) {
@@ -91,7 +121,7 @@ int launch_tile_t(const StepArgs &a, size_t smem, long long blocks, cudaStream_t
 }
 
 // Tile choice for the FFMA kernel: TI x TJ outputs per row, RPB rows per 256-thread block.
-int launch_tile(tqc_plan_t *pl, StepArgs &a, cudaStream_t st) {
+int launch_tile(tqc_plan_t *pl, StepArgs &a, int tag, cudaStream_t st) {
     const int MI = a.lgM >= 2 ? 4 : 1, MJ = a.lgN >= 2 ? 4 : 1;
     const long long M = 1ll << a.lgM, N = 1ll << a.lgN, K = 1ll << a.lgK;
     long long TI = MI == 4 ? std::min<long long>(M, 64) : M;
@@ -112,11 +142,11 @@ int launch_tile(tqc_plan_t *pl, StepArgs &a, cudaStream_t st) {
     const long long blocks = (long long)a.tiles_i * a.tiles_j * rgroups;
     if (blocks <= 0 || blocks > 0x7fffffffll) return fail(TQC_E_TOO_LARGE, "step needs more than 2^31 thread blocks");
     int rc;
+    if ((rc = note_launch(pl, tag, st))) return rc;
     if (MI == 4 && MJ == 4) rc = launch_tile_t<4, 4>(a, smem_of(TK), blocks, st);
     else if (MI == 4) rc = launch_tile_t<4, 1>(a, smem_of(TK), blocks, st);
     else if (MJ == 4) rc = launch_tile_t<1, 4>(a, smem_of(TK), blocks, st);
     else rc = launch_tile_t<1, 1>(a, smem_of(TK), blocks, st);
-    if (rc == 0) pl->launches++;
     return rc;
 }
 
@@ -215,7 +245,7 @@ int launch_cross_step(tqc_plan_t *pl, const CrossCtx &cx, int t, cudaStream_t st
         a.C = cx.ws + off;
     }
     if (!pa.build(a.outA) || !pb.build(a.outB)) return fail(TQC_E_TOO_LARGE, "bit map needs too many segments");
-    return launch_tile(pl, a, st);
+    return launch_tile(pl, a, t, st);
 }
 
 // ---- batch mode (one row per state of the chunk) ---------------------------------------------
@@ -254,9 +284,10 @@ int launch_batch_step(tqc_plan_t *pl, const BatchCtx &bx, int t, cudaStream_t st
         long long G = std::min<long long>(32, std::max<long long>(1, (1ll << lgK) / 4));
         const long long rows_per_block = (32 / G) * 8;
         const long long blocks = (bx.R + rows_per_block - 1) / rows_per_block;
+        int rc = note_launch(pl, t, st);
+        if (rc) return rc;
         tqc::dot_kernel<<<(unsigned)blocks, 256, 0, st>>>(d);
         TQC_CUDA(cudaGetLastError());
-        pl->launches++;
         return 0;
     }
     StepArgs a;
@@ -271,7 +302,7 @@ int launch_batch_step(tqc_plan_t *pl, const BatchCtx &bx, int t, cudaStream_t st
     add_digit_scatter(pa, s.outer_lhs, C.layout);
     add_digit_scatter(pb, s.outer_rhs, C.layout);
     if (!pa.build(a.outA) || !pb.build(a.outB)) return fail(TQC_E_TOO_LARGE, "bit map needs too many segments");
-    return launch_tile(pl, a, st);
+    return launch_tile(pl, a, t, st);
 }
 
 int ensure_meta(tqc_plan_t *pl) {
@@ -342,6 +373,7 @@ void tqc_plan_destroy(tqc_plan_t *pl) {
     if (pl->d_slot_ofs) cudaFree(pl->d_slot_ofs);
     if (pl->d_slot_qubits) cudaFree(pl->d_slot_qubits);
     if (pl->d_staging) cudaFree(pl->d_staging);
+    for (cudaEvent_t e : pl->ev_pool) cudaEventDestroy(e);
     delete pl;
 }
 
@@ -455,9 +487,13 @@ int tqc_load_subcircuit_tensors(tqc_plan_t *pl, int s, const float *data, size_t
     }
     if (!bp.build(a.row_of)) return fail(TQC_E_TOO_LARGE, "bit map needs too many segments");
     const long long tiles = (((1ll << o) + 31) / 32) * (((1ll << (2 * c)) + 31) / 32);
+    const bool prof = pl->profile;
+    pl->profile = false;                                   // loads are not part of the profiled contract call
+    rc = note_launch(pl, TAG_RELAYOUT, st);
+    pl->profile = prof;
+    if (rc) return rc;
     tqc::relayout_kernel<<<(unsigned)tiles, 256, 0, st>>>(a);
     TQC_CUDA(cudaGetLastError());
-    pl->launches++;
     pl->loaded[s] = 1;
     return 0;
 }
@@ -489,6 +525,7 @@ int tqc_contract_states(tqc_plan_t *pl, const uint64_t *states_dev, size_t n_sta
     float *batch = (float *)(ws + fixed + align256((size_t)hp.n_key_slots * 4 * (size_t)cap));
     // the alignment pad of the key region is covered by the +256 of tqc_plan_workspace_bytes
     int rc;
+    prof_begin(pl);
     // phase T: nodes evaluated once per key (tables), independent of the batch
     CrossCtx cx;
     cx.ws = tables;
@@ -508,9 +545,9 @@ int tqc_contract_states(tqc_plan_t *pl, const uint64_t *states_dev, size_t n_sta
             ka.keys = keys; ka.slot_ofs = pl->d_slot_ofs; ka.slot_qubits = pl->d_slot_qubits;
             ka.words = words; ka.R = bx.R; ka.cap = cap;
             dim3 grid((unsigned)((bx.R + 255) / 256), (unsigned)hp.n_key_slots);
+            if ((rc = note_launch(pl, TAG_KEYS, st))) return rc;
             tqc::key_kernel<<<grid, 256, 0, st>>>(ka);
             TQC_CUDA(cudaGetLastError());
-            pl->launches++;
         }
         for (int t = 0; t < hp.m - 1; ++t)
             if (hp.nodes[hp.m + t].kind == tqc::NODE_BATCH && (rc = launch_batch_step(pl, bx, t, st))) return rc;
@@ -520,12 +557,12 @@ int tqc_contract_states(tqc_plan_t *pl, const uint64_t *states_dev, size_t n_sta
             g.table = hp.m == 1 ? pl->d_leaf[0] : tables + root.table_offset;
             g.keys = keys + (long long)root.key_slot * cap;
             g.out = bx.out; g.R = bx.R;
+            if ((rc = note_launch(pl, TAG_GATHER, st))) return rc;
             tqc::gather_kernel<<<(unsigned)((bx.R + 255) / 256), 256, 0, st>>>(g);
             TQC_CUDA(cudaGetLastError());
-            pl->launches++;
         }
     }
-    return 0;
+    return prof_close(pl, st);
 }
 
 int tqc_contract_distribution(tqc_plan_t *pl, uint64_t prefix_value, int prefix_bits, float *out_dev, void *workspace_dev,
@@ -551,6 +588,7 @@ int tqc_contract_distribution(tqc_plan_t *pl, uint64_t prefix_value, int prefix_
     cx.free_bits = &fb; cx.offsets = &off;
     cx.ws = (float *)workspace_dev; cx.out = out_dev;
     int rc;
+    prof_begin(pl);
     for (int t = 0; t < hp.m - 1; ++t)
         if ((rc = launch_cross_step(pl, cx, t, st))) return rc;
     if (hp.m == 1) {
@@ -576,10 +614,85 @@ int tqc_contract_distribution(tqc_plan_t *pl, uint64_t prefix_value, int prefix_
         if (!in.build(g.map) || !om.build(g.out_map)) return fail(TQC_E_TOO_LARGE, "bit map needs too many segments");
         g.map_or = fixed;
         g.table = pl->d_leaf[0]; g.keys = nullptr; g.out = out_dev; g.R = 1ll << nf;
+        if ((rc = note_launch(pl, TAG_GATHER, st))) return rc;
         tqc::gather_kernel<<<(unsigned)((g.R + 255) / 256), 256, 0, st>>>(g);
         TQC_CUDA(cudaGetLastError());
-        pl->launches++;
     }
+    return prof_close(pl, st);
+}
+
+// ---- host-buffer entry points: staging carved from the front of the workspace ------------------
+size_t tqc_plan_workspace_bytes_host(const tqc_plan_t *pl, size_t n_states, int prefix_bits) {
+    if (!pl) return 0;
+    const HostPlan &hp = pl->hp;
+    if (hp.mode == TQC_MODE_STATES) {
+        const size_t words = (size_t)(hp.n + 63) / 64;
+        return align256(n_states * words * 8) + align256(n_states * 4) + tqc_plan_workspace_bytes(pl, n_states, 0);
+    }
+    const int pb = std::max(0, std::min(prefix_bits, hp.n));
+    return align256(((size_t)4) << (hp.n - pb)) + tqc_plan_workspace_bytes(pl, 0, pb);
+}
+
+int tqc_contract_states_host(tqc_plan_t *pl, const uint64_t *states_host, size_t n_states, float *out_host,
+                             void *workspace_dev, size_t workspace_bytes, void *stream) {
+    if (!pl) return fail(TQC_E_ARG, "null plan");
+    if (n_states == 0) return 0;
+    if (!states_host || !out_host) return fail(TQC_E_ARG, "null states/out pointer");
+    if (!workspace_dev || ((uintptr_t)workspace_dev & 255) != 0) return fail(TQC_E_ARG, "workspace must be non-null and 256-byte aligned");
+    const size_t words = (size_t)(pl->hp.n + 63) / 64;
+    const size_t sb = align256(n_states * words * 8), ob = align256(n_states * 4);
+    if (workspace_bytes < sb + ob + tqc_plan_workspace_min_bytes(pl)) return fail(TQC_E_WORKSPACE, "workspace smaller than staging + tqc_plan_workspace_min_bytes");
+    cudaStream_t st = (cudaStream_t)stream;
+    char *ws = (char *)workspace_dev;
+    uint64_t *sd = (uint64_t *)ws;
+    float *od = (float *)(ws + sb);
+    if (words > 0) TQC_CUDA(cudaMemcpyAsync(sd, states_host, n_states * words * 8, cudaMemcpyHostToDevice, st));
+    const int rc = tqc_contract_states(pl, sd, n_states, od, ws + sb + ob, workspace_bytes - sb - ob, stream);
+    if (rc) return rc;
+    TQC_CUDA(cudaMemcpyAsync(out_host, od, n_states * 4, cudaMemcpyDeviceToHost, st));
+    return 0;
+}
+
+int tqc_contract_distribution_host(tqc_plan_t *pl, uint64_t prefix_value, int prefix_bits, float *out_host,
+                                   void *workspace_dev, size_t workspace_bytes, void *stream) {
+    if (!pl) return fail(TQC_E_ARG, "null plan");
+    if (!out_host) return fail(TQC_E_ARG, "null out pointer");
+    if (prefix_bits < 0 || prefix_bits > pl->hp.n) return fail(TQC_E_ARG, "prefix_bits out of range");
+    if (pl->hp.n - prefix_bits > 34) return fail(TQC_E_TOO_LARGE, "more than 2^34 outputs; raise prefix_bits");
+    if (!workspace_dev || ((uintptr_t)workspace_dev & 255) != 0) return fail(TQC_E_ARG, "workspace must be non-null and 256-byte aligned");
+    const size_t ob = align256(((size_t)4) << (pl->hp.n - prefix_bits));
+    if (workspace_bytes < ob) return fail(TQC_E_WORKSPACE, "workspace smaller than tqc_plan_workspace_bytes_host");
+    cudaStream_t st = (cudaStream_t)stream;
+    char *ws = (char *)workspace_dev;
+    const int rc = tqc_contract_distribution(pl, prefix_value, prefix_bits, (float *)ws, ws + ob, workspace_bytes - ob, stream);
+    if (rc) return rc;
+    TQC_CUDA(cudaMemcpyAsync(out_host, ws, ((size_t)4) << (pl->hp.n - prefix_bits), cudaMemcpyDeviceToHost, st));
+    return 0;
+}
+
+// ---- per-launch timing --------------------------------------------------------------------------
+int tqc_plan_profile_enable(tqc_plan_t *pl, int on) {
+    if (!pl) return fail(TQC_E_ARG, "null plan");
+    pl->profile = on != 0;
+    pl->ev_used = 0;
+    pl->ev_tags.clear();
+    return 0;
+}
+
+int tqc_plan_profile_read(tqc_plan_t *pl, int32_t *tags, float *ms, size_t *n) {
+    if (!pl || !n) return fail(TQC_E_ARG, "null argument");
+    const size_t have = pl->ev_tags.size();
+    if (!tags || !ms) { *n = have; return 0; }
+    if (*n < have) { *n = have; return fail(TQC_E_ARG, "buffer too small"); }
+    if (have > 0) {
+        if (pl->ev_used != have + 1) return fail(TQC_E_STATE, "profiled call did not complete");
+        TQC_CUDA(cudaEventSynchronize(pl->ev_pool[have]));
+        for (size_t i = 0; i < have; ++i) {
+            tags[i] = pl->ev_tags[i];
+            TQC_CUDA(cudaEventElapsedTime(&ms[i], pl->ev_pool[i], pl->ev_pool[i + 1]));
+        }
+    }
+    *n = have;
     return 0;
 }
 
