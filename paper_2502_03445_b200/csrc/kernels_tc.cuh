@@ -1,0 +1,321 @@
+// Tensor-pipe contraction step for sm_100a: a pairwise contraction whose outer dimensions are large is a
+// batched GEMM (section 3.2; cost dim(i) dim(j) dim(k), lines 407-412)
+//     C_r[outA(i) | outB(j)] = sum_k A_r[i, k] * B_r[j, k],   M = 4^{#outer_lhs}, N = 4^{#outer_rhs}, K = 4^{#inner}
+// per state r.  Both operands are K-major fp32 in HBM/L2.  tcgen05 has no fp32-input MMA, so each operand
+// tile is split in shared memory into a_hi (top 19 bits, exactly a TF32 value) and a_lo = a - a_hi (exact in fp32)
+// and three TF32 MMAs hi*hi + hi*lo + lo*hi accumulate in fp32 in TMEM.
+//
+// Persistent, warp-specialised CTA (one per SM), 320 threads:
+//   warp 0      TMA producer: cp.async.bulk.tensor 3-D tiles {32 k, 128 or BN rows, 1 state} with 128-byte swizzle;
+//               the state coordinate of a LEAF/TABLE operand is the state's key (a3 gather = a TMA coordinate)
+//   warp 1      MMA issuer: one elected lane, 12 tcgen05.mma.kind::tf32 per k-block, tcgen05.commit frees the stage
+//   warps 2-5   accumulate + epilogue: tcgen05.ld -> fp32 round-to-nearest adds in registers -> scatter to C
+//   warps 6-9   splitter: fp32 tile -> hi (in place) and lo (second buffer), same swizzled byte offsets
+// Pipelines: full[s] (TMA -> splitter), ready[s] (splitter -> MMA), empty[s] (MMA -> TMA).
+// The tensor pipe's fp32 accumulator rounds toward zero on every add (measured: -5e-8 relative per accumulation,
+// profiles/r01c notes), a bias that grows with the number of k-steps.  So (i) the hi*hi products of at most
+// TC_CHUNK_KB k-blocks (8 MMAs) accumulate in a TMEM buffer D_hi that the accumulate warps then drain and add to
+// registers in round-to-nearest, two D_hi buffers alternating so draining overlaps the next chunk's MMAs; (ii) the
+// hi*lo + lo*hi products, 2^-11 smaller, accumulate over the whole K in their own buffer D_lo (two of them,
+// alternating per tile), where the same bias is negligible.  TMEM columns: 4 x BN <= 512.
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "device_args.h"
+
+namespace tqc {
+
+constexpr int TC_BM = 128;          // UMMA M
+constexpr int TC_BK = 32;           // fp32 elements per k-block = 128 bytes = one swizzle row
+constexpr int TC_THREADS = 320;
+constexpr int TC_SPLIT_THREADS = 128;
+constexpr int TC_CHUNK_KB = 2;       // k-blocks (of 32) whose hi*hi products accumulate in TMEM before a drain
+
+struct TcArgs {
+    const uint32_t *keysA, *keysB;  // state coordinate of a keyed operand (null: the row itself)
+    float *C;
+    long long c_row_stride;
+    BitMap outA, outB;              // i -> C offset bits, j -> C offset bits
+    int lgM, lgN, lgK;
+    int R;                          // states in this launch
+    int BN;                         // N tile: 16, 32, 64 or 128
+    int stages;
+    int mask_hi;                    // write the truncated hi part back in place (independent of how the MMA reads fp32 bits)
+    int vec4;                       // 4 consecutive j are contiguous in C
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t"
+        "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+
+__device__ __forceinline__ void tma_load_3d(const CUtensorMap *map, uint64_t *bar, void *dst, int c0, int c1, int c2) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+
+// K-major, 128-byte-swizzled operand tile: rows of 128 bytes, 8-row groups 1024 bytes apart.
+__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr) {
+    uint64_t d = 0;
+    d |= (uint64_t)((smem_addr & 0x3FFFFu) >> 4);          // start address, 16-byte units
+    d |= (uint64_t)1 << 16;                                // leading byte offset (unused for swizzled K-major)
+    d |= (uint64_t)(1024 >> 4) << 32;                      // stride byte offset between 8-row groups
+    d |= (uint64_t)1 << 46;                                // descriptor version (sm_100)
+    d |= (uint64_t)2 << 61;                                // SWIZZLE_128B
+    return d;
+}
+
+__device__ __forceinline__ void umma_tf32(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t"
+        "}" ::"r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint64_t *bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
+          "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]),
+          "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]),
+          "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[32]) {      // 16 columns into v[0..15]
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
+          "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+        : "r"(taddr));
+}
+
+
+template <int BN>
+__global__ void __launch_bounds__(TC_THREADS, 1)
+step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB, const TcArgs a) {
+    extern __shared__ unsigned char tc_smem_raw[];
+    __shared__ __align__(8) uint64_t full_bar[4], ready_bar[4], empty_bar[4];
+    __shared__ __align__(8) uint64_t hi_full_bar[2], hi_empty_bar[2], lo_full_bar[2], lo_empty_bar[2];
+    __shared__ uint32_t tmem_base_slot;
+    __shared__ uint32_t ob_tab[BN];
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int S = a.stages;
+    constexpr uint32_t bytesA = TC_BM * TC_BK * 4, bytesB = (uint32_t)BN * TC_BK * 4;
+    constexpr uint32_t stage_bytes = 2 * bytesA + 2 * bytesB;
+    unsigned char *tiles = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(tc_smem_raw) + 1023) & ~(uintptr_t)1023);
+    auto A_raw = [&](int s) { return tiles + (size_t)s * stage_bytes; };
+    auto A_lo = [&](int s) { return tiles + (size_t)s * stage_bytes + bytesA; };
+    auto B_raw = [&](int s) { return tiles + (size_t)s * stage_bytes + 2 * bytesA; };
+    auto B_lo = [&](int s) { return tiles + (size_t)s * stage_bytes + 2 * bytesA + bytesB; };
+
+    const int n_kb = 1 << (a.lgK - 5);
+    const int chunk_kb = n_kb < TC_CHUNK_KB ? n_kb : TC_CHUNK_KB;
+    const int n_chunks = n_kb / chunk_kb;
+    const long long tiles_m = 1ll << (a.lgM - 7);
+    const long long tiles_n = (1ll << a.lgN) / BN;
+    const long long total = tiles_m * tiles_n * a.R;
+    constexpr uint32_t tmem_cols = 4 * BN < 32 ? 32 : 4 * BN;      // D_hi[0], D_hi[1], D_lo[0], D_lo[1]
+
+    // ---- one-time setup -------------------------------------------------------------------------
+    for (int c = threadIdx.x; c < BN; c += TC_THREADS) ob_tab[c] = (uint32_t)bitmap_apply(a.outB, (unsigned long long)c);
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < S; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&ready_bar[s], TC_SPLIT_THREADS / 32); mbar_init(&empty_bar[s], 1); }
+        for (int s = 0; s < 2; ++s) {
+            mbar_init(&hi_full_bar[s], 1); mbar_init(&hi_empty_bar[s], 4);
+            mbar_init(&lo_full_bar[s], 1); mbar_init(&lo_empty_bar[s], 4);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 0 && lane == 0) {
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&mapA) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&mapB) : "memory");
+    }
+    if (warp == 1) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_slot)), "r"(tmem_cols) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem_base = tmem_base_slot;
+
+    if (warp == 0) {
+        // ===== TMA producer =====
+        if (lane == 0) {
+            long long it = 0;
+            for (long long t = blockIdx.x; t < total; t += gridDim.x) {
+                const long long nt = t % tiles_n, mt = (t / tiles_n) % tiles_m, r = t / (tiles_n * tiles_m);
+                const int rowA = a.keysA ? (int)a.keysA[r] : (int)r;
+                const int rowB = a.keysB ? (int)a.keysB[r] : (int)r;
+                for (int kb = 0; kb < n_kb; ++kb, ++it) {
+                    const int s = (int)(it % S);
+                    const uint32_t ph = (uint32_t)((it / S) & 1);
+                    mbar_wait(&empty_bar[s], ph ^ 1u);
+                    mbar_expect_tx(&full_bar[s], bytesA + bytesB);
+                    tma_load_3d(&mapA, &full_bar[s], A_raw(s), kb * TC_BK, (int)(mt * TC_BM), rowA);
+                    tma_load_3d(&mapB, &full_bar[s], B_raw(s), kb * TC_BK, (int)(nt * BN), rowB);
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer =====
+        constexpr uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(TC_BM >> 4) << 24);
+        long long it = 0, lt = 0, g = 0;
+        for (long long t = blockIdx.x; t < total; t += gridDim.x, ++lt) {
+            const uint32_t lb = (uint32_t)(lt & 1), lph = (uint32_t)((lt >> 1) & 1);
+            mbar_wait(&lo_empty_bar[lb], lph ^ 1u);
+            const uint32_t d_lo = tmem_base + (2u + lb) * (uint32_t)BN;
+            int kb = 0;
+            for (int c = 0; c < n_chunks; ++c, ++g) {
+                const uint32_t hb = (uint32_t)(g & 1), hph = (uint32_t)((g >> 1) & 1);
+                mbar_wait(&hi_empty_bar[hb], hph ^ 1u);
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                const uint32_t d_hi = tmem_base + hb * (uint32_t)BN;
+                for (int kc = 0; kc < chunk_kb; ++kc, ++kb, ++it) {
+                    const int s = (int)(it % S);
+                    const uint32_t ph = (uint32_t)((it / S) & 1);
+                    mbar_wait(&ready_bar[s], ph);
+                    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                    if (lane == 0) {
+                        const uint64_t dah = umma_desc_sw128(smem_u32(A_raw(s))), dal = umma_desc_sw128(smem_u32(A_lo(s)));
+                        const uint64_t dbh = umma_desc_sw128(smem_u32(B_raw(s))), dbl = umma_desc_sw128(smem_u32(B_lo(s)));
+#pragma unroll
+                        for (int k = 0; k < TC_BK / 8; ++k) {
+                            const uint64_t adv = (uint64_t)(k * 8 * 4 >> 4);       // 32 bytes per K=8 slice, 16-byte units
+                            umma_tf32(d_lo, dal + adv, dbh + adv, idesc, (kb | k) ? 1u : 0u);
+                            umma_tf32(d_lo, dah + adv, dbl + adv, idesc, 1u);
+                            umma_tf32(d_hi, dah + adv, dbh + adv, idesc, (kc | k) ? 1u : 0u);
+                        }
+                        umma_commit(&empty_bar[s]);                                 // frees the stage when these MMAs retire
+                        if (kc == chunk_kb - 1) umma_commit(&hi_full_bar[hb]);
+                        if (kb == n_kb - 1) umma_commit(&lo_full_bar[lb]);
+                    }
+                    __syncwarp();
+                }
+            }
+        }
+    } else if (warp < 6) {
+        // ===== accumulate (round-to-nearest, registers) + epilogue =====
+        const int w4 = warp & 3;
+        const int i_local = 32 * w4 + lane;
+        const uint32_t lane_base = (uint32_t)(32 * w4) << 16;
+        long long lt = 0, g = 0;
+        for (long long t = blockIdx.x; t < total; t += gridDim.x, ++lt) {
+            const long long nt = t % tiles_n, mt = (t / tiles_n) % tiles_m, r = t / (tiles_n * tiles_m);
+            float acc[BN];
+#pragma unroll
+            for (int q = 0; q < BN; ++q) acc[q] = 0.f;
+            for (int c = 0; c < n_chunks; ++c, ++g) {
+                const uint32_t hb = (uint32_t)(g & 1), hph = (uint32_t)((g >> 1) & 1);
+                mbar_wait(&hi_full_bar[hb], hph);
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                const uint32_t taddr = tmem_base + lane_base + hb * (uint32_t)BN;
+#pragma unroll
+                for (int c0 = 0; c0 < BN; c0 += 32) {
+                    uint32_t v[32];
+                    if (BN - c0 >= 32) tmem_ld32(taddr + c0, v); else tmem_ld16(taddr + c0, v);
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                    for (int q = 0; q < 32; ++q)
+                        if (c0 + q < BN) acc[c0 + q] += __uint_as_float(v[q]);
+                }
+                asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&hi_empty_bar[hb]);
+            }
+            const uint32_t lb = (uint32_t)(lt & 1), lph = (uint32_t)((lt >> 1) & 1);
+            mbar_wait(&lo_full_bar[lb], lph);
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            const unsigned long long oa = bitmap_apply(a.outA, (unsigned long long)(mt * TC_BM + i_local));
+            const unsigned long long obh = bitmap_apply(a.outB, (unsigned long long)(nt * BN));
+            float *crow = a.C + r * a.c_row_stride + (oa | obh);
+            const uint32_t laddr = tmem_base + lane_base + (2u + lb) * (uint32_t)BN;
+#pragma unroll
+            for (int c0 = 0; c0 < BN; c0 += 32) {
+                uint32_t v[32];
+                if (BN - c0 >= 32) tmem_ld32(laddr + c0, v); else tmem_ld16(laddr + c0, v);
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                for (int q = 0; q < 32; ++q)
+                    if (c0 + q < BN) acc[c0 + q] += __uint_as_float(v[q]);
+            }
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&lo_empty_bar[lb]);
+            if (a.vec4) {
+#pragma unroll
+                for (int q = 0; q < BN; q += 4)
+                    *reinterpret_cast<float4 *>(crow + ob_tab[q]) = make_float4(acc[q], acc[q + 1], acc[q + 2], acc[q + 3]);
+            } else {
+#pragma unroll
+                for (int q = 0; q < BN; ++q) crow[ob_tab[q]] = acc[q];
+            }
+        }
+    } else {
+        // ===== splitter: fp32 -> hi (in place) + lo =====
+        const int st = threadIdx.x - 6 * 32;
+        const bool mask_hi = a.mask_hi != 0;
+        long long it = 0;
+        for (long long t = blockIdx.x; t < total; t += gridDim.x) {
+            for (int kb = 0; kb < n_kb; ++kb, ++it) {
+                const int s = (int)(it % S);
+                const uint32_t ph = (uint32_t)((it / S) & 1);
+                mbar_wait(&full_bar[s], ph);
+                // per stage: [A_raw][A_lo][B_raw][B_lo]; element e of a raw tile and of its lo tile share the swizzled offset
+                constexpr int nva = (int)(bytesA >> 4), nvb = (int)(bytesB >> 4);
+#pragma unroll 2
+                for (int e = st; e < nva + nvb; e += TC_SPLIT_THREADS) {
+                    uint4 *xp = e < nva ? reinterpret_cast<uint4 *>(A_raw(s)) + e : reinterpret_cast<uint4 *>(B_raw(s)) + (e - nva);
+                    float4 *lp = e < nva ? reinterpret_cast<float4 *>(A_lo(s)) + e : reinterpret_cast<float4 *>(B_lo(s)) + (e - nva);
+                    const uint4 x = *xp;
+                    const uint4 h = make_uint4(x.x & 0xFFFFE000u, x.y & 0xFFFFE000u, x.z & 0xFFFFE000u, x.w & 0xFFFFE000u);
+                    *lp = make_float4(__uint_as_float(x.x) - __uint_as_float(h.x), __uint_as_float(x.y) - __uint_as_float(h.y),
+                                      __uint_as_float(x.z) - __uint_as_float(h.z), __uint_as_float(x.w) - __uint_as_float(h.w));
+                    if (mask_hi) *xp = h;
+                }
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // generic-proxy writes -> visible to the MMA's async proxy
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&ready_bar[s]);
+            }
+        }
+    }
+
+    // ---- teardown ---------------------------------------------------------------------------------
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (warp == 1) {
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(tmem_cols) : "memory");
+    }
+}
+
+}  // namespace tqc

@@ -5,6 +5,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -12,6 +13,7 @@
 #include "../../include/tqc.h"
 #include "device_args.h"
 #include "kernels_simt.cuh"
+#include "kernels_tc.cuh"
 #include "plan.hpp"
 
 namespace {
@@ -268,6 +270,94 @@ void batch_operand(tqc_plan_t *pl, const BatchCtx &bx, int v, const float *&base
     }
 }
 
+// ---- tensor-pipe step (kernels_tc.cuh) ----------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+int get_encode_fn(EncodeTiledFn *out) {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        TQC_CUDA(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres));
+        if (!p || qres != cudaDriverEntryPointSuccess) return fail(TQC_E_CUDA, "cuTensorMapEncodeTiled not available in this driver");
+        fn = (EncodeTiledFn)p;
+    }
+    *out = fn;
+    return 0;
+}
+
+// operand seen as a 3-D fp32 tensor {K, rows_inner, rows_outer}: one {32, box_rows, 1} box per TMA load
+int make_operand_map(CUtensorMap *map, const float *base, int lgK, int lgRows, long long n_outer, int box_rows) {
+    EncodeTiledFn enc;
+    int rc = get_encode_fn(&enc);
+    if (rc) return rc;
+    const cuuint64_t dims[3] = {(cuuint64_t)1 << lgK, (cuuint64_t)1 << lgRows, (cuuint64_t)std::max<long long>(n_outer, 1)};
+    const cuuint64_t strides[2] = {((cuuint64_t)4) << lgK, ((cuuint64_t)4) << (lgK + lgRows)};
+    const cuuint32_t box[3] = {(cuuint32_t)tqc::TC_BK, (cuuint32_t)box_rows, 1};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void *)base, dims, strides, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(TQC_E_CUDA, "cuTensorMapEncodeTiled failed with code " + std::to_string((int)r));
+    return 0;
+}
+
+bool tc_eligible(int lgM, int lgN, int lgK) {
+    return lgK >= 5 && std::max(lgM, lgN) >= 7 && std::min(lgM, lgN) >= 4;
+}
+
+struct TcOperand { const float *base; const uint32_t *keys; long long n_outer; };
+
+int launch_tc_step(tqc_plan_t *pl, TcOperand A, TcOperand B, BitMap outA, BitMap outB, int lgM, int lgN, int lgK, float *C,
+                   long long c_row_stride, int R, int tag, cudaStream_t st) {
+    static int sm_count = 0;
+    static bool attr = false;
+    if (!attr) {
+        int dev = 0;
+        TQC_CUDA(cudaGetDevice(&dev));
+        TQC_CUDA(cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 225 * 1024));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 225 * 1024));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, 225 * 1024));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 225 * 1024));
+        attr = true;
+    }
+    auto has_bit0 = [](const BitMap &m) { for (int s = 0; s < m.n; ++s) if (m.dst[s] == 0) return true; return false; };
+    // the M side needs >= 128 rows; with both sides large, the N side (vector stores run along it) takes C's lowest bits
+    bool swap = lgM < 7;
+    if (lgM >= 7 && lgN >= 7 && has_bit0(outA)) swap = true;
+    if (swap) { std::swap(A, B); std::swap(outA, outB); std::swap(lgM, lgN); }
+    tqc::TcArgs a;
+    memset(&a, 0, sizeof(a));
+    a.keysA = A.keys; a.keysB = B.keys;
+    a.C = C; a.c_row_stride = c_row_stride;
+    a.outA = outA; a.outB = outB;
+    a.lgM = lgM; a.lgN = lgN; a.lgK = lgK; a.R = R;
+    a.BN = (int)std::min<long long>(128, 1ll << lgN);
+    a.mask_hi = 0;      // the tensor pipe ignores the low 13 mantissa bits of an fp32 word read as TF32 (measured: bit-identical)
+    const size_t stage_bytes = 2 * (size_t)tqc::TC_BM * tqc::TC_BK * 4 + 2 * (size_t)a.BN * tqc::TC_BK * 4;
+    a.stages = (int)std::min<size_t>(4, (220 * 1024) / stage_bytes);
+    a.vec4 = (outB.n >= 1 && outB.src[0] == 0 && outB.dst[0] == 0 && outB.len[0] >= 2) ? 1 : 0;
+    CUtensorMap mapA, mapB;
+    int rc;
+    if ((rc = make_operand_map(&mapA, A.base, lgK, lgM, A.n_outer, tqc::TC_BM))) return rc;
+    if ((rc = make_operand_map(&mapB, B.base, lgK, lgN, B.n_outer, a.BN))) return rc;
+    const long long total = (1ll << (lgM - 7)) * ((1ll << lgN) / a.BN) * (long long)R;
+    const unsigned grid = (unsigned)std::min<long long>(total, sm_count);
+    if ((rc = note_launch(pl, tag, st))) return rc;
+    const size_t smem = a.stages * stage_bytes + 1024;
+    switch (a.BN) {
+        case 16: tqc::step_tc_kernel<16><<<grid, tqc::TC_THREADS, smem, st>>>(mapA, mapB, a); break;
+        case 32: tqc::step_tc_kernel<32><<<grid, tqc::TC_THREADS, smem, st>>>(mapA, mapB, a); break;
+        case 64: tqc::step_tc_kernel<64><<<grid, tqc::TC_THREADS, smem, st>>>(mapA, mapB, a); break;
+        default: tqc::step_tc_kernel<128><<<grid, tqc::TC_THREADS, smem, st>>>(mapA, mapB, a); break;
+    }
+    TQC_CUDA(cudaGetLastError());
+    return 0;
+}
+
 int launch_batch_step(tqc_plan_t *pl, const BatchCtx &bx, int t, cudaStream_t st) {
     const HostPlan &hp = pl->hp;
     const Step &s = hp.steps[t];
@@ -302,6 +392,14 @@ int launch_batch_step(tqc_plan_t *pl, const BatchCtx &bx, int t, cudaStream_t st
     add_digit_scatter(pa, s.outer_lhs, C.layout);
     add_digit_scatter(pb, s.outer_rhs, C.layout);
     if (!pa.build(a.outA) || !pb.build(a.outB)) return fail(TQC_E_TOO_LARGE, "bit map needs too many segments");
+    if (s.kernel_class == TQC_KERNEL_TCGEN05) {
+        auto n_outer = [&](int v) -> long long {
+            const Node &nd = hp.nodes[v];
+            return nd.kind == tqc::NODE_BATCH ? (long long)bx.R : (1ll << (int)nd.qubits.size());
+        };
+        TcOperand oa{a.A.base, a.A.keys, n_outer(s.lhs)}, ob{a.B.base, a.B.keys, n_outer(s.rhs)};
+        return launch_tc_step(pl, oa, ob, a.outA, a.outB, lgM, lgN, lgK, cbase, a.c_row_stride, bx.R, t, st);
+    }
     return launch_tile(pl, a, t, st);
 }
 
@@ -360,8 +458,10 @@ int tqc_plan(const tqc_network_desc *net, const tqc_plan_opts *opts, tqc_plan_t 
     pl->loaded.assign(pl->hp.m, 0);
     for (int t = 0; t < pl->hp.m - 1; ++t) {
         Step &s = pl->hp.steps[t];
-        s.kernel_class = (s.outer_lhs.empty() && s.outer_rhs.empty() && pl->hp.nodes[pl->hp.m + t].kind == tqc::NODE_BATCH)
-                             ? TQC_KERNEL_DOT : TQC_KERNEL_SIMT_TILE;
+        const bool batch = pl->hp.nodes[pl->hp.m + t].kind == tqc::NODE_BATCH;
+        s.kernel_class = (s.outer_lhs.empty() && s.outer_rhs.empty() && batch) ? TQC_KERNEL_DOT : TQC_KERNEL_SIMT_TILE;
+        if (batch && use_tc >= 0 && tc_eligible(2 * (int)s.outer_lhs.size(), 2 * (int)s.outer_rhs.size(), 2 * (int)s.inner.size()))
+            s.kernel_class = TQC_KERNEL_TCGEN05;
     }
     *out = pl;
     return 0;

@@ -1,0 +1,80 @@
+"""GPU parity of the tensor-pipe step (step_tc_kernel: TMA-fed 3xTF32 tcgen05 MMAs, TMEM accumulators) against the
+float64 direct sum of Eq. 1, on networks whose first contraction has large outer dimensions (M or N >= 128, K >= 32).
+Same bar as everywhere: |dp| <= 1e-5 * max p; the 3xTF32 split is also compared with the fp32 FFMA path."""
+import numpy as np
+import pytest
+import torch
+
+import paper_2502_03445_b200 as tqc
+from oracle.direct_sum_c import direct_sum_c
+from tqc_inputs import pack_states, random_states, random_tensors
+from tqc_inputs.network import Network
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-5
+KERNEL_TCGEN05 = 2
+
+
+def _triangle(na, nb, ni, oa=5, ob=5, od=2, flip=False):
+    """Subcircuits A, B, D: A-D share na cuts, B-D share nb, A-B share ni.  Contracting (A,B) first is a GEMM with
+    M = 4^na, N = 4^nb, K = 4^ni per state; then a dot with D over 4^(na+nb)."""
+    cuts, ca, cb, cd = [], [], [], []
+    for _ in range(na):
+        ca.append(len(cuts)); cd.append(len(cuts)); cuts.append((0, 2))
+    for _ in range(nb):
+        cb.append(len(cuts)); cd.append(len(cuts)); cuts.append((2, 1))
+    for _ in range(ni):
+        ca.append(len(cuts)); cb.append(len(cuts)); cuts.append((0, 1) if not flip else (1, 0))
+    rng = np.random.default_rng(na * 100 + nb * 10 + ni)
+    ca = [ca[i] for i in rng.permutation(len(ca))]            # caller axis order is arbitrary (G6)
+    cb = [cb[i] for i in rng.permutation(len(cb))]
+    cd = [cd[i] for i in rng.permutation(len(cd))]
+    q = list(rng.permutation(oa + ob + od))
+    net = Network(oa + ob + od, cuts, [ca, cb, cd], [[int(x) for x in q[:oa]], [int(x) for x in q[oa:oa + ob]],
+                                                      [int(x) for x in q[oa + ob:]]], name=f"tri{na}{nb}{ni}")
+    net.validate()
+    return net
+
+
+def _run(net, T, bits, **kw):
+    plan = tqc.tqc_plan(net, tqc.MODE_STATES, **kw)
+    for s, t in enumerate(T):
+        tqc.tqc_load_subcircuit_tensors(plan, s, t)
+    st = torch.from_numpy(pack_states(bits).view(np.int64)).cuda()
+    out = tqc.tqc_contract_states(plan, st)
+    torch.cuda.synchronize()
+    return out.cpu().numpy().astype(np.float64), plan
+
+
+@pytest.mark.parametrize("na,nb,ni,B", [(4, 2, 3, 67), (2, 4, 3, 33), (4, 3, 3, 40), (4, 4, 3, 9), (5, 2, 4, 21), (4, 2, 5, 16)])
+def test_tc_step_leaf_times_leaf(na, nb, ni, B):
+    net = _triangle(na, nb, ni)
+    T = random_tensors(net, 1000 + na * 100 + nb * 10 + ni)
+    bits = random_states(net.n_qubits, B, 5)
+    order = [(0, 1), (3, 2)]
+    got, plan = _run(net, T, bits, order=order, batch_hint=4)
+    assert plan.step(0)["kernel_class"] == KERNEL_TCGEN05
+    want, _ = direct_sum_c(net, T, bits)
+    err = np.abs(got - want).max() / want.max()
+    assert err <= TOL, err
+    ffma, plan2 = _run(net, T, bits, order=order, batch_hint=4, use_tcgen05=-1)
+    assert plan2.step(0)["kernel_class"] != KERNEL_TCGEN05
+    assert np.abs(got - ffma).max() / want.max() <= 3e-6
+
+
+def test_tc_step_with_batch_operand_and_signed_values():
+    """4 subcircuits: (A,B) first (FFMA, small), then (AB, C) as a tensor-pipe step whose lhs is a per-state
+    intermediate; signed values exercise the hi/lo split with cancellation."""
+    # A-B: 2 cuts; A-C: 2 cuts, B-C: 1 cut (inner of step 2 = 3 cuts); A-D: 2, B-D: 2 (outer lhs = 4 cuts); C-D: 2 (outer rhs)
+    cuts = [(0, 1), (1, 0), (0, 2), (2, 0), (1, 2), (0, 3), (3, 0), (1, 3), (3, 1), (2, 3), (3, 2)]
+    sub = [[0, 1, 2, 3, 5, 6], [0, 1, 4, 7, 8], [2, 3, 4, 9, 10], [5, 6, 7, 8, 9, 10]]
+    net = Network(14, cuts, sub, [[0, 1, 2, 3], [4, 5, 6, 7], [8, 9, 10, 11], [12, 13]], name="quad")
+    net.validate()
+    rng = np.random.default_rng(3)
+    T = [(rng.random(net.tensor_shape(s)) * 2 - 1).astype(np.float32) for s in range(net.m)]
+    bits = random_states(14, 50, 6)
+    order = [(0, 1), (4, 2), (5, 3)]
+    got, plan = _run(net, T, bits, order=order, batch_hint=4)
+    assert plan.step(1)["kernel_class"] == KERNEL_TCGEN05
+    want, _ = direct_sum_c(net, T, bits)
+    assert np.abs(got - want).max() <= TOL * np.abs(want).max(), np.abs(got - want).max() / np.abs(want).max()
