@@ -125,7 +125,13 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
     __shared__ __align__(8) uint64_t full_bar[4], ready_bar[4], empty_bar[4];
     __shared__ __align__(8) uint64_t hi_full_bar[2], hi_empty_bar[2], lo_full_bar[2], lo_empty_bar[2];
     __shared__ uint32_t tmem_base_slot;
-    __shared__ uint32_t ob_tab[BN];
+    // epilogue: each warp stages 32 rows x CB columns in its own scratch and writes them out in ascending C-offset
+    // order (perm tables), so a warp store covers the longest contiguous run the consumer's digit layout allows
+    constexpr int CB = BN < 32 ? BN : 32;
+    constexpr int LB = BN < 32 ? 4 : 5;
+    __shared__ uint32_t perm_off[32 * CB];
+    __shared__ uint16_t perm_src[32 * CB];
+    __shared__ float scratch[4][32 * 33];
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int S = a.stages;
@@ -146,7 +152,27 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
     constexpr uint32_t tmem_cols = 4 * BN < 32 ? 32 : 4 * BN;      // D_hi[0], D_hi[1], D_lo[0], D_lo[1]
 
     // ---- one-time setup -------------------------------------------------------------------------
-    for (int c = threadIdx.x; c < BN; c += TC_THREADS) ob_tab[c] = (uint32_t)bitmap_apply(a.outB, (unsigned long long)c);
+    for (int e = threadIdx.x; e < 32 * CB; e += TC_THREADS) {
+        // the 5 + LB index bits of a block, ordered by the C-offset bit they map to
+        uint32_t dst[5 + LB], src[5 + LB];
+#pragma unroll
+        for (int b = 0; b < 5 + LB; ++b) {
+            const unsigned long long o = b < 5 ? bitmap_apply(a.outA, 1ull << b) : bitmap_apply(a.outB, 1ull << (b - 5));
+            dst[b] = (uint32_t)(__ffsll((long long)o) - 1);
+            src[b] = (uint32_t)b;
+        }
+#pragma unroll
+        for (int x = 1; x < 5 + LB; ++x)                     // insertion sort by destination bit
+#pragma unroll
+            for (int y = x; y > 0; --y)
+                if (dst[y] < dst[y - 1]) { uint32_t t0 = dst[y]; dst[y] = dst[y - 1]; dst[y - 1] = t0; t0 = src[y]; src[y] = src[y - 1]; src[y - 1] = t0; }
+        uint32_t off = 0, ij = 0;
+#pragma unroll
+        for (int k = 0; k < 5 + LB; ++k)
+            if ((e >> k) & 1) { off |= 1u << dst[k]; ij |= 1u << src[k]; }
+        perm_off[e] = off;
+        perm_src[e] = (uint16_t)((ij & 31u) * 33u + (ij >> 5));      // scratch index: row i5, column j5
+    }
     if (threadIdx.x == 0) {
         for (int s = 0; s < S; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&ready_bar[s], TC_SPLIT_THREADS / 32); mbar_init(&empty_bar[s], 1); }
         for (int s = 0; s < 2; ++s) {
@@ -226,7 +252,6 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
     } else if (warp < 6) {
         // ===== accumulate (round-to-nearest, registers) + epilogue =====
         const int w4 = warp & 3;
-        const int i_local = 32 * w4 + lane;
         const uint32_t lane_base = (uint32_t)(32 * w4) << 16;
         long long lt = 0, g = 0;
         for (long long t = blockIdx.x; t < total; t += gridDim.x, ++lt) {
@@ -255,7 +280,7 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
             const uint32_t lb = (uint32_t)(lt & 1), lph = (uint32_t)((lt >> 1) & 1);
             mbar_wait(&lo_full_bar[lb], lph);
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-            const unsigned long long oa = bitmap_apply(a.outA, (unsigned long long)(mt * TC_BM + i_local));
+            const unsigned long long oa = bitmap_apply(a.outA, (unsigned long long)(mt * TC_BM + 32 * w4));
             const unsigned long long obh = bitmap_apply(a.outB, (unsigned long long)(nt * BN));
             float *crow = a.C + r * a.c_row_stride + (oa | obh);
             const uint32_t laddr = tmem_base + lane_base + (2u + lb) * (uint32_t)BN;
@@ -271,13 +296,28 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
             __syncwarp();
             if (lane == 0) mbar_arrive(&lo_empty_bar[lb]);
-            if (a.vec4) {
+            float *scr = scratch[warp - 2];
 #pragma unroll
-                for (int q = 0; q < BN; q += 4)
-                    *reinterpret_cast<float4 *>(crow + ob_tab[q]) = make_float4(acc[q], acc[q + 1], acc[q + 2], acc[q + 3]);
-            } else {
+            for (int c0 = 0; c0 < BN; c0 += CB) {
+                __syncwarp();
 #pragma unroll
-                for (int q = 0; q < BN; ++q) crow[ob_tab[q]] = acc[q];
+                for (int q = 0; q < CB; ++q) scr[lane * 33 + q] = acc[c0 + q];
+                __syncwarp();
+                float *cblk = crow + bitmap_apply(a.outB, (unsigned long long)c0);
+                if (a.vec4) {
+#pragma unroll
+                    for (int p = 0; p < CB / 4; ++p) {
+                        const int e = (p * 32 + lane) * 4;
+                        *reinterpret_cast<float4 *>(cblk + perm_off[e]) =
+                            make_float4(scr[perm_src[e]], scr[perm_src[e + 1]], scr[perm_src[e + 2]], scr[perm_src[e + 3]]);
+                    }
+                } else {
+#pragma unroll
+                    for (int p = 0; p < CB; ++p) {
+                        const int e = p * 32 + lane;
+                        cblk[perm_off[e]] = scr[perm_src[e]];
+                    }
+                }
             }
         }
     } else {

@@ -318,10 +318,10 @@ int launch_tc_step(tqc_plan_t *pl, TcOperand A, TcOperand B, BitMap outA, BitMap
         int dev = 0;
         TQC_CUDA(cudaGetDevice(&dev));
         TQC_CUDA(cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev));
-        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 225 * 1024));
-        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 225 * 1024));
-        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, 225 * 1024));
-        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 225 * 1024));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 201 * 1024));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 201 * 1024));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, 201 * 1024));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 201 * 1024));
         attr = true;
     }
     auto has_bit0 = [](const BitMap &m) { for (int s = 0; s < m.n; ++s) if (m.dst[s] == 0) return true; return false; };
@@ -338,7 +338,7 @@ int launch_tc_step(tqc_plan_t *pl, TcOperand A, TcOperand B, BitMap outA, BitMap
     a.BN = (int)std::min<long long>(128, 1ll << lgN);
     a.mask_hi = 0;      // the tensor pipe ignores the low 13 mantissa bits of an fp32 word read as TF32 (measured: bit-identical)
     const size_t stage_bytes = 2 * (size_t)tqc::TC_BM * tqc::TC_BK * 4 + 2 * (size_t)a.BN * tqc::TC_BK * 4;
-    a.stages = (int)std::min<size_t>(4, (220 * 1024) / stage_bytes);
+    a.stages = (int)std::min<size_t>(4, (200 * 1024) / stage_bytes);     // + 24 KB static (epilogue scratch, tables)
     a.vec4 = (outB.n >= 1 && outB.src[0] == 0 && outB.dst[0] == 0 && outB.len[0] >= 2) ? 1 : 0;
     CUtensorMap mapA, mapB;
     int rc;
