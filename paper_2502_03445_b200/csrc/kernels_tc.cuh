@@ -5,12 +5,12 @@
 // tile is split in shared memory into a_hi (top 19 bits, exactly a TF32 value) and a_lo = a - a_hi (exact in fp32)
 // and three TF32 MMAs hi*hi + hi*lo + lo*hi accumulate in fp32 in TMEM.
 //
-// Persistent, warp-specialised CTA (one per SM), 320 threads:
+// Persistent, warp-specialised CTA (one per SM), 256 threads:
 //   warp 0      TMA producer: cp.async.bulk.tensor 3-D tiles {32 k, 128 or BN rows, 1 state} with 128-byte swizzle;
 //               the state coordinate of a LEAF/TABLE operand is the state's key (a3 gather = a TMA coordinate)
 //   warp 1      MMA issuer: one elected lane, 12 tcgen05.mma.kind::tf32 per k-block, tcgen05.commit frees the stage
 //   warps 2-5   accumulate + epilogue: tcgen05.ld -> fp32 round-to-nearest adds in registers -> scatter to C
-//   warps 6-9   splitter: fp32 tile -> hi (in place) and lo (second buffer), same swizzled byte offsets
+//   warps 6-7   splitter: fp32 tile -> hi (in place) and lo (second buffer), same swizzled byte offsets
 // Pipelines: full[s] (TMA -> splitter), ready[s] (splitter -> MMA), empty[s] (MMA -> TMA).
 // The tensor pipe's fp32 accumulator rounds toward zero on every add (measured: -5e-8 relative per accumulation,
 // profiles/r01c notes), a bias that grows with the number of k-steps.  So (i) the hi*hi products of at most
@@ -29,8 +29,8 @@ namespace tqc {
 
 constexpr int TC_BM = 128;          // UMMA M
 constexpr int TC_BK = 32;           // fp32 elements per k-block = 128 bytes = one swizzle row
-constexpr int TC_THREADS = 320;
-constexpr int TC_SPLIT_THREADS = 128;
+constexpr int TC_THREADS = 256;      // 8 warps: up to 255 registers per thread for the accumulate warps
+constexpr int TC_SPLIT_THREADS = 64;
 constexpr int TC_CHUNK_KB = 2;       // k-blocks (of 32) whose hi*hi products accumulate in TMEM before a drain
 
 struct TcArgs {
@@ -44,6 +44,7 @@ struct TcArgs {
     int stages;
     int mask_hi;                    // write the truncated hi part back in place (independent of how the MMA reads fp32 bits)
     int vec4;                       // 4 consecutive j are contiguous in C
+    int debug;                      // development knobs (TQC_TC_DEBUG): 1 no global stores, 2 no store phase, 4 no split, 8 no drains
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -118,6 +119,26 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[32]) {  
 }
 
 
+// hi/lo split of NV 16-byte vectors per thread (stride TC_SPLIT_THREADS vectors), raw tile at `addr`, lo tile `lo_ofs` bytes
+// further: lo = x - (x & 0xFFFFE000) is exact in fp32; explicit shared-space accesses, all loads issued before the math
+template <int NV>
+__device__ __forceinline__ void split_tile(uint32_t addr, uint32_t lo_ofs, bool mask_hi) {
+    uint4 x[NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v)
+        asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(x[v].x), "=r"(x[v].y), "=r"(x[v].z), "=r"(x[v].w)
+                     : "r"(addr + (uint32_t)v * (TC_SPLIT_THREADS * 16u)));
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+        const uint32_t p = addr + (uint32_t)v * (TC_SPLIT_THREADS * 16u);
+        const uint4 h = make_uint4(x[v].x & 0xFFFFE000u, x[v].y & 0xFFFFE000u, x[v].z & 0xFFFFE000u, x[v].w & 0xFFFFE000u);
+        const float l0 = __uint_as_float(x[v].x) - __uint_as_float(h.x), l1 = __uint_as_float(x[v].y) - __uint_as_float(h.y);
+        const float l2 = __uint_as_float(x[v].z) - __uint_as_float(h.z), l3 = __uint_as_float(x[v].w) - __uint_as_float(h.w);
+        asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(p + lo_ofs), "f"(l0), "f"(l1), "f"(l2), "f"(l3) : "memory");
+        if (mask_hi) asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(p), "r"(h.x), "r"(h.y), "r"(h.z), "r"(h.w) : "memory");
+    }
+}
+
 template <int BN>
 __global__ void __launch_bounds__(TC_THREADS, 1)
 step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB, const TcArgs a) {
@@ -131,7 +152,7 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
     constexpr int LB = BN < 32 ? 4 : 5;
     __shared__ uint32_t perm_off[32 * CB];
     __shared__ uint16_t perm_src[32 * CB];
-    __shared__ float scratch[4][32 * 33];
+    __shared__ __align__(16) float scratch[4][32 * 32];     // row i5: 8 float4 slots, slot (j5 >> 2) ^ bitrev3(i5 & 7)
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int S = a.stages;
@@ -171,7 +192,11 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
         for (int k = 0; k < 5 + LB; ++k)
             if ((e >> k) & 1) { off |= 1u << dst[k]; ij |= 1u << src[k]; }
         perm_off[e] = off;
-        perm_src[e] = (uint16_t)((ij & 31u) * 33u + (ij >> 5));      // scratch index: row i5, column j5
+        {
+            const uint32_t i5 = ij & 31u, j5 = ij >> 5;
+            const uint32_t rev = ((i5 & 1u) << 2) | (i5 & 2u) | ((i5 >> 2) & 1u);
+            perm_src[e] = (uint16_t)(i5 * 32u + ((((j5 >> 2) ^ rev) & 7u) << 2) + (j5 & 3u));
+        }
     }
     if (threadIdx.x == 0) {
         for (int s = 0; s < S; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&ready_bar[s], TC_SPLIT_THREADS / 32); mbar_init(&empty_bar[s], 1); }
@@ -206,6 +231,7 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
                     const int s = (int)(it % S);
                     const uint32_t ph = (uint32_t)((it / S) & 1);
                     mbar_wait(&empty_bar[s], ph ^ 1u);
+                    if (a.debug & 16) { mbar_arrive(&full_bar[s]); continue; }
                     mbar_expect_tx(&full_bar[s], bytesA + bytesB);
                     tma_load_3d(&mapA, &full_bar[s], A_raw(s), kb * TC_BK, (int)(mt * TC_BM), rowA);
                     tma_load_3d(&mapB, &full_bar[s], B_raw(s), kb * TC_BK, (int)(nt * BN), rowB);
@@ -229,17 +255,31 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
                 for (int kc = 0; kc < chunk_kb; ++kc, ++kb, ++it) {
                     const int s = (int)(it % S);
                     const uint32_t ph = (uint32_t)((it / S) & 1);
-                    mbar_wait(&ready_bar[s], ph);
+                    // hi*hi reads only the raw tiles (TMA wrote them: no proxy fence needed), so it starts as soon as the
+                    // load lands and overlaps the splitter; the lo terms wait for the splitter's ready barrier
+                    mbar_wait(&full_bar[s], ph);
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                    if (lane == 0) {
-                        const uint64_t dah = umma_desc_sw128(smem_u32(A_raw(s))), dal = umma_desc_sw128(smem_u32(A_lo(s)));
-                        const uint64_t dbh = umma_desc_sw128(smem_u32(B_raw(s))), dbl = umma_desc_sw128(smem_u32(B_lo(s)));
+                    const uint64_t dah = umma_desc_sw128(smem_u32(A_raw(s))), dal = umma_desc_sw128(smem_u32(A_lo(s)));
+                    const uint64_t dbh = umma_desc_sw128(smem_u32(B_raw(s))), dbl = umma_desc_sw128(smem_u32(B_lo(s)));
+                    const bool run = !(a.debug & 32) || (kb | kc) == 0;
+                    if (lane == 0 && run) {
 #pragma unroll
                         for (int k = 0; k < TC_BK / 8; ++k) {
                             const uint64_t adv = (uint64_t)(k * 8 * 4 >> 4);       // 32 bytes per K=8 slice, 16-byte units
-                            umma_tf32(d_lo, dal + adv, dbh + adv, idesc, (kb | k) ? 1u : 0u);
-                            umma_tf32(d_lo, dah + adv, dbl + adv, idesc, 1u);
                             umma_tf32(d_hi, dah + adv, dbh + adv, idesc, (kc | k) ? 1u : 0u);
+                        }
+                    }
+                    __syncwarp();
+                    mbar_wait(&ready_bar[s], ph);
+                    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                    if (lane == 0) {
+                        if (run) {
+#pragma unroll
+                            for (int k = 0; k < TC_BK / 8; ++k) {
+                                const uint64_t adv = (uint64_t)(k * 8 * 4 >> 4);
+                                umma_tf32(d_lo, dal + adv, dbh + adv, idesc, (kb | k) ? 1u : 0u);
+                                umma_tf32(d_lo, dah + adv, dbl + adv, idesc, 1u);
+                            }
                         }
                         umma_commit(&empty_bar[s]);                                 // frees the stage when these MMAs retire
                         if (kc == chunk_kb - 1) umma_commit(&hi_full_bar[hb]);
@@ -253,6 +293,10 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
         // ===== accumulate (round-to-nearest, registers) + epilogue =====
         const int w4 = warp & 3;
         const uint32_t lane_base = (uint32_t)(32 * w4) << 16;
+        const uint32_t lane_rev = (((uint32_t)lane & 1u) << 2) | ((uint32_t)lane & 2u) | (((uint32_t)lane >> 2) & 1u);
+        uint32_t rd_ofs[CB / 4], st_ofs[CB / 4];           // this lane's float4 slots of a block, in ascending C-offset order
+#pragma unroll
+        for (int p = 0; p < CB / 4; ++p) { rd_ofs[p] = perm_src[(p * 32 + lane) * 4]; st_ofs[p] = perm_off[(p * 32 + lane) * 4]; }
         long long lt = 0, g = 0;
         for (long long t = blockIdx.x; t < total; t += gridDim.x, ++lt) {
             const long long nt = t % tiles_n, mt = (t / tiles_n) % tiles_m, r = t / (tiles_n * tiles_m);
@@ -264,6 +308,7 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
                 mbar_wait(&hi_full_bar[hb], hph);
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                 const uint32_t taddr = tmem_base + lane_base + hb * (uint32_t)BN;
+                if (!(a.debug & 8))
 #pragma unroll
                 for (int c0 = 0; c0 < BN; c0 += 32) {
                     uint32_t v[32];
@@ -297,19 +342,21 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
             __syncwarp();
             if (lane == 0) mbar_arrive(&lo_empty_bar[lb]);
             float *scr = scratch[warp - 2];
+            if (a.debug & 2) continue;
 #pragma unroll
             for (int c0 = 0; c0 < BN; c0 += CB) {
                 __syncwarp();
 #pragma unroll
-                for (int q = 0; q < CB; ++q) scr[lane * 33 + q] = acc[c0 + q];
+                for (int k = 0; k < CB / 4; ++k)
+                    *reinterpret_cast<float4 *>(scr + lane * 32 + (((uint32_t)k ^ lane_rev) << 2)) =
+                        make_float4(acc[c0 + 4 * k], acc[c0 + 4 * k + 1], acc[c0 + 4 * k + 2], acc[c0 + 4 * k + 3]);
                 __syncwarp();
                 float *cblk = crow + bitmap_apply(a.outB, (unsigned long long)c0);
                 if (a.vec4) {
 #pragma unroll
                     for (int p = 0; p < CB / 4; ++p) {
-                        const int e = (p * 32 + lane) * 4;
-                        *reinterpret_cast<float4 *>(cblk + perm_off[e]) =
-                            make_float4(scr[perm_src[e]], scr[perm_src[e + 1]], scr[perm_src[e + 2]], scr[perm_src[e + 3]]);
+                        const float4 val = *reinterpret_cast<const float4 *>(scr + rd_ofs[p]);
+                        if (!(a.debug & 1) || val.x == 123.456f) *reinterpret_cast<float4 *>(cblk + st_ofs[p]) = val;
                     }
                 } else {
 #pragma unroll
@@ -331,18 +378,12 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
                 const uint32_t ph = (uint32_t)((it / S) & 1);
                 mbar_wait(&full_bar[s], ph);
                 // per stage: [A_raw][A_lo][B_raw][B_lo]; element e of a raw tile and of its lo tile share the swizzled offset
-                constexpr int nva = (int)(bytesA >> 4), nvb = (int)(bytesB >> 4);
-#pragma unroll 2
-                for (int e = st; e < nva + nvb; e += TC_SPLIT_THREADS) {
-                    uint4 *xp = e < nva ? reinterpret_cast<uint4 *>(A_raw(s)) + e : reinterpret_cast<uint4 *>(B_raw(s)) + (e - nva);
-                    float4 *lp = e < nva ? reinterpret_cast<float4 *>(A_lo(s)) + e : reinterpret_cast<float4 *>(B_lo(s)) + (e - nva);
-                    const uint4 x = *xp;
-                    const uint4 h = make_uint4(x.x & 0xFFFFE000u, x.y & 0xFFFFE000u, x.z & 0xFFFFE000u, x.w & 0xFFFFE000u);
-                    *lp = make_float4(__uint_as_float(x.x) - __uint_as_float(h.x), __uint_as_float(x.y) - __uint_as_float(h.y),
-                                      __uint_as_float(x.z) - __uint_as_float(h.z), __uint_as_float(x.w) - __uint_as_float(h.w));
-                    if (mask_hi) *xp = h;
-                }
-                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // generic-proxy writes -> visible to the MMA's async proxy
+                const uint32_t sa = smem_u32(A_raw(s)) + (uint32_t)st * 16u;
+                if (!(a.debug & 4))
+                split_tile<(int)(bytesA >> 4) / TC_SPLIT_THREADS>(sa, bytesA, mask_hi);
+                if (!(a.debug & 4))
+                split_tile<(int)(bytesB >> 4) / TC_SPLIT_THREADS>(sa + 2u * bytesA, bytesB, mask_hi);
+                if (!(a.debug & 64)) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // generic-proxy writes -> visible to the MMA's async proxy
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&ready_bar[s]);
             }

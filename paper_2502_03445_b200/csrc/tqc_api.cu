@@ -336,6 +336,7 @@ int launch_tc_step(tqc_plan_t *pl, TcOperand A, TcOperand B, BitMap outA, BitMap
     a.outA = outA; a.outB = outB;
     a.lgM = lgM; a.lgN = lgN; a.lgK = lgK; a.R = R;
     a.BN = (int)std::min<long long>(128, 1ll << lgN);
+    { const char *dbg = std::getenv("TQC_TC_DEBUG"); a.debug = dbg ? std::atoi(dbg) : 0; }
     a.mask_hi = 0;      // the tensor pipe ignores the low 13 mantissa bits of an fp32 word read as TF32 (measured: bit-identical)
     const size_t stage_bytes = 2 * (size_t)tqc::TC_BM * tqc::TC_BK * 4 + 2 * (size_t)a.BN * tqc::TC_BK * 4;
     a.stages = (int)std::min<size_t>(4, (200 * 1024) / stage_bytes);     // + 24 KB static (epilogue scratch, tables)
