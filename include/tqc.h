@@ -52,8 +52,10 @@ enum { TQC_MODE_STATES = 0, TQC_MODE_DISTRIBUTION = 1 };
 /* Kernel class chosen per plan step (integer thresholds):
  * SIMT_TILE  register-tiled fp32 FFMA contraction (any shape);
  * DOT        final reduction: no outer cuts left, one dot product over the merged bond per state;
- * TCGEN05    3xTF32 tcgen05.mma / TMEM / TMA contraction for steps with large outer dimensions. */
-enum { TQC_KERNEL_SIMT_TILE = 0, TQC_KERNEL_DOT = 1, TQC_KERNEL_TCGEN05 = 2 };
+ * TCGEN05    3xTF32 tcgen05.mma / TMEM / TMA contraction for steps with large outer dimensions;
+ * CHAIN      the step is part of the fused small-bond chain: all per-state steps of the plan run in one kernel, one
+ *            warp per state, intermediates in shared memory, bond sums finished by warp shuffles. */
+enum { TQC_KERNEL_SIMT_TILE = 0, TQC_KERNEL_DOT = 1, TQC_KERNEL_TCGEN05 = 2, TQC_KERNEL_CHAIN = 3 };
 /* How a node of the contraction tree is evaluated. */
 enum { TQC_NODE_LEAF = 0, TQC_NODE_TABLE = 1, TQC_NODE_BATCH = 2 };
 
@@ -84,6 +86,7 @@ typedef struct {
                                        once per state.  Any n_states is still legal at contract time. */
     int32_t table_log2_floats_max;  /* 0 = default 24: cap on log2(entries) of such a table */
     int32_t use_tcgen05;            /* 0 = default (on where a step qualifies), -1 = never (fp32 FFMA everywhere) */
+    int32_t use_chain;              /* 0 = default (fused chain kernel when every per-state step is small), -1 = never */
 } tqc_plan_opts;
 
 /* ---- planning (host only; no CUDA call) -------------------------------------------------

@@ -29,7 +29,9 @@ EXPORTED = ["tqc_plan", "tqc_plan_destroy", "tqc_plan_mode", "tqc_plan_num_qubit
             "tqc_plan_num_cuts", "tqc_plan_num_steps", "tqc_plan_kmax", "tqc_plan_tensor_shape", "tqc_plan_step",
             "tqc_plan_node", "tqc_plan_cost_log2", "tqc_plan_serialize", "tqc_plan_workspace_bytes",
             "tqc_plan_workspace_min_bytes", "tqc_load_subcircuit_tensors", "tqc_contract_states",
-            "tqc_contract_distribution", "tqc_plan_launch_count", "tqc_last_error", "tqc_version"]
+            "tqc_contract_distribution", "tqc_plan_launch_count", "tqc_last_error", "tqc_version",
+            "tqc_plan_workspace_bytes_host", "tqc_contract_states_host", "tqc_contract_distribution_host",
+            "tqc_plan_profile_enable", "tqc_plan_profile_read"]
 
 
 class TqcError(RuntimeError):
@@ -48,7 +50,7 @@ class _NetworkDesc(ctypes.Structure):
 class _PlanOpts(ctypes.Structure):
     _fields_ = [("mode", c_int32), ("n_order_steps", c_int32), ("order", POINTER(c_int32)),
                 ("restarts", c_int32), ("seed", c_uint64), ("batch_hint", c_int64),
-                ("table_log2_floats_max", c_int32), ("use_tcgen05", c_int32)]
+                ("table_log2_floats_max", c_int32), ("use_tcgen05", c_int32), ("use_chain", c_int32)]
 
 
 def lib_path() -> str:
@@ -202,7 +204,7 @@ class Plan:
 
 
 def tqc_plan(net, mode: int = MODE_STATES, order=None, restarts: int = 0, seed: int = 0, batch_hint: int = 0,
-             table_log2_floats_max: int = 0, use_tcgen05: int = 0) -> Plan:
+             table_log2_floats_max: int = 0, use_tcgen05: int = 0, use_chain: int = 0) -> Plan:
     """net: any object with n_qubits, cuts [(up, down)], sub_cuts [[cut ids]], sub_qubits [[qubit ids]]
     (e.g. tqc_inputs.Network).  order: optional list of m-1 (lhs, rhs) node-id pairs."""
     m = len(net.sub_cuts)
@@ -215,7 +217,7 @@ def tqc_plan(net, mode: int = MODE_STATES, order=None, restarts: int = 0, seed: 
     desc = _NetworkDesc(net.n_qubits, m, len(net.cuts), up_p, down_p, cofs_p, cflat_p, qofs_p, qflat_p)
     oflat, oflat_p = _i32(v for ab in (order or []) for v in ab)
     opts = _PlanOpts(mode, len(order) if order else 0, oflat_p, restarts, seed, batch_hint,
-                     table_log2_floats_max, use_tcgen05)
+                     table_log2_floats_max, use_tcgen05, use_chain)
     h = c_void_p()
     _check(_lib.tqc_plan(byref(desc), byref(opts), byref(h)))
     return Plan(h.value)

@@ -14,6 +14,7 @@
 #include "device_args.h"
 #include "kernels_simt.cuh"
 #include "kernels_tc.cuh"
+#include "kernels_chain.cuh"
 #include "plan.hpp"
 
 namespace {
@@ -63,6 +64,12 @@ int index_of(const std::vector<int> &v, int x) {
 struct tqc_plan {
     tqc::HostPlan hp;
     int use_tcgen05 = 0;
+    // fused small-bond chain (kernels_chain.cuh): the per-state steps as one device step table
+    bool chain = false;
+    std::vector<tqc::ChainStep> chain_host;
+    std::vector<int> chain_leafA, chain_leafB;     // leaf id whose device pointer fills A.base / B.base (-1: none)
+    tqc::ChainStep *d_chain = nullptr;
+    int chain_scratch = 0;
     std::vector<float *> d_leaf;
     std::vector<char> loaded;
     int32_t *d_slot_ofs = nullptr, *d_slot_qubits = nullptr;
@@ -86,7 +93,7 @@ using tqc::Step;
 constexpr int kMaxDynSmem = 200 * 1024;
 
 // Tags of profiled launches: step index t >= 0, or one of these.
-enum { TAG_KEYS = -1, TAG_GATHER = -2, TAG_RELAYOUT = -3 };
+enum { TAG_KEYS = -1, TAG_GATHER = -2, TAG_RELAYOUT = -3, TAG_CHAIN = -4 };
 
 int prof_event(tqc_plan_t *pl, cudaStream_t st) {
     if (pl->ev_used == pl->ev_pool.size()) {
@@ -404,6 +411,98 @@ int launch_batch_step(tqc_plan_t *pl, const BatchCtx &bx, int t, cudaStream_t st
     return launch_tile(pl, a, t, st);
 }
 
+// ---- fused chain: plan-time step table --------------------------------------------------------
+// Eligible when every per-state (BATCH) step has at most 1024 outputs and small operands, so that all intermediates
+// of one state fit a warp's shared-memory scratch.
+bool build_chain(tqc_plan_t *pl) {
+    const HostPlan &hp = pl->hp;
+    if (hp.mode != TQC_MODE_STATES || hp.m < 2 || hp.nodes[hp.root()].kind != tqc::NODE_BATCH) return false;
+    std::vector<int> bsteps;
+    for (int t = 0; t < hp.m - 1; ++t) if (hp.nodes[hp.m + t].kind == tqc::NODE_BATCH) bsteps.push_back(t);
+    if (bsteps.empty() || (int)bsteps.size() > tqc::CHAIN_MAX_STEPS) return false;
+    auto pad = [](long long floats, int lgK) { return lgK >= 2 ? floats + ((floats >> lgK) << 2) : floats; };
+    long long stageA = 0, stageB = 0;
+    std::vector<tqc::ChainStep> tab;
+    std::vector<int> leafA, leafB;
+    std::vector<long long> node_ofs(hp.nodes.size(), -1);
+    // pass 1: shapes, staging sizes
+    for (int t : bsteps) {
+        const Step &s = hp.steps[t];
+        const int lgM = 2 * (int)s.outer_lhs.size(), lgN = 2 * (int)s.outer_rhs.size(), lgK = 2 * (int)s.inner.size();
+        if (lgM + lgN > 10) return false;
+        tqc::ChainStep cs;
+        memset(&cs, 0, sizeof(cs));
+        cs.lgM = lgM; cs.lgN = lgN; cs.lgK = lgK;
+        int la = -1, lb = -1;
+        for (int side = 0; side < 2; ++side) {
+            const int v = side ? s.rhs : s.lhs;
+            const Node &nd = hp.nodes[v];
+            tqc::ChainOperand &o = side ? cs.B : cs.A;
+            const int lgRows = side ? lgN : lgM, lgOther = side ? lgM : lgN;
+            const long long floats = 1ll << (lgRows + lgK);
+            o.table_ofs = -1;
+            if (nd.kind == tqc::NODE_BATCH) {
+                if (floats > 4096) return false;
+                o.gathered = 0;
+                o.pitch = (1 << lgK) + (lgK >= 2 ? 4 : 0);
+            } else {
+                o.gathered = 1;
+                o.key_slot = nd.key_slot;
+                if (v < hp.m) (side ? lb : la) = v; else o.table_ofs = nd.table_offset;
+                const bool reuse = lgOther > 0;
+                o.staged = (reuse && floats >= 4 && floats <= 2048) ? 1 : 0;
+                if (!o.staged && reuse && floats > 16384) return false;
+                o.pitch = (1 << lgK) + ((o.staged && lgK >= 2) ? 4 : 0);
+                if (o.staged) (side ? stageB : stageA) = std::max(side ? stageB : stageA, pad(floats, lgK));
+            }
+        }
+        tab.push_back(cs); leafA.push_back(la); leafB.push_back(lb);
+    }
+    // pass 2: scratch layout [stage A][stage B][intermediates...], result scatter maps
+    auto align4 = [](long long v) { return (v + 3) / 4 * 4; };
+    long long top = align4(stageA) + align4(stageB);
+    for (size_t x = 0; x < bsteps.size(); ++x) {
+        const int t = bsteps[x];
+        const Step &s = hp.steps[t];
+        const int vc = hp.m + t;
+        const Node &C = hp.nodes[vc];
+        tqc::ChainStep &cs = tab[x];
+        if (cs.A.gathered) cs.A.smem_ofs = 0; else cs.A.smem_ofs = (int)node_ofs[s.lhs];
+        if (cs.B.gathered) cs.B.smem_ofs = (int)align4(stageA); else cs.B.smem_ofs = (int)node_ofs[s.rhs];
+        if ((!cs.A.gathered && cs.A.smem_ofs < 0) || (!cs.B.gathered && cs.B.smem_ofs < 0)) return false;
+        if (vc == hp.root()) { cs.c_smem_ofs = -1; cs.c_lgK = 0; }
+        else {
+            const int c_lgK = 2 * (int)hp.steps[C.consumer].inner.size();
+            const long long floats = 1ll << (2 * (int)C.open.size());
+            if (floats > 4096) return false;
+            cs.c_smem_ofs = (int)top; cs.c_lgK = c_lgK;
+            node_ofs[vc] = top;
+            top += align4(pad(floats, c_lgK));
+        }
+        BitPairs pa, pb;
+        add_digit_scatter(pa, s.outer_lhs, C.layout);
+        add_digit_scatter(pb, s.outer_rhs, C.layout);
+        if (!pa.build(cs.outA) || !pb.build(cs.outB)) return false;
+    }
+    if (top > 2560) return false;                    // 10 KB of scratch per warp
+    pl->chain_host = tab; pl->chain_leafA = leafA; pl->chain_leafB = leafB;
+    pl->chain_scratch = (int)top;
+    return true;
+}
+
+int ensure_chain(tqc_plan_t *pl) {
+    if (!pl->chain || pl->d_chain) return 0;
+    std::vector<tqc::ChainStep> tab = pl->chain_host;
+    for (size_t x = 0; x < tab.size(); ++x) {
+        if (pl->chain_leafA[x] >= 0) tab[x].A.base = pl->d_leaf[pl->chain_leafA[x]];
+        if (pl->chain_leafB[x] >= 0) tab[x].B.base = pl->d_leaf[pl->chain_leafB[x]];
+    }
+    TQC_CUDA(cudaMalloc(&pl->d_chain, tab.size() * sizeof(tqc::ChainStep)));
+    TQC_CUDA(cudaMemcpy(pl->d_chain, tab.data(), tab.size() * sizeof(tqc::ChainStep), cudaMemcpyHostToDevice));
+    TQC_CUDA(cudaFuncSetAttribute(tqc::chain_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+    return 0;
+}
+
 int ensure_meta(tqc_plan_t *pl) {
     if (pl->d_slot_ofs || pl->hp.mode != TQC_MODE_STATES || pl->hp.n_key_slots == 0) return 0;
     const HostPlan &hp = pl->hp;
@@ -464,6 +563,11 @@ int tqc_plan(const tqc_network_desc *net, const tqc_plan_opts *opts, tqc_plan_t 
         if (batch && use_tc >= 0 && tc_eligible(2 * (int)s.outer_lhs.size(), 2 * (int)s.outer_rhs.size(), 2 * (int)s.inner.size()))
             s.kernel_class = TQC_KERNEL_TCGEN05;
     }
+    pl->chain = (opts ? opts->use_chain : 0) >= 0 && build_chain(pl);
+    if (pl->chain) pl->hp.ws_floats_per_state = 0;          // intermediates live in shared memory
+    if (pl->chain)
+        for (int t = 0; t < pl->hp.m - 1; ++t)
+            if (pl->hp.nodes[pl->hp.m + t].kind == tqc::NODE_BATCH) pl->hp.steps[t].kernel_class = TQC_KERNEL_CHAIN;
     *out = pl;
     return 0;
 }
@@ -474,6 +578,7 @@ void tqc_plan_destroy(tqc_plan_t *pl) {
     if (pl->d_slot_ofs) cudaFree(pl->d_slot_ofs);
     if (pl->d_slot_qubits) cudaFree(pl->d_slot_qubits);
     if (pl->d_staging) cudaFree(pl->d_staging);
+    if (pl->d_chain) cudaFree(pl->d_chain);
     for (cudaEvent_t e : pl->ev_pool) cudaEventDestroy(e);
     delete pl;
 }
@@ -626,6 +731,7 @@ int tqc_contract_states(tqc_plan_t *pl, const uint64_t *states_dev, size_t n_sta
     float *batch = (float *)(ws + fixed + align256((size_t)hp.n_key_slots * 4 * (size_t)cap));
     // the alignment pad of the key region is covered by the +256 of tqc_plan_workspace_bytes
     int rc;
+    if ((rc = ensure_chain(pl))) return rc;
     prof_begin(pl);
     // phase T: nodes evaluated once per key (tables), independent of the batch
     CrossCtx cx;
@@ -650,6 +756,17 @@ int tqc_contract_states(tqc_plan_t *pl, const uint64_t *states_dev, size_t n_sta
             tqc::key_kernel<<<grid, 256, 0, st>>>(ka);
             TQC_CUDA(cudaGetLastError());
         }
+        if (pl->chain) {
+            tqc::ChainArgs ca;
+            memset(&ca, 0, sizeof(ca));
+            ca.steps = pl->d_chain; ca.n_steps = (int)pl->chain_host.size();
+            ca.tables = tables; ca.keys = keys; ca.cap = cap; ca.out = bx.out; ca.R = bx.R;
+            ca.scratch_floats = pl->chain_scratch;
+            const long long blocks = std::min<long long>((bx.R + tqc::CHAIN_WARPS - 1) / tqc::CHAIN_WARPS, 148ll * 8);
+            if ((rc = note_launch(pl, TAG_CHAIN, st))) return rc;
+            tqc::chain_kernel<<<(unsigned)blocks, tqc::CHAIN_WARPS * 32, (size_t)tqc::CHAIN_WARPS * pl->chain_scratch * 4, st>>>(ca);
+            TQC_CUDA(cudaGetLastError());
+        } else
         for (int t = 0; t < hp.m - 1; ++t)
             if (hp.nodes[hp.m + t].kind == tqc::NODE_BATCH && (rc = launch_batch_step(pl, bx, t, st))) return rc;
         if (root.kind != tqc::NODE_BATCH) {
