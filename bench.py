@@ -162,6 +162,31 @@ def step_work(plan, t: int, B: int, mode_states: bool):
 
 def roofline_for(plan, tag: int, avg_ms: float, B: int, mode_states: bool, peaks: dict, traffic):
     """Roofline object for the dominant launch (tag = plan step index)."""
+    if tag == -4 and avg_ms > 0:
+        # fused chain kernel: every per-state step of the plan in one launch
+        NODE_BATCH = 2
+        flop, nbytes, seen = 0.0, 4.0 * B, set()
+        for t in range(plan.num_steps):
+            st = plan.step(t)
+            if st["kernel_class"] != 3:
+                continue
+            flop += 2.0 * (2.0 ** st["log2cost"]) * B
+            for v in (st["lhs"], st["rhs"]):
+                nd = plan.node(v)
+                if nd["kind"] != NODE_BATCH and v not in seen:          # gathered operand: distinct slices once + its keys
+                    seen.add(v)
+                    nbytes += 4.0 * min(B, 1 << nd["n_bits"]) * (4.0 ** nd["n_open"]) + 4.0 * B
+        alu_peak = SM_COUNT * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+        sec = avg_ms * 1e-3
+        t_alu, t_hbm = flop / (alu_peak * 1e12), nbytes / (peaks["hbm_gbs"] * 1e9)
+        if t_hbm > t_alu:
+            bound, peak, unit, achieved = "hbm", peaks["hbm_gbs"], "GB/s", nbytes / sec / 1e9
+        else:
+            bound, peak, unit, achieved = "alu", alu_peak, "TFLOP/s", flop / sec / 1e12
+        return {"bound": bound, "achieved": achieved, "peak": peak, "unit": unit, "frac": achieved / peak,
+                "traffic": traffic, "kernel": "chain_kernel (fused per-state chain, fp32 FFMA)", "plan_step": "all per-state steps",
+                "algorithmic_flop": flop, "algorithmic_bytes": nbytes, "avg_launch_ms": avg_ms,
+                "peak_source": peaks["source"] + (" hbm copy" if bound == "hbm" else " sm_max_mhz x 148 SMs x 128 lanes x 2")}
     if tag < 0 or avg_ms <= 0:
         return {"bound": "hbm", "achieved": None, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": None,
                 "traffic": traffic, "kernel": {-1: "key_kernel", -2: "gather_kernel"}.get(tag, "?")}

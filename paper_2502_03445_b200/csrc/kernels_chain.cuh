@@ -14,13 +14,16 @@ namespace tqc {
 constexpr int CHAIN_MAX_STEPS = 24;
 constexpr int CHAIN_WARPS = 8;                 // warps (states in flight) per block
 
+constexpr int CHAIN_MAX_GATHER = 16;
+constexpr int CHAIN_MAX_F4 = 6;                // float4 vectors per lane of one state's staged operands (768 floats)
+
 struct ChainOperand {
     const float *base;       // LEAF: its device tensor (rows of 2^{lgRows+lgK} floats)
     long long table_ofs;     // TABLE: float offset inside the workspace's table region (-1 otherwise)
     int gathered;            // 1: LEAF or TABLE row selected by the state's key; 0: intermediate in shared memory
     int key_slot;            // gathered: row = keys[key_slot * cap + r]
-    int smem_ofs;            // float offset in the warp's scratch: staging area (gathered, staged) or the intermediate itself
-    int staged;              // gathered operand copied to shared memory first (it is reused by several outputs)
+    int smem_ofs;            // float offset in the warp's scratch (staged gather or intermediate)
+    int staged;              // gathered operand copied to shared memory at the start of the state
     int pitch;               // floats between consecutive rows where the inner loop reads it (K, or K + 4 in shared memory)
 };
 
@@ -29,100 +32,179 @@ struct ChainStep {
     int lgM, lgN, lgK;
     int c_smem_ofs;          // result: float offset in the warp's scratch, or -1: the root, written to out[r]
     int c_lgK;               // log2 of the row length the consumer reads the result with (rows are padded by 4 floats)
+    int tab_ofs;             // offset of this step's index tables in the block's u16 table area: [M entries][N entries]
     BitMap outA, outB;       // i -> bits of the result's linear index, j -> bits (disjoint)
+};
+
+struct ChainGather {         // one staged operand: all of them are fetched together when a warp starts a state
+    const float *base;
+    long long table_ofs;
+    int key_slot, lg_floats, lgK, smem_ofs, f4_begin;
 };
 
 struct ChainArgs {
     const ChainStep *steps;  // DEVICE [n_steps]
     int n_steps;
+    int n_slots;             // key slots of the plan (<= 32 for the chain kernel)
+    int n_gather, total_f4;
+    ChainGather g[CHAIN_MAX_GATHER];
     const float *tables;     // states-mode table region of the workspace
     const uint32_t *keys;    // [n_slots][cap]
     long long cap;
     float *out;
     int R;
     int scratch_floats;      // per warp
+    int tab_entries;         // u16 index-table entries per block
 };
 
 // index of element x of a padded intermediate: rows of 2^lgK floats, 4 floats of padding per row (bank spread for float4 reads)
 __device__ __forceinline__ int chain_pad(int x, int lgK) { return lgK >= 2 ? x + ((x >> lgK) << 2) : x; }
 
-__device__ __forceinline__ float dot_range(const float *pa, const float *pb, int k_lo, int k_hi) {
+// KS floats of the bond per lane and output: fully unrolled float4 loads for the common small bonds
+template <int KS>
+__device__ __forceinline__ float dot_fixed(const float *pa, const float *pb) {
+    if (KS < 4) {
+        float s = 0.f;
+#pragma unroll
+        for (int k = 0; k < KS; ++k) s = fmaf(pa[k], pb[k], s);
+        return s;
+    }
     float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
-    if (k_hi - k_lo >= 4) {
-        for (int k = k_lo; k < k_hi; k += 4) {
-            const float4 x = *reinterpret_cast<const float4 *>(pa + k), y = *reinterpret_cast<const float4 *>(pb + k);
-            s0 = fmaf(x.x, y.x, s0); s1 = fmaf(x.y, y.y, s1); s2 = fmaf(x.z, y.z, s2); s3 = fmaf(x.w, y.w, s3);
-        }
-    } else {
-        for (int k = k_lo; k < k_hi; ++k) s0 = fmaf(pa[k], pb[k], s0);
+#pragma unroll
+    for (int k = 0; k < KS; k += 4) {
+        const float4 x = *reinterpret_cast<const float4 *>(pa + k), y = *reinterpret_cast<const float4 *>(pb + k);
+        s0 = fmaf(x.x, y.x, s0); s1 = fmaf(x.y, y.y, s1); s2 = fmaf(x.z, y.z, s2); s3 = fmaf(x.w, y.w, s3);
     }
     return (s0 + s1) + (s2 + s3);
 }
 
-__global__ void __launch_bounds__(CHAIN_WARPS * 32) chain_kernel(const ChainArgs a) {
-    extern __shared__ __align__(16) float chain_smem[];
+struct ChainStepCtx {           // per-step values every pass of the output loop needs
+    const float *pa, *pb;
+    const uint16_t *ta, *tb;
+    float *scr, *out_r;
+    int pitchA, pitchB, lgN, lgO, lgG, c_smem_ofs, c_lgK, lane;
+};
+
+// all outputs of one step for one state; KS = bond floats per lane (K / G), a multiple of 64 loops over 64-float pieces
+template <int KS>
+__device__ __forceinline__ void chain_outputs(const ChainStepCtx &c, int kspan) {
+    const int G = 1 << c.lgG, g = c.lane & (G - 1), per_pass = 32 >> c.lgG, n_out = 1 << c.lgO, nmask = (1 << c.lgN) - 1;
+    for (int o0 = 0; o0 < n_out; o0 += per_pass) {
+        const int o = o0 + (c.lane >> c.lgG);
+        const bool live = o < n_out;
+        const int i = o >> c.lgN, j = o & nmask;
+        float v = 0.f;
+        if (live) {
+            const float *qa = c.pa + i * c.pitchA + g * kspan, *qb = c.pb + j * c.pitchB + g * kspan;
+            if (KS <= 64) v = dot_fixed<KS>(qa, qb);
+            else for (int k = 0; k < kspan; k += 64) v += dot_fixed<64>(qa + k, qb + k);
+        }
+        for (int d = G >> 1; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+        if (live && g == 0) {
+            if (c.c_smem_ofs < 0) *c.out_r = v;
+            else c.scr[c.c_smem_ofs + chain_pad((int)(c.ta[i] | c.tb[j]), c.c_lgK)] = v;
+        }
+    }
+}
+
+__global__ void __launch_bounds__(CHAIN_WARPS * 32, 2) chain_kernel(const ChainArgs a) {
+    extern __shared__ __align__(16) unsigned char chain_smem_raw[];
+    // block layout: [step table][u16 index tables][per-warp scratch]
+    ChainStep *steps = reinterpret_cast<ChainStep *>(chain_smem_raw);
+    const size_t steps_bytes = ((size_t)a.n_steps * sizeof(ChainStep) + 15) & ~(size_t)15;
+    uint16_t *tabs = reinterpret_cast<uint16_t *>(chain_smem_raw + steps_bytes);
+    const size_t tabs_bytes = ((size_t)a.tab_entries * 2 + 15) & ~(size_t)15;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    float *scr = chain_smem + (size_t)warp * a.scratch_floats;
-    const long long n_warps = (long long)gridDim.x * CHAIN_WARPS;
-    for (long long r = (long long)blockIdx.x * CHAIN_WARPS + warp; r < a.R; r += n_warps) {
+    // gather table: for float4 number f of a state's staged operands: {source base, key slot, log2 row floats, float offset in
+    // the row, destination in the warp scratch} — the same for every state
+    uint4 *gtab = reinterpret_cast<uint4 *>(chain_smem_raw + steps_bytes + tabs_bytes);
+    const size_t gtab_bytes = (size_t)a.total_f4 * sizeof(uint4);
+    float *scr = reinterpret_cast<float *>(chain_smem_raw + steps_bytes + tabs_bytes + gtab_bytes) + (size_t)warp * a.scratch_floats;
+
+    {   // once per block: step table and result-index tables into shared memory
+        const uint32_t *src = reinterpret_cast<const uint32_t *>(a.steps);
+        uint32_t *dst = reinterpret_cast<uint32_t *>(steps);
+        for (int x = threadIdx.x; x < (int)(a.n_steps * sizeof(ChainStep) / 4); x += blockDim.x) dst[x] = src[x];
+        __syncthreads();
         for (int t = 0; t < a.n_steps; ++t) {
-            const ChainStep &s = a.steps[t];
-            const int M = 1 << s.lgM, N = 1 << s.lgN, K = 1 << s.lgK;
-            // ---- operands: shared-memory intermediate, staged gather, or direct gather ----
+            const ChainStep &s = steps[t];
+            const int M = 1 << s.lgM, N = 1 << s.lgN;
+            for (int x = threadIdx.x; x < M + N; x += blockDim.x)
+                tabs[s.tab_ofs + x] = (uint16_t)(x < M ? bitmap_apply(s.outA, (unsigned long long)x) : bitmap_apply(s.outB, (unsigned long long)(x - M)));
+        }
+        for (int f = threadIdx.x; f < a.total_f4; f += blockDim.x) {
+            int gi = 0;
+            for (int x = 1; x < a.n_gather; ++x) if (f >= a.g[x].f4_begin) gi = x;
+            const ChainGather &gg = a.g[gi];
+            const int x = (f - gg.f4_begin) * 4;
+            const unsigned long long src = (unsigned long long)((gg.table_ofs >= 0 ? a.tables + gg.table_ofs : gg.base) + x);
+            gtab[f] = make_uint4((uint32_t)src, (uint32_t)(src >> 32), (uint32_t)gg.key_slot | ((uint32_t)gg.lg_floats << 8),
+                                 (uint32_t)(gg.smem_ofs + chain_pad(x, gg.lgK)));
+        }
+        __syncthreads();
+    }
+
+    const long long n_warps = (long long)gridDim.x * CHAIN_WARPS;
+    // software pipeline over this warp's states: keys are fetched two states ahead and the staged operands one state
+    // ahead (held in registers while the current state computes), so no global-load latency sits on the critical path
+    auto load_key = [&](long long rr) -> uint32_t {
+        return (rr < a.R && lane < a.n_slots) ? a.keys[(long long)lane * a.cap + rr] : 0u;
+    };
+    float4 v[CHAIN_MAX_F4];
+    auto issue_gather = [&](uint32_t key_of_state) {
+#pragma unroll
+        for (int q = 0; q < CHAIN_MAX_F4; ++q) {
+            if (q * 32 < a.total_f4) {                                       // uniform
+                const uint4 e = gtab[min(q * 32 + lane, a.total_f4 - 1)];
+                const uint32_t key = __shfl_sync(0xffffffffu, key_of_state, e.z & 31u);
+                const float *src = reinterpret_cast<const float *>((unsigned long long)e.x | ((unsigned long long)e.y << 32)) +
+                                   ((size_t)key << (e.z >> 8));
+                v[q] = __ldg(reinterpret_cast<const float4 *>(src));
+            }
+        }
+    };
+    const long long r0 = (long long)blockIdx.x * CHAIN_WARPS + warp;
+    uint32_t mykey = load_key(r0), key_n1 = load_key(r0 + n_warps);
+    if (r0 < a.R) issue_gather(mykey);
+    for (long long r = r0; r < a.R; r += n_warps) {
+        const uint32_t key_n2 = load_key(r + 2 * n_warps);
+        __syncwarp();                                                   // the previous state's readers are done with scr
+#pragma unroll
+        for (int q = 0; q < CHAIN_MAX_F4; ++q)
+            if (q * 32 < a.total_f4 && q * 32 + lane < a.total_f4) *reinterpret_cast<float4 *>(scr + gtab[q * 32 + lane].w) = v[q];
+        if (r + n_warps < a.R) issue_gather(key_n1);                    // in flight while this state computes
+        __syncwarp();
+        for (int t = 0; t < a.n_steps; ++t) {
+            const ChainStep &s = steps[t];
+            const int K = 1 << s.lgK;
             const float *pa, *pb;
-            {
-                const ChainOperand &o = s.A;
-                if (!o.gathered) pa = scr + o.smem_ofs;
-                else {
-                    const float *g = (o.table_ofs >= 0 ? a.tables + o.table_ofs : o.base) +
-                                     ((size_t)a.keys[(long long)o.key_slot * a.cap + r] << (s.lgM + s.lgK));
-                    if (o.staged) {
-                        float *d = scr + o.smem_ofs;
-                        for (int x = lane * 4; x < M * K; x += 128)
-                            *reinterpret_cast<float4 *>(d + chain_pad(x, s.lgK)) = __ldg(reinterpret_cast<const float4 *>(g + x));
-                        pa = d;
-                    } else pa = g;
-                }
-            }
-            {
-                const ChainOperand &o = s.B;
-                if (!o.gathered) pb = scr + o.smem_ofs;
-                else {
-                    const float *g = (o.table_ofs >= 0 ? a.tables + o.table_ofs : o.base) +
-                                     ((size_t)a.keys[(long long)o.key_slot * a.cap + r] << (s.lgN + s.lgK));
-                    if (o.staged) {
-                        float *d = scr + o.smem_ofs;
-                        for (int x = lane * 4; x < N * K; x += 128)
-                            *reinterpret_cast<float4 *>(d + chain_pad(x, s.lgK)) = __ldg(reinterpret_cast<const float4 *>(g + x));
-                        pb = d;
-                    } else pb = g;
-                }
-            }
-            __syncwarp();
+            if (!s.A.gathered || s.A.staged) pa = scr + s.A.smem_ofs;
+            else pa = (s.A.table_ofs >= 0 ? a.tables + s.A.table_ofs : s.A.base) +
+                      ((size_t)__shfl_sync(0xffffffffu, mykey, s.A.key_slot) << (s.lgM + s.lgK));
+            if (!s.B.gathered || s.B.staged) pb = scr + s.B.smem_ofs;
+            else pb = (s.B.table_ofs >= 0 ? a.tables + s.B.table_ofs : s.B.base) +
+                      ((size_t)__shfl_sync(0xffffffffu, mykey, s.B.key_slot) << (s.lgN + s.lgK));
             // ---- outputs: G lanes share one output when there are fewer than 32 of them ----
-            const int lgO = s.lgM + s.lgN;
-            int lgG = lgO >= 5 ? 0 : 5 - lgO;
-            if (s.lgK - lgG < 2) lgG = s.lgK >= 2 ? s.lgK - 2 : 0;        // at least one float4 of k per lane
-            const int G = 1 << lgG, kspan = K >> lgG;
-            const int g = lane & (G - 1);
-            const int per_pass = 32 >> lgG;
-            for (int o0 = 0; o0 < (1 << lgO); o0 += per_pass) {
-                const int o = o0 + (lane >> lgG);
-                float v = 0.f;
-                const bool live = o < (1 << lgO);
-                const int i = o >> s.lgN, j = o & (N - 1);
-                if (live) v = dot_range(pa + (size_t)i * s.A.pitch, pb + (size_t)j * s.B.pitch, g * kspan, (g + 1) * kspan);
-                for (int d = G >> 1; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
-                if (live && g == 0) {
-                    if (s.c_smem_ofs < 0) a.out[r] = v;
-                    else {
-                        const int x = (int)(bitmap_apply(s.outA, (unsigned long long)i) | bitmap_apply(s.outB, (unsigned long long)j));
-                        scr[s.c_smem_ofs + chain_pad(x, s.c_lgK)] = v;
-                    }
-                }
+            ChainStepCtx c;
+            c.pa = pa; c.pb = pb; c.pitchA = s.A.pitch; c.pitchB = s.B.pitch;
+            c.lgN = s.lgN; c.lgO = s.lgM + s.lgN;
+            c.lgG = c.lgO >= 5 ? 0 : 5 - c.lgO;
+            if (s.lgK - c.lgG < 2) c.lgG = s.lgK >= 2 ? s.lgK - 2 : 0;        // at least one float4 of the bond per lane
+            c.ta = tabs + s.tab_ofs; c.tb = c.ta + (1 << s.lgM);
+            c.scr = scr; c.out_r = a.out + r; c.c_smem_ofs = s.c_smem_ofs; c.c_lgK = s.c_lgK; c.lane = lane;
+            const int kspan = K >> c.lgG;
+            switch (kspan) {
+                case 1: chain_outputs<1>(c, kspan); break;
+                case 4: chain_outputs<4>(c, kspan); break;
+                case 8: chain_outputs<8>(c, kspan); break;
+                case 16: chain_outputs<16>(c, kspan); break;
+                case 32: chain_outputs<32>(c, kspan); break;
+                case 64: chain_outputs<64>(c, kspan); break;
+                default: chain_outputs<128>(c, kspan); break;
             }
             __syncwarp();
         }
+        mykey = key_n1; key_n1 = key_n2;
     }
 }
 

@@ -69,7 +69,9 @@ struct tqc_plan {
     std::vector<tqc::ChainStep> chain_host;
     std::vector<int> chain_leafA, chain_leafB;     // leaf id whose device pointer fills A.base / B.base (-1: none)
     tqc::ChainStep *d_chain = nullptr;
-    int chain_scratch = 0;
+    std::vector<tqc::ChainGather> chain_gather;
+    std::vector<int> chain_gather_leaf;
+    int chain_scratch = 0, chain_f4 = 0, chain_tab_entries = 0;
     std::vector<float *> d_leaf;
     std::vector<char> loaded;
     int32_t *d_slot_ofs = nullptr, *d_slot_qubits = nullptr;
@@ -417,17 +419,21 @@ int launch_batch_step(tqc_plan_t *pl, const BatchCtx &bx, int t, cudaStream_t st
 bool build_chain(tqc_plan_t *pl) {
     const HostPlan &hp = pl->hp;
     if (hp.mode != TQC_MODE_STATES || hp.m < 2 || hp.nodes[hp.root()].kind != tqc::NODE_BATCH) return false;
+    if (hp.n_key_slots > 32) return false;
     std::vector<int> bsteps;
     for (int t = 0; t < hp.m - 1; ++t) if (hp.nodes[hp.m + t].kind == tqc::NODE_BATCH) bsteps.push_back(t);
     if (bsteps.empty() || (int)bsteps.size() > tqc::CHAIN_MAX_STEPS) return false;
     auto pad = [](long long floats, int lgK) { return lgK >= 2 ? floats + ((floats >> lgK) << 2) : floats; };
-    long long stageA = 0, stageB = 0;
+    auto align4 = [](long long v) { return (v + 3) / 4 * 4; };
     std::vector<tqc::ChainStep> tab;
-    std::vector<int> leafA, leafB;
+    std::vector<int> leafA, leafB, g_leaf;
+    std::vector<tqc::ChainGather> gathers;
     std::vector<long long> node_ofs(hp.nodes.size(), -1);
-    // pass 1: shapes, staging sizes
+    long long top = 0, f4 = 0, tab_entries = 0;
     for (int t : bsteps) {
         const Step &s = hp.steps[t];
+        const int vc = hp.m + t;
+        const Node &C = hp.nodes[vc];
         const int lgM = 2 * (int)s.outer_lhs.size(), lgN = 2 * (int)s.outer_rhs.size(), lgK = 2 * (int)s.inner.size();
         if (lgM + lgN > 10) return false;
         tqc::ChainStep cs;
@@ -442,34 +448,32 @@ bool build_chain(tqc_plan_t *pl) {
             const long long floats = 1ll << (lgRows + lgK);
             o.table_ofs = -1;
             if (nd.kind == tqc::NODE_BATCH) {
-                if (floats > 4096) return false;
+                if (node_ofs[v] < 0) return false;
                 o.gathered = 0;
+                o.smem_ofs = (int)node_ofs[v];
                 o.pitch = (1 << lgK) + (lgK >= 2 ? 4 : 0);
             } else {
                 o.gathered = 1;
                 o.key_slot = nd.key_slot;
                 if (v < hp.m) (side ? lb : la) = v; else o.table_ofs = nd.table_offset;
                 const bool reuse = lgOther > 0;
-                o.staged = (reuse && floats >= 4 && floats <= 2048) ? 1 : 0;
+                o.staged = (reuse && floats >= 4 && floats <= 1024) ? 1 : 0;
                 if (!o.staged && reuse && floats > 16384) return false;
                 o.pitch = (1 << lgK) + ((o.staged && lgK >= 2) ? 4 : 0);
-                if (o.staged) (side ? stageB : stageA) = std::max(side ? stageB : stageA, pad(floats, lgK));
+                if (o.staged) {
+                    if ((int)gathers.size() >= tqc::CHAIN_MAX_GATHER) return false;
+                    tqc::ChainGather gg;
+                    memset(&gg, 0, sizeof(gg));
+                    gg.table_ofs = o.table_ofs; gg.key_slot = nd.key_slot; gg.lg_floats = lgRows + lgK; gg.lgK = lgK;
+                    gg.smem_ofs = (int)top; gg.f4_begin = (int)f4;
+                    o.smem_ofs = (int)top;
+                    top += align4(pad(floats, lgK));
+                    f4 += floats / 4;
+                    gathers.push_back(gg);
+                    g_leaf.push_back(v < hp.m ? v : -1);
+                }
             }
         }
-        tab.push_back(cs); leafA.push_back(la); leafB.push_back(lb);
-    }
-    // pass 2: scratch layout [stage A][stage B][intermediates...], result scatter maps
-    auto align4 = [](long long v) { return (v + 3) / 4 * 4; };
-    long long top = align4(stageA) + align4(stageB);
-    for (size_t x = 0; x < bsteps.size(); ++x) {
-        const int t = bsteps[x];
-        const Step &s = hp.steps[t];
-        const int vc = hp.m + t;
-        const Node &C = hp.nodes[vc];
-        tqc::ChainStep &cs = tab[x];
-        if (cs.A.gathered) cs.A.smem_ofs = 0; else cs.A.smem_ofs = (int)node_ofs[s.lhs];
-        if (cs.B.gathered) cs.B.smem_ofs = (int)align4(stageA); else cs.B.smem_ofs = (int)node_ofs[s.rhs];
-        if ((!cs.A.gathered && cs.A.smem_ofs < 0) || (!cs.B.gathered && cs.B.smem_ofs < 0)) return false;
         if (vc == hp.root()) { cs.c_smem_ofs = -1; cs.c_lgK = 0; }
         else {
             const int c_lgK = 2 * (int)hp.steps[C.consumer].inner.size();
@@ -479,14 +483,18 @@ bool build_chain(tqc_plan_t *pl) {
             node_ofs[vc] = top;
             top += align4(pad(floats, c_lgK));
         }
+        cs.tab_ofs = (int)tab_entries;
+        tab_entries += (1ll << lgM) + (1ll << lgN);
         BitPairs pa, pb;
         add_digit_scatter(pa, s.outer_lhs, C.layout);
         add_digit_scatter(pb, s.outer_rhs, C.layout);
         if (!pa.build(cs.outA) || !pb.build(cs.outB)) return false;
+        tab.push_back(cs); leafA.push_back(la); leafB.push_back(lb);
     }
-    if (top > 2560) return false;                    // 10 KB of scratch per warp
+    if (top > 2560 || f4 > 32ll * tqc::CHAIN_MAX_F4 || tab_entries > 8192) return false;   // 10 KB of scratch per warp
     pl->chain_host = tab; pl->chain_leafA = leafA; pl->chain_leafB = leafB;
-    pl->chain_scratch = (int)top;
+    pl->chain_gather = gathers; pl->chain_gather_leaf = g_leaf;
+    pl->chain_scratch = (int)top; pl->chain_f4 = (int)f4; pl->chain_tab_entries = (int)tab_entries;
     return true;
 }
 
@@ -499,7 +507,7 @@ int ensure_chain(tqc_plan_t *pl) {
     }
     TQC_CUDA(cudaMalloc(&pl->d_chain, tab.size() * sizeof(tqc::ChainStep)));
     TQC_CUDA(cudaMemcpy(pl->d_chain, tab.data(), tab.size() * sizeof(tqc::ChainStep), cudaMemcpyHostToDevice));
-    TQC_CUDA(cudaFuncSetAttribute(tqc::chain_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+    TQC_CUDA(cudaFuncSetAttribute(tqc::chain_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 128 * 1024));
     return 0;
 }
 
@@ -762,9 +770,18 @@ int tqc_contract_states(tqc_plan_t *pl, const uint64_t *states_dev, size_t n_sta
             ca.steps = pl->d_chain; ca.n_steps = (int)pl->chain_host.size();
             ca.tables = tables; ca.keys = keys; ca.cap = cap; ca.out = bx.out; ca.R = bx.R;
             ca.scratch_floats = pl->chain_scratch;
+            ca.n_slots = hp.n_key_slots;
+            ca.n_gather = (int)pl->chain_gather.size(); ca.total_f4 = pl->chain_f4; ca.tab_entries = pl->chain_tab_entries;
+            for (int x = 0; x < ca.n_gather; ++x) {
+                ca.g[x] = pl->chain_gather[x];
+                if (pl->chain_gather_leaf[x] >= 0) ca.g[x].base = pl->d_leaf[pl->chain_gather_leaf[x]];
+            }
+            const size_t smem = (((size_t)ca.n_steps * sizeof(tqc::ChainStep) + 15) & ~(size_t)15) +
+                                (((size_t)ca.tab_entries * 2 + 15) & ~(size_t)15) + (size_t)ca.total_f4 * 16 +
+                                (size_t)tqc::CHAIN_WARPS * pl->chain_scratch * 4;
             const long long blocks = std::min<long long>((bx.R + tqc::CHAIN_WARPS - 1) / tqc::CHAIN_WARPS, 148ll * 8);
             if ((rc = note_launch(pl, TAG_CHAIN, st))) return rc;
-            tqc::chain_kernel<<<(unsigned)blocks, tqc::CHAIN_WARPS * 32, (size_t)tqc::CHAIN_WARPS * pl->chain_scratch * 4, st>>>(ca);
+            tqc::chain_kernel<<<(unsigned)blocks, tqc::CHAIN_WARPS * 32, smem, st>>>(ca);
             TQC_CUDA(cudaGetLastError());
         } else
         for (int t = 0; t < hp.m - 1; ++t)
