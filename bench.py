@@ -90,7 +90,7 @@ def workload_states(wl, rank: int) -> np.ndarray:
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled every 100 ms while the timed regions run."""
+    """nvidia-smi clocks / throttle reasons sampled every 20 ms while the timed regions run."""
     FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
               "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
               "clocks_event_reasons.sw_power_cap")
@@ -99,9 +99,12 @@ class ClockSampler:
         self.tmp = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits",
-                                          "-lms", "100", "-i", str(index)], stdout=self.tmp, stderr=subprocess.DEVNULL)
+                                          "-lms", "20", "-i", str(index)], stdout=self.tmp, stderr=subprocess.DEVNULL)
         except OSError:
             self.proc = None
+        t0 = time.time()
+        while self.proc is not None and time.time() - t0 < 3.0 and os.path.getsize(self.tmp.name) == 0:
+            time.sleep(0.02)                                            # first sample before the timed region starts
 
     def stop(self) -> dict:
         if self.proc is None:
@@ -212,15 +215,18 @@ def roofline_for(plan, tag: int, avg_ms: float, B: int, mode_states: bool, peaks
              else " bf16 x nominal tf32/bf16 ratio")}
 
 
-def committed_traffic(workload: str, tag: int):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture
-    (profiles/traffic.json, written by hand from the capture named there), else None."""
-    path = os.path.join(ROOT, "profiles", "traffic.json")
+def committed_traffic(workload: str, tag: int, states_per_launch: float):
+    """DRAM bytes per launch of the dominant kernel (dram__bytes_read.sum + dram__bytes_write.sum) from the committed
+    `ncu --set full` captures listed in profiles/traffic.csv, scaled to this run's states per launch; else None."""
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
     if not os.path.exists(path):
         return None
     with open(path) as f:
-        table = json.load(f)
-    return table.get(workload, {}).get(str(tag))
+        for line in f.read().splitlines()[1:]:
+            parts = line.split(",")
+            if len(parts) >= 4 and parts[0] == workload and parts[1] == str(tag):
+                return float(parts[3]) * states_per_launch / float(parts[2])
+    return None
 
 
 # ---------------------------------------------------------------------------------------------
@@ -242,8 +248,32 @@ def run_ours(args) -> None:
 
     import paper_2502_03445_b200 as tqc      # fails loudly if libtqc.so is missing
 
+    ctx = {"torch": torch, "dist": dist, "tqc": tqc, "world": world, "rank": rank, "local": local, "dev": dev}
+    line = measure(ctx, args, args.workload, args.batch, args.steps, args.warmup)
+    if rank == 0:
+        if world == 1 and args.others:
+            # the other BASELINE configs, shorter runs, same protocol (cfg5: a labelled prefix of its 10^6-state batch)
+            others = []
+            for name, batch, steps in (("cfg5", 1024, 2), ("cfg3", 0, 10), ("cfg2", 0, 10)):
+                if name == args.workload:
+                    continue
+                o = measure(ctx, args, name, batch, steps, 3)
+                others.append({k: o[k] for k in ("value", "unit", "ms_per_step", "steps", "gpu_launches", "roofline")} |
+                              {"workload": o["config"]["workload"], "e2e_value": o["e2e"]["value"]})
+            line["other_workloads"] = others
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(make_workload(args.workload, args.batch), args.cpu_seconds)
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def measure(ctx, args, workload: str, batch: int, steps: int, warmup: int):
+    """One workload through the full protocol; returns the JSON line as a dict (rank 0) or None."""
+    torch, dist, tqc = ctx["torch"], ctx["dist"], ctx["tqc"]
+    world, rank, local, dev = ctx["world"], ctx["rank"], ctx["local"], ctx["dev"]
     peaks = measured_peaks()
-    wl = make_workload(args.workload, args.batch)
+    wl = make_workload(workload, batch)
     net, B = wl["net"], wl["B"]
     states_mode = wl["mode"] == "states"
     plan = tqc.tqc_plan(net, tqc.MODE_STATES if states_mode else tqc.MODE_DISTRIBUTION, batch_hint=B,
@@ -304,13 +334,13 @@ def run_ours(args) -> None:
         return float(t.item()), plan.launch_count - l0
 
     sampler = ClockSampler(local) if rank == 0 else None
-    total_ms, launches = timed(step_device, args.steps, args.warmup)
-    e2e_ms, _ = timed(step_host, args.steps, args.warmup)
+    total_ms, launches = timed(step_device, steps, warmup)
+    e2e_ms, _ = timed(step_host, steps, warmup)
 
     # per-launch times of the same step, CUDA events on the launching stream inside the library
     plan.profile_enable(True)
     per_tag: dict = {}
-    for _ in range(args.steps):
+    for _ in range(steps):
         flush.zero_()
         step_device()
         for tag, ms in plan.profile_read():
@@ -321,28 +351,26 @@ def run_ours(args) -> None:
     torch.cuda.synchronize()
     clocks = sampler.stop() if sampler else None
 
-    ms_per_step = total_ms / args.steps
+    ms_per_step = total_ms / steps
     value = world * n_out / (ms_per_step * 1e-3)
-    e2e_value = world * n_out / (e2e_ms / args.steps * 1e-3)
+    e2e_value = world * n_out / (e2e_ms / steps * 1e-3)
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
-        return
+        return None
 
     dom = max(per_tag.items(), key=lambda kv: kv[1][0])
     dom_tag, (dom_total, dom_n) = dom
-    launches_per_step = dom_n / args.steps
+    launches_per_step = dom_n / steps
     rows_B = B / launches_per_step if states_mode else B          # a chunked batch runs the step once per chunk
     roof = roofline_for(plan, dom_tag, dom_total / dom_n, int(rows_B), states_mode, peaks,
-                        committed_traffic(wl["name"], dom_tag))
-    step_ms_sum = sum(v[0] for v in per_tag.values()) / args.steps
-    roof["share_of_step"] = (dom_total / args.steps) / step_ms_sum if step_ms_sum > 0 else None
-    kernels = {str(tag): {"ms_per_step": v[0] / args.steps, "launches_per_step": v[1] / args.steps}
+                        committed_traffic(wl["name"], dom_tag, rows_B))
+    step_ms_sum = sum(v[0] for v in per_tag.values()) / steps
+    roof["share_of_step"] = (dom_total / steps) / step_ms_sum if step_ms_sum > 0 else None
+    kernels = {str(tag): {"ms_per_step": v[0] / steps, "launches_per_step": v[1] / steps}
                for tag, v in sorted(per_tag.items())}
 
     words = (net.n_qubits + 63) // 64
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": workload_description(wl, plan), "states_per_step_per_gpu": n_out,
@@ -356,11 +384,10 @@ def run_ours(args) -> None:
         "roofline": roof,
         "kernels_ms": kernels,
     }
-    if world == 1 and not args.no_cpu_baseline:
-        line["cpu_baseline"] = cpu_baseline(wl, args.cpu_seconds)
-    print(json.dumps(line), flush=True)
-    if world > 1:
-        dist.destroy_process_group()
+    plan.close()
+    del workspace, flush, out_dev
+    torch.cuda.empty_cache()
+    return line
 
 
 def workload_description(wl, plan) -> str:
@@ -419,27 +446,57 @@ def cpu_baseline(wl, seconds: float) -> dict:
     return {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
 
 
+def oracle_run(wl, bits, order=None):
+    """One timed run of the oracle as it stands on the given states; returns (seconds, threads used)."""
+    from oracle import reconstruct as R
+    from oracle.direct_sum_c import direct_sum_c
+    t0 = time.perf_counter()
+    if wl["net"].K <= 16:
+        _, used = direct_sum_c(wl["net"], wl["tensors"], bits)
+    else:
+        R.bucket_elimination(wl["net"], wl["tensors"], bits, order=order, chunk=1)
+        used = os.cpu_count() or 1
+    return time.perf_counter() - t0, used
+
+
 def run_reference(args) -> None:
+    """The reference arm: the CPU oracle, as it stands, on rank 0's host cores; a step = a bounded sample of the batch."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
+    from oracle import reconstruct as R
     wl = make_workload(args.workload, args.batch)
-    per_step = max(2.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
-    rates, info = [], None
+    net = wl["net"]
+    cores = os.cpu_count() or 1
+    if wl["mode"] == "states":
+        bits_all = workload_states(wl, 0)
+    else:
+        idx = np.random.default_rng(1).choice(1 << net.n_qubits, size=min(1 << net.n_qubits, 1 << 16), replace=False)
+        bits_all = ((idx[:, None] >> (net.n_qubits - 1 - np.arange(net.n_qubits))[None, :]) & 1).astype(np.uint8)
+    order = R._elimination_order(net, trials=16) if net.K > 16 else None
+    per_step = max(0.5, min(20.0, 150.0 / max(1, args.steps + args.warmup)))     # seconds of oracle work per step
+    probe = 1 if net.K > 16 else min(len(bits_all), max(cores, 8))
+    dt, used = oracle_run(wl, bits_all[:probe], order)
+    n = int(max(probe, min(len(bits_all), probe * per_step / max(dt, 1e-6))))
+    total, done = 0.0, 0
     for i in range(args.warmup + args.steps):
-        rate, cores, sample = oracle_sample_rate(wl, per_step)
+        lo = (i * n) % max(1, len(bits_all) - n + 1)
+        dt, used = oracle_run(wl, bits_all[lo:lo + n], order)
         if i >= args.warmup:
-            rates.append(rate)
-        info = (cores, sample)
-    value = float(np.mean(rates))
-    n_out = wl["B"] if wl["mode"] == "states" else (1 << wl["net"].n_qubits)
+            total += dt
+            done += n
+    value = done / total
+    kind = ("direct sum over 4^%d cut assignments (C, OpenMP)" % net.K) if net.K <= 16 else \
+           ("bucket elimination (numpy float64; 4^K infeasible at K=%d)" % net.K)
+    sample = f"{kind}; {args.steps} timed steps of {n} states each from the seeded batch, {total:.1f} s"
+    n_out = wl["B"] if wl["mode"] == "states" else (1 << net.n_qubits)
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT,
             "n_gpus": int(os.environ.get("WORLD_SIZE", "1")), "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": 1e3 * n_out / value, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": 1e3 * total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload_description(wl, None), "states_per_step_per_gpu": n_out,
-                       "note": "CPU oracle on rank 0 only; ms_per_step extrapolated from the sampled rate"},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": info[0], "kind": "oracle", "sample": info[1]},
+            "config": {"workload": workload_description(wl, None), "states_per_step_per_gpu": n,
+                       "note": "CPU oracle on rank 0 only; a step is a bounded sample of the batch (states_per_step_per_gpu states)"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": used, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -448,7 +505,7 @@ def run_reference(args) -> None:
 def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg4", choices=["cfg2", "cfg3", "cfg4", "cfg5"])
@@ -458,6 +515,7 @@ def main() -> None:
     ap.add_argument("--max-workspace-gb", type=int, default=64)
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-others", dest="others", action="store_false", help="skip the secondary workloads")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
