@@ -53,7 +53,8 @@ struct ChainArgs {
     long long cap;
     float *out;
     int R;
-    int scratch_floats;      // per warp
+    int scratch_floats;      // per warp: [stage buffer 0][stage buffer 1][intermediates]
+    int stage_floats;        // one stage buffer (all staged operands of one state)
     int tab_entries;         // u16 index-table entries per block
 };
 
@@ -107,7 +108,7 @@ __device__ __forceinline__ void chain_outputs(const ChainStepCtx &c, int kspan) 
     }
 }
 
-__global__ void __launch_bounds__(CHAIN_WARPS * 32, 2) chain_kernel(const ChainArgs a) {
+__global__ void __launch_bounds__(CHAIN_WARPS * 32, 3) chain_kernel(const ChainArgs a) {
     extern __shared__ __align__(16) unsigned char chain_smem_raw[];
     // block layout: [step table][u16 index tables][per-warp scratch]
     ChainStep *steps = reinterpret_cast<ChainStep *>(chain_smem_raw);
@@ -145,13 +146,15 @@ __global__ void __launch_bounds__(CHAIN_WARPS * 32, 2) chain_kernel(const ChainA
     }
 
     const long long n_warps = (long long)gridDim.x * CHAIN_WARPS;
-    // software pipeline over this warp's states: keys are fetched two states ahead and the staged operands one state
-    // ahead (held in registers while the current state computes), so no global-load latency sits on the critical path
+    // software pipeline over this warp's states: keys are fetched two states ahead; the staged operands of the NEXT state
+    // are copied global -> shared by cp.async into the other stage buffer while the current state computes, so neither
+    // registers nor the critical path carry the gather latency
     auto load_key = [&](long long rr) -> uint32_t {
         return (rr < a.R && lane < a.n_slots) ? a.keys[(long long)lane * a.cap + rr] : 0u;
     };
-    float4 v[CHAIN_MAX_F4];
-    auto issue_gather = [&](uint32_t key_of_state) {
+    float *inter = scr + 2 * a.stage_floats;
+    auto issue_gather = [&](uint32_t key_of_state, int buf) {
+        const uint32_t dst_base = (uint32_t)__cvta_generic_to_shared(scr + buf * a.stage_floats);
 #pragma unroll
         for (int q = 0; q < CHAIN_MAX_F4; ++q) {
             if (q * 32 < a.total_f4) {                                       // uniform
@@ -159,29 +162,37 @@ __global__ void __launch_bounds__(CHAIN_WARPS * 32, 2) chain_kernel(const ChainA
                 const uint32_t key = __shfl_sync(0xffffffffu, key_of_state, e.z & 31u);
                 const float *src = reinterpret_cast<const float *>((unsigned long long)e.x | ((unsigned long long)e.y << 32)) +
                                    ((size_t)key << (e.z >> 8));
-                v[q] = __ldg(reinterpret_cast<const float4 *>(src));
+                if (q * 32 + lane < a.total_f4)
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst_base + e.w * 4u), "l"(src) : "memory");
             }
         }
+        asm volatile("cp.async.commit_group;" ::: "memory");
     };
     const long long r0 = (long long)blockIdx.x * CHAIN_WARPS + warp;
     uint32_t mykey = load_key(r0), key_n1 = load_key(r0 + n_warps);
-    if (r0 < a.R) issue_gather(mykey);
-    for (long long r = r0; r < a.R; r += n_warps) {
+    if (r0 < a.R) issue_gather(mykey, 0);
+    int buf = 0;
+    for (long long r = r0; r < a.R; r += n_warps, buf ^= 1) {
         const uint32_t key_n2 = load_key(r + 2 * n_warps);
-        __syncwarp();                                                   // the previous state's readers are done with scr
-#pragma unroll
-        for (int q = 0; q < CHAIN_MAX_F4; ++q)
-            if (q * 32 < a.total_f4 && q * 32 + lane < a.total_f4) *reinterpret_cast<float4 *>(scr + gtab[q * 32 + lane].w) = v[q];
-        if (r + n_warps < a.R) issue_gather(key_n1);                    // in flight while this state computes
+        __syncwarp();                                                   // the previous state's readers are done with the other buffer
+        if (r + n_warps < a.R) {
+            issue_gather(key_n1, buf ^ 1);                              // in flight while this state computes
+            asm volatile("cp.async.wait_group 1;" ::: "memory");
+        } else {
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+        }
         __syncwarp();
+        const float *stg = scr + buf * a.stage_floats;
         for (int t = 0; t < a.n_steps; ++t) {
             const ChainStep &s = steps[t];
             const int K = 1 << s.lgK;
             const float *pa, *pb;
-            if (!s.A.gathered || s.A.staged) pa = scr + s.A.smem_ofs;
+            if (!s.A.gathered) pa = inter + s.A.smem_ofs;
+            else if (s.A.staged) pa = stg + s.A.smem_ofs;
             else pa = (s.A.table_ofs >= 0 ? a.tables + s.A.table_ofs : s.A.base) +
                       ((size_t)__shfl_sync(0xffffffffu, mykey, s.A.key_slot) << (s.lgM + s.lgK));
-            if (!s.B.gathered || s.B.staged) pb = scr + s.B.smem_ofs;
+            if (!s.B.gathered) pb = inter + s.B.smem_ofs;
+            else if (s.B.staged) pb = stg + s.B.smem_ofs;
             else pb = (s.B.table_ofs >= 0 ? a.tables + s.B.table_ofs : s.B.base) +
                       ((size_t)__shfl_sync(0xffffffffu, mykey, s.B.key_slot) << (s.lgN + s.lgK));
             // ---- outputs: G lanes share one output when there are fewer than 32 of them ----
@@ -191,7 +202,7 @@ __global__ void __launch_bounds__(CHAIN_WARPS * 32, 2) chain_kernel(const ChainA
             c.lgG = c.lgO >= 5 ? 0 : 5 - c.lgO;
             if (s.lgK - c.lgG < 2) c.lgG = s.lgK >= 2 ? s.lgK - 2 : 0;        // at least one float4 of the bond per lane
             c.ta = tabs + s.tab_ofs; c.tb = c.ta + (1 << s.lgM);
-            c.scr = scr; c.out_r = a.out + r; c.c_smem_ofs = s.c_smem_ofs; c.c_lgK = s.c_lgK; c.lane = lane;
+            c.scr = inter; c.out_r = a.out + r; c.c_smem_ofs = s.c_smem_ofs; c.c_lgK = s.c_lgK; c.lane = lane;
             const int kspan = K >> c.lgG;
             switch (kspan) {
                 case 1: chain_outputs<1>(c, kspan); break;

@@ -71,7 +71,7 @@ struct tqc_plan {
     tqc::ChainStep *d_chain = nullptr;
     std::vector<tqc::ChainGather> chain_gather;
     std::vector<int> chain_gather_leaf;
-    int chain_scratch = 0, chain_f4 = 0, chain_tab_entries = 0;
+    int chain_scratch = 0, chain_stage = 0, chain_f4 = 0, chain_tab_entries = 0;
     std::vector<float *> d_leaf;
     std::vector<char> loaded;
     int32_t *d_slot_ofs = nullptr, *d_slot_qubits = nullptr;
@@ -429,7 +429,7 @@ bool build_chain(tqc_plan_t *pl) {
     std::vector<int> leafA, leafB, g_leaf;
     std::vector<tqc::ChainGather> gathers;
     std::vector<long long> node_ofs(hp.nodes.size(), -1);
-    long long top = 0, f4 = 0, tab_entries = 0;
+    long long top = 0, stop = 0, f4 = 0, tab_entries = 0;      // intermediates / staged operands / float4s / table entries
     for (int t : bsteps) {
         const Step &s = hp.steps[t];
         const int vc = hp.m + t;
@@ -465,9 +465,9 @@ bool build_chain(tqc_plan_t *pl) {
                     tqc::ChainGather gg;
                     memset(&gg, 0, sizeof(gg));
                     gg.table_ofs = o.table_ofs; gg.key_slot = nd.key_slot; gg.lg_floats = lgRows + lgK; gg.lgK = lgK;
-                    gg.smem_ofs = (int)top; gg.f4_begin = (int)f4;
-                    o.smem_ofs = (int)top;
-                    top += align4(pad(floats, lgK));
+                    gg.smem_ofs = (int)stop; gg.f4_begin = (int)f4;
+                    o.smem_ofs = (int)stop;
+                    stop += align4(pad(floats, lgK));
                     f4 += floats / 4;
                     gathers.push_back(gg);
                     g_leaf.push_back(v < hp.m ? v : -1);
@@ -491,10 +491,10 @@ bool build_chain(tqc_plan_t *pl) {
         if (!pa.build(cs.outA) || !pb.build(cs.outB)) return false;
         tab.push_back(cs); leafA.push_back(la); leafB.push_back(lb);
     }
-    if (top > 2560 || f4 > 32ll * tqc::CHAIN_MAX_F4 || tab_entries > 8192) return false;   // 10 KB of scratch per warp
+    if (top + 2 * stop > 3072 || f4 > 32ll * tqc::CHAIN_MAX_F4 || tab_entries > 8192) return false;   // 12 KB of scratch per warp
     pl->chain_host = tab; pl->chain_leafA = leafA; pl->chain_leafB = leafB;
     pl->chain_gather = gathers; pl->chain_gather_leaf = g_leaf;
-    pl->chain_scratch = (int)top; pl->chain_f4 = (int)f4; pl->chain_tab_entries = (int)tab_entries;
+    pl->chain_scratch = (int)(top + 2 * stop); pl->chain_stage = (int)stop; pl->chain_f4 = (int)f4; pl->chain_tab_entries = (int)tab_entries;
     return true;
 }
 
@@ -769,7 +769,7 @@ int tqc_contract_states(tqc_plan_t *pl, const uint64_t *states_dev, size_t n_sta
             memset(&ca, 0, sizeof(ca));
             ca.steps = pl->d_chain; ca.n_steps = (int)pl->chain_host.size();
             ca.tables = tables; ca.keys = keys; ca.cap = cap; ca.out = bx.out; ca.R = bx.R;
-            ca.scratch_floats = pl->chain_scratch;
+            ca.scratch_floats = pl->chain_scratch; ca.stage_floats = pl->chain_stage;
             ca.n_slots = hp.n_key_slots;
             ca.n_gather = (int)pl->chain_gather.size(); ca.total_f4 = pl->chain_f4; ca.tab_entries = pl->chain_tab_entries;
             for (int x = 0; x < ca.n_gather; ++x) {
