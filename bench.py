@@ -276,8 +276,9 @@ def measure(ctx, args, workload: str, batch: int, steps: int, warmup: int):
     wl = make_workload(workload, batch)
     net, B = wl["net"], wl["B"]
     states_mode = wl["mode"] == "states"
+    restarts = max(args.restarts, 0)
     plan = tqc.tqc_plan(net, tqc.MODE_STATES if states_mode else tqc.MODE_DISTRIBUTION, batch_hint=B,
-                        restarts=args.restarts, seed=args.plan_seed)
+                        restarts=restarts, seed=args.plan_seed)
     for s, t in enumerate(wl["tensors"]):
         tqc.tqc_load_subcircuit_tensors(plan, s, t)
     n_out = B if states_mode else (1 << net.n_qubits)
@@ -375,7 +376,7 @@ def measure(ctx, args, workload: str, batch: int, steps: int, warmup: int):
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": workload_description(wl, plan), "states_per_step_per_gpu": n_out,
                    "parallelism": f"states sharded over {world} GPU(s), tensors replicated, no collective",
-                   "l2": "flushed between timed iterations (256 MB write)", "plan_cost_log2_per_state": plan.cost_log2,
+                   "l2": "flushed between timed iterations (256 MB write)", "plan_cost_log2_per_state": plan.cost_log2, "planner_restarts": restarts,
                    "kmax": plan.kmax, "workspace_gb": ws_bytes / 2 ** 30},
         "e2e": {"value": e2e_value, "unit": UNIT,
                 "h2d_bytes_per_step": int(B * words * 8) if states_mode else 0, "d2h_bytes_per_step": int(n_out * 4)},
@@ -511,7 +512,7 @@ def main() -> None:
     ap.add_argument("--workload", default="cfg4", choices=["cfg2", "cfg3", "cfg4", "cfg5"])
     ap.add_argument("--batch", type=int, default=0, help="states per step per GPU (0: the config's own batch)")
     ap.add_argument("--restarts", type=int, default=0, help="planner restarts (0: deterministic greedy)")
-    ap.add_argument("--plan-seed", type=int, default=0)
+    ap.add_argument("--plan-seed", type=int, default=1)
     ap.add_argument("--max-workspace-gb", type=int, default=64)
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -159,3 +159,29 @@ def test_order_invariance_on_gpu():
     for order in ([(0, 1), (4, 2), (5, 3)], [(2, 3), (4, 1), (5, 0)], [(1, 2), (0, 3), (4, 5)]):
         got, _ = _gpu_states(net, T, bits, order=order)
         _assert_close(got, want)
+
+
+def test_host_buffer_entry_points_and_profile_hooks():
+    """tqc_contract_states_host / tqc_contract_distribution_host (pinned HOST buffers, the end-to-end form bench.py times)
+    give the same values as the device-pointer calls; the per-launch profile returns one entry per kernel launch."""
+    net = configs.random_network(5, 7, 91, o_lo=1, o_hi=3)
+    T = random_tensors(net, 92)
+    bits = random_states(net.n_qubits, 777, 93)
+    dev, plan = _gpu_states(net, T, bits)
+    sh = torch.from_numpy(pack_states(bits).view(np.int64)).pin_memory()
+    oh = torch.empty(bits.shape[0], dtype=torch.float32).pin_memory()
+    ws = torch.empty(plan.workspace_bytes_host(bits.shape[0]), dtype=torch.uint8, device="cuda")
+    plan.profile_enable(True)
+    l0 = plan.launch_count
+    tqc.tqc_contract_states_host(plan, sh, oh, ws)
+    torch.cuda.synchronize()
+    prof = plan.profile_read()
+    plan.profile_enable(False)
+    assert np.array_equal(oh.numpy().astype(np.float64), dev)
+    assert len(prof) == plan.launch_count - l0 and all(ms >= 0 for _, ms in prof)
+    ddev, pland = _gpu_distribution(net, T)
+    dh = torch.empty(1 << net.n_qubits, dtype=torch.float32).pin_memory()
+    wsd = torch.empty(pland.workspace_bytes_host(0, 0), dtype=torch.uint8, device="cuda")
+    tqc.tqc_contract_distribution_host(pland, dh, wsd)
+    torch.cuda.synchronize()
+    assert np.array_equal(dh.numpy().astype(np.float64), ddev)
