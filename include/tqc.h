@@ -86,7 +86,8 @@ typedef struct {
                                        once per state.  Any n_states is still legal at contract time. */
     int32_t table_log2_floats_max;  /* 0 = default 24: cap on log2(entries) of such a table */
     int32_t use_tcgen05;            /* 0 = default (on where a step qualifies), -1 = never (fp32 FFMA everywhere) */
-    int32_t use_chain;              /* 0 = default (fused chain kernel when every per-state step is small), -1 = never */
+    int32_t use_chain;              /* 0 = default (fused chain kernel when every per-state step is small, specialised for
+                                       the plan at the first contract call), -1 = never, -2 = fused but not specialised */
 } tqc_plan_opts;
 
 /* ---- planning (host only; no CUDA call) -------------------------------------------------
@@ -164,6 +165,11 @@ int tqc_contract_distribution_host(tqc_plan_t *plan, uint64_t prefix_value, int 
  * order, its tag (plan step index t >= 0; -1 key extraction; -2 root gather) and the time to the
  * next event in ms.  Call with tags = NULL to get the count in *n.  HOST arrays. */
 uint64_t tqc_plan_launch_count(const tqc_plan_t *plan);
+/* 0: the plan does not use the fused chain kernel; 1: it runs the generic (table-driven) chain kernel; 2: it runs the chain
+ * kernel specialised for this plan (the library generates the plan's steps as straight-line CUDA from its own templates
+ * in csrc/kernels_chain.cuh and compiles them with NVRTC at the first contract call; if NVRTC is not available the
+ * generic kernel runs).  note (HOST, may be NULL) receives a one-line explanation. */
+int tqc_plan_chain_status(const tqc_plan_t *plan, char *note, size_t note_len);
 int tqc_plan_profile_enable(tqc_plan_t *plan, int on);
 int tqc_plan_profile_read(tqc_plan_t *plan, int32_t *tags, float *ms, size_t *n);
 

@@ -31,7 +31,7 @@ EXPORTED = ["tqc_plan", "tqc_plan_destroy", "tqc_plan_mode", "tqc_plan_num_qubit
             "tqc_plan_workspace_min_bytes", "tqc_load_subcircuit_tensors", "tqc_contract_states",
             "tqc_contract_distribution", "tqc_plan_launch_count", "tqc_last_error", "tqc_version",
             "tqc_plan_workspace_bytes_host", "tqc_contract_states_host", "tqc_contract_distribution_host",
-            "tqc_plan_profile_enable", "tqc_plan_profile_read"]
+            "tqc_plan_profile_enable", "tqc_plan_profile_read", "tqc_plan_chain_status"]
 
 
 class TqcError(RuntimeError):
@@ -89,6 +89,7 @@ def _load() -> ctypes.CDLL:
     lib.tqc_plan_workspace_bytes_host.restype = c_size_t
     lib.tqc_contract_states_host.argtypes = [c_void_p, c_void_p, c_size_t, c_void_p, c_void_p, c_size_t, c_void_p]
     lib.tqc_contract_distribution_host.argtypes = [c_void_p, c_uint64, c_int, c_void_p, c_void_p, c_size_t, c_void_p]
+    lib.tqc_plan_chain_status.argtypes = [c_void_p, c_char_p, c_size_t]
     lib.tqc_plan_profile_enable.argtypes = [c_void_p, c_int]
     lib.tqc_plan_profile_read.argtypes = [c_void_p, c_void_p, c_void_p, POINTER(c_size_t)]
     return lib
@@ -189,6 +190,12 @@ class Plan:
 
     def workspace_bytes_host(self, n_states: int = 0, prefix_bits: int = 0) -> int:
         return int(_lib.tqc_plan_workspace_bytes_host(self._h, n_states, prefix_bits))
+
+    def chain_status(self):
+        """(0 no fused chain | 1 generic chain kernel | 2 plan-specialised chain kernel, note)."""
+        buf = ctypes.create_string_buffer(4096)
+        rc = _lib.tqc_plan_chain_status(self._h, buf, 4096)
+        return rc, buf.value.decode(errors="replace")
 
     def profile_enable(self, on: bool = True) -> None:
         _check(_lib.tqc_plan_profile_enable(self._h, 1 if on else 0))

@@ -7,7 +7,15 @@
 //   - the deposit of free output bits around a fixed prefix (a6), and
 //   - the product-order -> global-bit-order permutation of the distribution (a6, G4).
 #pragma once
+#if defined(__CUDACC_RTC__)      // run-time compilation (chain_jit.cpp): no standard headers
+typedef unsigned char uint8_t;
+typedef unsigned short uint16_t;
+typedef int int32_t;
+typedef unsigned int uint32_t;
+typedef unsigned long long uint64_t;
+#else
 #include <stdint.h>
+#endif
 
 #define TQC_MAXSEG 48
 

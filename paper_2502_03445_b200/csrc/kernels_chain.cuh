@@ -4,8 +4,10 @@
 // round-tripping through HBM.  Bond sums that have fewer than 32 outputs are split over lanes and finished with warp
 // shuffles.  The step table is plan data (built once on the host, read from global memory).
 #pragma once
+#if !defined(__CUDACC_RTC__)
 #include <cuda_runtime.h>
 #include <stdint.h>
+#endif
 
 #include "device_args.h"
 
@@ -108,7 +110,89 @@ __device__ __forceinline__ void chain_outputs(const ChainStepCtx &c, int kspan) 
     }
 }
 
-__global__ void __launch_bounds__(CHAIN_WARPS * 32, 3) chain_kernel(const ChainArgs a) {
+// Plan-specialised step (used by the run-time generated Spec): M = 2^LGM, N = 2^LGN, K = 2^LGK and both row pitches are
+// compile-time constants, so every loop unrolls and the index arithmetic folds away.  With >= 32 outputs a lane owns the
+// outputs o = lane + 32 p; they form an NI x NJ grid (NJ distinct j, NI distinct i) whose operand rows are loaded once per
+// 16-float slab of the bond and reused from registers.  With fewer outputs the bond is split over G lanes per output and
+// finished with warp shuffles.  emit(i, j, value) stores one result.
+template <int LGM, int LGN, int LGK, int PA, int PB, class Emit>
+__device__ __forceinline__ void chain_step_spec(const float *pa, const float *pb, int lane, Emit emit) {
+    constexpr int N = 1 << LGN, K = 1 << LGK, LGO = LGM + LGN, O = 1 << LGO;
+    if constexpr (O >= 32 && LGK >= 2) {
+        constexpr int PER = O / 32;
+        constexpr int NJ = N >= 32 ? (PER < N / 32 ? PER : N / 32) : 1;       // distinct j per lane (32 apart)
+        constexpr int NI = PER / NJ;                                           // distinct i per lane
+        constexpr int ISTR = N >= 32 ? 1 : 32 / N;                             // i step between a lane's rows
+        constexpr int KC = K < 16 ? K : 16;
+        const int j0 = lane & (N - 1), i0 = N >= 32 ? 0 : (lane >> LGN);
+        float acc[NI][NJ];
+#pragma unroll
+        for (int x = 0; x < NI; ++x)
+#pragma unroll
+            for (int y = 0; y < NJ; ++y) acc[x][y] = 0.f;
+#pragma unroll
+        for (int k0 = 0; k0 < K; k0 += KC) {
+            float4 b[NJ][KC / 4];
+#pragma unroll
+            for (int y = 0; y < NJ; ++y)
+#pragma unroll
+                for (int q = 0; q < KC / 4; ++q) b[y][q] = *reinterpret_cast<const float4 *>(pb + (j0 + 32 * y) * PB + k0 + 4 * q);
+#pragma unroll
+            for (int x = 0; x < NI; ++x) {
+                const int i = N >= 32 ? x : i0 + ISTR * x;
+#pragma unroll
+                for (int q = 0; q < KC / 4; ++q) {
+                    const float4 av = *reinterpret_cast<const float4 *>(pa + i * PA + k0 + 4 * q);
+#pragma unroll
+                    for (int y = 0; y < NJ; ++y) {
+                        acc[x][y] = fmaf(av.x, b[y][q].x, acc[x][y]); acc[x][y] = fmaf(av.y, b[y][q].y, acc[x][y]);
+                        acc[x][y] = fmaf(av.z, b[y][q].z, acc[x][y]); acc[x][y] = fmaf(av.w, b[y][q].w, acc[x][y]);
+                    }
+                }
+            }
+        }
+#pragma unroll
+        for (int x = 0; x < NI; ++x)
+#pragma unroll
+            for (int y = 0; y < NJ; ++y) emit(N >= 32 ? x : i0 + ISTR * x, j0 + 32 * y, acc[x][y]);
+    } else {
+        constexpr int LGG0 = LGO >= 5 ? 0 : 5 - LGO;
+        constexpr int LGG = (LGK - LGG0 < 2) ? (LGK >= 2 ? LGK - 2 : 0) : LGG0;
+        constexpr int G = 1 << LGG, KS = K >> LGG, PASS = 32 >> LGG;
+        const int g = lane & (G - 1);
+#pragma unroll
+        for (int o0 = 0; o0 < O; o0 += PASS) {
+            const int o = o0 + (lane >> LGG);
+            const bool live = o < O;
+            const int i = o >> LGN, j = o & (N - 1);
+            float v = 0.f;
+            if (live) {
+#pragma unroll
+                for (int k = 0; k < KS; k += 64)
+                    v += dot_fixed<(KS - 0 < 64 ? KS : 64)>(pa + i * PA + g * KS + k, pb + j * PB + g * KS + k);
+            }
+#pragma unroll
+            for (int d = G >> 1; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+            if (live && g == 0) emit(i, j, v);
+        }
+    }
+}
+
+// what a state's steps see: the warp's stage buffer of the current state, its intermediates, this state's keys (one per lane)
+struct ChainStateCtx {
+    const ChainArgs *a;
+    const ChainStep *steps;     // shared-memory copy of the step table
+    const uint16_t *tabs;       // result-index tables
+    const float *stg;
+    float *inter, *out_r;
+    uint32_t mykey;
+    int lane;
+};
+
+// Spec::run(ctx) executes every step of the plan for one state.  ChainInterp walks the step table; a plan-specialised Spec
+// (generated and compiled at run time by the library, chain_jit.cpp) has the same steps as straight-line code.
+template <class Spec>
+__device__ __forceinline__ void chain_body(const ChainArgs &a) {
     extern __shared__ __align__(16) unsigned char chain_smem_raw[];
     // block layout: [step table][u16 index tables][per-warp scratch]
     ChainStep *steps = reinterpret_cast<ChainStep *>(chain_smem_raw);
@@ -183,26 +267,36 @@ __global__ void __launch_bounds__(CHAIN_WARPS * 32, 3) chain_kernel(const ChainA
         }
         __syncwarp();
         const float *stg = scr + buf * a.stage_floats;
+        ChainStateCtx sc;
+        sc.a = &a; sc.steps = steps; sc.tabs = tabs; sc.stg = stg; sc.inter = inter; sc.out_r = a.out + r; sc.mykey = mykey; sc.lane = lane;
+        Spec::run(sc);
+        mykey = key_n1; key_n1 = key_n2;
+    }
+}
+
+struct ChainInterp {
+    static __device__ __forceinline__ void run(const ChainStateCtx &sc) {
+        const ChainArgs &a = *sc.a;
         for (int t = 0; t < a.n_steps; ++t) {
-            const ChainStep &s = steps[t];
+            const ChainStep &s = sc.steps[t];
             const int K = 1 << s.lgK;
             const float *pa, *pb;
-            if (!s.A.gathered) pa = inter + s.A.smem_ofs;
-            else if (s.A.staged) pa = stg + s.A.smem_ofs;
+            if (!s.A.gathered) pa = sc.inter + s.A.smem_ofs;
+            else if (s.A.staged) pa = sc.stg + s.A.smem_ofs;
             else pa = (s.A.table_ofs >= 0 ? a.tables + s.A.table_ofs : s.A.base) +
-                      ((size_t)__shfl_sync(0xffffffffu, mykey, s.A.key_slot) << (s.lgM + s.lgK));
-            if (!s.B.gathered) pb = inter + s.B.smem_ofs;
-            else if (s.B.staged) pb = stg + s.B.smem_ofs;
+                      ((size_t)__shfl_sync(0xffffffffu, sc.mykey, s.A.key_slot) << (s.lgM + s.lgK));
+            if (!s.B.gathered) pb = sc.inter + s.B.smem_ofs;
+            else if (s.B.staged) pb = sc.stg + s.B.smem_ofs;
             else pb = (s.B.table_ofs >= 0 ? a.tables + s.B.table_ofs : s.B.base) +
-                      ((size_t)__shfl_sync(0xffffffffu, mykey, s.B.key_slot) << (s.lgN + s.lgK));
+                      ((size_t)__shfl_sync(0xffffffffu, sc.mykey, s.B.key_slot) << (s.lgN + s.lgK));
             // ---- outputs: G lanes share one output when there are fewer than 32 of them ----
             ChainStepCtx c;
             c.pa = pa; c.pb = pb; c.pitchA = s.A.pitch; c.pitchB = s.B.pitch;
             c.lgN = s.lgN; c.lgO = s.lgM + s.lgN;
             c.lgG = c.lgO >= 5 ? 0 : 5 - c.lgO;
             if (s.lgK - c.lgG < 2) c.lgG = s.lgK >= 2 ? s.lgK - 2 : 0;        // at least one float4 of the bond per lane
-            c.ta = tabs + s.tab_ofs; c.tb = c.ta + (1 << s.lgM);
-            c.scr = inter; c.out_r = a.out + r; c.c_smem_ofs = s.c_smem_ofs; c.c_lgK = s.c_lgK; c.lane = lane;
+            c.ta = sc.tabs + s.tab_ofs; c.tb = c.ta + (1 << s.lgM);
+            c.scr = sc.inter; c.out_r = sc.out_r; c.c_smem_ofs = s.c_smem_ofs; c.c_lgK = s.c_lgK; c.lane = sc.lane;
             const int kspan = K >> c.lgG;
             switch (kspan) {
                 case 1: chain_outputs<1>(c, kspan); break;
@@ -215,8 +309,11 @@ __global__ void __launch_bounds__(CHAIN_WARPS * 32, 3) chain_kernel(const ChainA
             }
             __syncwarp();
         }
-        mykey = key_n1; key_n1 = key_n2;
     }
-}
+};
+
+#if !defined(__CUDACC_RTC__)
+__global__ void __launch_bounds__(CHAIN_WARPS * 32, 3) chain_kernel(const ChainArgs a) { chain_body<ChainInterp>(a); }
+#endif
 
 }  // namespace tqc

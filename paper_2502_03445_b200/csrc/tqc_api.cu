@@ -1,6 +1,9 @@
 // C ABI of libtqc.so (include/tqc.h): plan handle, tensor load, states / distribution contraction.
 // Host launch logic only; the arithmetic is in kernels_simt.cuh / kernels_tc.cuh.
+#include <cuda.h>
 #include <cuda_runtime.h>
+#include <dlfcn.h>
+#include <nvrtc.h>
 
 #include <algorithm>
 #include <cmath>
@@ -72,6 +75,10 @@ struct tqc_plan {
     std::vector<tqc::ChainGather> chain_gather;
     std::vector<int> chain_gather_leaf;
     int chain_scratch = 0, chain_stage = 0, chain_f4 = 0, chain_tab_entries = 0;
+    // plan-specialised chain kernel, generated and compiled at the first contract call (chain_jit_build)
+    int chain_mode = 0;                 // tqc_plan_opts.use_chain
+    void *jit_module = nullptr, *jit_fn = nullptr;
+    std::string jit_note;
     std::vector<float *> d_leaf;
     std::vector<char> loaded;
     int32_t *d_slot_ofs = nullptr, *d_slot_qubits = nullptr;
@@ -498,6 +505,133 @@ bool build_chain(tqc_plan_t *pl) {
     return true;
 }
 
+// ---- plan-specialised chain kernel: source generation + NVRTC + driver module ---------------------
+// The generated translation unit includes kernels_chain.cuh and defines ChainPlanSpec::run as the plan's steps in
+// straight-line form (chain_step_spec<...> per step, every shape, pitch, offset and index map a literal).
+struct JitApi {
+    void *nvrtc = nullptr;
+    nvrtcResult (*CreateProgram)(nvrtcProgram *, const char *, const char *, int, const char *const *, const char *const *) = nullptr;
+    nvrtcResult (*CompileProgram)(nvrtcProgram, int, const char *const *) = nullptr;
+    nvrtcResult (*GetProgramLogSize)(nvrtcProgram, size_t *) = nullptr;
+    nvrtcResult (*GetProgramLog)(nvrtcProgram, char *) = nullptr;
+    nvrtcResult (*GetCUBINSize)(nvrtcProgram, size_t *) = nullptr;
+    nvrtcResult (*GetCUBIN)(nvrtcProgram, char *) = nullptr;
+    nvrtcResult (*DestroyProgram)(nvrtcProgram *) = nullptr;
+    CUresult (*ModuleLoadData)(CUmodule *, const void *) = nullptr;
+    CUresult (*ModuleGetFunction)(CUfunction *, CUmodule, const char *) = nullptr;
+    CUresult (*FuncSetAttribute)(CUfunction, CUfunction_attribute, int) = nullptr;
+    CUresult (*LaunchKernel)(CUfunction, unsigned, unsigned, unsigned, unsigned, unsigned, unsigned, unsigned, CUstream, void **, void **) = nullptr;
+    CUresult (*ModuleUnload)(CUmodule) = nullptr;
+    bool ok = false;
+    std::string why;
+};
+
+JitApi &jit_api() {
+    static JitApi api;
+    static bool tried = false;
+    if (tried) return api;
+    tried = true;
+    const char *names[] = {"libnvrtc.so.12", "libnvrtc.so", "/usr/local/cuda/lib64/libnvrtc.so.12", "/usr/local/cuda/lib64/libnvrtc.so"};
+    for (const char *n : names) if ((api.nvrtc = dlopen(n, RTLD_NOW | RTLD_LOCAL))) break;
+    if (!api.nvrtc) { api.why = "libnvrtc not found"; return api; }
+#define TQC_SYM(field, sym) *(void **)(&api.field) = dlsym(api.nvrtc, sym); if (!api.field) { api.why = std::string("missing ") + sym; return api; }
+    TQC_SYM(CreateProgram, "nvrtcCreateProgram") TQC_SYM(CompileProgram, "nvrtcCompileProgram")
+    TQC_SYM(GetProgramLogSize, "nvrtcGetProgramLogSize") TQC_SYM(GetProgramLog, "nvrtcGetProgramLog")
+    TQC_SYM(GetCUBINSize, "nvrtcGetCUBINSize") TQC_SYM(GetCUBIN, "nvrtcGetCUBIN") TQC_SYM(DestroyProgram, "nvrtcDestroyProgram")
+#undef TQC_SYM
+    auto drv = [&](const char *sym, void **out) {
+        cudaDriverEntryPointQueryResult q;
+        return cudaGetDriverEntryPoint(sym, out, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess && *out;
+    };
+    if (!drv("cuModuleLoadData", (void **)&api.ModuleLoadData) || !drv("cuModuleGetFunction", (void **)&api.ModuleGetFunction) ||
+        !drv("cuFuncSetAttribute", (void **)&api.FuncSetAttribute) || !drv("cuLaunchKernel", (void **)&api.LaunchKernel) ||
+        !drv("cuModuleUnload", (void **)&api.ModuleUnload)) { api.why = "driver entry points not available"; return api; }
+    api.ok = true;
+    return api;
+}
+
+std::string bitmap_expr(const BitMap &m, const char *var) {
+    if (m.n == 0) return "0";
+    std::string e;
+    for (int s = 0; s < m.n; ++s) {
+        if (s) e += " | ";
+        e += "(((" + std::string(var) + " >> " + std::to_string((int)m.src[s]) + ") & " + std::to_string((1 << m.len[s]) - 1) + ") << " +
+             std::to_string((int)m.dst[s]) + ")";
+    }
+    return e;
+}
+
+std::string chain_source(const tqc_plan_t *pl) {
+    std::string src = "#include \"kernels_chain.cuh\"\nnamespace tqc {\nstruct ChainPlanSpec {\n"
+                      "  static __device__ __forceinline__ void run(const ChainStateCtx &c) {\n";
+    for (size_t t = 0; t < pl->chain_host.size(); ++t) {
+        const tqc::ChainStep &s = pl->chain_host[t];
+        auto operand = [&](const tqc::ChainOperand &o, const char *which, int lgRows) {
+            if (!o.gathered) return "c.inter + " + std::to_string(o.smem_ofs);
+            if (o.staged) return "c.stg + " + std::to_string(o.smem_ofs);
+            const std::string base = o.table_ofs >= 0 ? "c.a->tables + " + std::to_string(o.table_ofs) + "ll"
+                                                      : "c.steps[" + std::to_string(t) + "]." + which + ".base";
+            return "(" + base + ") + ((size_t)__shfl_sync(0xffffffffu, c.mykey, " + std::to_string(o.key_slot) + ") << " +
+                   std::to_string(lgRows + s.lgK) + ")";
+        };
+        src += "    { const float *pa = " + operand(s.A, "A", s.lgM) + ";\n      const float *pb = " + operand(s.B, "B", s.lgN) + ";\n";
+        src += "      chain_step_spec<" + std::to_string(s.lgM) + ", " + std::to_string(s.lgN) + ", " + std::to_string(s.lgK) + ", " +
+               std::to_string(s.A.pitch) + ", " + std::to_string(s.B.pitch) + ">(pa, pb, c.lane, [&](int i, int j, float v) {\n";
+        if (s.c_smem_ofs < 0) src += "        *c.out_r = v;\n";
+        else {
+            src += "        const int x = (" + bitmap_expr(s.outA, "i") + ") | (" + bitmap_expr(s.outB, "j") + ");\n";
+            src += "        c.inter[" + std::to_string(s.c_smem_ofs) + " + " +
+                   (s.c_lgK >= 2 ? "x + ((x >> " + std::to_string(s.c_lgK) + ") << 2)" : std::string("x")) + "] = v;\n";
+        }
+        src += "      });\n      __syncwarp(); }\n";
+    }
+    src += "  }\n};\n}  // namespace tqc\n"
+           "extern \"C\" __global__ void __launch_bounds__(256, 3) chain_spec_kernel(const tqc::ChainArgs a) {\n"
+           "  tqc::chain_body<tqc::ChainPlanSpec>(a);\n}\n";
+    return src;
+}
+
+// fills pl->jit_fn, or leaves it null with the reason in pl->jit_note (the interpreter kernel then runs the chain)
+void chain_jit_build(tqc_plan_t *pl) {
+    JitApi &api = jit_api();
+    if (!api.ok) { pl->jit_note = "chain kernel not specialised: " + api.why; return; }
+    Dl_info info;
+    if (!dladdr((void *)&tqc_version, &info) || !info.dli_fname) { pl->jit_note = "chain kernel not specialised: library path unknown"; return; }
+    std::string dir(info.dli_fname);
+    dir = dir.substr(0, dir.find_last_of('/')) + "/csrc";
+    const std::string src = chain_source(pl);
+    nvrtcProgram prog;
+    if (api.CreateProgram(&prog, src.c_str(), "chain_spec.cu", 0, nullptr, nullptr) != NVRTC_SUCCESS) { pl->jit_note = "nvrtcCreateProgram failed"; return; }
+    const std::string inc = "-I" + dir;
+    const char *opts[] = {"--gpu-architecture=sm_100a", "-std=c++17", inc.c_str(), "-lineinfo"};
+    const nvrtcResult rc = api.CompileProgram(prog, 4, opts);
+    if (rc != NVRTC_SUCCESS) {
+        size_t n = 0;
+        api.GetProgramLogSize(prog, &n);
+        std::string log(n, '\0');
+        if (n) api.GetProgramLog(prog, &log[0]);
+        pl->jit_note = "chain kernel not specialised: compile failed: " + log.substr(0, 2000);
+        api.DestroyProgram(&prog);
+        return;
+    }
+    size_t n = 0;
+    api.GetCUBINSize(prog, &n);
+    std::vector<char> cubin(n);
+    api.GetCUBIN(prog, cubin.data());
+    api.DestroyProgram(&prog);
+    CUmodule mod;
+    CUfunction fn;
+    if (api.ModuleLoadData(&mod, cubin.data()) != CUDA_SUCCESS) { pl->jit_note = "chain kernel not specialised: cuModuleLoadData failed"; return; }
+    if (api.ModuleGetFunction(&fn, mod, "chain_spec_kernel") != CUDA_SUCCESS ||
+        api.FuncSetAttribute(fn, CU_FUNC_ATTRIBUTE_MAX_DYNAMIC_SHARED_SIZE_BYTES, 128 * 1024) != CUDA_SUCCESS) {
+        api.ModuleUnload(mod);
+        pl->jit_note = "chain kernel not specialised: kernel not found in module";
+        return;
+    }
+    pl->jit_module = (void *)mod; pl->jit_fn = (void *)fn;
+    pl->jit_note = "chain kernel specialised for this plan (" + std::to_string(src.size()) + " bytes of generated source)";
+}
+
 int ensure_chain(tqc_plan_t *pl) {
     if (!pl->chain || pl->d_chain) return 0;
     std::vector<tqc::ChainStep> tab = pl->chain_host;
@@ -508,6 +642,7 @@ int ensure_chain(tqc_plan_t *pl) {
     TQC_CUDA(cudaMalloc(&pl->d_chain, tab.size() * sizeof(tqc::ChainStep)));
     TQC_CUDA(cudaMemcpy(pl->d_chain, tab.data(), tab.size() * sizeof(tqc::ChainStep), cudaMemcpyHostToDevice));
     TQC_CUDA(cudaFuncSetAttribute(tqc::chain_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 128 * 1024));
+    if (pl->chain_mode == 0) chain_jit_build(pl);
     return 0;
 }
 
@@ -571,8 +706,14 @@ int tqc_plan(const tqc_network_desc *net, const tqc_plan_opts *opts, tqc_plan_t 
         if (batch && use_tc >= 0 && tc_eligible(2 * (int)s.outer_lhs.size(), 2 * (int)s.outer_rhs.size(), 2 * (int)s.inner.size()))
             s.kernel_class = TQC_KERNEL_TCGEN05;
     }
-    pl->chain = (opts ? opts->use_chain : 0) >= 0 && build_chain(pl);
+    pl->chain_mode = opts ? opts->use_chain : 0;
+    pl->chain = pl->chain_mode != -1 && build_chain(pl);
     if (pl->chain) pl->hp.ws_floats_per_state = 0;          // intermediates live in shared memory
+    if (pl->chain) {
+        if (const char *dump = std::getenv("TQC_CHAIN_SRC_DUMP")) {      // development aid: the generated specialisation
+            if (FILE *f = fopen(dump, "w")) { fputs(chain_source(pl).c_str(), f); fclose(f); }
+        }
+    }
     if (pl->chain)
         for (int t = 0; t < pl->hp.m - 1; ++t)
             if (pl->hp.nodes[pl->hp.m + t].kind == tqc::NODE_BATCH) pl->hp.steps[t].kernel_class = TQC_KERNEL_CHAIN;
@@ -587,6 +728,7 @@ void tqc_plan_destroy(tqc_plan_t *pl) {
     if (pl->d_slot_qubits) cudaFree(pl->d_slot_qubits);
     if (pl->d_staging) cudaFree(pl->d_staging);
     if (pl->d_chain) cudaFree(pl->d_chain);
+    if (pl->jit_module && jit_api().ok) jit_api().ModuleUnload((CUmodule)pl->jit_module);
     for (cudaEvent_t e : pl->ev_pool) cudaEventDestroy(e);
     delete pl;
 }
@@ -781,6 +923,12 @@ int tqc_contract_states(tqc_plan_t *pl, const uint64_t *states_dev, size_t n_sta
                                 (size_t)tqc::CHAIN_WARPS * pl->chain_scratch * 4;
             const long long blocks = std::min<long long>((bx.R + tqc::CHAIN_WARPS - 1) / tqc::CHAIN_WARPS, 148ll * 8);
             if ((rc = note_launch(pl, TAG_CHAIN, st))) return rc;
+            if (pl->jit_fn) {
+                void *params[] = {&ca};
+                const CUresult lr = jit_api().LaunchKernel((CUfunction)pl->jit_fn, (unsigned)blocks, 1, 1, tqc::CHAIN_WARPS * 32, 1, 1,
+                                                           (unsigned)smem, (CUstream)st, params, nullptr);
+                if (lr != CUDA_SUCCESS) return fail(TQC_E_CUDA, "cuLaunchKernel(chain_spec_kernel) failed with code " + std::to_string((int)lr));
+            } else
             tqc::chain_kernel<<<(unsigned)blocks, tqc::CHAIN_WARPS * 32, smem, st>>>(ca);
             TQC_CUDA(cudaGetLastError());
         } else
@@ -932,5 +1080,11 @@ int tqc_plan_profile_read(tqc_plan_t *pl, int32_t *tags, float *ms, size_t *n) {
 }
 
 uint64_t tqc_plan_launch_count(const tqc_plan_t *pl) { return pl ? pl->launches : 0; }
+
+int tqc_plan_chain_status(const tqc_plan_t *pl, char *note, size_t note_len) {
+    if (!pl) return fail(TQC_E_ARG, "null plan");
+    if (note && note_len) { snprintf(note, note_len, "%s", pl->jit_note.c_str()); }
+    return !pl->chain ? 0 : (pl->jit_fn ? 2 : 1);
+}
 
 }  // extern "C"

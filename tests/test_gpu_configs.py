@@ -82,7 +82,8 @@ def test_cfg3_all_states_vs_direct_sum():
     want, _ = direct_sum_c(net, T, bits)
     assert np.abs(got - want).max() <= TOL * want.max(), (np.abs(got - want).max(), want.max())
     assert (got >= -TOL * want.max()).all()
-    assert all(s["kernel_class"] == 3 for s in plan.steps())             # the fused chain kernel ran
+    assert all(s["kernel_class"] == 3 for s in plan.steps())             # the fused chain kernel ran ...
+    assert plan.chain_status()[0] == 2, plan.chain_status()              # ... specialised for this plan
     plan2 = _loaded_plan(net, T, tqc.MODE_STATES, batch_hint=configs.BATCH[3], use_chain=-1)
     got2 = _run_states(plan2, bits)                                      # one kernel per step
     assert np.abs(got2 - want).max() <= TOL * want.max()

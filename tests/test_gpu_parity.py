@@ -69,7 +69,7 @@ def test_states_random_networks(seed):
     bits = random_states(net.n_qubits, B, 700 + seed)
     want = R.direct_sum(net, T, bits)
     for hint in (0, 4):                       # default (tables where possible) and per-state evaluation
-        for chain in (0, -1):                 # fused chain kernel / one kernel per step
+        for chain in (0, -2, -1):             # fused chain kernel specialised for the plan / generic / one kernel per step
             got, _ = _gpu_states(net, T, bits, batch_hint=hint, use_chain=chain)
             _assert_close(got, want)
 
