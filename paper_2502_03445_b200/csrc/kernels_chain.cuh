@@ -119,12 +119,18 @@ template <int LGM, int LGN, int LGK, int PA, int PB, class Emit>
 __device__ __forceinline__ void chain_step_spec(const float *pa, const float *pb, int lane, Emit emit) {
     constexpr int N = 1 << LGN, K = 1 << LGK, LGO = LGM + LGN, O = 1 << LGO;
     if constexpr (O >= 32 && LGK >= 2) {
-        constexpr int PER = O / 32;
-        constexpr int NJ = N >= 32 ? (PER < N / 32 ? PER : N / 32) : 1;       // distinct j per lane (32 apart)
-        constexpr int NI = PER / NJ;                                           // distinct i per lane
-        constexpr int ISTR = N >= 32 ? 1 : 32 / N;                             // i step between a lane's rows
+        // a lane owns an NI x NJ block of outputs: rows i0 + x * SI, columns j0 + y * SJ, with the 32 lanes laid out LI x LJ
+        // over the M x N outputs.  Shared-memory traffic per lane is (NI + NJ) rows per bond slab, so the block is kept as
+        // square as the shape allows (16 x 16 outputs: 2 x 4 instead of 8 x 1, a third fewer loads).
+        constexpr int M = 1 << LGM, PER = O / 32;
+        constexpr int LGPER = LGO - 5;
+        constexpr int LGNJ0 = (LGPER + 1) / 2;                                     // aim for NJ >= NI
+        constexpr int LGNJ = LGNJ0 > LGN ? LGN : (LGPER - LGNJ0 > LGM ? LGPER - LGM : LGNJ0);
+        constexpr int NJ = 1 << LGNJ, NI = PER / NJ;
+        constexpr int LJ = N / NJ, LI = M / NI;                                    // lane grid, LI * LJ == 32
+        static_assert(LI * LJ == 32 && NI * NJ == PER, "lane tiling");
         constexpr int KC = K < 16 ? K : 16;
-        const int j0 = lane & (N - 1), i0 = N >= 32 ? 0 : (lane >> LGN);
+        const int j0 = lane % LJ, i0 = lane / LJ;
         float acc[NI][NJ];
 #pragma unroll
         for (int x = 0; x < NI; ++x)
@@ -136,13 +142,12 @@ __device__ __forceinline__ void chain_step_spec(const float *pa, const float *pb
 #pragma unroll
             for (int y = 0; y < NJ; ++y)
 #pragma unroll
-                for (int q = 0; q < KC / 4; ++q) b[y][q] = *reinterpret_cast<const float4 *>(pb + (j0 + 32 * y) * PB + k0 + 4 * q);
+                for (int q = 0; q < KC / 4; ++q) b[y][q] = *reinterpret_cast<const float4 *>(pb + (j0 + LJ * y) * PB + k0 + 4 * q);
 #pragma unroll
             for (int x = 0; x < NI; ++x) {
-                const int i = N >= 32 ? x : i0 + ISTR * x;
 #pragma unroll
                 for (int q = 0; q < KC / 4; ++q) {
-                    const float4 av = *reinterpret_cast<const float4 *>(pa + i * PA + k0 + 4 * q);
+                    const float4 av = *reinterpret_cast<const float4 *>(pa + (i0 + LI * x) * PA + k0 + 4 * q);
 #pragma unroll
                     for (int y = 0; y < NJ; ++y) {
                         acc[x][y] = fmaf(av.x, b[y][q].x, acc[x][y]); acc[x][y] = fmaf(av.y, b[y][q].y, acc[x][y]);
@@ -154,7 +159,7 @@ __device__ __forceinline__ void chain_step_spec(const float *pa, const float *pb
 #pragma unroll
         for (int x = 0; x < NI; ++x)
 #pragma unroll
-            for (int y = 0; y < NJ; ++y) emit(N >= 32 ? x : i0 + ISTR * x, j0 + 32 * y, acc[x][y]);
+            for (int y = 0; y < NJ; ++y) emit(i0 + LI * x, j0 + LJ * y, acc[x][y]);
     } else {
         constexpr int LGG0 = LGO >= 5 ? 0 : 5 - LGO;
         constexpr int LGG = (LGK - LGG0 < 2) ? (LGK >= 2 ? LGK - 2 : 0) : LGG0;
