@@ -115,10 +115,37 @@ __device__ __forceinline__ void chain_outputs(const ChainStepCtx &c, int kspan) 
 // outputs o = lane + 32 p; they form an NI x NJ grid (NJ distinct j, NI distinct i) whose operand rows are loaded once per
 // 16-float slab of the bond and reused from registers.  With fewer outputs the bond is split over G lanes per output and
 // finished with warp shuffles.  emit(i, j, value) stores one result.
-template <int LGM, int LGN, int LGK, int PA, int PB, class Emit>
+template <int LGM, int LGN, int LGK, int PA, int PB, bool ROWSPLIT = false, class Emit>
 __device__ __forceinline__ void chain_step_spec(const float *pa, const float *pb, int lane, Emit emit) {
     constexpr int N = 1 << LGN, K = 1 << LGK, LGO = LGM + LGN, O = 1 << LGO;
-    if constexpr (O >= 32 && LGK >= 2) {
+    if constexpr (ROWSPLIT) {
+        // M == 1 and B is read straight from global memory (each element is used once per state): out[j] = sum_k a[k] B[j][k].
+        // The lanes split the bond so that every load of B is a contiguous 16 B x G segment of one row (coalesced), the
+        // partial sums of a row meet by warp shuffles.
+        static_assert(LGM == 0 && LGK >= 4, "row-split step");
+        constexpr int G = K / 4 < 32 ? K / 4 : 32;          // lanes per row
+        constexpr int RP = 32 / G;                           // rows per pass
+        constexpr int NQ = K / (4 * G);                      // float4 per lane per row
+        const int g = lane % G, rr = lane / G;
+        float4 a4[NQ];
+#pragma unroll
+        for (int q = 0; q < NQ; ++q) a4[q] = *reinterpret_cast<const float4 *>(pa + 4 * g + 4 * G * q);
+#pragma unroll 4
+        for (int jb = 0; jb < N; jb += RP) {
+            const int j = jb + rr;
+            float v = 0.f;
+            if (j < N) {
+#pragma unroll
+                for (int q = 0; q < NQ; ++q) {
+                    const float4 b = __ldg(reinterpret_cast<const float4 *>(pb + (size_t)j * PB + 4 * g + 4 * G * q));
+                    v = fmaf(a4[q].x, b.x, v); v = fmaf(a4[q].y, b.y, v); v = fmaf(a4[q].z, b.z, v); v = fmaf(a4[q].w, b.w, v);
+                }
+            }
+#pragma unroll
+            for (int d = G >> 1; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+            if (j < N && g == 0) emit(0, j, v);
+        }
+    } else if constexpr (O >= 32 && LGK >= 2) {
         // a lane owns an NI x NJ block of outputs: rows i0 + x * SI, columns j0 + y * SJ, with the 32 lanes laid out LI x LJ
         // over the M x N outputs.  Shared-memory traffic per lane is (NI + NJ) rows per bond slab, so the block is kept as
         // square as the shape allows (16 x 16 outputs: 2 x 4 instead of 8 x 1, a third fewer loads).

@@ -574,9 +574,20 @@ std::string chain_source(const tqc_plan_t *pl) {
             return "(" + base + ") + ((size_t)__shfl_sync(0xffffffffu, c.mykey, " + std::to_string(o.key_slot) + ") << " +
                    std::to_string(lgRows + s.lgK) + ")";
         };
-        src += "    { const float *pa = " + operand(s.A, "A", s.lgM) + ";\n      const float *pb = " + operand(s.B, "B", s.lgN) + ";\n";
-        src += "      chain_step_spec<" + std::to_string(s.lgM) + ", " + std::to_string(s.lgN) + ", " + std::to_string(s.lgK) + ", " +
-               std::to_string(s.A.pitch) + ", " + std::to_string(s.B.pitch) + ">(pa, pb, c.lane, [&](int i, int j, float v) {\n";
+        // a bond-wide operand read straight from global memory with a single row on the other side: row-split step
+        // (coalesced reads); if that operand is A, the roles are swapped in the generated call
+        const bool direct_a = s.A.gathered && !s.A.staged, direct_b = s.B.gathered && !s.B.staged;
+        const bool split_b = direct_b && s.lgM == 0 && s.lgK >= 4 && s.lgN >= 1;
+        const bool split_a = !split_b && direct_a && s.lgN == 0 && s.lgK >= 4 && s.lgM >= 1;
+        if (split_a) {
+            src += "    { const float *pa = " + operand(s.B, "B", s.lgN) + ";\n      const float *pb = " + operand(s.A, "A", s.lgM) + ";\n";
+            src += "      chain_step_spec<0, " + std::to_string(s.lgM) + ", " + std::to_string(s.lgK) + ", " + std::to_string(s.B.pitch) + ", " +
+                   std::to_string(s.A.pitch) + ", true>(pa, pb, c.lane, [&](int j, int i, float v) {\n";
+        } else {
+            src += "    { const float *pa = " + operand(s.A, "A", s.lgM) + ";\n      const float *pb = " + operand(s.B, "B", s.lgN) + ";\n";
+            src += "      chain_step_spec<" + std::to_string(s.lgM) + ", " + std::to_string(s.lgN) + ", " + std::to_string(s.lgK) + ", " +
+                   std::to_string(s.A.pitch) + ", " + std::to_string(s.B.pitch) + (split_b ? ", true" : "") + ">(pa, pb, c.lane, [&](int i, int j, float v) {\n";
+        }
         if (s.c_smem_ofs < 0) src += "        *c.out_r = v;\n";
         else {
             src += "        const int x = (" + bitmap_expr(s.outA, "i") + ") | (" + bitmap_expr(s.outB, "j") + ");\n";
