@@ -5,12 +5,13 @@
 // tile is split in shared memory into a_hi (top 19 bits, exactly a TF32 value) and a_lo = a - a_hi (exact in fp32)
 // and three TF32 MMAs hi*hi + hi*lo + lo*hi accumulate in fp32 in TMEM.
 //
-// Persistent, warp-specialised CTA (one per SM), 256 threads:
+// Persistent, warp-specialised CTA (one per SM), 384 threads:
 //   warp 0      TMA producer: cp.async.bulk.tensor 3-D tiles {32 k, 128 or BN rows, 1 state} with 128-byte swizzle;
 //               the state coordinate of a LEAF/TABLE operand is the state's key (a3 gather = a TMA coordinate)
 //   warp 1      MMA issuer: one elected lane, 12 tcgen05.mma.kind::tf32 per k-block, tcgen05.commit frees the stage
-//   warps 2-5   accumulate + epilogue: tcgen05.ld -> fp32 round-to-nearest adds in registers -> scatter to C
-//   warps 6-7   splitter: fp32 tile -> hi (in place) and lo (second buffer), same swizzled byte offsets
+//   warps 2-9   accumulate + epilogue: tcgen05.ld -> fp32 round-to-nearest adds in registers -> scatter to C; two groups of
+//               four warps (one per TMEM lane quadrant), each group owning half of the tile's columns when BN >= 64
+//   warps 10-11 splitter: fp32 tile -> hi (in place) and lo (second buffer), same swizzled byte offsets
 // Pipelines: full[s] (TMA -> splitter), ready[s] (splitter -> MMA), empty[s] (MMA -> TMA).
 // The tensor pipe's fp32 accumulator rounds toward zero on every add (measured: -5e-8 relative per accumulation,
 // profiles/r01c notes), a bias that grows with the number of k-steps.  So (i) the hi*hi products of at most
@@ -29,7 +30,7 @@ namespace tqc {
 
 constexpr int TC_BM = 128;          // UMMA M
 constexpr int TC_BK = 32;           // fp32 elements per k-block = 128 bytes = one swizzle row
-constexpr int TC_THREADS = 256;      // 8 warps: up to 255 registers per thread for the accumulate warps
+constexpr int TC_THREADS = 384;      // 12 warps: TMA, MMA, 2 x 4 accumulate/epilogue warps, 2 splitter warps
 constexpr int TC_SPLIT_THREADS = 64;
 constexpr int TC_CHUNK_KB = 2;       // k-blocks (of 32) whose hi*hi products accumulate in TMEM before a drain
 
@@ -139,6 +140,18 @@ __device__ __forceinline__ void split_tile(uint32_t addr, uint32_t lo_ofs, bool 
     }
 }
 
+// float index of element (row i5, column j5) of a warp's staging block: rows of CB floats (32-float pitch for CB = 32,
+// 16-float pitch otherwise), float4 slot XOR-swizzled by the row so that row-wise float4 writes and the permuted float4
+// reads of the store phase are bank-conflict free
+template <int CB>
+__device__ __forceinline__ uint32_t scratch_index(uint32_t i5, uint32_t j5) {
+    if (CB == 32) {
+        const uint32_t rev = ((i5 & 1u) << 2) | (i5 & 2u) | ((i5 >> 2) & 1u);
+        return i5 * 32u + ((((j5 >> 2) ^ rev) & 7u) << 2) + (j5 & 3u);
+    }
+    return i5 * 16u + ((((j5 >> 2) ^ (i5 >> 1)) & 3u) << 2) + (j5 & 3u);
+}
+
 template <int BN>
 __global__ void __launch_bounds__(TC_THREADS, 1)
 step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB, const TcArgs a) {
@@ -148,11 +161,15 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
     __shared__ uint32_t tmem_base_slot;
     // epilogue: each warp stages 32 rows x CB columns in its own scratch and writes them out in ascending C-offset
     // order (perm tables), so a warp store covers the longest contiguous run the consumer's digit layout allows
-    constexpr int CB = BN < 32 ? BN : 32;
-    constexpr int LB = BN < 32 ? 4 : 5;
+    constexpr int EG = BN >= 64 ? 2 : 1;             // epilogue warp groups
+    constexpr int EC = BN / EG;                       // columns each epilogue warp accumulates
+    constexpr int CB = EG == 2 ? 16 : (BN < 32 ? BN : 32);   // columns per staged block
+    constexpr int LB = CB == 32 ? 5 : 4;
+    // C-offset tables (bit maps applied once per kernel, not per tile): m-tile, lane quadrant, n-tile, column block
+    __shared__ uint32_t oa_mt[256], oa_q[4], ob_nt[256], ob_blk[BN / CB];
     __shared__ uint32_t perm_off[32 * CB];
-    __shared__ uint16_t perm_src[32 * CB];
-    __shared__ __align__(16) float scratch[4][32 * 32];     // row i5: 8 float4 slots, slot (j5 >> 2) ^ bitrev3(i5 & 7)
+    __shared__ __align__(8) uint16_t perm_src[32 * CB];
+    __shared__ __align__(16) float scratch[4 * EG][32 * (CB == 32 ? 32 : 16)];   // row i5: CB/4 float4 slots, XOR-swizzled by the row
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int S = a.stages;
@@ -173,6 +190,12 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
     constexpr uint32_t tmem_cols = 4 * BN < 32 ? 32 : 4 * BN;      // D_hi[0], D_hi[1], D_lo[0], D_lo[1]
 
     // ---- one-time setup -------------------------------------------------------------------------
+    for (int x = threadIdx.x; x < 256; x += TC_THREADS) {
+        oa_mt[x] = x < tiles_m ? (uint32_t)bitmap_apply(a.outA, (unsigned long long)x * TC_BM) : 0u;
+        ob_nt[x] = x < tiles_n ? (uint32_t)bitmap_apply(a.outB, (unsigned long long)x * BN) : 0u;
+        if (x < 4) oa_q[x] = (uint32_t)bitmap_apply(a.outA, (unsigned long long)x * 32);
+        if (x < BN / CB) ob_blk[x] = (uint32_t)bitmap_apply(a.outB, (unsigned long long)x * CB);
+    }
     for (int e = threadIdx.x; e < 32 * CB; e += TC_THREADS) {
         // the 5 + LB index bits of a block, ordered by the C-offset bit they map to
         uint32_t dst[5 + LB], src[5 + LB];
@@ -194,15 +217,14 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
         perm_off[e] = off;
         {
             const uint32_t i5 = ij & 31u, j5 = ij >> 5;
-            const uint32_t rev = ((i5 & 1u) << 2) | (i5 & 2u) | ((i5 >> 2) & 1u);
-            perm_src[e] = (uint16_t)(i5 * 32u + ((((j5 >> 2) ^ rev) & 7u) << 2) + (j5 & 3u));
+            perm_src[e] = (uint16_t)scratch_index<CB>(i5, j5);
         }
     }
     if (threadIdx.x == 0) {
         for (int s = 0; s < S; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&ready_bar[s], TC_SPLIT_THREADS / 32); mbar_init(&empty_bar[s], 1); }
         for (int s = 0; s < 2; ++s) {
-            mbar_init(&hi_full_bar[s], 1); mbar_init(&hi_empty_bar[s], 4);
-            mbar_init(&lo_full_bar[s], 1); mbar_init(&lo_empty_bar[s], 4);
+            mbar_init(&hi_full_bar[s], 1); mbar_init(&hi_empty_bar[s], 4 * EG);
+            mbar_init(&lo_full_bar[s], 1); mbar_init(&lo_empty_bar[s], 4 * EG);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -289,34 +311,34 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
                 }
             }
         }
-    } else if (warp < 6) {
+    } else if (warp < 2 + 4 * EG) {
         // ===== accumulate (round-to-nearest, registers) + epilogue =====
         const int w4 = warp & 3;
+        const int col_base = ((warp - 2) >> 2) * EC;             // this warp's first column of the tile
         const uint32_t lane_base = (uint32_t)(32 * w4) << 16;
-        const uint32_t lane_rev = (((uint32_t)lane & 1u) << 2) | ((uint32_t)lane & 2u) | (((uint32_t)lane >> 2) & 1u);
         uint32_t rd_ofs[CB / 4], st_ofs[CB / 4];           // this lane's float4 slots of a block, in ascending C-offset order
 #pragma unroll
         for (int p = 0; p < CB / 4; ++p) { rd_ofs[p] = perm_src[(p * 32 + lane) * 4]; st_ofs[p] = perm_off[(p * 32 + lane) * 4]; }
         long long lt = 0, g = 0;
         for (long long t = blockIdx.x; t < total; t += gridDim.x, ++lt) {
             const long long nt = t % tiles_n, mt = (t / tiles_n) % tiles_m, r = t / (tiles_n * tiles_m);
-            float acc[BN];
+            float acc[EC];
 #pragma unroll
-            for (int q = 0; q < BN; ++q) acc[q] = 0.f;
+            for (int q = 0; q < EC; ++q) acc[q] = 0.f;
             for (int c = 0; c < n_chunks; ++c, ++g) {
                 const uint32_t hb = (uint32_t)(g & 1), hph = (uint32_t)((g >> 1) & 1);
                 mbar_wait(&hi_full_bar[hb], hph);
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                const uint32_t taddr = tmem_base + lane_base + hb * (uint32_t)BN;
+                const uint32_t taddr = tmem_base + lane_base + hb * (uint32_t)BN + (uint32_t)col_base;
                 if (!(a.debug & 8))
 #pragma unroll
-                for (int c0 = 0; c0 < BN; c0 += 32) {
+                for (int c0 = 0; c0 < EC; c0 += 32) {
                     uint32_t v[32];
-                    if (BN - c0 >= 32) tmem_ld32(taddr + c0, v); else tmem_ld16(taddr + c0, v);
+                    if (EC - c0 >= 32) tmem_ld32(taddr + c0, v); else tmem_ld16(taddr + c0, v);
                     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
                     for (int q = 0; q < 32; ++q)
-                        if (c0 + q < BN) acc[c0 + q] += __uint_as_float(v[q]);
+                        if (c0 + q < EC) acc[c0 + q] += __uint_as_float(v[q]);
                 }
                 asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
                 __syncwarp();
@@ -325,18 +347,16 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
             const uint32_t lb = (uint32_t)(lt & 1), lph = (uint32_t)((lt >> 1) & 1);
             mbar_wait(&lo_full_bar[lb], lph);
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-            const unsigned long long oa = bitmap_apply(a.outA, (unsigned long long)(mt * TC_BM + 32 * w4));
-            const unsigned long long obh = bitmap_apply(a.outB, (unsigned long long)(nt * BN));
-            float *crow = a.C + r * a.c_row_stride + (oa | obh);
-            const uint32_t laddr = tmem_base + lane_base + (2u + lb) * (uint32_t)BN;
+            float *crow = a.C + r * a.c_row_stride + (oa_mt[mt] | oa_q[w4] | ob_nt[nt]);
+            const uint32_t laddr = tmem_base + lane_base + (2u + lb) * (uint32_t)BN + (uint32_t)col_base;
 #pragma unroll
-            for (int c0 = 0; c0 < BN; c0 += 32) {
+            for (int c0 = 0; c0 < EC; c0 += 32) {
                 uint32_t v[32];
-                if (BN - c0 >= 32) tmem_ld32(laddr + c0, v); else tmem_ld16(laddr + c0, v);
+                if (EC - c0 >= 32) tmem_ld32(laddr + c0, v); else tmem_ld16(laddr + c0, v);
                 asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
                 for (int q = 0; q < 32; ++q)
-                    if (c0 + q < BN) acc[c0 + q] += __uint_as_float(v[q]);
+                    if (c0 + q < EC) acc[c0 + q] += __uint_as_float(v[q]);
             }
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
             __syncwarp();
@@ -344,19 +364,29 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
             float *scr = scratch[warp - 2];
             if (a.debug & 2) continue;
 #pragma unroll
-            for (int c0 = 0; c0 < BN; c0 += CB) {
+            for (int c0 = 0; c0 < EC; c0 += CB) {
                 __syncwarp();
 #pragma unroll
                 for (int k = 0; k < CB / 4; ++k)
-                    *reinterpret_cast<float4 *>(scr + lane * 32 + (((uint32_t)k ^ lane_rev) << 2)) =
+                    *reinterpret_cast<float4 *>(scr + scratch_index<CB>((uint32_t)lane, (uint32_t)(4 * k))) =
                         make_float4(acc[c0 + 4 * k], acc[c0 + 4 * k + 1], acc[c0 + 4 * k + 2], acc[c0 + 4 * k + 3]);
                 __syncwarp();
-                float *cblk = crow + bitmap_apply(a.outB, (unsigned long long)c0);
+                float *cblk = crow + ob_blk[(col_base + c0) / CB];
                 if (a.vec4) {
 #pragma unroll
                     for (int p = 0; p < CB / 4; ++p) {
                         const float4 val = *reinterpret_cast<const float4 *>(scr + rd_ofs[p]);
                         if (!(a.debug & 1) || val.x == 123.456f) *reinterpret_cast<float4 *>(cblk + st_ofs[p]) = val;
+                    }
+                } else if (perm_off[1] == 1u && perm_off[2] == 2u && perm_off[3] == 3u) {
+                    // four consecutive elements of the ascending order are contiguous in C (the two lowest C bits lie inside
+                    // the block) but not in the staging block: four scalar reads, one 16-byte store
+#pragma unroll
+                    for (int p = 0; p < CB / 4; ++p) {
+                        const int e = (p * 32 + lane) * 4;
+                        const uint2 ps = *reinterpret_cast<const uint2 *>(perm_src + e);
+                        const float4 val = make_float4(scr[ps.x & 0xFFFFu], scr[ps.x >> 16], scr[ps.y & 0xFFFFu], scr[ps.y >> 16]);
+                        *reinterpret_cast<float4 *>(cblk + st_ofs[p]) = val;
                     }
                 } else {
 #pragma unroll
@@ -367,9 +397,9 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
                 }
             }
         }
-    } else {
+    } else if (warp >= (TC_THREADS - TC_SPLIT_THREADS) / 32) {
         // ===== splitter: fp32 -> hi (in place) + lo =====
-        const int st = threadIdx.x - 6 * 32;
+        const int st = threadIdx.x - (TC_THREADS - TC_SPLIT_THREADS);
         const bool mask_hi = a.mask_hi != 0;
         long long it = 0;
         for (long long t = blockIdx.x; t < total; t += gridDim.x) {

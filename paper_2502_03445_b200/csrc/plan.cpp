@@ -258,6 +258,21 @@ int build_plan(int n, int m, int K, const int32_t *cut_up, const int32_t *cut_do
         A.n_inner = B.n_inner = (int)st.inner.size();
     }
     if (m > 1 && !p.nodes[2 * m - 2].open.empty()) { err = "internal: root has open cuts"; return E_ARG; }
+    // Outer digits of each operand in the order they have in the RESULT's layout (root first, so the result's layout is
+    // final when its operands are ordered): the result index maps i -> C and j -> C are then order-preserving, the lowest
+    // digits of one operand are the lowest digits of C, and a tile of the step covers long contiguous runs of C.
+    for (int t = m - 2; t >= 0; --t) {
+        const Step &st = p.steps[t];
+        const Node &C = p.nodes[m + t];
+        for (int op : {st.lhs, st.rhs}) {
+            Node &X = p.nodes[op];
+            const size_t no = X.layout.size() - (size_t)X.n_inner;
+            std::stable_sort(X.layout.begin(), X.layout.begin() + (long)no, [&](int a, int b) {
+                const auto ia = std::find(C.layout.begin(), C.layout.end(), a), ib = std::find(C.layout.begin(), C.layout.end(), b);
+                return ia < ib;
+            });
+        }
+    }
 
     // ---- node kinds ----
     {

@@ -168,6 +168,9 @@ int launch_tile(tqc_plan_t *pl, StepArgs &a, int tag, cudaStream_t st) {
     return rc;
 }
 
+// outer digits of a node in its device order (most significant first): the layout minus the trailing inner digits
+std::vector<int> outer_of(const Node &nd) { return std::vector<int>(nd.layout.begin(), nd.layout.end() - nd.n_inner); }
+
 // digits of an operand's outer index (most significant first) -> bit positions inside C's row
 void add_digit_scatter(BitPairs &bp, const std::vector<int> &outer, const std::vector<int> &c_layout) {
     const int no = (int)outer.size(), nc = (int)c_layout.size();
@@ -245,8 +248,8 @@ int launch_cross_step(tqc_plan_t *pl, const CrossCtx &cx, int t, cudaStream_t st
     const bool dist_root = cx.out != nullptr && vc == hp.root();
     const int cdig = 2 * (int)C.layout.size();
     BitPairs pa, pb;
-    add_digit_scatter(pa, s.outer_lhs, C.layout);
-    add_digit_scatter(pb, s.outer_rhs, C.layout);
+    add_digit_scatter(pa, outer_of(hp.nodes[s.lhs]), C.layout);
+    add_digit_scatter(pb, outer_of(hp.nodes[s.rhs]), C.layout);
     const int na = 2 * (int)s.outer_lhs.size(), nb = 2 * (int)s.outer_rhs.size();
     if (dist_root) {
         // product-order row bits -> global bit order: free qubits ascending, lowest id = MSB (G4)
@@ -321,6 +324,7 @@ int make_operand_map(CUtensorMap *map, const float *base, int lgK, int lgRows, l
 }
 
 bool tc_eligible(int lgM, int lgN, int lgK) {
+    if (std::max(lgM, lgN) > 14) return false;                  // at most 256 tiles per side (C-offset tables of the kernel)
     return lgK >= 5 && std::max(lgM, lgN) >= 7 && std::min(lgM, lgN) >= 4;
 }
 
@@ -406,8 +410,8 @@ int launch_batch_step(tqc_plan_t *pl, const BatchCtx &bx, int t, cudaStream_t st
     a.C = cbase;
     a.c_row_stride = 1ll << (2 * (int)C.open.size());
     BitPairs pa, pb;
-    add_digit_scatter(pa, s.outer_lhs, C.layout);
-    add_digit_scatter(pb, s.outer_rhs, C.layout);
+    add_digit_scatter(pa, outer_of(hp.nodes[s.lhs]), C.layout);
+    add_digit_scatter(pb, outer_of(hp.nodes[s.rhs]), C.layout);
     if (!pa.build(a.outA) || !pb.build(a.outB)) return fail(TQC_E_TOO_LARGE, "bit map needs too many segments");
     if (s.kernel_class == TQC_KERNEL_TCGEN05) {
         auto n_outer = [&](int v) -> long long {
@@ -493,8 +497,8 @@ bool build_chain(tqc_plan_t *pl) {
         cs.tab_ofs = (int)tab_entries;
         tab_entries += (1ll << lgM) + (1ll << lgN);
         BitPairs pa, pb;
-        add_digit_scatter(pa, s.outer_lhs, C.layout);
-        add_digit_scatter(pb, s.outer_rhs, C.layout);
+        add_digit_scatter(pa, outer_of(hp.nodes[s.lhs]), C.layout);
+        add_digit_scatter(pb, outer_of(hp.nodes[s.rhs]), C.layout);
         if (!pa.build(cs.outA) || !pb.build(cs.outB)) return false;
         tab.push_back(cs); leafA.push_back(la); leafB.push_back(lb);
     }
