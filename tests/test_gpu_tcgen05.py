@@ -46,7 +46,8 @@ def _run(net, T, bits, **kw):
     return out.cpu().numpy().astype(np.float64), plan
 
 
-@pytest.mark.parametrize("na,nb,ni,B", [(4, 2, 3, 67), (2, 4, 3, 33), (4, 3, 3, 40), (4, 4, 3, 9), (5, 2, 4, 21), (4, 2, 5, 16)])
+@pytest.mark.parametrize("na,nb,ni,B", [(4, 2, 3, 67), (2, 4, 3, 33), (4, 3, 3, 40), (4, 4, 3, 9), (5, 2, 4, 21), (4, 2, 5, 16),
+                                        (4, 5, 3, 5), (5, 4, 3, 3)])        # the last two: N >= 256, the wide-tile kernel
 def test_tc_step_leaf_times_leaf(na, nb, ni, B):
     net = _triangle(na, nb, ni)
     T = random_tensors(net, 1000 + na * 100 + nb * 10 + ni)
