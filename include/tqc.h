@@ -157,6 +157,23 @@ int tqc_contract_distribution_host(tqc_plan_t *plan, uint64_t prefix_value, int 
                                    float *out_host, void *workspace_dev, size_t workspace_bytes,
                                    void *stream);
 
+/* ---- Heavy State Selection (section 4, Algorithm 1) -- first row of SURVEY 8(f) -----------------
+ * tqc_hss_scores: scores_dev[i] = ||p_{s,i}|| = sqrt(sum_e T_s[e, i]^2) for every binary state i of subcircuit s
+ *   (the L2 norm over all edge permutations, Alg. 1 line 3), DEVICE [2^{o_s}], asynchronous on `stream`; the tensor
+ *   must be loaded.  Scores refer to the caller's values (the 2^{-d_s} folded in at load is undone exactly).
+ * tqc_hss_select (host only): Alg. 1 on the m score arrays (HOST, scores_host[j] has 2^{o_j} entries): every subcircuit
+ *   is seeded with its heaviest state (ties: smaller i), the remaining (j, i) are taken in descending norm (ties: smaller
+ *   j, then smaller i) while prod_j |x_j| < s_max (readings: seeds count toward the product, the last addition may
+ *   overshoot s_max, the loop also ends when everything is selected).  counts[j] = |x_j|; keys = the selected states of
+ *   subcircuit 0, then 1, ..., each ascending (HOST, capacity >= sum_j 2^{o_j}).
+ * tqc_hss_expand (host only): the prod_j |x_j| composite states in the batch format of tqc_contract_states (G5), product
+ *   order with subcircuit 0 slowest.  Call with states_host = NULL to get *n_states. */
+int tqc_hss_scores(tqc_plan_t *plan, int s, float *scores_dev, void *stream);
+int tqc_hss_select(const tqc_plan_t *plan, const float *const *scores_host, uint64_t s_max, int32_t *counts, int32_t *keys,
+                   size_t keys_capacity);
+int tqc_hss_expand(const tqc_plan_t *plan, const int32_t *counts, const int32_t *keys, uint64_t *states_host, size_t capacity,
+                   size_t *n_states);
+
 /* ---- measurement hooks (bench.py) --------------------------------------------------------------
  * tqc_plan_launch_count: kernels launched so far on behalf of this plan.
  * tqc_plan_profile_enable(plan, 1): every later contract call records one CUDA event on the

@@ -31,7 +31,8 @@ EXPORTED = ["tqc_plan", "tqc_plan_destroy", "tqc_plan_mode", "tqc_plan_num_qubit
             "tqc_plan_workspace_min_bytes", "tqc_load_subcircuit_tensors", "tqc_contract_states",
             "tqc_contract_distribution", "tqc_plan_launch_count", "tqc_last_error", "tqc_version",
             "tqc_plan_workspace_bytes_host", "tqc_contract_states_host", "tqc_contract_distribution_host",
-            "tqc_plan_profile_enable", "tqc_plan_profile_read", "tqc_plan_chain_status"]
+            "tqc_plan_profile_enable", "tqc_plan_profile_read", "tqc_plan_chain_status", "tqc_hss_scores", "tqc_hss_select",
+            "tqc_hss_expand"]
 
 
 class TqcError(RuntimeError):
@@ -92,6 +93,9 @@ def _load() -> ctypes.CDLL:
     lib.tqc_plan_chain_status.argtypes = [c_void_p, c_char_p, c_size_t]
     lib.tqc_plan_profile_enable.argtypes = [c_void_p, c_int]
     lib.tqc_plan_profile_read.argtypes = [c_void_p, c_void_p, c_void_p, POINTER(c_size_t)]
+    lib.tqc_hss_scores.argtypes = [c_void_p, c_int, c_void_p, c_void_p]
+    lib.tqc_hss_select.argtypes = [c_void_p, POINTER(c_void_p), c_uint64, c_void_p, c_void_p, c_size_t]
+    lib.tqc_hss_expand.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_size_t, POINTER(c_size_t)]
     return lib
 
 
@@ -299,3 +303,45 @@ def tqc_contract_distribution_host(plan: Plan, out_host, workspace, prefix_value
                                                workspace.data_ptr(), workspace.numel() * workspace.element_size(),
                                                _stream_ptr(stream)))
     return out_host
+
+
+def tqc_hss_scores(plan: Plan, s: int, out=None, stream=None, device="cuda"):
+    """||p_{s,i}|| for every binary state i of subcircuit s (Alg. 1): CUDA fp32 [2^{o_s}]."""
+    import torch
+    _, o = plan.tensor_shape(s)
+    if out is None:
+        out = torch.empty(1 << o, dtype=torch.float32, device=device)
+    _check(_lib.tqc_hss_scores(plan._h, s, out.data_ptr(), _stream_ptr(stream)))
+    return out
+
+
+def tqc_hss_select(plan: Plan, scores_host, s_max: int):
+    """Alg. 1 lines 480-491 on host score arrays (one float32 numpy array per subcircuit).  Returns x_j as a list of
+    int32 arrays, each ascending."""
+    import numpy as np
+    m = plan.m
+    arrs = [np.ascontiguousarray(a, dtype=np.float32) for a in scores_host]
+    if len(arrs) != m or any(a.size != 1 << plan.tensor_shape(j)[1] for j, a in enumerate(arrs)):
+        raise ValueError("one score array of 2^{o_j} entries per subcircuit")
+    ptrs = (c_void_p * m)(*[a.ctypes.data for a in arrs])
+    counts = np.zeros(m, dtype=np.int32)
+    keys = np.zeros(sum(a.size for a in arrs), dtype=np.int32)
+    _check(_lib.tqc_hss_select(plan._h, ptrs, s_max, counts.ctypes.data, keys.ctypes.data, keys.size))
+    ofs = np.concatenate([[0], np.cumsum(counts)])
+    return [keys[ofs[j]:ofs[j + 1]].copy() for j in range(m)]
+
+
+def tqc_hss_expand(plan: Plan, x):
+    """The prod_j |x_j| composite states of a selection, packed as tqc_contract_states takes them:
+    numpy uint64 [B, ceil(n/64)], product order with subcircuit 0 slowest."""
+    import numpy as np
+    counts = np.array([len(k) for k in x], dtype=np.int32)
+    keys = np.ascontiguousarray(np.concatenate([np.asarray(k, dtype=np.int32) for k in x]) if len(x) else
+                                np.zeros(0, np.int32))
+    n = c_size_t(0)
+    _check(_lib.tqc_hss_expand(plan._h, counts.ctypes.data, keys.ctypes.data, None, 0, ctypes.byref(n)))
+    words = (plan.n_qubits + 63) // 64
+    states = np.zeros((n.value, words), dtype=np.uint64)
+    _check(_lib.tqc_hss_expand(plan._h, counts.ctypes.data, keys.ctypes.data, states.ctypes.data, n.value,
+                               ctypes.byref(n)))
+    return states

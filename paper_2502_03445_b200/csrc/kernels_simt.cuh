@@ -237,4 +237,34 @@ __global__ void __launch_bounds__(256) gather_kernel(const GatherArgs a) {
     else a.out[bitmap_apply(a.out_map, (unsigned long long)r)] = a.table[bitmap_apply(a.map, (unsigned long long)r) | a.map_or];
 }
 
+// ---------------------------------------------------------------------------------------------
+// Heavy State Selection, scoring pass (section 4, Alg. 1):
+//   ||p_{j,i}|| = sqrt( sum_e (p_{j,i}^e)^2 )  for every binary state i of subcircuit j.
+// In the state-major device layout state i is one contiguous row of 4^{c_j} floats, so the pass is a row norm: one warp
+// per row, float4 loads, shuffle tree; HBM-bound (each tensor element read once).  `unscale` = 2^{d_j} undoes the exact
+// power of two folded in at load, so the score is that of the caller's values.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) hss_norm_kernel(const float *__restrict__ t, float *__restrict__ score, long long rows,
+                                                        int lgCols, float unscale) {
+    const int lane = threadIdx.x & 31;
+    const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const long long n_warps = ((long long)gridDim.x * blockDim.x) >> 5;
+    const long long cols = 1ll << lgCols;
+    for (long long r = warp; r < rows; r += n_warps) {
+        const float *p = t + (r << lgCols);
+        float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
+        if (cols >= 4) {
+            for (long long k = lane * 4; k < cols; k += 128) {
+                const float4 v = __ldg(reinterpret_cast<const float4 *>(p + k));
+                s0 = fmaf(v.x, v.x, s0); s1 = fmaf(v.y, v.y, s1); s2 = fmaf(v.z, v.z, s2); s3 = fmaf(v.w, v.w, s3);
+            }
+        } else if (lane < cols) {
+            s0 = p[lane] * p[lane];
+        }
+        float s = (s0 + s1) + (s2 + s3);
+        for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
+        if (lane == 0) score[r] = sqrtf(s) * unscale;
+    }
+}
+
 }  // namespace tqc

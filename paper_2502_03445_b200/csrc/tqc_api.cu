@@ -102,7 +102,7 @@ using tqc::Step;
 constexpr int kMaxDynSmem = 200 * 1024;
 
 // Tags of profiled launches: step index t >= 0, or one of these.
-enum { TAG_KEYS = -1, TAG_GATHER = -2, TAG_RELAYOUT = -3, TAG_CHAIN = -4 };
+enum { TAG_KEYS = -1, TAG_GATHER = -2, TAG_RELAYOUT = -3, TAG_CHAIN = -4, TAG_HSS = -5 };
 
 int prof_event(tqc_plan_t *pl, cudaStream_t st) {
     if (pl->ev_used == pl->ev_pool.size()) {
@@ -1117,6 +1117,91 @@ int tqc_plan_profile_read(tqc_plan_t *pl, int32_t *tags, float *ms, size_t *n) {
         }
     }
     *n = have;
+    return 0;
+}
+
+// ---- NEXT row 1: Heavy State Selection (section 4, Alg. 1) ------------------------------------------------
+int tqc_hss_scores(tqc_plan_t *pl, int s, float *scores_dev, void *stream) {
+    if (!pl || !scores_dev) return fail(TQC_E_ARG, "null argument");
+    const HostPlan &hp = pl->hp;
+    if (s < 0 || s >= hp.m) return fail(TQC_E_ARG, "subcircuit id out of range");
+    if (!pl->loaded[s]) return fail(TQC_E_STATE, "tensor of subcircuit " + std::to_string(s) + " not loaded");
+    const long long rows = 1ll << hp.o(s);
+    const int lgCols = 2 * hp.c(s);
+    const long long warps = std::min<long long>(rows, 148ll * 64);
+    const unsigned blocks = (unsigned)((warps * 32 + 255) / 256);
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = note_launch(pl, TAG_HSS, st);
+    if (rc) return rc;
+    tqc::hss_norm_kernel<<<blocks, 256, 0, st>>>(pl->d_leaf[s], scores_dev, rows, lgCols, std::ldexp(1.0f, hp.d[s]));
+    TQC_CUDA(cudaGetLastError());
+    return 0;
+}
+
+int tqc_hss_select(const tqc_plan_t *pl, const float *const *scores_host, uint64_t s_max, int32_t *counts, int32_t *keys,
+                   size_t keys_capacity) {
+    if (!pl || !scores_host || !counts || !keys) return fail(TQC_E_ARG, "null argument");
+    const HostPlan &hp = pl->hp;
+    struct Cand { float norm; int j, i; };
+    std::vector<std::vector<char>> chosen(hp.m);
+    std::vector<Cand> rest;
+    std::vector<uint64_t> cnt(hp.m, 0);
+    size_t total_rows = 0;
+    for (int j = 0; j < hp.m; ++j) {
+        if (!scores_host[j]) return fail(TQC_E_ARG, "null score array");
+        const int n = 1 << hp.o(j);
+        total_rows += (size_t)n;
+        chosen[j].assign(n, 0);
+        int best = 0;                                       // seed: the heaviest state of every subcircuit (ties: smaller i)
+        for (int i = 1; i < n; ++i) if (scores_host[j][i] > scores_host[j][best]) best = i;
+        chosen[j][best] = 1; cnt[j] = 1;
+        for (int i = 0; i < n; ++i) if (i != best) rest.push_back({scores_host[j][i], j, i});
+    }
+    if (keys_capacity < total_rows) return fail(TQC_E_ARG, "keys buffer must hold sum_j 2^{o_j} entries");
+    // descending norm; ties by smaller subcircuit id, then smaller state (total order: the selection is reproducible)
+    std::sort(rest.begin(), rest.end(), [](const Cand &a, const Cand &b) {
+        if (a.norm != b.norm) return a.norm > b.norm;
+        if (a.j != b.j) return a.j < b.j;
+        return a.i < b.i;
+    });
+    auto product_reached = [&]() {                          // prod_j |x_j| >= s_max, without overflow
+        unsigned __int128 p = 1;
+        for (int j = 0; j < hp.m; ++j) { p *= cnt[j]; if (p >= s_max) return true; }
+        return p >= s_max;
+    };
+    for (size_t k = 0; k < rest.size() && !product_reached(); ++k) { chosen[rest[k].j][rest[k].i] = 1; cnt[rest[k].j]++; }
+    size_t w = 0;
+    for (int j = 0; j < hp.m; ++j) {
+        counts[j] = (int32_t)cnt[j];
+        for (int i = 0; i < (int)chosen[j].size(); ++i) if (chosen[j][i]) keys[w++] = i;      // ascending key order
+    }
+    return 0;
+}
+
+int tqc_hss_expand(const tqc_plan_t *pl, const int32_t *counts, const int32_t *keys, uint64_t *states_host, size_t capacity,
+                   size_t *n_states) {
+    if (!pl || !counts || !keys || !n_states) return fail(TQC_E_ARG, "null argument");
+    const HostPlan &hp = pl->hp;
+    unsigned __int128 total = 1;
+    for (int j = 0; j < hp.m; ++j) { total *= (uint64_t)std::max(counts[j], 0); if (total > ((unsigned __int128)1 << 40)) return fail(TQC_E_TOO_LARGE, "more than 2^40 composite states"); }
+    *n_states = (size_t)total;
+    if (!states_host) return 0;
+    if (capacity < (size_t)total) return fail(TQC_E_ARG, "states buffer too small");
+    const size_t words = (size_t)(hp.n + 63) / 64;
+    std::vector<size_t> ofs(hp.m + 1, 0);
+    for (int j = 0; j < hp.m; ++j) ofs[j + 1] = ofs[j] + (size_t)counts[j];
+    std::vector<int> idx(hp.m, 0);                          // odometer, subcircuit 0 slowest
+    for (size_t b = 0; b < (size_t)total; ++b) {
+        uint64_t *w = states_host + b * words;
+        for (size_t x = 0; x < words; ++x) w[x] = 0;
+        for (int j = 0; j < hp.m; ++j) {
+            const int key = keys[ofs[j] + idx[j]];
+            const int nq = hp.o(j);
+            for (int pq = 0; pq < nq; ++pq)                 // first listed qubit = MSB of the key (G4), qubit q = bit q%64 of word q/64 (G5)
+                if ((key >> (nq - 1 - pq)) & 1) { const int q = hp.sub_qubits[j][pq]; w[q >> 6] |= 1ull << (q & 63); }
+        }
+        for (int j = hp.m - 1; j >= 0; --j) { if (++idx[j] < counts[j]) break; idx[j] = 0; }
+    }
     return 0;
 }
 
