@@ -260,6 +260,7 @@ def run_ours(args) -> None:
                 o = measure(ctx, args, name, batch, steps, 3)
                 others.append({k: o[k] for k in ("value", "unit", "ms_per_step", "steps", "gpu_launches", "roofline")} |
                               {"workload": o["config"]["workload"], "e2e_value": o["e2e"]["value"]})
+            others.append(measure_hss(ctx, 10, 3))
             line["other_workloads"] = others
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(make_workload(args.workload, args.batch), args.cpu_seconds)
@@ -389,6 +390,48 @@ def measure(ctx, args, workload: str, batch: int, steps: int, warmup: int):
     del workspace, flush, out_dev
     torch.cuda.empty_cache()
     return line
+
+
+def measure_hss(ctx, steps: int, warmup: int) -> dict:
+    """NEXT row 1 (Alg. 1): the state-norm pass over two 4^6 x 2^14 tensors (512 MB, larger than L2), one launch
+    per subcircuit, against the HBM copy peak.  Selection and expansion are host work and are not timed here."""
+    torch, tqc, dev = ctx["torch"], ctx["tqc"], ctx["dev"]
+    from tqc_inputs.network import Network
+    K, o = 6, 14
+    net = Network(2 * o, [(0, 1)] * K, [list(range(K)), list(range(K))], [list(range(o)), list(range(o, 2 * o))],
+                  name="hss-2x(4^6 x 2^14)")
+    net.validate()
+    plan = tqc.tqc_plan(net, tqc.MODE_STATES)
+    rng = np.random.default_rng(250203445)
+    for s in range(net.m):
+        tqc.tqc_load_subcircuit_tensors(plan, s, rng.random((4 ** K, 2 ** o), dtype=np.float32))
+    scores = [torch.empty(2 ** o, dtype=torch.float32, device=dev) for _ in range(net.m)]
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    l0 = plan.launch_count
+    for _ in range(warmup):
+        for s in range(net.m):
+            tqc.tqc_hss_scores(plan, s, out=scores[s], stream=stream)
+    torch.cuda.synchronize()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for a, b in evs:
+        flush.zero_()
+        a.record(stream)
+        for s in range(net.m):
+            tqc.tqc_hss_scores(plan, s, out=scores[s], stream=stream)
+        b.record(stream)
+    torch.cuda.synchronize()
+    ms = sum(a.elapsed_time(b) for a, b in evs) / steps
+    nbytes = net.m * (4 ** K * 2 ** o + 2 ** o) * 4
+    peaks = measured_peaks()
+    gbs = nbytes / (ms * 1e-3) / 1e9
+    launches = plan.launch_count - l0
+    plan.close()
+    return {"workload": f"{net.name}: tqc_hss_scores over both subcircuits", "value": net.m * 2 ** o / (ms * 1e-3),
+            "unit": "subcircuit states scored/s", "ms_per_step": ms, "steps": steps, "gpu_launches": int(launches),
+            "roofline": {"bound": "hbm", "kernel": "hss_norm_kernel<32>", "achieved": gbs, "peak": peaks["hbm_gbs"],
+                         "unit": "GB/s", "frac": gbs / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"],
+                         "algorithmic_bytes_per_launch": nbytes // net.m}}
 
 
 def workload_description(wl, plan) -> str:

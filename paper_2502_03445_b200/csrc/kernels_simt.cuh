@@ -244,17 +244,20 @@ __global__ void __launch_bounds__(256) gather_kernel(const GatherArgs a) {
 // per row, float4 loads, shuffle tree; HBM-bound (each tensor element read once).  `unscale` = 2^{d_j} undoes the exact
 // power of two folded in at load, so the score is that of the caller's values.
 // ---------------------------------------------------------------------------------------------
+template <int LANES>   // LANES = 32: one warp per row (many rows); LANES = 256: one block per row (few, long rows)
 __global__ void __launch_bounds__(256) hss_norm_kernel(const float *__restrict__ t, float *__restrict__ score, long long rows,
                                                         int lgCols, float unscale) {
-    const int lane = threadIdx.x & 31;
-    const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const long long n_warps = ((long long)gridDim.x * blockDim.x) >> 5;
+    __shared__ float part[8];
+    const int lane = threadIdx.x & (LANES - 1);
+    const long long group = LANES == 32 ? ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5 : blockIdx.x;
+    const long long n_groups = LANES == 32 ? ((long long)gridDim.x * blockDim.x) >> 5 : gridDim.x;
     const long long cols = 1ll << lgCols;
-    for (long long r = warp; r < rows; r += n_warps) {
+    for (long long r = group; r < rows; r += n_groups) {
         const float *p = t + (r << lgCols);
         float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
         if (cols >= 4) {
-            for (long long k = lane * 4; k < cols; k += 128) {
+#pragma unroll 4
+            for (long long k = lane * 4; k < cols; k += LANES * 4) {
                 const float4 v = __ldg(reinterpret_cast<const float4 *>(p + k));
                 s0 = fmaf(v.x, v.x, s0); s1 = fmaf(v.y, v.y, s1); s2 = fmaf(v.z, v.z, s2); s3 = fmaf(v.w, v.w, s3);
             }
@@ -263,6 +266,12 @@ __global__ void __launch_bounds__(256) hss_norm_kernel(const float *__restrict__
         }
         float s = (s0 + s1) + (s2 + s3);
         for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
+        if (LANES == 256) {                              // fixed-order sum of the 8 warp partials
+            if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = s;
+            __syncthreads();
+            s = ((part[0] + part[1]) + (part[2] + part[3])) + ((part[4] + part[5]) + (part[6] + part[7]));
+            __syncthreads();
+        }
         if (lane == 0) score[r] = sqrtf(s) * unscale;
     }
 }

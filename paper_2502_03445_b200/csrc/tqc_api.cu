@@ -1128,12 +1128,17 @@ int tqc_hss_scores(tqc_plan_t *pl, int s, float *scores_dev, void *stream) {
     if (!pl->loaded[s]) return fail(TQC_E_STATE, "tensor of subcircuit " + std::to_string(s) + " not loaded");
     const long long rows = 1ll << hp.o(s);
     const int lgCols = 2 * hp.c(s);
-    const long long warps = std::min<long long>(rows, 148ll * 64);
-    const unsigned blocks = (unsigned)((warps * 32 + 255) / 256);
     cudaStream_t st = (cudaStream_t)stream;
     int rc = note_launch(pl, TAG_HSS, st);
     if (rc) return rc;
-    tqc::hss_norm_kernel<<<blocks, 256, 0, st>>>(pl->d_leaf[s], scores_dev, rows, lgCols, std::ldexp(1.0f, hp.d[s]));
+    const float unscale = std::ldexp(1.0f, hp.d[s]);
+    if (rows < 148 * 16 && lgCols >= 10) {                  // few long rows: a block per row keeps every SM loading
+        tqc::hss_norm_kernel<256><<<(unsigned)rows, 256, 0, st>>>(pl->d_leaf[s], scores_dev, rows, lgCols, unscale);
+    } else {
+        const long long warps = std::min<long long>(rows, 148ll * 64);
+        const unsigned blocks = (unsigned)((warps * 32 + 255) / 256);
+        tqc::hss_norm_kernel<32><<<blocks, 256, 0, st>>>(pl->d_leaf[s], scores_dev, rows, lgCols, unscale);
+    }
     TQC_CUDA(cudaGetLastError());
     return 0;
 }
