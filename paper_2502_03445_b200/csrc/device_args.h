@@ -52,8 +52,8 @@ struct StepArgs {
     long long c_row_stride;     // batch mode: floats per row of C (4^{#open cuts of C})
     int lgM, lgN, lgK;          // log2 of the virtual dimensions M' x N' x K (batch mode: per row)
     int R;                      // rows (states of the chunk) in batch mode; 1 in cross mode
-    int TI, TJ, TK, RPB;        // tile of one block: RPB rows x TI x TJ outputs, K in slabs of TK
-    int tiles_i, tiles_j;
+    int lgTI, lgTJ, lgTK, lgRPB;        // log2 of the tile of one block: RPB rows x TI x TJ outputs, K in slabs of TK
+    int lgTilesI, lgTilesJ;             // log2 of the tile counts M / TI, N / TJ
     int vec_store;              // the 4 consecutive j of a thread are contiguous in C
 };
 

@@ -61,33 +61,38 @@ __global__ void __launch_bounds__(256) key_kernel(const KeyArgs a) {
 // float4s that are broadcast (A) or contiguous (B) across a warp.
 // ---------------------------------------------------------------------------------------------
 template <int MI, int MJ>
-__global__ void __launch_bounds__(256) step_tile_kernel(const StepArgs a) {
+__global__ void __launch_bounds__(256, 4) step_tile_kernel(const StepArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int TI = a.TI, TJ = a.TJ, TK = a.TK, RPB = a.RPB;
+    // every tile dimension is a power of two: all index splitting below is shifts and masks
+    constexpr int LGMI = MI == 4 ? 2 : 0, LGMJ = MJ == 4 ? 2 : 0;
+    const int lgTI = a.lgTI, lgTJ = a.lgTJ, lgTK = a.lgTK;
+    const int TI = 1 << lgTI, TJ = 1 << lgTJ, TK = 1 << lgTK, RPB = 1 << a.lgRPB;
     const int TIp = TI + (MI == 4 ? 4 : 1), TJp = TJ + (MJ == 4 ? 4 : 1);
     unsigned long long *rowA = reinterpret_cast<unsigned long long *>(smem_raw);     // [RPB*TI] float offsets
     unsigned long long *rowB = rowA + RPB * TI;                                       // [RPB*TJ]
-    float *As = reinterpret_cast<float *>(rowB + RPB * TJ);                           // [RPB][TK][TIp]
-    float *Bs = As + RPB * TK * TIp;                                                  // [RPB][TK][TJp]
+    unsigned long long *offA = rowB + RPB * TJ;                                       // [TI] C offset bits of i'
+    unsigned long long *offB = offA + TI;                                             // [TJ] C offset bits of j'
+    float *As = reinterpret_cast<float *>(offB + TJ + ((RPB * (TI + TJ) + TI + TJ) & 1));   // [RPB][TK][TIp], 16 B aligned
+    float *Bs = As + ((RPB * TK * TIp + 3) & ~3);                                     // [RPB][TK][TJp], 16 B aligned
 
     const long long bid = blockIdx.x;
-    const int tjb = (int)(bid % a.tiles_j);
-    const int tib = (int)((bid / a.tiles_j) % a.tiles_i);
-    const long long rg = bid / ((long long)a.tiles_j * a.tiles_i);
-    const int nti = TI / MI, ntj = TJ / MJ, tpr = nti * ntj;
+    const int tjb = (int)(bid & ((1ll << a.lgTilesJ) - 1));
+    const int tib = (int)((bid >> a.lgTilesJ) & ((1ll << a.lgTilesI) - 1));
+    const long long rg = bid >> (a.lgTilesJ + a.lgTilesI);
+    const int lg_ntj = lgTJ - LGMJ, lg_tpr = (lgTI - LGMI) + lg_ntj;
     const int tid = threadIdx.x;
-    const int row_l = tid / tpr, within = tid % tpr;
-    const int ti = within / ntj, tj = within % ntj;
+    const int row_l = tid >> lg_tpr, within = tid & ((1 << lg_tpr) - 1);
+    const int ti = within >> lg_ntj, tj = within & ((1 << lg_ntj) - 1);
     const long long K = 1ll << a.lgK;
     const long long M = 1ll << a.lgM, N = 1ll << a.lgN;
 
-    // operand row offsets (in floats) of every (row, i) and (row, j) this block touches
+    // operand row offsets (in floats) of every (row, i) and (row, j) this block touches; C offset bits of i' and j'
     for (int e = tid; e < RPB * TI; e += 256) {
-        const int rl = e / TI, i = e % TI;
-        const long long r = rg * RPB + rl;
+        const int rl = e >> lgTI, i = e & (TI - 1);
+        const long long r = (rg << a.lgRPB) + rl;
+        const unsigned long long ip = ((unsigned long long)tib << lgTI) + i;
         unsigned long long off = ~0ull;
         if (r < a.R) {
-            const unsigned long long ip = (unsigned long long)tib * TI + i;
             if (a.A.use_map) off = (bitmap_apply(a.A.in_map, ip) | a.A.in_or) << a.lgK;
             else {
                 const unsigned long long row = a.A.keys ? (unsigned long long)a.A.keys[r] : (unsigned long long)r;
@@ -95,13 +100,14 @@ __global__ void __launch_bounds__(256) step_tile_kernel(const StepArgs a) {
             }
         }
         rowA[e] = off;
+        if (rl == 0) offA[i] = bitmap_apply(a.outA, ip);
     }
     for (int e = tid; e < RPB * TJ; e += 256) {
-        const int rl = e / TJ, j = e % TJ;
-        const long long r = rg * RPB + rl;
+        const int rl = e >> lgTJ, j = e & (TJ - 1);
+        const long long r = (rg << a.lgRPB) + rl;
+        const unsigned long long jp = ((unsigned long long)tjb << lgTJ) + j;
         unsigned long long off = ~0ull;
         if (r < a.R) {
-            const unsigned long long jp = (unsigned long long)tjb * TJ + j;
             if (a.B.use_map) off = (bitmap_apply(a.B.in_map, jp) | a.B.in_or) << a.lgK;
             else {
                 const unsigned long long row = a.B.keys ? (unsigned long long)a.B.keys[r] : (unsigned long long)r;
@@ -109,6 +115,7 @@ __global__ void __launch_bounds__(256) step_tile_kernel(const StepArgs a) {
             }
         }
         rowB[e] = off;
+        if (rl == 0) offB[j] = bitmap_apply(a.outB, jp);
     }
     __syncthreads();
 
@@ -119,40 +126,40 @@ __global__ void __launch_bounds__(256) step_tile_kernel(const StepArgs a) {
         for (int y = 0; y < MJ; ++y) acc[x][y] = 0.f;
 
     for (long long k0 = 0; k0 < K; k0 += TK) {
-        if (TK >= 4) {
-            const int kq = TK / 4;
-            for (int e = tid; e < RPB * TI * kq; e += 256) {
-                const int k4 = e % kq, ri = e / kq;                 // ri = rl * TI + i
+        if (lgTK >= 2) {
+            const int lgkq = lgTK - 2;
+            for (int e = tid; e < (RPB << (lgTI + lgkq)); e += 256) {
+                const int k4 = e & ((1 << lgkq) - 1), ri = e >> lgkq;          // ri = rl * TI + i
                 const unsigned long long off = rowA[ri];
                 float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
                 if (off != ~0ull) v = __ldg(reinterpret_cast<const float4 *>(a.A.base + off + k0) + k4);
-                float *dst = As + ((ri / TI) * TK + k4 * 4) * TIp + (ri % TI);
+                float *dst = As + (((ri >> lgTI) << lgTK) + k4 * 4) * TIp + (ri & (TI - 1));
                 dst[0] = v.x; dst[TIp] = v.y; dst[2 * TIp] = v.z; dst[3 * TIp] = v.w;
             }
-            for (int e = tid; e < RPB * TJ * kq; e += 256) {
-                const int k4 = e % kq, rj = e / kq;
+            for (int e = tid; e < (RPB << (lgTJ + lgkq)); e += 256) {
+                const int k4 = e & ((1 << lgkq) - 1), rj = e >> lgkq;
                 const unsigned long long off = rowB[rj];
                 float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
                 if (off != ~0ull) v = __ldg(reinterpret_cast<const float4 *>(a.B.base + off + k0) + k4);
-                float *dst = Bs + ((rj / TJ) * TK + k4 * 4) * TJp + (rj % TJ);
+                float *dst = Bs + (((rj >> lgTJ) << lgTK) + k4 * 4) * TJp + (rj & (TJ - 1));
                 dst[0] = v.x; dst[TJp] = v.y; dst[2 * TJp] = v.z; dst[3 * TJp] = v.w;
             }
         } else {
-            for (int e = tid; e < RPB * TI * TK; e += 256) {
-                const int k = e % TK, ri = e / TK;
+            for (int e = tid; e < (RPB << (lgTI + lgTK)); e += 256) {
+                const int k = e & (TK - 1), ri = e >> lgTK;
                 const unsigned long long off = rowA[ri];
-                As[((ri / TI) * TK + k) * TIp + (ri % TI)] = (off != ~0ull) ? __ldg(a.A.base + off + k0 + k) : 0.f;
+                As[(((ri >> lgTI) << lgTK) + k) * TIp + (ri & (TI - 1))] = (off != ~0ull) ? __ldg(a.A.base + off + k0 + k) : 0.f;
             }
-            for (int e = tid; e < RPB * TJ * TK; e += 256) {
-                const int k = e % TK, rj = e / TK;
+            for (int e = tid; e < (RPB << (lgTJ + lgTK)); e += 256) {
+                const int k = e & (TK - 1), rj = e >> lgTK;
                 const unsigned long long off = rowB[rj];
-                Bs[((rj / TJ) * TK + k) * TJp + (rj % TJ)] = (off != ~0ull) ? __ldg(a.B.base + off + k0 + k) : 0.f;
+                Bs[(((rj >> lgTJ) << lgTK) + k) * TJp + (rj & (TJ - 1))] = (off != ~0ull) ? __ldg(a.B.base + off + k0 + k) : 0.f;
             }
         }
         __syncthreads();
         if (row_l < RPB) {
-            const float *ap = As + row_l * TK * TIp + ti * MI;
-            const float *bp = Bs + row_l * TK * TJp + tj * MJ;
+            const float *ap = As + (row_l << lgTK) * TIp + ti * MI;
+            const float *bp = Bs + (row_l << lgTK) * TJp + tj * MJ;
 #pragma unroll 4
             for (int k = 0; k < TK; ++k) {
                 float av[MI], bv[MJ];
@@ -169,18 +176,18 @@ __global__ void __launch_bounds__(256) step_tile_kernel(const StepArgs a) {
         __syncthreads();
     }
 
-    const long long r = rg * RPB + row_l;
+    const long long r = (rg << a.lgRPB) + row_l;
     if (row_l >= RPB || r >= a.R) return;
-    const unsigned long long i0 = (unsigned long long)tib * TI + ti * MI;
-    const unsigned long long j0 = (unsigned long long)tjb * TJ + tj * MJ;
+    const unsigned long long i0 = ((unsigned long long)tib << lgTI) + ti * MI;
+    const unsigned long long j0 = ((unsigned long long)tjb << lgTJ) + tj * MJ;
     if (i0 >= (unsigned long long)M || j0 >= (unsigned long long)N) return;
     float *crow = a.C + r * a.c_row_stride;
     unsigned long long ob[MJ];
 #pragma unroll
-    for (int y = 0; y < MJ; ++y) ob[y] = bitmap_apply(a.outB, j0 + y);
+    for (int y = 0; y < MJ; ++y) ob[y] = offB[tj * MJ + y];
 #pragma unroll
     for (int x = 0; x < MI; ++x) {
-        const unsigned long long oa = bitmap_apply(a.outA, i0 + x);
+        const unsigned long long oa = offA[ti * MI + x];
         if (MJ == 4 && a.vec_store) {
             *reinterpret_cast<float4 *>(crow + (oa | ob[0])) = make_float4(acc[x][0], acc[x][1], acc[x][2], acc[x][3]);
         } else {

@@ -91,6 +91,11 @@ struct tqc_plan {
     std::vector<cudaEvent_t> ev_pool;
     std::vector<int> ev_tags;          // tag of the launch that follows event i (same length as used events - 1)
     size_t ev_used = 0;
+    // independent table steps run on side streams next to the key kernel (fork/join by events on the caller's stream)
+    enum { N_LANES = 3 };
+    cudaStream_t lane[N_LANES] = {nullptr, nullptr, nullptr};
+    cudaEvent_t ev_fork = nullptr, ev_join[N_LANES] = {nullptr, nullptr, nullptr};
+    int tables_parallel = -1;          // -1 not decided; 0 serial; 1 fork/join
 };
 
 namespace {
@@ -150,14 +155,17 @@ int launch_tile(tqc_plan_t *pl, StepArgs &a, int tag, cudaStream_t st) {
     const long long RPB = std::max<long long>(1, 256 / tpr);
     long long TK = std::min<long long>(K, 16);
     const long long TIp = TI + (MI == 4 ? 4 : 1), TJp = TJ + (MJ == 4 ? 4 : 1);
-    auto smem_of = [&](long long tk) { return (size_t)(8 * RPB * (TI + TJ) + 4 * RPB * tk * (TIp + TJp)); };
+    auto smem_of = [&](long long tk) { return (size_t)(8 * RPB * (TI + TJ) + 8 * (TI + TJ) + 4 * RPB * tk * (TIp + TJp) + 32); };
     while (TK > 1 && smem_of(TK) > (size_t)96 * 1024) TK /= 2;
     if (smem_of(TK) > (size_t)kMaxDynSmem) return fail(TQC_E_TOO_LARGE, "internal: tile does not fit shared memory");
-    a.TI = (int)TI; a.TJ = (int)TJ; a.TK = (int)TK; a.RPB = (int)RPB;
-    a.tiles_i = (int)(M / TI); a.tiles_j = (int)(N / TJ);
+    auto lg = [](long long v) { int l = 0; while ((1ll << l) < v) ++l; return l; };
+    a.lgTI = lg(TI); a.lgTJ = lg(TJ); a.lgTK = lg(TK); a.lgRPB = lg(RPB);
+    a.lgTilesI = lg(M / TI); a.lgTilesJ = lg(N / TJ);
+    if ((1ll << a.lgTI) != TI || (1ll << a.lgTJ) != TJ || (1ll << a.lgTK) != TK || (1ll << a.lgRPB) != RPB)
+        return fail(TQC_E_TOO_LARGE, "internal: tile dimensions must be powers of two");
     a.vec_store = (MJ == 4 && a.outB.n >= 1 && a.outB.src[0] == 0 && a.outB.dst[0] == 0 && a.outB.len[0] >= 2) ? 1 : 0;
     const long long rgroups = (a.R + RPB - 1) / RPB;
-    const long long blocks = (long long)a.tiles_i * a.tiles_j * rgroups;
+    const long long blocks = ((M / TI) * (N / TJ)) * rgroups;
     if (blocks <= 0 || blocks > 0x7fffffffll) return fail(TQC_E_TOO_LARGE, "step needs more than 2^31 thread blocks");
     int rc;
     if ((rc = note_launch(pl, tag, st))) return rc;
@@ -771,6 +779,11 @@ void tqc_plan_destroy(tqc_plan_t *pl) {
     if (pl->d_chain) cudaFree(pl->d_chain);
     if (pl->jit_module && jit_api().ok) jit_api().ModuleUnload((CUmodule)pl->jit_module);
     for (cudaEvent_t e : pl->ev_pool) cudaEventDestroy(e);
+    if (pl->ev_fork) cudaEventDestroy(pl->ev_fork);
+    for (int l = 0; l < tqc_plan::N_LANES; ++l) {
+        if (pl->ev_join[l]) cudaEventDestroy(pl->ev_join[l]);
+        if (pl->lane[l]) { cudaStreamSynchronize(pl->lane[l]); cudaStreamDestroy(pl->lane[l]); }
+    }
     delete pl;
 }
 
@@ -927,6 +940,38 @@ int tqc_contract_states(tqc_plan_t *pl, const uint64_t *states_dev, size_t n_sta
     // phase T: nodes evaluated once per key (tables), independent of the batch
     CrossCtx cx;
     cx.ws = tables;
+    // Table steps whose operands are all leaves neither depend on one another nor share storage (plan.cpp releases a
+    // table's block only when another table step consumes it): they go to side streams and overlap the key kernel.
+    if (pl->tables_parallel < 0) {
+        int n_tab = 0;
+        bool leaf_only = true;
+        for (int t = 0; t < hp.m - 1; ++t) {
+            if (hp.nodes[hp.m + t].kind != tqc::NODE_TABLE) continue;
+            ++n_tab;
+            if (hp.steps[t].lhs >= hp.m || hp.steps[t].rhs >= hp.m) leaf_only = false;
+        }
+        pl->tables_parallel = (n_tab >= 1 && leaf_only && !getenv("TQC_NO_FORK")) ? 1 : 0;
+        if (pl->tables_parallel) {
+            TQC_CUDA(cudaEventCreateWithFlags(&pl->ev_fork, cudaEventDisableTiming));
+            for (int l = 0; l < tqc_plan::N_LANES; ++l) {
+                TQC_CUDA(cudaStreamCreateWithFlags(&pl->lane[l], cudaStreamNonBlocking));
+                TQC_CUDA(cudaEventCreateWithFlags(&pl->ev_join[l], cudaEventDisableTiming));
+            }
+        }
+    }
+    const bool fork = pl->tables_parallel == 1 && !pl->profile;
+    int lanes_used = 0;
+    if (fork) {
+        TQC_CUDA(cudaEventRecord(pl->ev_fork, st));
+        int next = 0;
+        for (int t = 0; t < hp.m - 1; ++t) {
+            if (hp.nodes[hp.m + t].kind != tqc::NODE_TABLE) continue;
+            const int l = next++ % tqc_plan::N_LANES;
+            if (l >= lanes_used) { TQC_CUDA(cudaStreamWaitEvent(pl->lane[l], pl->ev_fork, 0)); lanes_used = l + 1; }
+            if ((rc = launch_cross_step(pl, cx, t, pl->lane[l]))) return rc;
+        }
+        for (int l = 0; l < lanes_used; ++l) TQC_CUDA(cudaEventRecord(pl->ev_join[l], pl->lane[l]));
+    } else
     for (int t = 0; t < hp.m - 1; ++t)
         if (hp.nodes[hp.m + t].kind == tqc::NODE_TABLE && (rc = launch_cross_step(pl, cx, t, st))) return rc;
     // phase B: chunks of states
@@ -947,6 +992,7 @@ int tqc_contract_states(tqc_plan_t *pl, const uint64_t *states_dev, size_t n_sta
             tqc::key_kernel<<<grid, 256, 0, st>>>(ka);
             TQC_CUDA(cudaGetLastError());
         }
+        if (lo == 0) for (int l = 0; l < lanes_used; ++l) TQC_CUDA(cudaStreamWaitEvent(st, pl->ev_join[l], 0));   // join
         if (pl->chain) {
             tqc::ChainArgs ca;
             memset(&ca, 0, sizeof(ca));
