@@ -115,9 +115,85 @@ __device__ __forceinline__ void chain_outputs(const ChainStepCtx &c, int kspan) 
 // outputs o = lane + 32 p; they form an NI x NJ grid (NJ distinct j, NI distinct i) whose operand rows are loaded once per
 // 16-float slab of the bond and reused from registers.  With fewer outputs the bond is split over G lanes per output and
 // finished with warp shuffles.  emit(i, j, value) stores one result.
+// x = hi + lo with hi the nearest TF32 and lo the exact remainder (the tensor core reads its top 19 bits): the operands of
+// a 3xTF32 product
+__device__ __forceinline__ void tf32_split(float x, uint32_t &hi, uint32_t &lo) {
+    hi = (__float_as_uint(x) + 0x1000u) & 0xFFFFE000u;          // round-to-nearest TF32 of a finite x
+    lo = __float_as_uint(x - __uint_as_float(hi));              // exact remainder
+#if defined(TQC_MMA_MASK_LO)
+    lo &= 0xFFFFE000u;                                          // what the tensor core does with the low 13 bits anyway
+#endif
+}
+__device__ __forceinline__ void mma_tf32_16x8x8(float (&d)[4], const uint32_t (&a)[4], const uint32_t (&b)[2]) {
+    asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]));
+}
+
+// Warp-level tensor-core step for the larger outputs of a chain (M >= 16, N >= 8, K >= 8; at most 1024 outputs): the warp's
+// one state is an M x N x K product small enough for mma.sync fragments, far too small for a tcgen05 tile.  3xTF32
+// (lo*hi + hi*lo + hi*hi, fp32 accumulate); each lane loads 4 A and 2 B scalars per 16x8x8 block from the K-major rows
+// (conflict-free with the 4-float row pad) and splits them once per k-step.
+template <int LGM, int LGN, int LGK, int PA, int PB, class Emit>
+__device__ __forceinline__ void chain_step_mma(const float *pa, const float *pb, int lane, Emit emit) {
+    constexpr int MT = (1 << LGM) / 16, NT = (1 << LGN) / 8, K = 1 << LGK;
+    const int g = lane >> 2, t = lane & 3;
+    float acc[MT][NT][4];
+#pragma unroll
+    for (int mi = 0; mi < MT; ++mi)
+#pragma unroll
+        for (int nj = 0; nj < NT; ++nj)
+#pragma unroll
+            for (int e = 0; e < 4; ++e) acc[mi][nj][e] = 0.f;
+#pragma unroll
+    for (int k0 = 0; k0 < K; k0 += 8) {
+        uint32_t ah[MT][4], al[MT][4], bh[NT][2], bl[NT][2];
+#pragma unroll
+        for (int mi = 0; mi < MT; ++mi) {
+            const float *p = pa + (mi * 16 + g) * PA + k0 + t;
+            tf32_split(p[0], ah[mi][0], al[mi][0]);
+            tf32_split(p[8 * PA], ah[mi][1], al[mi][1]);
+            tf32_split(p[4], ah[mi][2], al[mi][2]);
+            tf32_split(p[8 * PA + 4], ah[mi][3], al[mi][3]);
+        }
+#pragma unroll
+        for (int nj = 0; nj < NT; ++nj) {
+            const float *q = pb + (nj * 8 + g) * PB + k0 + t;
+            tf32_split(q[0], bh[nj][0], bl[nj][0]);
+            tf32_split(q[4], bh[nj][1], bl[nj][1]);
+        }
+#pragma unroll
+        for (int mi = 0; mi < MT; ++mi)
+#pragma unroll
+            for (int nj = 0; nj < NT; ++nj) {
+                mma_tf32_16x8x8(acc[mi][nj], al[mi], bh[nj]);       // small terms first
+                mma_tf32_16x8x8(acc[mi][nj], ah[mi], bl[nj]);
+                mma_tf32_16x8x8(acc[mi][nj], ah[mi], bh[nj]);
+            }
+    }
+#pragma unroll
+    for (int mi = 0; mi < MT; ++mi)
+#pragma unroll
+        for (int nj = 0; nj < NT; ++nj) {
+            emit(mi * 16 + g, nj * 8 + 2 * t, acc[mi][nj][0]);
+            emit(mi * 16 + g, nj * 8 + 2 * t + 1, acc[mi][nj][1]);
+            emit(mi * 16 + g + 8, nj * 8 + 2 * t, acc[mi][nj][2]);
+            emit(mi * 16 + g + 8, nj * 8 + 2 * t + 1, acc[mi][nj][3]);
+        }
+}
+
 template <int LGM, int LGN, int LGK, int PA, int PB, bool ROWSPLIT = false, class Emit>
 __device__ __forceinline__ void chain_step_spec(const float *pa, const float *pb, int lane, Emit emit) {
     constexpr int N = 1 << LGN, K = 1 << LGK, LGO = LGM + LGN, O = 1 << LGO;
+#if !defined(TQC_CHAIN_NO_MMA)
+    if constexpr (!ROWSPLIT && LGK >= 3 && LGO <= 10 && LGM >= 4 && LGN >= 3) {
+        chain_step_mma<LGM, LGN, LGK, PA, PB>(pa, pb, lane, emit);
+        return;
+    } else if constexpr (!ROWSPLIT && LGK >= 3 && LGO <= 10 && LGN >= 4 && LGM >= 3) {
+        chain_step_mma<LGN, LGM, LGK, PB, PA>(pb, pa, lane, [&](int j, int i, float v) { emit(i, j, v); });
+        return;
+    }
+#endif
     if constexpr (ROWSPLIT) {
         // M == 1 and B is read straight from global memory (each element is used once per state): out[j] = sum_k a[k] B[j][k].
         // The lanes split the bond so that every load of B is a contiguous 16 B x G segment of one row (coalesced), the

@@ -652,8 +652,9 @@ void chain_jit_build(tqc_plan_t *pl) {
     nvrtcProgram prog;
     if (api.CreateProgram(&prog, src.c_str(), "chain_spec.cu", 0, nullptr, nullptr) != NVRTC_SUCCESS) { pl->jit_note = "nvrtcCreateProgram failed"; return; }
     const std::string inc = "-I" + dir;
-    const char *opts[] = {"--gpu-architecture=sm_100a", "-std=c++17", inc.c_str(), "-lineinfo"};
-    const nvrtcResult rc = api.CompileProgram(prog, 4, opts);
+    const char *opts[] = {"--gpu-architecture=sm_100a", "-std=c++17", inc.c_str(), "-lineinfo", "-DTQC_CHAIN_NO_MMA"};
+    if (getenv("TQC_MMA_MASK_LO")) opts[4] = "-DTQC_MMA_MASK_LO";
+    const nvrtcResult rc = api.CompileProgram(prog, getenv("TQC_CHAIN_NO_MMA") || getenv("TQC_MMA_MASK_LO") ? 5 : 4, opts);
     if (rc != NVRTC_SUCCESS) {
         size_t n = 0;
         api.GetProgramLogSize(prog, &n);
