@@ -286,6 +286,10 @@ __device__ __forceinline__ void chain_step_spec(const float *pa, const float *pb
     }
 }
 
+__device__ __forceinline__ void chain_cp16(uint32_t dst_smem, const float *src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst_smem), "l"(src) : "memory");
+}
+
 // what a state's steps see: the warp's stage buffer of the current state, its intermediates, this state's keys (one per lane)
 struct ChainStateCtx {
     const ChainArgs *a;
@@ -347,6 +351,11 @@ __device__ __forceinline__ void chain_body(const ChainArgs &a) {
     float *inter = scr + 2 * a.stage_floats;
     auto issue_gather = [&](uint32_t key_of_state, int buf) {
         const uint32_t dst_base = (uint32_t)__cvta_generic_to_shared(scr + buf * a.stage_floats);
+        if constexpr (Spec::kOwnGather) {                                    // plan-specialised: straight-line copies
+            Spec::gather(a, key_of_state, dst_base, lane);
+            asm volatile("cp.async.commit_group;" ::: "memory");
+            return;
+        }
 #pragma unroll
         for (int q = 0; q < CHAIN_MAX_F4; ++q) {
             if (q * 32 < a.total_f4) {                                       // uniform
@@ -383,6 +392,8 @@ __device__ __forceinline__ void chain_body(const ChainArgs &a) {
 }
 
 struct ChainInterp {
+    static constexpr bool kOwnGather = false;
+    static __device__ __forceinline__ void gather(const ChainArgs &, uint32_t, uint32_t, int) {}
     static __device__ __forceinline__ void run(const ChainStateCtx &sc) {
         const ChainArgs &a = *sc.a;
         for (int t = 0; t < a.n_steps; ++t) {

@@ -634,7 +634,37 @@ std::string chain_source(const tqc_plan_t *pl) {
         }
         src += "      });\n      __syncwarp(); }\n";
     }
-    src += "  }\n};\n}  // namespace tqc\n"
+    src += "  }\n";
+    // the staged operands of one state: for every 32-chunk slot the lane ranges of the gathers it covers, with the row
+    // size, the padding and the destination as constants (the generic kernel reads the same from a shared-memory table)
+    if (getenv("TQC_CHAIN_TABLE_GATHER")) src += "  static constexpr bool kOwnGather = false;\n  static __device__ __forceinline__ void gather(const ChainArgs &, uint32_t, uint32_t, int) {}\n";
+    else {
+        src += "  static constexpr bool kOwnGather = true;\n"
+               "  static __device__ __forceinline__ void gather(const ChainArgs &a, uint32_t key, uint32_t dst, int lane) {\n";
+        const int ng = (int)pl->chain_gather.size();
+        for (int gi = 0; gi < ng; ++gi) {
+            const tqc::ChainGather &gg = pl->chain_gather[gi];
+            const std::string base = gg.table_ofs >= 0 ? "a.tables + " + std::to_string(gg.table_ofs) + "ll" : "a.g[" + std::to_string(gi) + "].base";
+            src += "    const float *s" + std::to_string(gi) + " = (" + base + ") + ((size_t)__shfl_sync(0xffffffffu, key, " +
+                   std::to_string(gg.key_slot) + ") << " + std::to_string(gg.lg_floats) + ");\n";
+        }
+        for (int q = 0; q * 32 < pl->chain_f4; ++q) {
+            for (int gi = 0; gi < ng; ++gi) {
+                const tqc::ChainGather &gg = pl->chain_gather[gi];
+                const int f_end = gi + 1 < ng ? pl->chain_gather[gi + 1].f4_begin : pl->chain_f4;
+                const int lo = std::max(gg.f4_begin, q * 32), hi = std::min(f_end, q * 32 + 32);
+                if (lo >= hi) continue;
+                const int l0 = lo - q * 32, l1 = hi - q * 32, c0 = lo - gg.f4_begin;
+                const std::string cexp = std::to_string(c0 - l0) + " + lane";
+                const std::string pad = gg.lgK >= 2 ? "x + ((x >> " + std::to_string(gg.lgK) + ") << 2)" : std::string("x");
+                src += "    " + (l0 == 0 && l1 == 32 ? std::string("") : "if (lane >= " + std::to_string(l0) + " && lane < " + std::to_string(l1) + ") ") +
+                       "{ const int x = 4 * (" + cexp + "); chain_cp16(dst + 4u * (uint32_t)(" + std::to_string(gg.smem_ofs) + " + " + pad +
+                       "), s" + std::to_string(gi) + " + x); }\n";
+            }
+        }
+        src += "  }\n";
+    }
+    src += "};\n}  // namespace tqc\n"
            "extern \"C\" __global__ void __launch_bounds__(256, 3) chain_spec_kernel(const tqc::ChainArgs a) {\n"
            "  tqc::chain_body<tqc::ChainPlanSpec>(a);\n}\n";
     return src;
