@@ -287,7 +287,7 @@ __device__ __forceinline__ void chain_step_spec(const float *pa, const float *pb
 }
 
 __device__ __forceinline__ void chain_cp16(uint32_t dst_smem, const float *src) {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst_smem), "l"(src) : "memory");
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst_smem), "l"(src) : "memory");   // .ca measured slower
 }
 
 // what a state's steps see: the warp's stage buffer of the current state, its intermediates, this state's keys (one per lane)
