@@ -18,6 +18,7 @@
 #include "kernels_simt.cuh"
 #include "kernels_tc.cuh"
 #include "kernels_chain.cuh"
+#include "kernels_cross.cuh"
 #include "plan.hpp"
 
 namespace {
@@ -274,6 +275,33 @@ int launch_cross_step(tqc_plan_t *pl, const CrossCtx &cx, int t, cudaStream_t st
         a.C = cx.ws + off;
     }
     if (!pa.build(a.outA) || !pb.build(a.outB)) return fail(TQC_E_TOO_LARGE, "bit map needs too many segments");
+    // short bond, many rows on both sides: warp-level 3xTF32 tensor-core tiles (kernels_cross.cuh)
+    if (pl->use_tcgen05 >= 0 && a.lgK >= 3 && a.lgK <= 6 && std::min(a.lgM, a.lgN) >= 6 && std::max(a.lgM, a.lgN) >= 7 &&
+        !getenv("TQC_NO_CROSS_MMA")) {
+        if (a.lgN < 7) { std::swap(a.A, a.B); std::swap(a.outA, a.outB); std::swap(a.lgM, a.lgN); }
+        a.lgTilesI = a.lgM - 6; a.lgTilesJ = a.lgN - 7;
+        a.vec_store = (a.outB.n >= 1 && a.outB.src[0] == 0 && a.outB.dst[0] == 0 && a.outB.len[0] >= 2) ? 1 : 0;
+        const long long blocks = 1ll << (a.lgTilesI + a.lgTilesJ);
+        if (blocks > 0x7fffffffll) return fail(TQC_E_TOO_LARGE, "step needs more than 2^31 thread blocks");
+        const size_t smem = tqc::cross_mma_smem(a.lgK);
+        static bool attr = false;
+        if (!attr) {
+            TQC_CUDA(cudaFuncSetAttribute(tqc::cross_mma_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+            TQC_CUDA(cudaFuncSetAttribute(tqc::cross_mma_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+            TQC_CUDA(cudaFuncSetAttribute(tqc::cross_mma_kernel<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+            TQC_CUDA(cudaFuncSetAttribute(tqc::cross_mma_kernel<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+            attr = true;
+        }
+        if ((rc = note_launch(pl, t, st))) return rc;
+        switch (a.lgK) {
+            case 3: tqc::cross_mma_kernel<3><<<(unsigned)blocks, 256, smem, st>>>(a); break;
+            case 4: tqc::cross_mma_kernel<4><<<(unsigned)blocks, 256, smem, st>>>(a); break;
+            case 5: tqc::cross_mma_kernel<5><<<(unsigned)blocks, 256, smem, st>>>(a); break;
+            default: tqc::cross_mma_kernel<6><<<(unsigned)blocks, 256, smem, st>>>(a); break;
+        }
+        TQC_CUDA(cudaGetLastError());
+        return 0;
+    }
     return launch_tile(pl, a, t, st);
 }
 
