@@ -79,3 +79,22 @@ def test_tc_step_with_batch_operand_and_signed_values():
     assert plan.step(1)["kernel_class"] == KERNEL_TCGEN05
     want, _ = direct_sum_c(net, T, bits)
     assert np.abs(got - want).max() <= TOL * np.abs(want).max(), np.abs(got - want).max() / np.abs(want).max()
+
+
+def test_warp_mma_paths_signed_values_and_ffma_agreement():
+    """cfg4's plan has both warp-level 3xTF32 paths: a 16x16x16 step inside the fused chain kernel and table steps with a
+    16-long bond and >= 2^10 rows per side (cross_mma_kernel).  Signed values (cancellation) against the direct sum, and
+    against the same plan with use_tcgen05 = -1 / use_chain = -2 (fp32 FFMA tables, generic chain kernel)."""
+    from tqc_inputs import configs
+    net = configs.cfg4_network()
+    rng = np.random.default_rng(17)
+    T = [(rng.random(net.tensor_shape(s)) * 2 - 1).astype(np.float32) for s in range(net.m)]
+    bits = random_states(net.n_qubits, 3000, 9)                         # ragged: not a multiple of 8 warps
+    got, plan = _run(net, T, bits, batch_hint=1 << 18)
+    assert plan.chain_status()[0] >= 1
+    ffma, _ = _run(net, T, bits, batch_hint=1 << 18, use_tcgen05=-1, use_chain=-2)
+    want, _ = direct_sum_c(net, T, bits[:48])
+    scale = np.abs(want).max()
+    assert np.abs(got[:48] - want).max() <= TOL * scale, np.abs(got[:48] - want).max() / scale
+    assert np.abs(ffma[:48] - want).max() <= TOL * scale
+    assert np.abs(got - ffma).max() <= TOL * np.abs(ffma).max()
