@@ -88,6 +88,12 @@ typedef struct {
     int32_t use_tcgen05;            /* 0 = default (on where a step qualifies), -1 = never (fp32 FFMA everywhere) */
     int32_t use_chain;              /* 0 = default (fused chain kernel when every per-state step is small, specialised for
                                        the plan at the first contract call), -1 = never, -2 = fused but not specialised */
+    int32_t n_slice_cuts;           /* index slicing (Fig. 6): these cut edges are not contracted as   */
+    const int32_t *slice_cuts;      /* bonds; the network is evaluated once per assignment of their bases (4^{n_slice_cuts}
+                                       smaller networks, planned once) and the results are summed.  HOST [n_slice_cuts] distinct
+                                       cut ids.  Tensors are still loaded whole; every intermediate that carried a sliced cut is 4x
+                                       smaller per cut.  Sliced plans run step by step (no fused chain); workspace sizes include
+                                       one partial-sum buffer (4 bytes per output; add it to tqc_plan_workspace_min_bytes). */
 } tqc_plan_opts;
 
 /* ---- planning (host only; no CUDA call) -------------------------------------------------
@@ -100,7 +106,8 @@ void tqc_plan_destroy(tqc_plan_t *plan);
 int tqc_plan_mode(const tqc_plan_t *plan);
 int tqc_plan_num_qubits(const tqc_plan_t *plan);
 int tqc_plan_num_subcircuits(const tqc_plan_t *plan);
-int tqc_plan_num_cuts(const tqc_plan_t *plan);
+int tqc_plan_num_cuts(const tqc_plan_t *plan);                   /* K of the caller's network (sliced cuts included) */
+int tqc_plan_num_sliced_cuts(const tqc_plan_t *plan);
 int tqc_plan_num_steps(const tqc_plan_t *plan);
 int tqc_plan_kmax(const tqc_plan_t *plan);                       /* max_t |E_a u E_b| */
 int tqc_plan_tensor_shape(const tqc_plan_t *plan, int s, int *c_s, int *o_s);

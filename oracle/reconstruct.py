@@ -176,3 +176,32 @@ def pairwise_contract(net, tensors, bits: np.ndarray, steps) -> np.ndarray:
         assert lab == [BATCH]
         val = val * v
     return val / (2.0 ** net.K)
+
+
+def slice_network(net, tensors, slice_cuts, assignment):
+    """Index slicing (Fig. 6): fix every cut in slice_cuts to the basis given by `assignment`
+    (same order).  Returns the smaller network (remaining cuts renumbered in order) and its tensors: each incident tensor
+    keeps only the rows whose digit on the sliced axis equals the fixed basis."""
+    from tqc_inputs.network import Network
+    fixed = dict(zip(slice_cuts, assignment))
+    keep = [e for e in range(net.K) if e not in fixed]
+    relabel = {e: i for i, e in enumerate(keep)}
+    Ts, sub_cuts = [], []
+    for s in range(net.m):
+        t = np.asarray(tensors[s], dtype=np.float64).reshape((4,) * net.c(s) + (-1,))
+        index = tuple(fixed[e] if e in fixed else slice(None) for e in net.sub_cuts[s]) + (slice(None),)
+        t = t[index]
+        left = [e for e in net.sub_cuts[s] if e not in fixed]
+        Ts.append(t.reshape(4 ** len(left), -1))
+        sub_cuts.append([relabel[e] for e in left])
+    return Network(net.n_qubits, [net.cuts[e] for e in keep], sub_cuts, net.sub_qubits), Ts
+
+
+def sliced_sum(net, tensors, bits: np.ndarray, slice_cuts) -> np.ndarray:
+    """The network as "a summation of smaller tensor networks": one direct sum per assignment of the sliced
+    cuts' bases, each with its own 2^{-K'}; the 1/2 of every sliced cut (reading G1) is applied to the total."""
+    acc = np.zeros(bits.shape[0], dtype=np.float64)
+    for assignment in itertools.product(range(4), repeat=len(slice_cuts)):
+        small, Ts = slice_network(net, tensors, list(slice_cuts), assignment)
+        acc += direct_sum(small, Ts, bits)
+    return acc / (2.0 ** len(slice_cuts))

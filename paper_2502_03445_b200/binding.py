@@ -32,7 +32,7 @@ EXPORTED = ["tqc_plan", "tqc_plan_destroy", "tqc_plan_mode", "tqc_plan_num_qubit
             "tqc_contract_distribution", "tqc_plan_launch_count", "tqc_last_error", "tqc_version",
             "tqc_plan_workspace_bytes_host", "tqc_contract_states_host", "tqc_contract_distribution_host",
             "tqc_plan_profile_enable", "tqc_plan_profile_read", "tqc_plan_chain_status", "tqc_hss_scores", "tqc_hss_select",
-            "tqc_hss_expand"]
+            "tqc_hss_expand", "tqc_plan_num_sliced_cuts"]
 
 
 class TqcError(RuntimeError):
@@ -51,7 +51,8 @@ class _NetworkDesc(ctypes.Structure):
 class _PlanOpts(ctypes.Structure):
     _fields_ = [("mode", c_int32), ("n_order_steps", c_int32), ("order", POINTER(c_int32)),
                 ("restarts", c_int32), ("seed", c_uint64), ("batch_hint", c_int64),
-                ("table_log2_floats_max", c_int32), ("use_tcgen05", c_int32), ("use_chain", c_int32)]
+                ("table_log2_floats_max", c_int32), ("use_tcgen05", c_int32), ("use_chain", c_int32),
+                ("n_slice_cuts", c_int32), ("slice_cuts", POINTER(c_int32))]
 
 
 def lib_path() -> str:
@@ -69,7 +70,7 @@ def _load() -> ctypes.CDLL:
     lib.tqc_plan_destroy.argtypes = [c_void_p]
     lib.tqc_plan_destroy.restype = None
     for name in ("tqc_plan_mode", "tqc_plan_num_qubits", "tqc_plan_num_subcircuits", "tqc_plan_num_cuts",
-                 "tqc_plan_num_steps", "tqc_plan_kmax"):
+                 "tqc_plan_num_steps", "tqc_plan_kmax", "tqc_plan_num_sliced_cuts"):
         getattr(lib, name).argtypes = [c_void_p]
     lib.tqc_plan_tensor_shape.argtypes = [c_void_p, c_int, POINTER(c_int), POINTER(c_int)]
     lib.tqc_plan_step.argtypes = [c_void_p, c_int] + [POINTER(c_int)] * 7
@@ -152,6 +153,8 @@ class Plan:
     @property
     def K(self) -> int: return _lib.tqc_plan_num_cuts(self._h)
     @property
+    def n_sliced_cuts(self) -> int: return _lib.tqc_plan_num_sliced_cuts(self._h)
+    @property
     def num_steps(self) -> int: return _lib.tqc_plan_num_steps(self._h)
     @property
     def kmax(self) -> int: return _lib.tqc_plan_kmax(self._h)
@@ -215,9 +218,10 @@ class Plan:
 
 
 def tqc_plan(net, mode: int = MODE_STATES, order=None, restarts: int = 0, seed: int = 0, batch_hint: int = 0,
-             table_log2_floats_max: int = 0, use_tcgen05: int = 0, use_chain: int = 0) -> Plan:
+             table_log2_floats_max: int = 0, use_tcgen05: int = 0, use_chain: int = 0, slice_cuts=None) -> Plan:
     """net: any object with n_qubits, cuts [(up, down)], sub_cuts [[cut ids]], sub_qubits [[qubit ids]]
-    (e.g. tqc_inputs.Network).  order: optional list of m-1 (lhs, rhs) node-id pairs."""
+    (e.g. tqc_inputs.Network).  order: optional list of m-1 (lhs, rhs) node-id pairs.  slice_cuts: cut ids evaluated by
+    index slicing (summed over their 4 bases) instead of being contracted as bonds."""
     m = len(net.sub_cuts)
     up, up_p = _i32(c[0] for c in net.cuts)
     down, down_p = _i32(c[1] for c in net.cuts)
@@ -227,8 +231,9 @@ def tqc_plan(net, mode: int = MODE_STATES, order=None, restarts: int = 0, seed: 
     qflat, qflat_p = _i32(q for x in net.sub_qubits for q in x)
     desc = _NetworkDesc(net.n_qubits, m, len(net.cuts), up_p, down_p, cofs_p, cflat_p, qofs_p, qflat_p)
     oflat, oflat_p = _i32(v for ab in (order or []) for v in ab)
+    sflat, sflat_p = _i32(slice_cuts or [])
     opts = _PlanOpts(mode, len(order) if order else 0, oflat_p, restarts, seed, batch_hint,
-                     table_log2_floats_max, use_tcgen05, use_chain)
+                     table_log2_floats_max, use_tcgen05, use_chain, len(slice_cuts) if slice_cuts else 0, sflat_p)
     h = c_void_p()
     _check(_lib.tqc_plan(byref(desc), byref(opts), byref(h)))
     return Plan(h.value)

@@ -77,6 +77,7 @@ struct RelayoutArgs {           // a1: dst[x][j] = scale * src[row_of(j)][x]
     const float *src;
     float *dst;
     BitMap row_of;              // device digit index j -> caller row index
+    unsigned long long row_or;  // fixed digits of the caller row index (sliced axes), 0 without slicing
     int lgRows, lgCols;         // caller layout: 2^lgRows rows (4^{c_s}) x 2^lgCols columns (2^{o_s})
     float scale;                // exact power of two 2^{-d_s}
 };

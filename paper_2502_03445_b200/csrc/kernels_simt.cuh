@@ -22,7 +22,7 @@ __global__ void __launch_bounds__(256) relayout_kernel(const RelayoutArgs a) {
     for (int jj = ty; jj < 32; jj += 8) {
         const long long j = bj * 32 + jj;
         if (j < rows && x < cols) {
-            const unsigned long long row = bitmap_apply(a.row_of, (unsigned long long)j);
+            const unsigned long long row = bitmap_apply(a.row_of, (unsigned long long)j) | a.row_or;
             tile[jj][tx] = a.src[row * cols + x];
         }
     }
@@ -251,6 +251,12 @@ __global__ void __launch_bounds__(256) gather_kernel(const GatherArgs a) {
 // per row, float4 loads, shuffle tree; HBM-bound (each tensor element read once).  `unscale` = 2^{d_j} undoes the exact
 // power of two folded in at load, so the score is that of the caller's values.
 // ---------------------------------------------------------------------------------------------
+// out[i] += part[i]: the sum over sliced-bond sub-networks
+__global__ void __launch_bounds__(256) accumulate_kernel(float *__restrict__ out, const float *__restrict__ part, long long n) {
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) out[i] += part[i];
+}
+
 template <int LANES>   // LANES = 32: one warp per row (many rows); LANES = 256: one block per row (few, long rows)
 __global__ void __launch_bounds__(256) hss_norm_kernel(const float *__restrict__ t, float *__restrict__ score, long long rows,
                                                         int lgCols, float unscale) {

@@ -10,6 +10,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <functional>
 #include <string>
 #include <vector>
 
@@ -97,6 +98,15 @@ struct tqc_plan {
     cudaStream_t lane[N_LANES] = {nullptr, nullptr, nullptr};
     cudaEvent_t ev_fork = nullptr, ev_join[N_LANES] = {nullptr, nullptr, nullptr};
     int tables_parallel = -1;          // -1 not decided; 0 serial; 1 fork/join
+    // bond slicing: hp describes the network WITHOUT the sliced cuts; a leaf keeps one re-laid-out
+    // sub-tensor per value of its sliced axes, the contract calls sum over all 4^{n_sliced} assignments
+    int K_full = 0;
+    std::vector<int> slice_cuts;                            // caller's cut ids; the first is the most significant digit
+    std::vector<std::vector<int>> full_axis;                // per leaf: caller axis position (0 = MS) of every kept axis
+    std::vector<std::vector<std::pair<int, int>>> sliced_axis;   // per leaf: (caller axis position, index into slice_cuts)
+    std::vector<int> c_full, d_extra;                       // per leaf: caller's c_s; sliced cuts whose downstream end it holds
+    std::vector<float *> d_leaf_all;                        // allocation per leaf: [4^{#sliced axes}][2^o][4^{c'}]
+    int n_sliced() const { return (int)slice_cuts.size(); }
 };
 
 namespace {
@@ -801,10 +811,51 @@ int tqc_plan(const tqc_network_desc *net, const tqc_plan_opts *opts, tqc_plan_t 
     }
     tqc_plan_t *pl = new tqc_plan_t();
     std::string err;
-    const int rc = tqc::build_plan(net->n_qubits, net->m, net->K, net->cut_up, net->cut_down, net->sub_cut_ofs,
-                                   net->sub_cuts, net->sub_qubit_ofs, net->sub_qubits, po, pl->hp, err);
+    int rc;
+    const int ns = opts ? opts->n_slice_cuts : 0;
+    if (ns < 0 || (ns > 0 && !opts->slice_cuts)) { delete pl; return fail(TQC_E_ARG, "n_slice_cuts > 0 but slice_cuts is null"); }
+    if (ns > 12) { delete pl; return fail(TQC_E_TOO_LARGE, "at most 12 sliced cuts (4^12 sub-networks)"); }
+    pl->K_full = net->K;
+    if (ns == 0) {
+        rc = tqc::build_plan(net->n_qubits, net->m, net->K, net->cut_up, net->cut_down, net->sub_cut_ofs,
+                             net->sub_cuts, net->sub_qubit_ofs, net->sub_qubits, po, pl->hp, err);
+    } else {
+        // the network without the sliced cuts: kept cuts renumbered in order, axis lists filtered
+        if (net->m < 1 || net->K < 0 || !net->sub_cut_ofs) { delete pl; return fail(TQC_E_ARG, "bad network description"); }
+        std::vector<int> relabel(net->K, 0), is_sliced(net->K, -1);
+        for (int i = 0; i < ns; ++i) {
+            const int e = opts->slice_cuts[i];
+            if (e < 0 || e >= net->K || is_sliced[e] >= 0) { delete pl; return fail(TQC_E_ARG, "slice_cuts must be distinct cut ids"); }
+            is_sliced[e] = i;
+            pl->slice_cuts.push_back(e);
+        }
+        std::vector<int32_t> up, down, ofs(1, 0), flat;
+        for (int e = 0; e < net->K; ++e)
+            if (is_sliced[e] < 0) { relabel[e] = (int)up.size(); up.push_back(net->cut_up[e]); down.push_back(net->cut_down[e]); }
+        pl->full_axis.resize(net->m); pl->sliced_axis.resize(net->m);
+        pl->c_full.assign(net->m, 0); pl->d_extra.assign(net->m, 0);
+        for (int s = 0; s < net->m; ++s) {
+            const int b = net->sub_cut_ofs[s], e1 = net->sub_cut_ofs[s + 1];
+            pl->c_full[s] = e1 - b;
+            for (int x = b; x < e1; ++x) {
+                const int e = net->sub_cuts[x];
+                if (e < 0 || e >= net->K) { delete pl; return fail(TQC_E_ARG, "cut id out of range in sub_cuts"); }
+                if (is_sliced[e] >= 0) {
+                    pl->sliced_axis[s].emplace_back(x - b, is_sliced[e]);
+                    if (net->cut_down[e] == s) pl->d_extra[s]++;
+                } else { flat.push_back(relabel[e]); pl->full_axis[s].push_back(x - b); }
+            }
+            // local slice digits in the order of slice_cuts (first = most significant)
+            std::sort(pl->sliced_axis[s].begin(), pl->sliced_axis[s].end(),
+                      [](const std::pair<int, int> &a, const std::pair<int, int> &b2) { return a.second < b2.second; });
+            ofs.push_back((int32_t)flat.size());
+        }
+        rc = tqc::build_plan(net->n_qubits, net->m, (int)up.size(), up.data(), down.data(), ofs.data(), flat.data(),
+                             net->sub_qubit_ofs, net->sub_qubits, po, pl->hp, err);
+    }
     if (rc != 0) { delete pl; return fail(rc, err); }
     pl->use_tcgen05 = use_tc;
+    pl->d_leaf_all.assign(pl->hp.m, nullptr);
     pl->d_leaf.assign(pl->hp.m, nullptr);
     pl->loaded.assign(pl->hp.m, 0);
     for (int t = 0; t < pl->hp.m - 1; ++t) {
@@ -815,6 +866,7 @@ int tqc_plan(const tqc_network_desc *net, const tqc_plan_opts *opts, tqc_plan_t 
             s.kernel_class = TQC_KERNEL_TCGEN05;
     }
     pl->chain_mode = opts ? opts->use_chain : 0;
+    if (pl->n_sliced()) pl->chain_mode = -1;                // the chain's device step table holds leaf pointers; sliced plans run per step
     pl->chain = pl->chain_mode != -1 && build_chain(pl);
     if (pl->chain) pl->hp.ws_floats_per_state = 0;          // intermediates live in shared memory
     if (pl->chain) {
@@ -831,7 +883,10 @@ int tqc_plan(const tqc_network_desc *net, const tqc_plan_opts *opts, tqc_plan_t 
 
 void tqc_plan_destroy(tqc_plan_t *pl) {
     if (!pl) return;
-    for (float *p : pl->d_leaf) if (p) cudaFree(p);
+    for (size_t x = 0; x < pl->d_leaf.size(); ++x) {
+        float *p = pl->n_sliced() ? pl->d_leaf_all[x] : pl->d_leaf[x];
+        if (p) cudaFree(p);
+    }
     if (pl->d_slot_ofs) cudaFree(pl->d_slot_ofs);
     if (pl->d_slot_qubits) cudaFree(pl->d_slot_qubits);
     if (pl->d_staging) cudaFree(pl->d_staging);
@@ -849,13 +904,14 @@ void tqc_plan_destroy(tqc_plan_t *pl) {
 int tqc_plan_mode(const tqc_plan_t *pl) { return pl ? pl->hp.mode : TQC_E_ARG; }
 int tqc_plan_num_qubits(const tqc_plan_t *pl) { return pl ? pl->hp.n : TQC_E_ARG; }
 int tqc_plan_num_subcircuits(const tqc_plan_t *pl) { return pl ? pl->hp.m : TQC_E_ARG; }
-int tqc_plan_num_cuts(const tqc_plan_t *pl) { return pl ? pl->hp.K : TQC_E_ARG; }
+int tqc_plan_num_cuts(const tqc_plan_t *pl) { return pl ? pl->K_full : TQC_E_ARG; }
+int tqc_plan_num_sliced_cuts(const tqc_plan_t *pl) { return pl ? pl->n_sliced() : TQC_E_ARG; }
 int tqc_plan_num_steps(const tqc_plan_t *pl) { return pl ? (int)pl->hp.steps.size() : TQC_E_ARG; }
 int tqc_plan_kmax(const tqc_plan_t *pl) { return pl ? pl->hp.kmax : TQC_E_ARG; }
 
 int tqc_plan_tensor_shape(const tqc_plan_t *pl, int s, int *c_s, int *o_s) {
     if (!pl || s < 0 || s >= pl->hp.m) return fail(TQC_E_ARG, "bad plan or subcircuit id");
-    if (c_s) *c_s = pl->hp.c(s);
+    if (c_s) *c_s = pl->n_sliced() ? pl->c_full[s] : pl->hp.c(s);
     if (o_s) *o_s = pl->hp.o(s);
     return 0;
 }
@@ -911,25 +967,31 @@ size_t tqc_plan_workspace_bytes(const tqc_plan_t *pl, size_t n_states, int prefi
     const HostPlan &hp = pl->hp;
     if (hp.mode == TQC_MODE_STATES) {
         const size_t cap = (std::max<size_t>(n_states, 1) + 63) / 64 * 64;
-        return states_fixed_bytes(hp) + align256(states_bytes_per_state(hp) * cap) + 256;
+        return states_fixed_bytes(hp) + align256(states_bytes_per_state(hp) * cap) + 256 + (pl->n_sliced() ? align256(n_states * 4) : 0);
     }
     std::vector<int> fb;
     std::vector<int64_t> off;
-    const int64_t floats = tqc::distribution_layout(hp, std::max(0, std::min(prefix_bits, hp.n)), fb, off);
-    return align256((size_t)floats * 4) + 256;
+    const int pbits = std::max(0, std::min(prefix_bits, hp.n));
+    const int64_t floats = tqc::distribution_layout(hp, pbits, fb, off);
+    return align256((size_t)floats * 4) + 256 + (pl->n_sliced() ? align256(((size_t)4) << (hp.n - pbits)) : 0);
 }
 
 int tqc_load_subcircuit_tensors(tqc_plan_t *pl, int s, const float *data, size_t n_elems, int on_device, void *stream) {
     if (!pl || !data) return fail(TQC_E_ARG, "null argument");
     HostPlan &hp = pl->hp;
     if (s < 0 || s >= hp.m) return fail(TQC_E_ARG, "subcircuit id out of range");
-    const int c = hp.c(s), o = hp.o(s);
-    const size_t need = (size_t)1 << (2 * c + o);
+    const bool sliced = pl->n_sliced() > 0;
+    const int c = hp.c(s), o = hp.o(s);                     // c: axes the plan contracts (without the sliced ones)
+    const int cf = sliced ? pl->c_full[s] : c;              // axes of the caller's tensor
+    const int nsl = sliced ? (int)pl->sliced_axis[s].size() : 0;
+    const size_t need = (size_t)1 << (2 * cf + o);
     if (n_elems != need) return fail(TQC_E_SHAPE, "n_elems must be 4^c_s * 2^o_s = " + std::to_string(need));
     cudaStream_t st = (cudaStream_t)stream;
     int rc = ensure_meta(pl);
     if (rc) return rc;
-    if (!pl->d_leaf[s]) TQC_CUDA(cudaMalloc(&pl->d_leaf[s], need * sizeof(float)));
+    float *&store = sliced ? pl->d_leaf_all[s] : pl->d_leaf[s];
+    if (!store) TQC_CUDA(cudaMalloc(&store, need * sizeof(float)));
+    if (sliced) pl->d_leaf[s] = store;
     const float *src = data;
     if (!on_device) {
         if (pl->staging_elems < need) {
@@ -942,32 +1004,106 @@ int tqc_load_subcircuit_tensors(tqc_plan_t *pl, int s, const float *data, size_t
     }
     RelayoutArgs a;
     memset(&a, 0, sizeof(a));
-    a.src = src; a.dst = pl->d_leaf[s];
+    a.src = src;
     a.lgRows = 2 * c; a.lgCols = o;
-    a.scale = std::ldexp(1.0f, -hp.d[s]);
+    // 2^{-d_s}: one factor 1/2 per cut whose downstream end is s (reading G2), the sliced ones included
+    a.scale = std::ldexp(1.0f, -(hp.d[s] + (sliced ? pl->d_extra[s] : 0)));
     // device digit x (most significant first) holds cut layout[x]; the caller's digit order is sub_cuts[s]
     const Node &leaf = hp.nodes[s];
     std::vector<int> layout = leaf.layout;
     if (layout.empty()) layout = leaf.open;               // m == 1 has no consumer: keep ascending order
     BitPairs bp;
     for (int x = 0; x < c; ++x) {
-        const int y = index_of(hp.sub_cuts[s], layout[x]);
-        bp.add_run(2 * (c - 1 - x), 2 * (c - 1 - y), 2);
+        const int y = index_of(hp.sub_cuts[s], layout[x]);            // position among the kept axes
+        const int yf = sliced ? pl->full_axis[s][y] : y;              // position among the caller's axes
+        bp.add_run(2 * (c - 1 - x), 2 * (cf - 1 - yf), 2);
     }
     if (!bp.build(a.row_of)) return fail(TQC_E_TOO_LARGE, "bit map needs too many segments");
     const long long tiles = (((1ll << o) + 31) / 32) * (((1ll << (2 * c)) + 31) / 32);
     const bool prof = pl->profile;
     pl->profile = false;                                   // loads are not part of the profiled contract call
-    rc = note_launch(pl, TAG_RELAYOUT, st);
+    // one re-laid-out sub-tensor per value of the sliced axes (a single one without slicing)
+    for (long long v = 0; v < (1ll << (2 * nsl)); ++v) {
+        a.dst = store + (size_t)v * ((size_t)1 << (2 * c + o));
+        a.row_or = 0;
+        for (int x = 0; x < nsl; ++x) {                                // local digit x, first = most significant
+            const unsigned long long digit = (unsigned long long)(v >> (2 * (nsl - 1 - x))) & 3ull;
+            a.row_or |= digit << (2 * (cf - 1 - pl->sliced_axis[s][x].first));
+        }
+        rc = note_launch(pl, TAG_RELAYOUT, st);
+        if (rc) break;
+        tqc::relayout_kernel<<<(unsigned)tiles, 256, 0, st>>>(a);
+    }
     pl->profile = prof;
     if (rc) return rc;
-    tqc::relayout_kernel<<<(unsigned)tiles, 256, 0, st>>>(a);
     TQC_CUDA(cudaGetLastError());
     pl->loaded[s] = 1;
     return 0;
 }
 
+namespace {
+// point every leaf at the sub-tensor of slice assignment `assign` (base-4 digits in the order of slice_cuts, first = MS)
+void select_slice(tqc_plan_t *pl, long long assign) {
+    const int ns = pl->n_sliced();
+    for (int s = 0; s < pl->hp.m; ++s) {
+        if (!pl->d_leaf_all[s]) continue;
+        size_t local = 0;
+        for (const auto &ax : pl->sliced_axis[s]) local = local * 4 + (size_t)((assign >> (2 * (ns - 1 - ax.second))) & 3);
+        pl->d_leaf[s] = pl->d_leaf_all[s] + local * ((size_t)1 << (2 * pl->hp.c(s) + pl->hp.o(s)));
+    }
+}
+int contract_states_impl(tqc_plan_t *pl, const uint64_t *states_dev, size_t n_states, float *out_dev, void *workspace_dev,
+                         size_t workspace_bytes, void *stream);
+int contract_distribution_impl(tqc_plan_t *pl, uint64_t prefix_value, int prefix_bits, float *out_dev, void *workspace_dev,
+                               size_t workspace_bytes, void *stream);
+// sum over the 4^{n_sliced} sub-networks: the first lands in out, the others in a partial-sum buffer at the head of the
+// workspace and are added ("a summation of smaller tensor networks")
+int sliced_sum(tqc_plan_t *pl, float *out_dev, size_t n_out, void *workspace_dev, size_t workspace_bytes, void *stream,
+               const std::function<int(float *, void *, size_t)> &once) {
+    if (!workspace_dev || ((uintptr_t)workspace_dev & 255) != 0) return fail(TQC_E_ARG, "workspace must be non-null and 256-byte aligned");
+    const size_t tb = align256(n_out * 4);
+    if (workspace_bytes < tb) return fail(TQC_E_WORKSPACE, "workspace smaller than the partial-sum buffer of a sliced plan");
+    float *tmp = (float *)workspace_dev;
+    char *rest = (char *)workspace_dev + tb;
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = 0;
+    for (long long a = 0; a < (1ll << (2 * pl->n_sliced())) && !rc; ++a) {
+        select_slice(pl, a);
+        rc = once(a == 0 ? out_dev : tmp, rest, workspace_bytes - tb);
+        if (!rc && a > 0) {
+            pl->launches++;
+            tqc::accumulate_kernel<<<(unsigned)std::min<size_t>((n_out + 1023) / 1024, 148 * 16), 256, 0, st>>>(out_dev, tmp, (long long)n_out);
+            if (cudaGetLastError() != cudaSuccess) rc = fail(TQC_E_CUDA, "accumulate_kernel launch failed");
+        }
+    }
+    select_slice(pl, 0);
+    return rc;
+}
+}  // namespace
+
 int tqc_contract_states(tqc_plan_t *pl, const uint64_t *states_dev, size_t n_states, float *out_dev, void *workspace_dev,
+                        size_t workspace_bytes, void *stream) {
+    if (!pl) return fail(TQC_E_ARG, "null plan");
+    if (pl->n_sliced() == 0 || n_states == 0) return contract_states_impl(pl, states_dev, n_states, out_dev, workspace_dev, workspace_bytes, stream);
+    if (!out_dev) return fail(TQC_E_ARG, "null states/out pointer");
+    return sliced_sum(pl, out_dev, n_states, workspace_dev, workspace_bytes, stream, [&](float *dst, void *ws, size_t wb) {
+        return contract_states_impl(pl, states_dev, n_states, dst, ws, wb, stream);
+    });
+}
+
+int tqc_contract_distribution(tqc_plan_t *pl, uint64_t prefix_value, int prefix_bits, float *out_dev, void *workspace_dev,
+                              size_t workspace_bytes, void *stream) {
+    if (!pl) return fail(TQC_E_ARG, "null plan");
+    if (pl->n_sliced() == 0) return contract_distribution_impl(pl, prefix_value, prefix_bits, out_dev, workspace_dev, workspace_bytes, stream);
+    if (!out_dev) return fail(TQC_E_ARG, "null out pointer");
+    if (prefix_bits < 0 || prefix_bits > pl->hp.n) return fail(TQC_E_ARG, "prefix_bits out of range");
+    if (pl->hp.n - prefix_bits > 34) return fail(TQC_E_TOO_LARGE, "more than 2^34 outputs; raise prefix_bits");
+    return sliced_sum(pl, out_dev, (size_t)1 << (pl->hp.n - prefix_bits), workspace_dev, workspace_bytes, stream,
+                      [&](float *dst, void *ws, size_t wb) { return contract_distribution_impl(pl, prefix_value, prefix_bits, dst, ws, wb, stream); });
+}
+
+namespace {
+int contract_states_impl(tqc_plan_t *pl, const uint64_t *states_dev, size_t n_states, float *out_dev, void *workspace_dev,
                         size_t workspace_bytes, void *stream) {
     if (!pl) return fail(TQC_E_ARG, "null plan");
     HostPlan &hp = pl->hp;
@@ -1094,7 +1230,7 @@ int tqc_contract_states(tqc_plan_t *pl, const uint64_t *states_dev, size_t n_sta
     return prof_close(pl, st);
 }
 
-int tqc_contract_distribution(tqc_plan_t *pl, uint64_t prefix_value, int prefix_bits, float *out_dev, void *workspace_dev,
+int contract_distribution_impl(tqc_plan_t *pl, uint64_t prefix_value, int prefix_bits, float *out_dev, void *workspace_dev,
                               size_t workspace_bytes, void *stream) {
     if (!pl) return fail(TQC_E_ARG, "null plan");
     HostPlan &hp = pl->hp;
@@ -1149,6 +1285,7 @@ int tqc_contract_distribution(tqc_plan_t *pl, uint64_t prefix_value, int prefix_
     }
     return prof_close(pl, st);
 }
+}  // namespace
 
 // ---- host-buffer entry points: staging carved from the front of the workspace ------------------
 size_t tqc_plan_workspace_bytes_host(const tqc_plan_t *pl, size_t n_states, int prefix_bits) {
@@ -1231,6 +1368,7 @@ int tqc_hss_scores(tqc_plan_t *pl, int s, float *scores_dev, void *stream) {
     const HostPlan &hp = pl->hp;
     if (s < 0 || s >= hp.m) return fail(TQC_E_ARG, "subcircuit id out of range");
     if (!pl->loaded[s]) return fail(TQC_E_STATE, "tensor of subcircuit " + std::to_string(s) + " not loaded");
+    if (pl->n_sliced()) return fail(TQC_E_STATE, "state norms need the whole tensor: build the plan without slice_cuts");
     const long long rows = 1ll << hp.o(s);
     const int lgCols = 2 * hp.c(s);
     cudaStream_t st = (cudaStream_t)stream;

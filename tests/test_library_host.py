@@ -112,3 +112,25 @@ def test_restarts_never_worse_and_deterministic():
     b = tqc.tqc_plan(net, restarts=16, seed=7)
     assert a.serialize() == b.serialize()
     assert a.cost_log2 <= base.cost_log2 + 1e-9
+
+
+def test_sliced_plan_is_the_plan_of_the_smaller_network():
+    """Index slicing: the library plans the network without the sliced cuts once; its blob is
+    byte-identical to the reference planner's on the oracle-side reduced network; shapes still describe the caller's tensors."""
+    from oracle import reconstruct as R
+    from tqc_inputs import random_tensors
+    net = configs.random_network(5, 8, seed=77, o_lo=1, o_hi=3)
+    T = random_tensors(net, 1)
+    for slice_cuts in ([3], [0, 5], [7, 2, 4]):
+        small, _ = R.slice_network(net, T, slice_cuts, [0] * len(slice_cuts))
+        plan = tqc.tqc_plan(net, tqc.MODE_STATES, slice_cuts=slice_cuts, use_chain=-1)
+        ref = tqc.tqc_plan(small, tqc.MODE_STATES, use_chain=-1)
+        assert plan.serialize() == ref.serialize()
+        assert plan.serialize() == P.serialize(P.plan(small, 0))
+        assert plan.K == net.K and plan.n_sliced_cuts == len(slice_cuts)
+        assert [plan.tensor_shape(s) for s in range(net.m)] == [(net.c(s), net.o(s)) for s in range(net.m)]
+        assert plan.workspace_bytes(1000) >= ref.workspace_bytes(1000) + 4000
+    with pytest.raises(tqc.TqcError):
+        tqc.tqc_plan(net, tqc.MODE_STATES, slice_cuts=[1, 1])
+    with pytest.raises(tqc.TqcError):
+        tqc.tqc_plan(net, tqc.MODE_STATES, slice_cuts=[net.K])

@@ -193,3 +193,14 @@ def test_cfg5_network_shape_and_rank_one():
     assert all(2 <= net.o(s) <= 4 for s in range(52))
     p = P.plan(net)
     assert len(p["steps"]) == 51
+
+
+@pytest.mark.parametrize("slice_cuts", [[2], [0, 3], [4, 1, 2]])
+def test_sliced_sum_is_the_network(slice_cuts):
+    """Pi-5 for oracle.reconstruct.sliced_sum: any set of sliced cuts (two on one tensor, parallel ones) sums back to Eq. 1."""
+    net = configs.random_network(4, 6, 131, o_lo=1, o_hi=2)
+    T = random_tensors(net, 132)
+    bits = random_states(net.n_qubits, 10, 133)
+    assert np.allclose(R.sliced_sum(net, T, bits, slice_cuts), R.direct_sum(net, T, bits), rtol=1e-12)
+    small, Ts = R.slice_network(net, T, slice_cuts, [1] * len(slice_cuts))
+    assert small.K == net.K - len(slice_cuts) and [t.shape[0] for t in Ts] == [4 ** small.c(s) for s in range(net.m)]
