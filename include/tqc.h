@@ -101,6 +101,17 @@ typedef struct {
  * the paper delegates this to CoTenGra, this library ships a deterministic greedy planner)
  * + device layouts + kernel class per step.  *out is library-owned until tqc_plan_destroy. */
 int tqc_plan(const tqc_network_desc *net, const tqc_plan_opts *opts, tqc_plan_t **out);
+/* Which cuts to slice: the paper's two-level strategy, host only, deterministic.
+ * Level 1 - while a subcircuit tensor of one sub-network (4^{c'_s} 2^{o_s} floats, c'_s = unsliced incident cuts) exceeds
+ *   2^{max_log2_input_floats}: slice "the most size-reducing cut edge", i.e. among the cuts touching an oversize tensor
+ *   the one whose two tensors are largest (larger one first, then the smaller one; tie: smaller cut id).
+ * Level 2 - while the largest intermediate of the greedy plan (4^{open cuts} floats per state, x 2^{carried output bits}
+ *   in distribution mode) exceeds 2^{max_log2_intermediate_floats}: slice the cut whose removal leaves the smallest
+ *   largest-intermediate, then the smallest total multiplication count, then the smaller id (one plan per candidate).
+ * slice_cuts: HOST [K] out, in pick order; *n_slice_cuts out.  opts supplies mode / planner options (order is ignored).
+ * TQC_E_INFEASIBLE when a limit cannot be met.  Pass the result as tqc_plan_opts.slice_cuts. */
+int tqc_choose_slice_cuts(const tqc_network_desc *net, const tqc_plan_opts *opts, int max_log2_input_floats,
+                          int max_log2_intermediate_floats, int32_t *slice_cuts, int32_t *n_slice_cuts);
 void tqc_plan_destroy(tqc_plan_t *plan);
 
 int tqc_plan_mode(const tqc_plan_t *plan);

@@ -88,3 +88,67 @@ def serialize(p) -> bytes:
 
 def step_pairs(p):
     return [(s["lhs"], s["rhs"]) for s in p["steps"]]
+
+
+def _without(net, slice_cuts):
+    """The network with the given cuts removed (remaining cuts renumbered in order) - structure only."""
+    from tqc_inputs.network import Network
+    gone = set(slice_cuts)
+    keep = [e for e in range(net.K) if e not in gone]
+    relabel = {e: i for i, e in enumerate(keep)}
+    return Network(net.n_qubits, [net.cuts[e] for e in keep],
+                   [[relabel[e] for e in net.sub_cuts[s] if e not in gone] for s in range(net.m)], net.sub_qubits)
+
+
+def choose_slice_cuts(net, mode, max_log2_input_floats, max_log2_intermediate_floats):
+    """Two-level slicing, the reading written in include/tqc.h / DESIGN.md G19.
+    Level 1: while a tensor of one sub-network exceeds the input limit, slice the most size-reducing cut among those
+    touching an oversize tensor (its two tensors compared larger first, then smaller; tie: smaller id).
+    Level 2: while the plan's largest intermediate exceeds its limit, slice the cut that leaves the smallest largest
+    intermediate, then the smallest exact multiplication count, then the smaller id.  Returns None when infeasible."""
+    S = []
+    while True:
+        small = _without(net, S)
+        lg = [2 * small.c(s) + small.o(s) for s in range(net.m)]
+        if max(lg) <= max_log2_input_floats:
+            break
+        best = None
+        for e in range(net.K):
+            if e in S:
+                continue
+            a, b = lg[net.cuts[e][0]], lg[net.cuts[e][1]]
+            if max(a, b) <= max_log2_input_floats:
+                continue
+            key = (-max(a, b), -min(a, b), e)
+            if best is None or key < best:
+                best = key
+        if best is None:
+            return None
+        S.append(best[2])
+
+    def score(cuts):
+        small = _without(net, cuts)
+        p = plan(small, mode)
+        bits = {s: small.o(s) for s in range(net.m)}
+        worst = 0
+        for t, st in enumerate(p["steps"]):
+            bits[net.m + t] = bits[st["lhs"]] + bits[st["rhs"]]
+            size = 2 * (len(st["outer_lhs"]) + len(st["outer_rhs"])) + (bits[net.m + t] if mode == MODE_DISTRIBUTION else 0)
+            worst = max(worst, size)
+        return worst, sum(1 << st["log2cost"] for st in p["steps"])
+
+    while True:
+        worst, _ = score(S)
+        if worst <= max_log2_intermediate_floats:
+            return S
+        best = None
+        for e in range(net.K):
+            if e in S:
+                continue
+            w, c = score(S + [e])
+            key = (w, c, e)
+            if best is None or key < best:
+                best = key
+        if best is None:
+            return None
+        S.append(best[2])

@@ -32,7 +32,7 @@ EXPORTED = ["tqc_plan", "tqc_plan_destroy", "tqc_plan_mode", "tqc_plan_num_qubit
             "tqc_contract_distribution", "tqc_plan_launch_count", "tqc_last_error", "tqc_version",
             "tqc_plan_workspace_bytes_host", "tqc_contract_states_host", "tqc_contract_distribution_host",
             "tqc_plan_profile_enable", "tqc_plan_profile_read", "tqc_plan_chain_status", "tqc_hss_scores", "tqc_hss_select",
-            "tqc_hss_expand", "tqc_plan_num_sliced_cuts"]
+            "tqc_hss_expand", "tqc_plan_num_sliced_cuts", "tqc_choose_slice_cuts"]
 
 
 class TqcError(RuntimeError):
@@ -67,6 +67,7 @@ def _load() -> ctypes.CDLL:
     lib.tqc_last_error.restype = c_char_p
     lib.tqc_version.restype = c_char_p
     lib.tqc_plan.argtypes = [POINTER(_NetworkDesc), POINTER(_PlanOpts), POINTER(c_void_p)]
+    lib.tqc_choose_slice_cuts.argtypes = [POINTER(_NetworkDesc), POINTER(_PlanOpts), c_int, c_int, c_void_p, POINTER(c_int32)]
     lib.tqc_plan_destroy.argtypes = [c_void_p]
     lib.tqc_plan_destroy.restype = None
     for name in ("tqc_plan_mode", "tqc_plan_num_qubits", "tqc_plan_num_subcircuits", "tqc_plan_num_cuts",
@@ -217,19 +218,21 @@ class Plan:
         return [(int(tags[i]), float(ms[i])) for i in range(n.value)]
 
 
+def _network_desc(net):
+    m = len(net.sub_cuts)
+    keep = [_i32(c[0] for c in net.cuts), _i32(c[1] for c in net.cuts),
+            _i32(np.concatenate([[0], np.cumsum([len(x) for x in net.sub_cuts])])), _i32(e for x in net.sub_cuts for e in x),
+            _i32(np.concatenate([[0], np.cumsum([len(x) for x in net.sub_qubits])])), _i32(q for x in net.sub_qubits for q in x)]
+    desc = _NetworkDesc(net.n_qubits, m, len(net.cuts), *[k[1] for k in keep])
+    return desc, keep                      # keep: the arrays the descriptor points into
+
+
 def tqc_plan(net, mode: int = MODE_STATES, order=None, restarts: int = 0, seed: int = 0, batch_hint: int = 0,
              table_log2_floats_max: int = 0, use_tcgen05: int = 0, use_chain: int = 0, slice_cuts=None) -> Plan:
     """net: any object with n_qubits, cuts [(up, down)], sub_cuts [[cut ids]], sub_qubits [[qubit ids]]
     (e.g. tqc_inputs.Network).  order: optional list of m-1 (lhs, rhs) node-id pairs.  slice_cuts: cut ids evaluated by
     index slicing (summed over their 4 bases) instead of being contracted as bonds."""
-    m = len(net.sub_cuts)
-    up, up_p = _i32(c[0] for c in net.cuts)
-    down, down_p = _i32(c[1] for c in net.cuts)
-    cofs, cofs_p = _i32(np.concatenate([[0], np.cumsum([len(x) for x in net.sub_cuts])]))
-    cflat, cflat_p = _i32(e for x in net.sub_cuts for e in x)
-    qofs, qofs_p = _i32(np.concatenate([[0], np.cumsum([len(x) for x in net.sub_qubits])]))
-    qflat, qflat_p = _i32(q for x in net.sub_qubits for q in x)
-    desc = _NetworkDesc(net.n_qubits, m, len(net.cuts), up_p, down_p, cofs_p, cflat_p, qofs_p, qflat_p)
+    desc, _keep = _network_desc(net)
     oflat, oflat_p = _i32(v for ab in (order or []) for v in ab)
     sflat, sflat_p = _i32(slice_cuts or [])
     opts = _PlanOpts(mode, len(order) if order else 0, oflat_p, restarts, seed, batch_hint,
@@ -237,6 +240,18 @@ def tqc_plan(net, mode: int = MODE_STATES, order=None, restarts: int = 0, seed: 
     h = c_void_p()
     _check(_lib.tqc_plan(byref(desc), byref(opts), byref(h)))
     return Plan(h.value)
+
+
+def tqc_choose_slice_cuts(net, mode: int = MODE_STATES, max_log2_input_floats: int = 62,
+                          max_log2_intermediate_floats: int = 62, batch_hint: int = 0):
+    """The paper's two-level slicing choice (include/tqc.h): list of cut ids in pick order."""
+    desc, _keep = _network_desc(net)
+    opts = _PlanOpts(mode, 0, None, 0, 0, batch_hint, 0, 0, 0, 0, None)
+    out = np.zeros(max(1, len(net.cuts)), dtype=np.int32)
+    n = c_int32(0)
+    _check(_lib.tqc_choose_slice_cuts(byref(desc), byref(opts), max_log2_input_floats, max_log2_intermediate_floats,
+                                      out.ctypes.data, byref(n)))
+    return [int(x) for x in out[:n.value]]
 
 
 def tqc_load_subcircuit_tensors(plan: Plan, s: int, data, stream=None) -> None:

@@ -793,6 +793,132 @@ extern "C" {
 const char *tqc_last_error(void) { return g_err.c_str(); }
 const char *tqc_version(void) { return "tqc-b200 0.1 (sm_100a)"; }
 
+namespace {
+// the network without the sliced cuts: kept cuts renumbered in order, axis lists filtered
+struct ReducedNet {
+    std::vector<int32_t> up, down, ofs, flat;
+    std::vector<std::vector<int>> full_axis;
+    std::vector<std::vector<std::pair<int, int>>> sliced_axis;
+    std::vector<int> c_full, d_extra;
+};
+bool reduce_network(const tqc_network_desc *net, const int32_t *slice_cuts, int ns, ReducedNet &rn, std::string &why) {
+    if (net->m < 1 || net->K < 0 || !net->sub_cut_ofs || (net->K > 0 && (!net->cut_up || !net->cut_down || !net->sub_cuts))) {
+        why = "bad network description"; return false;
+    }
+    std::vector<int> relabel(net->K, 0), is_sliced(net->K, -1);
+    for (int i = 0; i < ns; ++i) {
+        const int e = slice_cuts[i];
+        if (e < 0 || e >= net->K || is_sliced[e] >= 0) { why = "slice_cuts must be distinct cut ids"; return false; }
+        is_sliced[e] = i;
+    }
+    rn.ofs.assign(1, 0);
+    for (int e = 0; e < net->K; ++e)
+        if (is_sliced[e] < 0) { relabel[e] = (int)rn.up.size(); rn.up.push_back(net->cut_up[e]); rn.down.push_back(net->cut_down[e]); }
+    rn.full_axis.assign(net->m, {}); rn.sliced_axis.assign(net->m, {});
+    rn.c_full.assign(net->m, 0); rn.d_extra.assign(net->m, 0);
+    for (int s = 0; s < net->m; ++s) {
+        const int b = net->sub_cut_ofs[s], e1 = net->sub_cut_ofs[s + 1];
+        rn.c_full[s] = e1 - b;
+        for (int x = b; x < e1; ++x) {
+            const int e = net->sub_cuts[x];
+            if (e < 0 || e >= net->K) { why = "cut id out of range in sub_cuts"; return false; }
+            if (is_sliced[e] >= 0) {
+                rn.sliced_axis[s].emplace_back(x - b, is_sliced[e]);
+                if (net->cut_down[e] == s) rn.d_extra[s]++;
+            } else { rn.flat.push_back(relabel[e]); rn.full_axis[s].push_back(x - b); }
+        }
+        // local slice digits in the order of slice_cuts (first = most significant)
+        std::sort(rn.sliced_axis[s].begin(), rn.sliced_axis[s].end(),
+                  [](const std::pair<int, int> &a, const std::pair<int, int> &b2) { return a.second < b2.second; });
+        rn.ofs.push_back((int32_t)rn.flat.size());
+    }
+    return true;
+}
+void plan_options_from(const tqc_plan_opts *opts, tqc::PlanOptions &po) {
+    if (!opts) return;
+    po.mode = opts->mode;
+    po.restarts = opts->restarts;
+    po.seed = opts->seed;
+    po.batch_hint = opts->batch_hint;
+    po.table_log2_floats_max = opts->table_log2_floats_max;
+    for (int i = 0; i < opts->n_order_steps && opts->order; ++i) po.order.emplace_back(opts->order[2 * i], opts->order[2 * i + 1]);
+}
+}  // namespace
+
+// Which cuts to slice (the two-level strategy).  Level 1: while a subcircuit tensor of a single
+// sub-network, 4^{c'_s} 2^{o_s} floats, exceeds 2^{max_log2_input_floats}, slice "the most size-reducing cut edge": among
+// the cuts incident on an oversize tensor the one whose two tensors are largest (compare the larger, then the smaller;
+// tie: smaller cut id).  Level 2: while the largest intermediate of the plan exceeds 2^{max_log2_intermediate_floats}
+// (4^{open cuts} floats per state; x 2^{carried bits} in distribution mode), slice the cut whose removal gives the smallest
+// largest-intermediate, then the smallest total multiplication count, then the smaller id (one greedy plan per candidate).
+int tqc_choose_slice_cuts(const tqc_network_desc *net, const tqc_plan_opts *opts, int max_log2_input_floats,
+                          int max_log2_intermediate_floats, int32_t *slice_cuts, int32_t *n_slice_cuts) {
+    if (!net || !slice_cuts || !n_slice_cuts) return fail(TQC_E_ARG, "null argument");
+    tqc::PlanOptions po;
+    plan_options_from(opts, po);
+    po.order.clear();                                   // an explicit order names nodes of one particular network
+    std::vector<int32_t> S;
+    std::vector<char> used(std::max(net->K, 0), 0);
+    auto sizes = [&](std::vector<int> &lg) -> bool {
+        ReducedNet rn; std::string why;
+        if (!reduce_network(net, S.data(), (int)S.size(), rn, why)) { fail(TQC_E_ARG, why); return false; }
+        lg.assign(net->m, 0);
+        for (int s = 0; s < net->m; ++s)
+            lg[s] = 2 * (rn.ofs[s + 1] - rn.ofs[s]) + (net->sub_qubit_ofs ? net->sub_qubit_ofs[s + 1] - net->sub_qubit_ofs[s] : 0);
+        return true;
+    };
+    for (;;) {                                          // level 1: inputs
+        std::vector<int> lg;
+        if (!sizes(lg)) return TQC_E_ARG;
+        if (*std::max_element(lg.begin(), lg.end()) <= max_log2_input_floats) break;
+        int best = -1, bhi = -1, blo = -1;
+        for (int e = 0; e < net->K; ++e) {
+            if (used[e]) continue;
+            const int a = lg[net->cut_up[e]], b = lg[net->cut_down[e]];
+            if (std::max(a, b) <= max_log2_input_floats) continue;
+            const int hi = std::max(a, b), lo = std::min(a, b);
+            if (hi > bhi || (hi == bhi && lo > blo)) { best = e; bhi = hi; blo = lo; }
+        }
+        if (best < 0) return fail(TQC_E_INFEASIBLE, "a subcircuit tensor exceeds max_log2_input_floats with every incident cut sliced");
+        used[best] = 1; S.push_back(best);
+    }
+    struct Score { int max_inter; unsigned __int128 cost; };
+    auto score = [&](const std::vector<int32_t> &cuts, Score &sc) -> int {
+        ReducedNet rn; std::string why;
+        if (!reduce_network(net, cuts.data(), (int)cuts.size(), rn, why)) return fail(TQC_E_ARG, why);
+        tqc::HostPlan hp; std::string err;
+        const int rc = tqc::build_plan(net->n_qubits, net->m, (int)rn.up.size(), rn.up.data(), rn.down.data(), rn.ofs.data(),
+                                       rn.flat.data(), net->sub_qubit_ofs, net->sub_qubits, po, hp, err);
+        if (rc) return fail(rc, err);
+        sc.max_inter = 0; sc.cost = 0;
+        for (int t = 0; t < hp.m - 1; ++t) {
+            const Node &C = hp.nodes[hp.m + t];
+            sc.max_inter = std::max(sc.max_inter, 2 * (int)C.open.size() + (hp.mode == TQC_MODE_DISTRIBUTION ? (int)C.qubits.size() : 0));
+            sc.cost += (unsigned __int128)1 << std::min(hp.steps[t].log2cost, 120);
+        }
+        return 0;
+    };
+    for (;;) {                                          // level 2: intermediates
+        Score cur;
+        int rc = score(S, cur);
+        if (rc) return rc;
+        if (cur.max_inter <= max_log2_intermediate_floats) break;
+        int best = -1; Score bs{0, 0};
+        for (int e = 0; e < net->K; ++e) {
+            if (used[e]) continue;
+            std::vector<int32_t> T = S; T.push_back(e);
+            Score sc;
+            if ((rc = score(T, sc))) return rc;
+            if (best < 0 || sc.max_inter < bs.max_inter || (sc.max_inter == bs.max_inter && sc.cost < bs.cost)) { best = e; bs = sc; }
+        }
+        if (best < 0) return fail(TQC_E_INFEASIBLE, "an intermediate exceeds max_log2_intermediate_floats with every cut sliced");
+        used[best] = 1; S.push_back(best);
+    }
+    for (size_t i = 0; i < S.size(); ++i) slice_cuts[i] = S[i];
+    *n_slice_cuts = (int32_t)S.size();
+    return 0;
+}
+
 int tqc_plan(const tqc_network_desc *net, const tqc_plan_opts *opts, tqc_plan_t **out) {
     if (!net || !out) return fail(TQC_E_ARG, "null argument");
     tqc::PlanOptions po;
@@ -820,36 +946,12 @@ int tqc_plan(const tqc_network_desc *net, const tqc_plan_opts *opts, tqc_plan_t 
         rc = tqc::build_plan(net->n_qubits, net->m, net->K, net->cut_up, net->cut_down, net->sub_cut_ofs,
                              net->sub_cuts, net->sub_qubit_ofs, net->sub_qubits, po, pl->hp, err);
     } else {
-        // the network without the sliced cuts: kept cuts renumbered in order, axis lists filtered
-        if (net->m < 1 || net->K < 0 || !net->sub_cut_ofs) { delete pl; return fail(TQC_E_ARG, "bad network description"); }
-        std::vector<int> relabel(net->K, 0), is_sliced(net->K, -1);
-        for (int i = 0; i < ns; ++i) {
-            const int e = opts->slice_cuts[i];
-            if (e < 0 || e >= net->K || is_sliced[e] >= 0) { delete pl; return fail(TQC_E_ARG, "slice_cuts must be distinct cut ids"); }
-            is_sliced[e] = i;
-            pl->slice_cuts.push_back(e);
-        }
-        std::vector<int32_t> up, down, ofs(1, 0), flat;
-        for (int e = 0; e < net->K; ++e)
-            if (is_sliced[e] < 0) { relabel[e] = (int)up.size(); up.push_back(net->cut_up[e]); down.push_back(net->cut_down[e]); }
-        pl->full_axis.resize(net->m); pl->sliced_axis.resize(net->m);
-        pl->c_full.assign(net->m, 0); pl->d_extra.assign(net->m, 0);
-        for (int s = 0; s < net->m; ++s) {
-            const int b = net->sub_cut_ofs[s], e1 = net->sub_cut_ofs[s + 1];
-            pl->c_full[s] = e1 - b;
-            for (int x = b; x < e1; ++x) {
-                const int e = net->sub_cuts[x];
-                if (e < 0 || e >= net->K) { delete pl; return fail(TQC_E_ARG, "cut id out of range in sub_cuts"); }
-                if (is_sliced[e] >= 0) {
-                    pl->sliced_axis[s].emplace_back(x - b, is_sliced[e]);
-                    if (net->cut_down[e] == s) pl->d_extra[s]++;
-                } else { flat.push_back(relabel[e]); pl->full_axis[s].push_back(x - b); }
-            }
-            // local slice digits in the order of slice_cuts (first = most significant)
-            std::sort(pl->sliced_axis[s].begin(), pl->sliced_axis[s].end(),
-                      [](const std::pair<int, int> &a, const std::pair<int, int> &b2) { return a.second < b2.second; });
-            ofs.push_back((int32_t)flat.size());
-        }
+        ReducedNet rn;
+        std::string why;
+        if (!reduce_network(net, opts->slice_cuts, ns, rn, why)) { delete pl; return fail(TQC_E_ARG, why); }
+        pl->slice_cuts.assign(opts->slice_cuts, opts->slice_cuts + ns);
+        pl->full_axis = rn.full_axis; pl->sliced_axis = rn.sliced_axis; pl->c_full = rn.c_full; pl->d_extra = rn.d_extra;
+        const std::vector<int32_t> &up = rn.up, &down = rn.down, &ofs = rn.ofs, &flat = rn.flat;
         rc = tqc::build_plan(net->n_qubits, net->m, (int)up.size(), up.data(), down.data(), ofs.data(), flat.data(),
                              net->sub_qubit_ofs, net->sub_qubits, po, pl->hp, err);
     }

@@ -90,3 +90,20 @@ def test_sliced_plan_with_tensor_pipe_step_and_host_buffers():
     assert np.array_equal(oh.numpy().astype(np.float64), got)
     with pytest.raises(tqc.TqcError):
         tqc.tqc_hss_scores(plan, 0)
+
+
+def test_two_level_choice_end_to_end():
+    """tqc_choose_slice_cuts -> tqc_plan(slice_cuts) -> contract: limits met and the values are still Eq. 1."""
+    net = configs.random_network(6, 11, seed=611, o_lo=1, o_hi=3)
+    T = [np.asarray(t, dtype=np.float32) for t in random_tensors(net, 612)]
+    bits = random_states(net.n_qubits, 500, 613)
+    full = tqc.tqc_plan(net, tqc.MODE_STATES, use_chain=-1)
+    inter = max(2 * full.node(net.m + t)["n_open"] for t in range(net.m - 1))
+    big_in = max(2 * net.c(s) + net.o(s) for s in range(net.m))
+    cuts = tqc.tqc_choose_slice_cuts(net, tqc.MODE_STATES, big_in - 2, max(inter - 4, 2))
+    assert len(cuts) >= 2
+    plan = _loaded(net, T, tqc.MODE_STATES, slice_cuts=cuts)
+    assert max(2 * plan.node(net.m + t)["n_open"] for t in range(net.m - 1)) <= max(inter - 4, 2)
+    want, _ = direct_sum_c(net, T, bits)
+    got = _states(plan, bits)
+    assert np.abs(got - want).max() <= TOL * want.max()

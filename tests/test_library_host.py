@@ -134,3 +134,30 @@ def test_sliced_plan_is_the_plan_of_the_smaller_network():
         tqc.tqc_plan(net, tqc.MODE_STATES, slice_cuts=[1, 1])
     with pytest.raises(tqc.TqcError):
         tqc.tqc_plan(net, tqc.MODE_STATES, slice_cuts=[net.K])
+
+
+def test_choose_slice_cuts_matches_reference_and_meets_limits():
+    """Two-level slicing choice: library == oracle-side reference on random networks in both
+    modes; the chosen set meets both limits (checked through the plan it leads to); infeasible limits are reported."""
+    for seed in range(12):
+        net = configs.random_network(3 + seed % 5, 6 + seed % 6, seed=500 + seed, o_lo=0, o_hi=4)
+        for mode in (tqc.MODE_STATES, tqc.MODE_DISTRIBUTION):
+            full = tqc.tqc_plan(net, mode, use_chain=-1)
+            inter = max(2 * full.node(net.m + t)["n_open"] + (full.node(net.m + t)["n_bits"] if mode else 0)
+                        for t in range(net.m - 1))
+            big_in = max(2 * net.c(s) + net.o(s) for s in range(net.m))
+            for lim_in, lim_inter in ((62, 62), (big_in - 2, 62), (62, max(inter - 3, 2)), (big_in - 3, max(inter - 4, 2))):
+                want = P.choose_slice_cuts(net, mode, lim_in, lim_inter)
+                if want is None:
+                    with pytest.raises(tqc.TqcError):
+                        tqc.tqc_choose_slice_cuts(net, mode, lim_in, lim_inter)
+                    continue
+                got = tqc.tqc_choose_slice_cuts(net, mode, lim_in, lim_inter)
+                assert got == want, (seed, mode, lim_in, lim_inter)
+                if (lim_in, lim_inter) == (62, 62):
+                    assert got == []
+                plan = tqc.tqc_plan(net, mode, slice_cuts=got, use_chain=-1)
+                left = [net.c(s) - sum(1 for e in got if e in net.sub_cuts[s]) for s in range(net.m)]
+                assert max(2 * left[s] + net.o(s) for s in range(net.m)) <= lim_in
+                assert max([2 * plan.node(net.m + t)["n_open"] + (plan.node(net.m + t)["n_bits"] if mode else 0)
+                            for t in range(net.m - 1)] or [0]) <= lim_inter
