@@ -192,6 +192,19 @@ int tqc_hss_select(const tqc_plan_t *plan, const float *const *scores_host, uint
 int tqc_hss_expand(const tqc_plan_t *plan, const int32_t *counts, const int32_t *keys, uint64_t *states_host, size_t capacity,
                    size_t *n_states);
 
+/* Product-structured contraction of a selection ("prune subcircuit outputs prior to tensor network
+ * contraction", output dimension prod_j |x_j|): every subcircuit tensor is restricted to its selected states and the
+ * network is contracted ONCE with those pruned output axes open, so the prod_j |x_j| composite states share every
+ * intermediate - the same values as tqc_contract_states on tqc_hss_expand's batch, at a fraction of the work.
+ * tqc_hss_prepare (allocates, like a load): counts HOST [m] = |x_j|; keys_dev DEVICE [sum_j counts[j]] = the selected
+ *   states of subcircuit 0, then 1, ... (the order of tqc_hss_select's keys).  Builds the pruned tensors on `stream` from
+ *   the loaded ones and plans the pruned network (axes padded to powers of two; at most 2^34 padded composite states).
+ * tqc_hss_contract: out_dev DEVICE [prod_j counts[j]] in product order, subcircuit 0 slowest (tqc_hss_expand's order);
+ *   workspace >= tqc_hss_workspace_bytes(plan), 256-byte aligned; asynchronous on `stream`, no allocation. */
+int tqc_hss_prepare(tqc_plan_t *plan, const int32_t *counts, const int32_t *keys_dev, void *stream);
+size_t tqc_hss_workspace_bytes(const tqc_plan_t *plan);
+int tqc_hss_contract(tqc_plan_t *plan, float *out_dev, void *workspace_dev, size_t workspace_bytes, void *stream);
+
 /* ---- measurement hooks (bench.py) --------------------------------------------------------------
  * tqc_plan_launch_count: kernels launched so far on behalf of this plan.
  * tqc_plan_profile_enable(plan, 1): every later contract call records one CUDA event on the

@@ -4,10 +4,10 @@ in the CUDA kernels under csrc/.  There is no CPU fallback: without the built li
 of `binding` fails, and without a CUDA device the compute calls return TQC_E_CUDA."""
 from .binding import (MODE_DISTRIBUTION, MODE_STATES, Plan, TqcError, lib_path, tqc_contract_distribution,
                       tqc_contract_distribution_host, tqc_contract_states, tqc_contract_states_host,
-                      tqc_choose_slice_cuts, tqc_hss_expand, tqc_hss_scores, tqc_hss_select, tqc_load_subcircuit_tensors, tqc_plan,
+                      tqc_choose_slice_cuts, tqc_hss_contract, tqc_hss_expand, tqc_hss_scores, tqc_hss_select, tqc_load_subcircuit_tensors, tqc_plan,
                       version)
 
 __all__ = ["MODE_STATES", "MODE_DISTRIBUTION", "Plan", "TqcError", "tqc_plan", "tqc_load_subcircuit_tensors",
            "tqc_contract_states", "tqc_contract_distribution", "tqc_contract_states_host",
-           "tqc_contract_distribution_host", "tqc_hss_scores", "tqc_hss_select", "tqc_hss_expand", "tqc_choose_slice_cuts", "version",
+           "tqc_contract_distribution_host", "tqc_hss_scores", "tqc_hss_select", "tqc_hss_expand", "tqc_hss_contract", "tqc_choose_slice_cuts", "version",
            "lib_path"]

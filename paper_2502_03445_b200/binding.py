@@ -32,7 +32,8 @@ EXPORTED = ["tqc_plan", "tqc_plan_destroy", "tqc_plan_mode", "tqc_plan_num_qubit
             "tqc_contract_distribution", "tqc_plan_launch_count", "tqc_last_error", "tqc_version",
             "tqc_plan_workspace_bytes_host", "tqc_contract_states_host", "tqc_contract_distribution_host",
             "tqc_plan_profile_enable", "tqc_plan_profile_read", "tqc_plan_chain_status", "tqc_hss_scores", "tqc_hss_select",
-            "tqc_hss_expand", "tqc_plan_num_sliced_cuts", "tqc_choose_slice_cuts"]
+            "tqc_hss_expand", "tqc_plan_num_sliced_cuts", "tqc_choose_slice_cuts", "tqc_hss_prepare",
+            "tqc_hss_workspace_bytes", "tqc_hss_contract"]
 
 
 class TqcError(RuntimeError):
@@ -98,6 +99,10 @@ def _load() -> ctypes.CDLL:
     lib.tqc_hss_scores.argtypes = [c_void_p, c_int, c_void_p, c_void_p]
     lib.tqc_hss_select.argtypes = [c_void_p, POINTER(c_void_p), c_uint64, c_void_p, c_void_p, c_size_t]
     lib.tqc_hss_expand.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_size_t, POINTER(c_size_t)]
+    lib.tqc_hss_prepare.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p]
+    lib.tqc_hss_workspace_bytes.argtypes = [c_void_p]
+    lib.tqc_hss_workspace_bytes.restype = c_size_t
+    lib.tqc_hss_contract.argtypes = [c_void_p, c_void_p, c_void_p, c_size_t, c_void_p]
     return lib
 
 
@@ -365,3 +370,19 @@ def tqc_hss_expand(plan: Plan, x):
     _check(_lib.tqc_hss_expand(plan._h, counts.ctypes.data, keys.ctypes.data, states.ctypes.data, n.value,
                                ctypes.byref(n)))
     return states
+
+
+def tqc_hss_contract(plan: Plan, x, out=None, workspace=None, stream=None, device="cuda"):
+    """Product-structured contraction of a selection x (list of key arrays, as tqc_hss_select returns): CUDA fp32
+    [prod_j |x_j|] in the order of tqc_hss_expand, every intermediate shared between the composite states."""
+    import torch
+    counts = np.array([len(k) for k in x], dtype=np.int32)
+    keys = torch.from_numpy(np.ascontiguousarray(np.concatenate([np.asarray(k, dtype=np.int32) for k in x]))).to(device)
+    _check(_lib.tqc_hss_prepare(plan._h, counts.ctypes.data, keys.data_ptr(), _stream_ptr(stream)))
+    n = int(np.prod(counts.astype(np.int64)))
+    if out is None:
+        out = torch.empty(n, dtype=torch.float32, device=device)
+    if workspace is None:
+        workspace = torch.empty(max(256, int(_lib.tqc_hss_workspace_bytes(plan._h))), dtype=torch.uint8, device=device)
+    _check(_lib.tqc_hss_contract(plan._h, out.data_ptr(), workspace.data_ptr(), workspace.numel(), _stream_ptr(stream)))
+    return out

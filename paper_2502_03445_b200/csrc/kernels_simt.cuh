@@ -289,4 +289,42 @@ __global__ void __launch_bounds__(256) hss_norm_kernel(const float *__restrict__
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// NEXT row 1, pruned output axes: the tensor of subcircuit j restricted to its heavy states x_j,
+//     dst[i][q] = i < count ? src[keys[i]][perm(q)] : 0          i < 2^{ceil log2 count}
+// a row gather on the state-major layout (rows are contiguous 4^{c} floats), with the digit order of the pruned plan.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) hss_rows_kernel(const float *__restrict__ src, float *__restrict__ dst,
+                                                        const int32_t *__restrict__ keys, int count, long long rows_out,
+                                                        int lgCols, const BitMap perm) {
+    const long long n = rows_out << lgCols, stride = (long long)gridDim.x * blockDim.x;
+    const long long cmask = (1ll << lgCols) - 1;
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += stride) {
+        const long long i = e >> lgCols;
+        float v = 0.f;
+        if (i < count) v = src[((long long)keys[i] << lgCols) + (long long)bitmap_apply(perm, (unsigned long long)(e & cmask))];
+        dst[e] = v;
+    }
+}
+
+struct HssCompactArgs {          // product order over the |x_j| (subcircuit 0 slowest) -> index in the padded 2^{v_j} table
+    int m;
+    int32_t count[64];
+    uint8_t shift[64];
+};
+__global__ void __launch_bounds__(256) hss_compact_kernel(const float *__restrict__ padded, float *__restrict__ out, long long n,
+                                                           const HssCompactArgs a) {
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x; b < n; b += stride) {
+        long long rest = b;
+        unsigned long long idx = 0;
+        for (int j = a.m - 1; j >= 0; --j) {
+            const long long cj = a.count[j];
+            idx |= (unsigned long long)(rest % cj) << a.shift[j];
+            rest /= cj;
+        }
+        out[b] = padded[idx];
+    }
+}
+
 }  // namespace tqc

@@ -107,6 +107,10 @@ struct tqc_plan {
     std::vector<int> c_full, d_extra;                       // per leaf: caller's c_s; sliced cuts whose downstream end it holds
     std::vector<float *> d_leaf_all;                        // allocation per leaf: [4^{#sliced axes}][2^o][4^{c'}]
     int n_sliced() const { return (int)slice_cuts.size(); }
+    // Heavy State Selection, pruned output axes: a distribution-mode plan of the same cut network whose subcircuit j
+    // carries ceil(log2 |x_j|) virtual output bits (tqc_hss_prepare / tqc_hss_contract)
+    tqc_plan *hss_sub = nullptr;
+    std::vector<int32_t> hss_counts;
 };
 
 namespace {
@@ -995,6 +999,7 @@ void tqc_plan_destroy(tqc_plan_t *pl) {
     if (pl->d_chain) cudaFree(pl->d_chain);
     if (pl->jit_module && jit_api().ok) jit_api().ModuleUnload((CUmodule)pl->jit_module);
     for (cudaEvent_t e : pl->ev_pool) cudaEventDestroy(e);
+    if (pl->hss_sub) tqc_plan_destroy(pl->hss_sub);
     if (pl->ev_fork) cudaEventDestroy(pl->ev_fork);
     for (int l = 0; l < tqc_plan::N_LANES; ++l) {
         if (pl->ev_join[l]) cudaEventDestroy(pl->ev_join[l]);
@@ -1552,6 +1557,107 @@ int tqc_hss_expand(const tqc_plan_t *pl, const int32_t *counts, const int32_t *k
         }
         for (int j = hp.m - 1; j >= 0; --j) { if (++idx[j] < counts[j]) break; idx[j] = 0; }
     }
+    return 0;
+}
+
+// ---- Heavy State Selection, product-structured contraction ---------------------------------
+int tqc_hss_prepare(tqc_plan_t *pl, const int32_t *counts, const int32_t *keys_dev, void *stream) {
+    if (!pl || !counts || !keys_dev) return fail(TQC_E_ARG, "null argument");
+    const HostPlan &hp = pl->hp;
+    if (pl->n_sliced()) return fail(TQC_E_STATE, "pruned contraction needs whole tensors: build the plan without slice_cuts");
+    if (hp.m > 64) return fail(TQC_E_TOO_LARGE, "more than 64 subcircuits");
+    std::vector<int> v(hp.m, 0);
+    int total_bits = 0;
+    for (int j = 0; j < hp.m; ++j) {
+        if (!pl->loaded[j]) return fail(TQC_E_STATE, "tensor of subcircuit " + std::to_string(j) + " not loaded");
+        if (counts[j] < 1 || counts[j] > (1 << hp.o(j))) return fail(TQC_E_ARG, "counts[j] must be in 1 .. 2^{o_j}");
+        while ((1 << v[j]) < counts[j]) ++v[j];
+        total_bits += v[j];
+    }
+    if (total_bits > 34) return fail(TQC_E_TOO_LARGE, "padded product of the selections exceeds 2^34 states");
+    // same pattern of padded sizes as the last call: keep the plan and its allocations
+    bool reuse = pl->hss_sub != nullptr;
+    if (reuse) for (int j = 0; j < hp.m; ++j) reuse &= pl->hss_sub->hp.o(j) == v[j];
+    if (!reuse) {
+        if (pl->hss_sub) { tqc_plan_destroy(pl->hss_sub); pl->hss_sub = nullptr; }
+        std::vector<int32_t> cofs(1, 0), cflat, qofs(1, 0), qflat;
+        int next_q = 0;                                    // subcircuit 0 owns the most significant virtual bits
+        for (int j = 0; j < hp.m; ++j) {
+            for (int e : hp.sub_cuts[j]) cflat.push_back(e);
+            cofs.push_back((int32_t)cflat.size());
+            for (int b = 0; b < v[j]; ++b) qflat.push_back(next_q++);
+            qofs.push_back((int32_t)qflat.size());
+        }
+        std::vector<int32_t> up(hp.cut_up.begin(), hp.cut_up.end()), down(hp.cut_down.begin(), hp.cut_down.end());
+        tqc_network_desc d;
+        d.n_qubits = total_bits; d.m = hp.m; d.K = hp.K;
+        d.cut_up = up.data(); d.cut_down = down.data(); d.sub_cut_ofs = cofs.data(); d.sub_cuts = cflat.data();
+        d.sub_qubit_ofs = qofs.data(); d.sub_qubits = qflat.data();
+        tqc_plan_opts o;
+        memset(&o, 0, sizeof(o));
+        o.mode = TQC_MODE_DISTRIBUTION;
+        o.use_tcgen05 = pl->use_tcgen05;
+        const int rc = tqc_plan(&d, &o, &pl->hss_sub);
+        if (rc) { pl->hss_sub = nullptr; return rc; }
+    }
+    tqc_plan_t *sub = pl->hss_sub;
+    cudaStream_t st = (cudaStream_t)stream;
+    size_t kofs = 0;
+    for (int j = 0; j < hp.m; ++j) {
+        const int c = hp.c(j);
+        const size_t floats = (size_t)1 << (2 * c + v[j]);
+        if (!sub->d_leaf[j]) TQC_CUDA(cudaMalloc(&sub->d_leaf[j], floats * sizeof(float)));
+        // digit x of the pruned plan's leaf layout (most significant first) <- the same cut's digit in this plan's layout
+        std::vector<int> la = hp.nodes[j].layout, lp = sub->hp.nodes[j].layout;
+        if (la.empty()) la = hp.nodes[j].open;
+        if (lp.empty()) lp = sub->hp.nodes[j].open;
+        BitPairs bp;
+        for (int x = 0; x < c; ++x) bp.add_run(2 * (c - 1 - x), 2 * (c - 1 - index_of(la, lp[x])), 2);
+        BitMap perm;
+        memset(&perm, 0, sizeof(perm));
+        if (!bp.build(perm)) return fail(TQC_E_TOO_LARGE, "bit map needs too many segments");
+        pl->launches++;
+        tqc::hss_rows_kernel<<<(unsigned)std::min<size_t>((floats + 255) / 256, 148 * 32), 256, 0, st>>>(
+            pl->d_leaf[j], sub->d_leaf[j], keys_dev + kofs, counts[j], 1ll << v[j], 2 * c, perm);
+        TQC_CUDA(cudaGetLastError());
+        sub->loaded[j] = 1;
+        kofs += (size_t)counts[j];
+    }
+    pl->hss_counts.assign(counts, counts + hp.m);
+    return 0;
+}
+
+size_t tqc_hss_workspace_bytes(const tqc_plan_t *pl) {
+    if (!pl || !pl->hss_sub) return 0;
+    return align256(((size_t)4) << pl->hss_sub->hp.n) + tqc_plan_workspace_bytes(pl->hss_sub, 0, 0);
+}
+
+int tqc_hss_contract(tqc_plan_t *pl, float *out_dev, void *workspace_dev, size_t workspace_bytes, void *stream) {
+    if (!pl || !out_dev) return fail(TQC_E_ARG, "null argument");
+    if (!pl->hss_sub) return fail(TQC_E_STATE, "call tqc_hss_prepare first");
+    if (!workspace_dev || ((uintptr_t)workspace_dev & 255) != 0) return fail(TQC_E_ARG, "workspace must be non-null and 256-byte aligned");
+    if (workspace_bytes < tqc_hss_workspace_bytes(pl)) return fail(TQC_E_WORKSPACE, "workspace smaller than tqc_hss_workspace_bytes");
+    tqc_plan_t *sub = pl->hss_sub;
+    const size_t pb = align256(((size_t)4) << sub->hp.n);
+    float *padded = (float *)workspace_dev;
+    const uint64_t before = sub->launches;
+    int rc = contract_distribution_impl(sub, 0, 0, padded, (char *)workspace_dev + pb, workspace_bytes - pb, stream);
+    pl->launches += sub->launches - before;
+    if (rc) return rc;
+    tqc::HssCompactArgs a;
+    memset(&a, 0, sizeof(a));
+    a.m = sub->hp.m;
+    long long n = 1;
+    int shift = 0;
+    for (int j = a.m - 1; j >= 0; --j) {                   // subcircuit 0 owns the most significant bits
+        a.count[j] = pl->hss_counts[j];
+        a.shift[j] = (uint8_t)shift;
+        shift += sub->hp.o(j);
+        n *= pl->hss_counts[j];
+    }
+    pl->launches++;
+    tqc::hss_compact_kernel<<<(unsigned)std::min<long long>((n + 255) / 256, 148 * 32), 256, 0, (cudaStream_t)stream>>>(padded, out_dev, n, a);
+    TQC_CUDA(cudaGetLastError());
     return 0;
 }
 

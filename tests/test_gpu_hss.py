@@ -95,3 +95,31 @@ def test_scores_require_loaded_tensor():
     plan = tqc.tqc_plan(net, tqc.MODE_STATES)
     with pytest.raises(tqc.TqcError):
         tqc.tqc_hss_scores(plan, 0)
+
+
+@pytest.mark.parametrize("seed,s_max", [(0, 37), (1, 1000), (2, 1), (3, 20000)])
+def test_product_structured_contraction(seed, s_max):
+    """tqc_hss_contract (pruned output axes, one contraction) == the oracle's direct sum on the oracle's expansion ==
+    tqc_contract_states on tqc_hss_expand's batch; |x_j| not powers of two, |x_j| = 1, o_j = 0 included."""
+    net = configs.random_network(3 + seed, 6 + seed, seed=700 + seed, o_lo=0 if seed else 1, o_hi=5)
+    tensors = [np.asarray(t, dtype=np.float32) for t in random_tensors(net, 710 + seed)]
+    plan = _loaded(net, tensors)
+    x = tqc.tqc_hss_select(plan, _gpu_scores(plan), s_max)
+    got = tqc.tqc_hss_contract(plan, x)
+    torch.cuda.synchronize()
+    got = got.cpu().numpy().astype(np.float64)
+    bits = H.expand(net, [v.tolist() for v in x])
+    assert got.shape == (bits.shape[0],)
+    sample = np.arange(bits.shape[0]) if bits.shape[0] <= 4096 else np.random.default_rng(1).choice(bits.shape[0], 4096, replace=False)
+    ref = direct_sum_c(net, tensors, bits[sample])[0]
+    assert np.abs(got[sample] - ref).max() <= 1e-5 * np.abs(ref).max()
+    states = tqc.tqc_hss_expand(plan, x)
+    per_state = tqc.tqc_contract_states(plan, torch.from_numpy(states.view(np.int64)).cuda())
+    torch.cuda.synchronize()
+    assert np.abs(got - per_state.cpu().numpy()).max() <= 1e-5 * np.abs(ref).max()
+    # a second selection with the same padded sizes reuses the pruned plan; a different one rebuilds it
+    x2 = [np.sort(np.random.default_rng(2).permutation(1 << net.o(j))[:len(v)]).astype(np.int32) for j, v in enumerate(x)]
+    got2 = tqc.tqc_hss_contract(plan, x2)
+    torch.cuda.synchronize()
+    ref2 = direct_sum_c(net, tensors, H.expand(net, [v.tolist() for v in x2])[:64])[0]
+    assert np.abs(got2.cpu().numpy()[:64] - ref2).max() <= 1e-5 * max(np.abs(ref2).max(), np.abs(ref).max())
