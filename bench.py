@@ -261,6 +261,7 @@ def run_ours(args) -> None:
                 others.append({k: o[k] for k in ("value", "unit", "ms_per_step", "steps", "gpu_launches", "roofline")} |
                               {"workload": o["config"]["workload"], "e2e_value": o["e2e"]["value"]})
             others.append(measure_hss(ctx, 10, 3))
+            others.append(measure_hss_contract(ctx, 10, 3))
             line["other_workloads"] = others
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(make_workload(args.workload, args.batch), args.cpu_seconds)
@@ -432,6 +433,54 @@ def measure_hss(ctx, steps: int, warmup: int) -> dict:
             "roofline": {"bound": "hbm", "kernel": "hss_norm_kernel<32>", "achieved": gbs, "peak": peaks["hbm_gbs"],
                          "unit": "GB/s", "frac": gbs / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"],
                          "algorithmic_bytes_per_launch": nbytes // net.m}}
+
+
+def measure_hss_contract(ctx, steps: int, warmup: int) -> dict:
+    """NEXT row 1, pruned contraction: Alg. 1 selection of >= 2^20 composite states on the cfg3-shaped network, contracted
+    once with pruned output axes (tqc_hss_contract) and, for comparison, state by state (tqc_contract_states on the
+    expanded batch).  A step = scores + (host) selection excluded; prepare + contract timed."""
+    torch, tqc, dev = ctx["torch"], ctx["tqc"], ctx["dev"]
+    wl = make_workload("cfg3")
+    net = wl["net"]
+    plan = tqc.tqc_plan(net, tqc.MODE_STATES, batch_hint=1 << 20)
+    for s, t in enumerate(wl["tensors"]):
+        tqc.tqc_load_subcircuit_tensors(plan, s, t)
+    scores = [tqc.tqc_hss_scores(plan, s) for s in range(net.m)]
+    torch.cuda.synchronize()
+    x = tqc.tqc_hss_select(plan, [v.cpu().numpy() for v in scores], 1 << 20)
+    n = int(np.prod([len(v) for v in x], dtype=np.int64))
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    out = torch.empty(n, dtype=torch.float32, device=dev)
+    l0 = plan.launch_count
+
+    def timed(fn):
+        for _ in range(warmup):
+            fn()
+        torch.cuda.synchronize()
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        for a, b in evs:
+            flush.zero_()
+            a.record(stream)
+            fn()
+            b.record(stream)
+        torch.cuda.synchronize()
+        return sum(a.elapsed_time(b) for a, b in evs) / steps
+
+    ms_product = timed(lambda: tqc.tqc_hss_contract(plan, x, out=out, stream=stream))
+    launches = (plan.launch_count - l0) // (steps + warmup)
+    states = torch.from_numpy(tqc.tqc_hss_expand(plan, x).view(np.int64)).to(dev)
+    ws = torch.empty(plan.workspace_bytes(n), dtype=torch.uint8, device=dev)
+    out2 = torch.empty(n, dtype=torch.float32, device=dev)
+    ms_states = timed(lambda: tqc.tqc_contract_states(plan, states, out=out2, workspace=ws, stream=stream))
+    torch.cuda.synchronize()
+    agree = float((out - out2).abs().max() / out2.abs().max())
+    plan.close()
+    return {"workload": f"hss-contract: cfg3-shaped network, |x_j| = {[len(v) for v in x]}, {n} composite states",
+            "value": n / (ms_product * 1e-3), "unit": UNIT, "ms_per_step": ms_product, "steps": steps,
+            "gpu_launches": int(launches), "per_state_path_ms": ms_states, "max_rel_diff_vs_per_state_path": agree,
+            "roofline": {"bound": "hbm", "kernel": "pruned distribution-mode contraction (step_tile / cross_mma) + hss_compact_kernel",
+                         "achieved": None, "peak": None, "unit": "GB/s", "frac": None, "traffic": None}}
 
 
 def workload_description(wl, plan) -> str:
