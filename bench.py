@@ -187,7 +187,7 @@ def roofline_for(plan, tag: int, avg_ms: float, B: int, mode_states: bool, peaks
         else:
             bound, peak, unit, achieved = "alu", alu_peak, "TFLOP/s", flop / sec / 1e12
         return {"bound": bound, "achieved": achieved, "peak": peak, "unit": unit, "frac": achieved / peak,
-                "traffic": traffic, "kernel": "chain_spec_kernel / chain_kernel (fused per-state chain, fp32 FFMA; specialised per plan when NVRTC is present)", "plan_step": "all per-state steps",
+                "traffic": traffic, "kernel": "chain_spec_kernel / chain_kernel (fused per-state chain: fp32 FFMA steps + 3xTF32 mma.sync blocks for 16x16x16-class steps; specialised per plan when NVRTC is present; the FP32-ALU peak is the reference for its algorithmic flops)", "plan_step": "all per-state steps",
                 "algorithmic_flop": flop, "algorithmic_bytes": nbytes, "avg_launch_ms": avg_ms,
                 "peak_source": peaks["source"] + (" hbm copy" if bound == "hbm" else " sm_max_mhz x 148 SMs x 128 lanes x 2")}
     if tag < 0 or avg_ms <= 0:
