@@ -98,3 +98,31 @@ def test_warp_mma_paths_signed_values_and_ffma_agreement():
     assert np.abs(got[:48] - want).max() <= TOL * scale, np.abs(got[:48] - want).max() / scale
     assert np.abs(ffma[:48] - want).max() <= TOL * scale
     assert np.abs(got - ffma).max() <= TOL * np.abs(ffma).max()
+
+
+@pytest.mark.parametrize("oa,ob,na,nb,ni", [(3, 2, 2, 2, 2), (2, 3, 2, 2, 2), (4, 4, 1, 2, 3), (1, 5, 3, 1, 1)])
+def test_cross_mma_tables_both_orientations_distribution_mode(oa, ob, na, nb, ni):
+    """Distribution mode on a triangle A-B-D: step (A, B) is a cross-mode product with M' = 2^oa 4^na, N' = 2^ob 4^nb,
+    K = 4^ni.  The cases put the >= 128 side on either operand (the launcher swaps them) and cover K = 4, 16, 64;
+    (1, 5, 3, 1, 1) has K = 4 < 8 and must stay on the FFMA kernel.  Against the direct sum and the FFMA-only plan."""
+    net = _triangle(na, nb, ni, oa=oa, ob=ob, od=1)
+    T = [np.asarray(t, dtype=np.float32) for t in random_tensors(net, 40 + oa)]
+    n = net.n_qubits
+    idx = np.arange(2 ** n, dtype=np.int64)
+    bits = ((idx[:, None] >> (n - 1 - np.arange(n))[None, :]) & 1).astype(np.uint8)
+    want, _ = direct_sum_c(net, T, bits)
+    outs = []
+    for use_tc in (0, -1):
+        plan = tqc.tqc_plan(net, tqc.MODE_DISTRIBUTION, order=[(0, 1), (3, 2)], use_tcgen05=use_tc)
+        for s, t in enumerate(T):
+            tqc.tqc_load_subcircuit_tensors(plan, s, t)
+        out = tqc.tqc_contract_distribution(plan)
+        torch.cuda.synchronize()
+        outs.append(out.cpu().numpy().astype(np.float64))
+        assert np.abs(outs[-1] - want).max() <= TOL * want.max()
+        for pv in (1, 2):                                       # prefix slices: leaves addressed through a bit map
+            part = tqc.tqc_contract_distribution(plan, pv, 2)
+            torch.cuda.synchronize()
+            w = want[pv << (n - 2):(pv + 1) << (n - 2)]
+            assert np.abs(part.cpu().numpy() - w).max() <= TOL * want.max()
+    assert np.abs(outs[0] - outs[1]).max() <= TOL * want.max()
