@@ -98,6 +98,7 @@ struct tqc_plan {
     cudaStream_t lane[N_LANES] = {nullptr, nullptr, nullptr};
     cudaEvent_t ev_fork = nullptr, ev_join[N_LANES] = {nullptr, nullptr, nullptr};
     int tables_parallel = -1;          // -1 not decided; 0 serial; 1 fork/join
+    bool fork_recorded = false;        // the host-buffer entry point recorded ev_fork before its H2D copy
     // bond slicing: hp describes the network WITHOUT the sliced cuts; a leaf keeps one re-laid-out
     // sub-tensor per value of its sliced axes, the contract calls sum over all 4^{n_sliced} assignments
     int K_full = 0;
@@ -1210,6 +1211,28 @@ int tqc_contract_distribution(tqc_plan_t *pl, uint64_t prefix_value, int prefix_
 }
 
 namespace {
+// decides once whether the table steps of a states-mode plan fork onto side streams, and creates the streams / events
+int ensure_lanes(tqc_plan_t *pl) {
+    if (pl->tables_parallel >= 0) return 0;
+    const HostPlan &hp = pl->hp;
+    int n_tab = 0;
+    bool leaf_only = true;
+    for (int t = 0; t < hp.m - 1; ++t) {
+        if (hp.nodes[hp.m + t].kind != tqc::NODE_TABLE) continue;
+        ++n_tab;
+        if (hp.steps[t].lhs >= hp.m || hp.steps[t].rhs >= hp.m) leaf_only = false;
+    }
+    pl->tables_parallel = (hp.mode == TQC_MODE_STATES && n_tab >= 1 && leaf_only && !getenv("TQC_NO_FORK")) ? 1 : 0;
+    if (pl->tables_parallel) {
+        TQC_CUDA(cudaEventCreateWithFlags(&pl->ev_fork, cudaEventDisableTiming));
+        for (int l = 0; l < tqc_plan::N_LANES; ++l) {
+            TQC_CUDA(cudaStreamCreateWithFlags(&pl->lane[l], cudaStreamNonBlocking));
+            TQC_CUDA(cudaEventCreateWithFlags(&pl->ev_join[l], cudaEventDisableTiming));
+        }
+    }
+    return 0;
+}
+
 int contract_states_impl(tqc_plan_t *pl, const uint64_t *states_dev, size_t n_states, float *out_dev, void *workspace_dev,
                         size_t workspace_bytes, void *stream) {
     if (!pl) return fail(TQC_E_ARG, "null plan");
@@ -1244,27 +1267,12 @@ int contract_states_impl(tqc_plan_t *pl, const uint64_t *states_dev, size_t n_st
     cx.ws = tables;
     // Table steps whose operands are all leaves neither depend on one another nor share storage (plan.cpp releases a
     // table's block only when another table step consumes it): they go to side streams and overlap the key kernel.
-    if (pl->tables_parallel < 0) {
-        int n_tab = 0;
-        bool leaf_only = true;
-        for (int t = 0; t < hp.m - 1; ++t) {
-            if (hp.nodes[hp.m + t].kind != tqc::NODE_TABLE) continue;
-            ++n_tab;
-            if (hp.steps[t].lhs >= hp.m || hp.steps[t].rhs >= hp.m) leaf_only = false;
-        }
-        pl->tables_parallel = (n_tab >= 1 && leaf_only && !getenv("TQC_NO_FORK")) ? 1 : 0;
-        if (pl->tables_parallel) {
-            TQC_CUDA(cudaEventCreateWithFlags(&pl->ev_fork, cudaEventDisableTiming));
-            for (int l = 0; l < tqc_plan::N_LANES; ++l) {
-                TQC_CUDA(cudaStreamCreateWithFlags(&pl->lane[l], cudaStreamNonBlocking));
-                TQC_CUDA(cudaEventCreateWithFlags(&pl->ev_join[l], cudaEventDisableTiming));
-            }
-        }
-    }
+    if ((rc = ensure_lanes(pl))) return rc;
     const bool fork = pl->tables_parallel == 1 && !pl->profile;
     int lanes_used = 0;
     if (fork) {
-        TQC_CUDA(cudaEventRecord(pl->ev_fork, st));
+        if (!pl->fork_recorded) TQC_CUDA(cudaEventRecord(pl->ev_fork, st));
+        pl->fork_recorded = false;
         int next = 0;
         for (int t = 0; t < hp.m - 1; ++t) {
             if (hp.nodes[hp.m + t].kind != tqc::NODE_TABLE) continue;
@@ -1419,8 +1427,16 @@ int tqc_contract_states_host(tqc_plan_t *pl, const uint64_t *states_host, size_t
     char *ws = (char *)workspace_dev;
     uint64_t *sd = (uint64_t *)ws;
     float *od = (float *)(ws + sb);
+    // the table steps do not depend on the states: fork their side streams off BEFORE the host-to-device copy so that
+    // they run under it (only for the plain path: a sliced plan loops over sub-networks, profile mode stays serial)
+    if (pl->hp.mode == TQC_MODE_STATES && pl->n_sliced() == 0 && !pl->profile) {
+        const int lrc = ensure_lanes(pl);
+        if (lrc) return lrc;
+        if (pl->tables_parallel == 1) { TQC_CUDA(cudaEventRecord(pl->ev_fork, st)); pl->fork_recorded = true; }
+    }
     if (words > 0) TQC_CUDA(cudaMemcpyAsync(sd, states_host, n_states * words * 8, cudaMemcpyHostToDevice, st));
     const int rc = tqc_contract_states(pl, sd, n_states, od, ws + sb + ob, workspace_bytes - sb - ob, stream);
+    pl->fork_recorded = false;
     if (rc) return rc;
     TQC_CUDA(cudaMemcpyAsync(out_host, od, n_states * 4, cudaMemcpyDeviceToHost, st));
     return 0;
