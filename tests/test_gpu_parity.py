@@ -185,3 +185,33 @@ def test_host_buffer_entry_points_and_profile_hooks():
     tqc.tqc_contract_distribution_host(pland, dh, wsd)
     torch.cuda.synchronize()
     assert np.array_equal(dh.numpy().astype(np.float64), ddev)
+
+
+@pytest.mark.parametrize("net_name", ["cfg4", "rand"])
+def test_host_buffer_pipeline_large_batch(net_name):
+    """A large ragged batch through tqc_contract_states_host on a non-default stream: the table steps are forked off
+    before the host-to-device copy.  Same values as the device-pointer call, repeated calls on the same buffers (the
+    staging area is reused), and the caller's stream order covering the copy back."""
+    if net_name == "cfg4":
+        net = configs.cfg4_network()
+    else:
+        net = configs.random_network(5, 7, 191, o_lo=2, o_hi=4)
+    T = random_tensors(net, 192)
+    plan = _loaded_plan(net, T, tqc.MODE_STATES, batch_hint=1 << 17)
+    B = 70001
+    ws = torch.empty(plan.workspace_bytes_host(B), dtype=torch.uint8, device="cuda")
+    oh = torch.empty(B, dtype=torch.float32).pin_memory()
+    stream = torch.cuda.Stream()
+    for rep in range(3):
+        bits = random_states(net.n_qubits, B, 193 + rep)
+        sh = torch.from_numpy(pack_states(bits).view(np.int64)).pin_memory()
+        oh.fill_(-1.0)
+        with torch.cuda.stream(stream):
+            tqc.tqc_contract_states_host(plan, sh, oh, ws, stream=stream)
+        stream.synchronize()                                  # only the caller's stream: the side streams must be joined
+        got = oh.numpy().copy()
+        dev = tqc.tqc_contract_states(plan, sh.cuda())
+        torch.cuda.synchronize()
+        assert np.array_equal(got, dev.cpu().numpy())
+    want = direct_sum_c(net, T, bits[:24])[0] if net_name == "cfg4" else R.direct_sum(net, T, bits[:200])
+    assert np.abs(got[:len(want)] - want).max() <= TOL * np.abs(want).max()
