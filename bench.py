@@ -200,6 +200,14 @@ def roofline_for(plan, tag: int, avg_ms: float, B: int, mode_states: bool, peaks
     t_hbm = nbytes / (peaks["hbm_gbs"] * 1e9)
     sec = avg_ms * 1e-3
     name = {0: "step_tile_kernel (fp32 FFMA)", 1: "dot_kernel", 2: "step_tc_kernel (3xTF32 tcgen05)"}.get(kclass, "?")
+    st_ = plan.step(tag)
+    if kclass == 0 and (not mode_states or plan.node(plan.m + tag)["kind"] == 1):
+        # cross-mode step: the launcher's integer rule for the warp-level tensor-core tile kernel
+        la, lb = plan.node(st_["lhs"]), plan.node(st_["rhs"])
+        lgm = la["n_bits"] + 2 * st_["n_outer_lhs"]
+        lgn = lb["n_bits"] + 2 * st_["n_outer_rhs"]
+        if 3 <= 2 * st_["n_inner"] <= 6 and min(lgm, lgn) >= 6 and max(lgm, lgn) >= 7:
+            name = "cross_mma_kernel (3xTF32 mma.sync tiles; FP32-ALU peak as reference)"
     if kclass == 2:
         t_cmp, peak, unit, bound = 3.0 * flop / (tf32_peak * 1e12), tf32_peak, "TFLOP/s", "tensor"
         achieved = 3.0 * flop / sec / 1e12            # issued tensor flops: 3 TF32 MMAs per fp32-accurate product
