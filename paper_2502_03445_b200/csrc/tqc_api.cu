@@ -1501,7 +1501,7 @@ int tqc_hss_scores(tqc_plan_t *pl, int s, float *scores_dev, void *stream) {
     if (rows < 148 * 16 && lgCols >= 10) {                  // few long rows: a block per row keeps every SM loading
         tqc::hss_norm_kernel<256><<<(unsigned)rows, 256, 0, st>>>(pl->d_leaf[s], scores_dev, rows, lgCols, unscale);
     } else {
-        const long long warps = std::min<long long>(rows, 148ll * 64);
+        const long long warps = std::min<long long>(rows, 148ll * 64 * 32);     // one warp per row: blocks are scheduled as SMs free up
         const unsigned blocks = (unsigned)((warps * 32 + 255) / 256);
         tqc::hss_norm_kernel<32><<<blocks, 256, 0, st>>>(pl->d_leaf[s], scores_dev, rows, lgCols, unscale);
     }
