@@ -206,20 +206,54 @@ __device__ __forceinline__ void chain_step_spec(const float *pa, const float *pb
         float4 a4[NQ];
 #pragma unroll
         for (int q = 0; q < NQ; ++q) a4[q] = *reinterpret_cast<const float4 *>(pa + 4 * g + 4 * G * q);
-#pragma unroll 4
-        for (int jb = 0; jb < N; jb += RP) {
-            const int j = jb + rr;
-            float v = 0.f;
-            if (j < N) {
+        // U passes (U * RP rows) per round: all their loads are issued before the first use (the step is bound by the
+        // latency of these L2 reads, not by their bandwidth), and the U partial sums of a lane meet their G - 1 partners by
+        // recursive halving - each level a lane keeps half of its values and sends the other half - so U rows cost about
+        // U shuffles instead of U log2 G.  Lane g ends with the row whose pass number is the top log2 U bits of g.
+        constexpr int UMAX = NQ >= 8 ? 1 : 8 / NQ;
+        constexpr int U = G < UMAX ? G : UMAX;
+        constexpr int LGG = G == 32 ? 5 : G == 16 ? 4 : G == 8 ? 3 : 2, LGU = U == 8 ? 3 : U == 4 ? 2 : U == 2 ? 1 : 0;
+        static_assert((1 << LGG) == G && (1 << LGU) == U, "row-split lane groups");
+#pragma unroll 1
+        for (int jb = 0; jb < N; jb += U * RP) {
+            float4 b[U][NQ];
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int j = jb + u * RP + rr;
+#pragma unroll
+                for (int q = 0; q < NQ; ++q)
+                    b[u][q] = j < N ? __ldg(reinterpret_cast<const float4 *>(pb + (size_t)j * PB + 4 * g + 4 * G * q))
+                                    : make_float4(0.f, 0.f, 0.f, 0.f);
+            }
+            float v[U];
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                float s0 = 0.f, s1 = 0.f;
 #pragma unroll
                 for (int q = 0; q < NQ; ++q) {
-                    const float4 b = __ldg(reinterpret_cast<const float4 *>(pb + (size_t)j * PB + 4 * g + 4 * G * q));
-                    v = fmaf(a4[q].x, b.x, v); v = fmaf(a4[q].y, b.y, v); v = fmaf(a4[q].z, b.z, v); v = fmaf(a4[q].w, b.w, v);
+                    s0 = fmaf(a4[q].x, b[u][q].x, s0); s1 = fmaf(a4[q].y, b[u][q].y, s1);
+                    s0 = fmaf(a4[q].z, b[u][q].z, s0); s1 = fmaf(a4[q].w, b[u][q].w, s1);
+                }
+                v[u] = s0 + s1;
+            }
+            int cnt = U;
+#pragma unroll
+            for (int d = G >> 1; d > 0; d >>= 1) {
+                if (cnt > 1) {
+                    const bool up = (g & d) != 0;
+#pragma unroll
+                    for (int i = 0; i < cnt / 2; ++i) {
+                        const float send = up ? v[i] : v[i + cnt / 2];
+                        const float keep = up ? v[i + cnt / 2] : v[i];
+                        v[i] = keep + __shfl_xor_sync(0xffffffffu, send, d);
+                    }
+                    cnt /= 2;
+                } else {
+                    v[0] += __shfl_xor_sync(0xffffffffu, v[0], d);
                 }
             }
-#pragma unroll
-            for (int d = G >> 1; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
-            if (j < N && g == 0) emit(0, j, v);
+            const int j = jb + (g >> (LGG - LGU)) * RP + rr;
+            if (j < N && (g & ((1 << (LGG - LGU)) - 1)) == 0) emit(0, j, v[0]);
         }
     } else if constexpr (O >= 32 && LGK >= 2) {
         // a lane owns an NI x NJ block of outputs: rows i0 + x * SI, columns j0 + y * SJ, with the 32 lanes laid out LI x LJ
