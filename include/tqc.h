@@ -94,6 +94,9 @@ typedef struct {
                                        cut ids.  Tensors are still loaded whole; every intermediate that carried a sliced cut is 4x
                                        smaller per cut.  Sliced plans run step by step (no fused chain); workspace sizes include
                                        one partial-sum buffer (4 bytes per output; add it to tqc_plan_workspace_min_bytes). */
+    int32_t kmax_cap;               /* restarts > 0 only: among the randomised-greedy orders keep the cheapest one whose widest
+                                       step K_max = max_t |E_a u E_b| is <= kmax_cap; while no order meets the
+                                       cap the smaller K_max wins.  0 = no cap (total multiplication count only). */
 } tqc_plan_opts;
 
 /* ---- planning (host only; no CUDA call) -------------------------------------------------

@@ -53,7 +53,7 @@ class _PlanOpts(ctypes.Structure):
     _fields_ = [("mode", c_int32), ("n_order_steps", c_int32), ("order", POINTER(c_int32)),
                 ("restarts", c_int32), ("seed", c_uint64), ("batch_hint", c_int64),
                 ("table_log2_floats_max", c_int32), ("use_tcgen05", c_int32), ("use_chain", c_int32),
-                ("n_slice_cuts", c_int32), ("slice_cuts", POINTER(c_int32))]
+                ("n_slice_cuts", c_int32), ("slice_cuts", POINTER(c_int32)), ("kmax_cap", c_int32)]
 
 
 def lib_path() -> str:
@@ -233,7 +233,8 @@ def _network_desc(net):
 
 
 def tqc_plan(net, mode: int = MODE_STATES, order=None, restarts: int = 0, seed: int = 0, batch_hint: int = 0,
-             table_log2_floats_max: int = 0, use_tcgen05: int = 0, use_chain: int = 0, slice_cuts=None) -> Plan:
+             table_log2_floats_max: int = 0, use_tcgen05: int = 0, use_chain: int = 0, slice_cuts=None,
+             kmax_cap: int = 0) -> Plan:
     """net: any object with n_qubits, cuts [(up, down)], sub_cuts [[cut ids]], sub_qubits [[qubit ids]]
     (e.g. tqc_inputs.Network).  order: optional list of m-1 (lhs, rhs) node-id pairs.  slice_cuts: cut ids evaluated by
     index slicing (summed over their 4 bases) instead of being contracted as bonds."""
@@ -241,7 +242,8 @@ def tqc_plan(net, mode: int = MODE_STATES, order=None, restarts: int = 0, seed: 
     oflat, oflat_p = _i32(v for ab in (order or []) for v in ab)
     sflat, sflat_p = _i32(slice_cuts or [])
     opts = _PlanOpts(mode, len(order) if order else 0, oflat_p, restarts, seed, batch_hint,
-                     table_log2_floats_max, use_tcgen05, use_chain, len(slice_cuts) if slice_cuts else 0, sflat_p)
+                     table_log2_floats_max, use_tcgen05, use_chain, len(slice_cuts) if slice_cuts else 0, sflat_p,
+                     kmax_cap)
     h = c_void_p()
     _check(_lib.tqc_plan(byref(desc), byref(opts), byref(h)))
     return Plan(h.value)
@@ -251,7 +253,7 @@ def tqc_choose_slice_cuts(net, mode: int = MODE_STATES, max_log2_input_floats: i
                           max_log2_intermediate_floats: int = 62, batch_hint: int = 0):
     """The paper's two-level slicing choice (include/tqc.h): list of cut ids in pick order."""
     desc, _keep = _network_desc(net)
-    opts = _PlanOpts(mode, 0, None, 0, 0, batch_hint, 0, 0, 0, 0, None)
+    opts = _PlanOpts(mode, 0, None, 0, 0, batch_hint, 0, 0, 0, 0, None, 0)
     out = np.zeros(max(1, len(net.cuts)), dtype=np.int32)
     n = c_int32(0)
     _check(_lib.tqc_choose_slice_cuts(byref(desc), byref(opts), max_log2_input_floats, max_log2_intermediate_floats,

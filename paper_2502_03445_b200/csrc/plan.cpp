@@ -222,14 +222,21 @@ int build_plan(int n, int m, int K, const int32_t *cut_up, const int32_t *cut_do
         order = greedy_order(p, leaf_open, 0.0, nullptr, &too_large);
         if (too_large) { err = "plan would need a tensor of more than 2^120 entries"; return E_TOO_LARGE; }
         if (opts.restarts > 0) {
-            double best = order_cost_log2(p, leaf_open, order, nullptr);
+            // objective: total multiplication count, among the orders whose K_max (the widest step)
+            // stays within kmax_cap; while no order meets the cap the smaller K_max wins
+            int best_k = 0;
+            double best = order_cost_log2(p, leaf_open, order, &best_k);
+            const int cap = opts.kmax_cap > 0 ? opts.kmax_cap : 1 << 30;
             SplitMix64 rng(opts.seed);
             for (int r = 0; r < opts.restarts; ++r) {
                 const double noise = 0.5 + 2.5 * (double)(r % 8) / 8.0;
                 auto cand = greedy_order(p, leaf_open, noise, &rng, &too_large);
                 if (too_large) { too_large = false; continue; }
-                const double c = order_cost_log2(p, leaf_open, cand, nullptr);
-                if (c < best - 1e-12) { best = c; order = cand; }
+                int k = 0;
+                const double c = order_cost_log2(p, leaf_open, cand, &k);
+                const bool ok = k <= cap, best_ok = best_k <= cap;
+                const bool better = (ok && !best_ok) || (ok == best_ok && (ok ? c < best - 1e-12 : (k < best_k || (k == best_k && c < best - 1e-12))));
+                if (better) { best = c; best_k = k; order = cand; }
             }
         }
     }

@@ -106,6 +106,7 @@ struct PlanOptions {
     std::vector<std::pair<int, int>> order;     // explicit order (empty: greedy)
     int restarts = 0;
     uint64_t seed = 0;
+    int kmax_cap = 0;                           // restarts only: prefer orders with K_max <= cap (0: no cap)
     int64_t batch_hint = 0;                     // expected states per call (0: 2^20); sets table_bits_max
     int table_log2_floats_max = 0;              // 0: default 24 (64 MB per table)
 };

@@ -846,6 +846,7 @@ void plan_options_from(const tqc_plan_opts *opts, tqc::PlanOptions &po) {
     po.seed = opts->seed;
     po.batch_hint = opts->batch_hint;
     po.table_log2_floats_max = opts->table_log2_floats_max;
+    po.kmax_cap = opts->kmax_cap;
     for (int i = 0; i < opts->n_order_steps && opts->order; ++i) po.order.emplace_back(opts->order[2 * i], opts->order[2 * i + 1]);
 }
 }  // namespace
@@ -934,6 +935,7 @@ int tqc_plan(const tqc_network_desc *net, const tqc_plan_opts *opts, tqc_plan_t 
         po.seed = opts->seed;
         po.batch_hint = opts->batch_hint;
         po.table_log2_floats_max = opts->table_log2_floats_max;
+        po.kmax_cap = opts->kmax_cap;
         use_tc = opts->use_tcgen05;
         if (opts->n_order_steps > 0) {
             if (!opts->order) return fail(TQC_E_ARG, "n_order_steps > 0 but order is null");

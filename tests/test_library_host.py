@@ -161,3 +161,21 @@ def test_choose_slice_cuts_matches_reference_and_meets_limits():
                 assert max(2 * left[s] + net.o(s) for s in range(net.m)) <= lim_in
                 assert max([2 * plan.node(net.m + t)["n_open"] + (plan.node(net.m + t)["n_bits"] if mode else 0)
                             for t in range(net.m - 1)] or [0]) <= lim_inter
+
+
+def test_restarts_respect_kmax_cap_and_are_deterministic():
+    """Order search (PAPER.md 441-450: the role CoTenGra plays there): seeded randomised-greedy restarts keep the cheapest
+    order, optionally among those whose widest step stays within kmax_cap; the same seed gives the same plan."""
+    net = configs.cfg5_network()
+    greedy = tqc.tqc_plan(net, tqc.MODE_STATES)
+    a = tqc.tqc_plan(net, tqc.MODE_STATES, restarts=64, seed=7)
+    b = tqc.tqc_plan(net, tqc.MODE_STATES, restarts=64, seed=7)
+    assert a.serialize() == b.serialize()
+    assert a.cost_log2 <= greedy.cost_log2 + 1e-9
+    capped = tqc.tqc_plan(net, tqc.MODE_STATES, restarts=64, seed=7, kmax_cap=greedy.kmax - 1)
+    assert capped.kmax <= max(greedy.kmax - 1, min(a.kmax, greedy.kmax))
+    if capped.kmax <= greedy.kmax - 1:
+        loose = tqc.tqc_plan(net, tqc.MODE_STATES, restarts=64, seed=7, kmax_cap=capped.kmax)
+        assert loose.kmax <= capped.kmax and loose.cost_log2 <= capped.cost_log2 + 1e-9
+    impossible = tqc.tqc_plan(net, tqc.MODE_STATES, restarts=16, seed=3, kmax_cap=2)      # nothing meets it: smallest K_max wins
+    assert impossible.kmax <= greedy.kmax
