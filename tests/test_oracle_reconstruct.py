@@ -204,3 +204,38 @@ def test_sliced_sum_is_the_network(slice_cuts):
     assert np.allclose(R.sliced_sum(net, T, bits, slice_cuts), R.direct_sum(net, T, bits), rtol=1e-12)
     small, Ts = R.slice_network(net, T, slice_cuts, [1] * len(slice_cuts))
     assert small.K == net.K - len(slice_cuts) and [t.shape[0] for t in Ts] == [4 ** small.c(s) for s in range(net.m)]
+
+
+def _limits(net, mode, cuts):
+    """Largest single-network input tensor and largest plan intermediate (log2 floats) with `cuts` sliced - recomputed here
+    from the reduced network and the reference planner's steps."""
+    small = P._without(net, cuts)
+    big_in = max(2 * small.c(s) + small.o(s) for s in range(net.m))
+    plan = P.plan(small, mode)
+    bits = {s: small.o(s) for s in range(net.m)}
+    worst = 0
+    for t, st in enumerate(plan["steps"]):
+        bits[net.m + t] = bits[st["lhs"]] + bits[st["rhs"]]
+        worst = max(worst, 2 * (len(st["outer_lhs"]) + len(st["outer_rhs"])) + (bits[net.m + t] if mode else 0))
+    return big_in, worst
+
+
+@pytest.mark.parametrize("seed", range(8))
+def test_choose_slice_cuts_reference_invariants(seed):
+    """planner_ref.choose_slice_cuts (two-level slicing, PAPER.md 460-472): the chosen set meets both limits, nothing is
+    sliced when nothing exceeds them, picks are distinct, and every pick was needed when it was made (the limit it serves
+    was still violated by the picks before it)."""
+    net = configs.random_network(3 + seed % 4, 6 + seed % 5, seed=900 + seed, o_lo=0, o_hi=4)
+    for mode in (0, 1):
+        in0, inter0 = _limits(net, mode, [])
+        assert P.choose_slice_cuts(net, mode, in0, inter0) == []
+        for lim_in, lim_inter in ((in0 - 2, 62), (62, max(inter0 - 3, 2)), (in0 - 2, max(inter0 - 4, 2))):
+            S = P.choose_slice_cuts(net, mode, lim_in, lim_inter)
+            if S is None:
+                continue
+            assert len(set(S)) == len(S) and all(0 <= e < net.K for e in S)
+            got_in, got_inter = _limits(net, mode, S)
+            assert got_in <= lim_in and got_inter <= lim_inter
+            for k in range(len(S)):
+                before_in, before_inter = _limits(net, mode, S[:k])
+                assert before_in > lim_in or before_inter > lim_inter
