@@ -2,8 +2,10 @@
 //     C[outA(i') | outB(j')] = sum_k A[rowA(i'), k] * B[rowB(j'), k]
 // is one M' x N' x K product per step (PAPER.md lines 318-330 merged bond).  With K this
 // short the fp32 FFMA kernel is bound by instruction issue, not by the result write, so the products run on the tensor
-// pipe as warp-level 3xTF32 mma.sync blocks (kernels_chain.cuh: chain_step_mma), 64 x 128 outputs per 256-thread block,
-// and the tile leaves through shared memory so that every store is a full 16-byte piece of a C row.
+// pipe as warp-level 3xTF32 mma.sync blocks (kernels_chain.cuh: chain_step_mma), 64 x 128 outputs per 256-thread block.
+// Where j' and j' + 1 are neighbours in C (the usual case: the result layout keeps the operand's digit order) the results
+// leave straight from the fragments as 8-byte stores, four lanes per 32-byte sector; otherwise the tile goes through
+// shared memory and leaves row by row.
 #pragma once
 #include "device_args.h"
 #include "kernels_chain.cuh"
@@ -49,6 +51,17 @@ __global__ void __launch_bounds__(256) cross_mma_kernel(const StepArgs a) {
         *reinterpret_cast<float4 *>(Bs + row * P + 4 * k4) = __ldg(reinterpret_cast<const float4 *>(a.B.base + rowB[row]) + k4);
     }
     __syncthreads();
+    if (a.vec_store == 2) {
+        // j' and j' + 1 are neighbours in C: the two results a lane holds per fragment row leave as one 8-byte store, four
+        // lanes fill a 32-byte sector, no trip through shared memory
+        const int wi = warp >> 2, wj = warp & 3;
+        float keep = 0.f;
+        chain_step_mma<5, 5, LGK, P, P>(As + 32 * wi * P, Bs + 32 * wj * P, lane, [&](int i, int j, float v) {
+            if ((j & 1) == 0) keep = v;
+            else *reinterpret_cast<float2 *>(a.C + (offA[32 * wi + i] | offB[32 * wj + j - 1])) = make_float2(keep, v);
+        });
+        return;
+    }
     {   // warp grid 2 x 4 over the 64 x 128 tile: 32 x 32 outputs per warp
         const int wi = warp >> 2, wj = warp & 3;
         float *cw = Cs + (32 * wi) * CROSS_CP + 32 * wj;
@@ -66,9 +79,9 @@ __global__ void __launch_bounds__(256) cross_mma_kernel(const StepArgs a) {
     }
 }
 
-inline size_t cross_mma_smem(int lgK) {
+inline size_t cross_mma_smem(int lgK, bool staged_c) {
     const size_t P = ((size_t)1 << lgK) + 4;
-    return 8 * 2 * (size_t)(CROSS_TI + CROSS_TJ) + 4 * (size_t)(CROSS_TI + CROSS_TJ) * P + 4 * (size_t)CROSS_TI * CROSS_CP;
+    return 8 * 2 * (size_t)(CROSS_TI + CROSS_TJ) + 4 * (size_t)(CROSS_TI + CROSS_TJ) * P + (staged_c ? 4 * (size_t)CROSS_TI * CROSS_CP : 0);
 }
 
 }  // namespace tqc

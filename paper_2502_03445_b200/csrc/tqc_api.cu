@@ -296,9 +296,10 @@ int launch_cross_step(tqc_plan_t *pl, const CrossCtx &cx, int t, cudaStream_t st
         if (a.lgN < 7) { std::swap(a.A, a.B); std::swap(a.outA, a.outB); std::swap(a.lgM, a.lgN); }
         a.lgTilesI = a.lgM - 6; a.lgTilesJ = a.lgN - 7;
         a.vec_store = (a.outB.n >= 1 && a.outB.src[0] == 0 && a.outB.dst[0] == 0 && a.outB.len[0] >= 2) ? 1 : 0;
+        if (a.vec_store && !getenv("TQC_CROSS_STAGED")) a.vec_store = 2;          // 8-byte stores straight from the fragments
         const long long blocks = 1ll << (a.lgTilesI + a.lgTilesJ);
         if (blocks > 0x7fffffffll) return fail(TQC_E_TOO_LARGE, "step needs more than 2^31 thread blocks");
-        const size_t smem = tqc::cross_mma_smem(a.lgK);
+        const size_t smem = tqc::cross_mma_smem(a.lgK, a.vec_store != 2);
         static bool attr = false;
         if (!attr) {
             TQC_CUDA(cudaFuncSetAttribute(tqc::cross_mma_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
