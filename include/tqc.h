@@ -208,6 +208,43 @@ int tqc_hss_prepare(tqc_plan_t *plan, const int32_t *counts, const int32_t *keys
 size_t tqc_hss_workspace_bytes(const tqc_plan_t *plan);
 int tqc_hss_contract(tqc_plan_t *plan, float *out_dev, void *workspace_dev, size_t workspace_bytes, void *stream);
 
+/* ---- Subcircuit variants on the device (section 2.1) -- fourth row of SURVEY 8(f) ---------------
+ * The quantum half of the method runs every subcircuit in 4^{d_s} * 3^{u_s} variants - each downstream cut wire
+ * initialised in |0>, |1>, |+> or |i>, each upstream cut wire measured in Z, X or Y (I shares the Z setting, lines
+ * 184-185) - and the Pauli bases of a downstream cut are "constructed as a linear combination from the initialization
+ * states" (line 188; coefficients: DESIGN.md reading G3).  tqc_simulate_subcircuit_tensor stands in for the QPU with a
+ * noiseless fp64 statevector simulation of all variants on the device ("noiseless classical simulators", line 722) and
+ * writes T_s in the layout tqc_load_subcircuit_tensors takes with on_device = 1.
+ *
+ * sub (HOST, read before the call returns):
+ *   w wires; wire 0 is the most significant bit of the amplitude index (G4); all wires start in |0> unless listed in D.
+ *     w = 0 (a subcircuit no gate was assigned to) gives the 1 x 1 tensor [1].
+ *   gates[n_gates] applied in order; kind = TQC_GATE_*, wire0 (and wire1 for two-qubit gates; CX controls on wire0),
+ *     param = angle of RX/RY/RZ (exp(-i param P / 2)) and RZZ (exp(-i param Z(x)Z)); SX/SY/SW = exp(-i pi/4 P) for
+ *     P = X, Y, (X+Y)/sqrt2.
+ *   D_wires[d]: wires that begin at a downstream cut end;  U_wires[u]: wires that end at an upstream cut end;
+ *   O_wires[o]: wires that end at a circuit output, in the order of x_s (first = MSB).  u + o = w.
+ *   bond_pos[d + u]: bond j (D_wires in order, then U_wires in order) is digit bond_pos[j] of the row index of T_s
+ *     (0 = most significant = the subcircuit's first listed incident cut).
+ * out_dev DEVICE [4^{d+u}][2^o] fp32.  workspace DEVICE, 256-byte aligned, >= tqc_simulate_workspace_bytes(sub) (0 if the
+ * description is out of range).  Asynchronous on `stream`, no allocation.  Errors: TQC_E_ARG (inconsistent lists, unknown
+ * gate), TQC_E_TOO_LARGE (w > 13 or 4^{d+u} 2^o > 2^31), TQC_E_WORKSPACE, TQC_E_CUDA. */
+enum { TQC_GATE_H = 0, TQC_GATE_X = 1, TQC_GATE_S = 2, TQC_GATE_SDG = 3, TQC_GATE_SX = 4, TQC_GATE_SY = 5, TQC_GATE_SW = 6,
+       TQC_GATE_RX = 7, TQC_GATE_RY = 8, TQC_GATE_RZ = 9, TQC_GATE_CZ = 10, TQC_GATE_CX = 11, TQC_GATE_RZZ = 12 };
+typedef struct {
+    int32_t kind, wire0, wire1, reserved;
+    double param;
+} tqc_gate;
+typedef struct {
+    int32_t w, n_gates;
+    const tqc_gate *gates;
+    int32_t d, u, o, reserved;
+    const int32_t *D_wires, *U_wires, *O_wires, *bond_pos;
+} tqc_subcircuit_desc;
+size_t tqc_simulate_workspace_bytes(const tqc_subcircuit_desc *sub);
+int tqc_simulate_subcircuit_tensor(const tqc_subcircuit_desc *sub, float *out_dev, void *workspace_dev,
+                                   size_t workspace_bytes, void *stream);
+
 /* ---- measurement hooks (bench.py) --------------------------------------------------------------
  * tqc_plan_launch_count: kernels launched so far on behalf of this plan.
  * tqc_plan_profile_enable(plan, 1): every later contract call records one CUDA event on the

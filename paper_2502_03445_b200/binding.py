@@ -33,7 +33,8 @@ EXPORTED = ["tqc_plan", "tqc_plan_destroy", "tqc_plan_mode", "tqc_plan_num_qubit
             "tqc_plan_workspace_bytes_host", "tqc_contract_states_host", "tqc_contract_distribution_host",
             "tqc_plan_profile_enable", "tqc_plan_profile_read", "tqc_plan_chain_status", "tqc_hss_scores", "tqc_hss_select",
             "tqc_hss_expand", "tqc_plan_num_sliced_cuts", "tqc_choose_slice_cuts", "tqc_hss_prepare",
-            "tqc_hss_workspace_bytes", "tqc_hss_contract"]
+            "tqc_hss_workspace_bytes", "tqc_hss_contract", "tqc_simulate_workspace_bytes",
+            "tqc_simulate_subcircuit_tensor"]
 
 
 class TqcError(RuntimeError):
@@ -54,6 +55,21 @@ class _PlanOpts(ctypes.Structure):
                 ("restarts", c_int32), ("seed", c_uint64), ("batch_hint", c_int64),
                 ("table_log2_floats_max", c_int32), ("use_tcgen05", c_int32), ("use_chain", c_int32),
                 ("n_slice_cuts", c_int32), ("slice_cuts", POINTER(c_int32)), ("kmax_cap", c_int32)]
+
+
+class _Gate(ctypes.Structure):
+    _fields_ = [("kind", c_int32), ("wire0", c_int32), ("wire1", c_int32), ("reserved", c_int32), ("param", c_double)]
+
+
+class _SubcircuitDesc(ctypes.Structure):
+    _fields_ = [("w", c_int32), ("n_gates", c_int32), ("gates", POINTER(_Gate)),
+                ("d", c_int32), ("u", c_int32), ("o", c_int32), ("reserved", c_int32),
+                ("D_wires", POINTER(c_int32)), ("U_wires", POINTER(c_int32)), ("O_wires", POINTER(c_int32)),
+                ("bond_pos", POINTER(c_int32))]
+
+
+GATE_KINDS = {"h": 0, "x": 1, "s": 2, "sdg": 3, "sx": 4, "sy": 5, "sw": 6, "rx": 7, "ry": 8, "rz": 9, "cz": 10, "cx": 11,
+              "rzz": 12}
 
 
 def lib_path() -> str:
@@ -103,6 +119,9 @@ def _load() -> ctypes.CDLL:
     lib.tqc_hss_workspace_bytes.argtypes = [c_void_p]
     lib.tqc_hss_workspace_bytes.restype = c_size_t
     lib.tqc_hss_contract.argtypes = [c_void_p, c_void_p, c_void_p, c_size_t, c_void_p]
+    lib.tqc_simulate_workspace_bytes.argtypes = [POINTER(_SubcircuitDesc)]
+    lib.tqc_simulate_workspace_bytes.restype = c_size_t
+    lib.tqc_simulate_subcircuit_tensor.argtypes = [POINTER(_SubcircuitDesc), c_void_p, c_void_p, c_size_t, c_void_p]
     return lib
 
 
@@ -387,4 +406,42 @@ def tqc_hss_contract(plan: Plan, x, out=None, workspace=None, stream=None, devic
     if workspace is None:
         workspace = torch.empty(max(256, int(_lib.tqc_hss_workspace_bytes(plan._h))), dtype=torch.uint8, device=device)
     _check(_lib.tqc_hss_contract(plan._h, out.data_ptr(), workspace.data_ptr(), workspace.numel(), _stream_ptr(stream)))
+    return out
+
+
+def _subcircuit_desc(w, gates, D_wires, U_wires, O_wires, bond_pos):
+    garr = (_Gate * max(1, len(gates)))()
+    for t, (name, params, wires) in enumerate(gates):
+        if name not in GATE_KINDS:
+            raise TqcError(-1, f"unknown gate {name}")
+        garr[t].kind = GATE_KINDS[name]
+        garr[t].wire0 = int(wires[0])
+        garr[t].wire1 = int(wires[1]) if len(wires) > 1 else 0
+        garr[t].param = float(params[0]) if len(params) else 0.0
+    keep = [garr] + [_i32(v) for v in (D_wires, U_wires, O_wires, bond_pos)]
+    desc = _SubcircuitDesc(int(w), len(gates), garr, len(D_wires), len(U_wires), len(O_wires), 0,
+                           *[ptr for (_arr, ptr) in keep[1:]])
+    return desc, keep
+
+
+def tqc_simulate_workspace_bytes(w, gates, D_wires, U_wires, O_wires, bond_pos) -> int:
+    desc, _keep = _subcircuit_desc(w, gates, D_wires, U_wires, O_wires, bond_pos)
+    return int(_lib.tqc_simulate_workspace_bytes(byref(desc)))
+
+
+def tqc_simulate_subcircuit_tensor(w, gates, D_wires, U_wires, O_wires, bond_pos, out=None, workspace=None, stream=None,
+                                   device="cuda"):
+    """T_s of one subcircuit from a device simulation of its 4^d 3^u variants (section 2.1): CUDA fp32
+    [4^{d+u}, 2^o] in the layout tqc_load_subcircuit_tensors takes.  gates: (name, params, local wires) in order;
+    bond_pos[j]: digit position (0 = most significant) of bond j (D_wires, then U_wires) in the row index."""
+    import torch
+    desc, _keep = _subcircuit_desc(w, gates, D_wires, U_wires, O_wires, bond_pos)
+    c, o = len(D_wires) + len(U_wires), len(O_wires)
+    if out is None:
+        out = torch.empty((4 ** c, 2 ** o), dtype=torch.float32, device=device)
+    if workspace is None:
+        workspace = torch.empty(max(256, int(_lib.tqc_simulate_workspace_bytes(byref(desc)))), dtype=torch.uint8,
+                                device=device)
+    _check(_lib.tqc_simulate_subcircuit_tensor(byref(desc), out.data_ptr(), workspace.data_ptr(), workspace.numel(),
+                                               _stream_ptr(stream)))
     return out

@@ -20,6 +20,7 @@
 #include "kernels_tc.cuh"
 #include "kernels_chain.cuh"
 #include "kernels_cross.cuh"
+#include "kernels_sim.cuh"
 #include "plan.hpp"
 
 namespace {
@@ -1686,6 +1687,138 @@ int tqc_plan_chain_status(const tqc_plan_t *pl, char *note, size_t note_len) {
     if (!pl) return fail(TQC_E_ARG, "null plan");
     if (note && note_len) { snprintf(note, note_len, "%s", pl->jit_note.c_str()); }
     return !pl->chain ? 0 : (pl->jit_fn ? 2 : 1);
+}
+
+// ---- NEXT row 4: subcircuit variants simulated on the device -> T_s (section 2.1) ----------
+namespace {
+typedef std::pair<double, double> cplx;
+// Standard gate definitions written out entry by entry (row-major, first operand = more significant index bit).
+bool sim_gate_matrix(int kind, double t, tqc::SimGate &g) {
+    const double r = std::sqrt(0.5);
+    std::vector<cplx> m;
+    auto rot = [&](cplx px00, cplx px01, cplx px10, cplx px11) {       // cos(t/2) I - i sin(t/2) P
+        const double c = std::cos(t / 2.0), s = std::sin(t / 2.0);
+        auto mi = [&](cplx p) { return cplx(s * p.second, -s * p.first); };   // -i s p
+        cplx a = mi(px00), b = mi(px01), cc = mi(px10), d = mi(px11);
+        m = {cplx(c + a.first, a.second), b, cc, cplx(c + d.first, d.second)};
+    };
+    switch (kind) {
+    case TQC_GATE_H: m = {{r, 0}, {r, 0}, {r, 0}, {-r, 0}}; break;
+    case TQC_GATE_X: m = {{0, 0}, {1, 0}, {1, 0}, {0, 0}}; break;
+    case TQC_GATE_S: m = {{1, 0}, {0, 0}, {0, 0}, {0, 1}}; break;
+    case TQC_GATE_SDG: m = {{1, 0}, {0, 0}, {0, 0}, {0, -1}}; break;
+    // exp(-i pi/4 P) = (I - iP)/sqrt2 for P = X, Y, W = (X + Y)/sqrt2 (reading G11)
+    case TQC_GATE_SX: m = {{r, 0}, {0, -r}, {0, -r}, {r, 0}}; break;
+    case TQC_GATE_SY: m = {{r, 0}, {-r, 0}, {r, 0}, {r, 0}}; break;
+    case TQC_GATE_SW: m = {{r, 0}, {-0.5, -0.5}, {0.5, -0.5}, {r, 0}}; break;
+    case TQC_GATE_RX: rot({0, 0}, {1, 0}, {1, 0}, {0, 0}); break;
+    case TQC_GATE_RY: rot({0, 0}, {0, -1}, {0, 1}, {0, 0}); break;
+    case TQC_GATE_RZ: rot({1, 0}, {0, 0}, {0, 0}, {-1, 0}); break;
+    case TQC_GATE_CZ:
+        m.assign(16, cplx(0, 0));
+        m[0] = m[5] = m[10] = cplx(1, 0); m[15] = cplx(-1, 0);
+        break;
+    case TQC_GATE_CX:                                                   // control = first operand
+        m.assign(16, cplx(0, 0));
+        m[0] = m[5] = m[11] = m[14] = cplx(1, 0);
+        break;
+    case TQC_GATE_RZZ: {                                                // exp(-i t Z(x)Z): diag e^{-it}, e^{it}, e^{it}, e^{-it}
+        m.assign(16, cplx(0, 0));
+        const double c = std::cos(t), s = std::sin(t);
+        m[0] = m[15] = cplx(c, -s); m[5] = m[10] = cplx(c, s);
+        break;
+    }
+    default: return false;
+    }
+    g.nq = m.size() == 4 ? 1 : 2;
+    for (size_t i = 0; i < m.size(); ++i) g.m[i] = make_double2(m[i].first, m[i].second);
+    return true;
+}
+size_t sim_align(size_t b) { return (b + 255) & ~size_t(255); }
+}  // namespace
+
+size_t tqc_simulate_workspace_bytes(const tqc_subcircuit_desc *sub) {
+    if (!sub || sub->d < 0 || sub->u < 0 || sub->o < 0 || sub->n_gates < 0) return 0;
+    const int lg = 2 * (sub->d + sub->u) + sub->o;
+    if (lg > 31) return 0;
+    return sim_align(sizeof(tqc::SimGate) * (size_t)std::max(sub->n_gates, 1)) + sim_align(sizeof(double) << lg);
+}
+
+int tqc_simulate_subcircuit_tensor(const tqc_subcircuit_desc *sub, float *out_dev, void *workspace_dev,
+                                   size_t workspace_bytes, void *stream) {
+    if (!sub || !out_dev || !workspace_dev) return fail(TQC_E_ARG, "null argument");
+    const int w = sub->w, d = sub->d, u = sub->u, o = sub->o, c = d + u;
+    if (w < 0 || d < 0 || u < 0 || o < 0 || sub->n_gates < 0) return fail(TQC_E_ARG, "negative size");
+    if (u + o != w) return fail(TQC_E_ARG, "every wire ends in an upstream cut or an output: u + o must equal w");
+    if (d > w) return fail(TQC_E_ARG, "more downstream wires than wires");
+    if (w > 13) return fail(TQC_E_TOO_LARGE, "w > 13: 2^w complex128 amplitudes do not fit one block's shared memory");
+    if (d > 15 || u > 15 || 2 * c + o > 31) return fail(TQC_E_TOO_LARGE, "4^c 2^o exceeds 2^31 entries");
+    if ((d && !sub->D_wires) || (u && !sub->U_wires) || (o && !sub->O_wires) || (c && !sub->bond_pos) ||
+        (sub->n_gates && !sub->gates))
+        return fail(TQC_E_ARG, "null wire / gate list");
+    if ((uintptr_t)workspace_dev & 255) return fail(TQC_E_ARG, "workspace must be 256-byte aligned");
+    if (workspace_bytes < tqc_simulate_workspace_bytes(sub)) return fail(TQC_E_WORKSPACE, "workspace too small");
+    tqc::SimArgs a{};
+    a.w = w; a.d = d; a.u = u; a.o = o; a.n_gates = sub->n_gates;
+    std::vector<char> ends(w, 0), begins(w, 0);
+    auto wire_ok = [&](int q) { return q >= 0 && q < w; };
+    for (int i = 0; i < d; ++i) {
+        if (!wire_ok(sub->D_wires[i]) || begins[sub->D_wires[i]]++) return fail(TQC_E_ARG, "bad downstream wire list");
+        a.D_bit[i] = w - 1 - sub->D_wires[i];                             // wire 0 = most significant index bit (G4)
+    }
+    for (int j = 0; j < u; ++j) {
+        if (!wire_ok(sub->U_wires[j]) || ends[sub->U_wires[j]]++) return fail(TQC_E_ARG, "bad upstream wire list");
+        a.U_bit[j] = w - 1 - sub->U_wires[j];
+    }
+    for (int j = 0; j < o; ++j) {
+        if (!wire_ok(sub->O_wires[j]) || ends[sub->O_wires[j]]++) return fail(TQC_E_ARG, "bad output wire list");
+        a.O_bit[j] = w - 1 - sub->O_wires[j];
+    }
+    tqc::SimPermArgs pa{};
+    pa.c = c; pa.o = o;
+    std::vector<char> seen(c, 0);
+    for (int j = 0; j < c; ++j) {
+        const int p = sub->bond_pos[j];
+        if (p < 0 || p >= c || seen[p]++) return fail(TQC_E_ARG, "bond_pos is not a permutation of 0..c-1");
+        pa.pos[j] = p;
+    }
+    std::vector<tqc::SimGate> hg((size_t)std::max(sub->n_gates, 1));
+    for (int t = 0; t < sub->n_gates; ++t) {
+        const tqc_gate &g = sub->gates[t];
+        if (!sim_gate_matrix(g.kind, g.param, hg[t])) return fail(TQC_E_ARG, "unknown gate kind " + std::to_string(g.kind));
+        if (!wire_ok(g.wire0) || (hg[t].nq == 2 && (!wire_ok(g.wire1) || g.wire1 == g.wire0)))
+            return fail(TQC_E_ARG, "gate " + std::to_string(t) + ": wire out of range");
+        hg[t].b0 = w - 1 - g.wire0;
+        hg[t].b1 = hg[t].nq == 2 ? w - 1 - g.wire1 : 0;
+        hg[t].pad = 0;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    tqc::SimGate *d_gates = (tqc::SimGate *)workspace_dev;
+    a.gates = d_gates;
+    a.R = (double *)((char *)workspace_dev + sim_align(sizeof(tqc::SimGate) * hg.size()));
+    // pageable source: the runtime stages the bytes before the call returns, so hg may go out of scope
+    TQC_CUDA(cudaMemcpyAsync(d_gates, hg.data(), sizeof(tqc::SimGate) * hg.size(), cudaMemcpyHostToDevice, st));
+    const size_t smem = sizeof(double2) << w;
+    static bool attr_set = false;
+    if (!attr_set) {
+        TQC_CUDA(cudaFuncSetAttribute(tqc::sim_variant_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 16 << 13));
+        attr_set = true;
+    }
+    unsigned variants = 1;
+    for (int i = 0; i < d; ++i) variants *= 4;
+    for (int j = 0; j < u; ++j) variants *= 3;
+    tqc::sim_variant_kernel<<<variants, 256, smem, st>>>(a);
+    TQC_CUDA(cudaGetLastError());
+    const size_t total = size_t(1) << (2 * c + o);
+    for (int i = 0; i < d; ++i) {
+        const size_t inner = size_t(1) << (2 * (d - 1 - i) + 2 * u + o), tuples = total >> 2;
+        const unsigned blocks = (unsigned)std::min<size_t>((tuples + 255) / 256, 148 * 16);
+        tqc::sim_kappa_axis_kernel<<<blocks, 256, 0, st>>>(a.R, inner, tuples);
+    }
+    const unsigned blocks = (unsigned)std::min<size_t>((total + 255) / 256, 148 * 16);
+    tqc::sim_permute_cast_kernel<<<blocks, 256, 0, st>>>(a.R, out_dev, pa, total);
+    TQC_CUDA(cudaGetLastError());
+    return 0;
 }
 
 }  // extern "C"

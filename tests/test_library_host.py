@@ -179,3 +179,22 @@ def test_restarts_respect_kmax_cap_and_are_deterministic():
         assert loose.kmax <= capped.kmax and loose.cost_log2 <= capped.cost_log2 + 1e-9
     impossible = tqc.tqc_plan(net, tqc.MODE_STATES, restarts=16, seed=3, kmax_cap=2)      # nothing meets it: smallest K_max wins
     assert impossible.kmax <= greedy.kmax
+
+
+def test_simulate_description_checks_run_without_a_gpu():
+    # tqc_simulate_subcircuit_tensor validates its description on the host before any CUDA call (include/tqc.h)
+    import ctypes
+    from paper_2502_03445_b200.binding import _lib, _subcircuit_desc
+    gates = [("h", (), (0,)), ("rzz", (0.3,), (0, 1))]
+    ws = binding.tqc_simulate_workspace_bytes(2, gates, [0], [1], [0], [1, 0])
+    # gate table (272 B per gate, rounded to 256) + 4^2 * 2 float64 entries
+    assert ws == 768 + 256
+    assert binding.tqc_simulate_workspace_bytes(20, [], list(range(8)), list(range(8)), list(range(8, 20)), list(range(16))) == 0
+    fake = ctypes.c_void_p(256)
+    for bad, code in (((2, gates, [0], [0], [], [1, 0]), -1),           # u + o != w
+                      ((2, [("h", (), (5,))], [], [], [0, 1], []), -1),  # gate wire out of range
+                      ((14, [], [], [], list(range(14)), []), -6)):      # too wide for one block
+        desc, _keep = _subcircuit_desc(*bad)
+        assert _lib.tqc_simulate_subcircuit_tensor(ctypes.byref(desc), fake, fake, 1 << 30, None) == code
+    with pytest.raises(binding.TqcError):
+        binding.tqc_simulate_workspace_bytes(1, [("nope", (), (0,))], [], [], [0], [])
