@@ -270,6 +270,7 @@ def run_ours(args) -> None:
                               {"workload": o["config"]["workload"], "e2e_value": o["e2e"]["value"]})
             others.append(measure_hss(ctx, 10, 3))
             others.append(measure_hss_contract(ctx, 10, 3))
+            others.append(measure_variants(ctx, 10, 3))
             line["other_workloads"] = others
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(make_workload(args.workload, args.batch), args.cpu_seconds)
@@ -441,6 +442,59 @@ def measure_hss(ctx, steps: int, warmup: int) -> dict:
             "roofline": {"bound": "hbm", "kernel": "hss_norm_kernel<32>", "achieved": gbs, "peak": peaks["hbm_gbs"],
                          "unit": "GB/s", "frac": gbs / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"],
                          "algorithmic_bytes_per_launch": nbytes // net.m}}
+
+
+def measure_variants(ctx, steps: int, warmup: int) -> dict:
+    """NEXT row 4 (section 2.1): T_s of one subcircuit from a device simulation of its 4^d 3^u variants.  Synthetic
+    subcircuit with the shape of cfg3's middle one (12 wires, d = u = 3, o = 9; three RY/RZ layers, two CX ladders, seeded
+    angles): 1728 variants, one block each.  The amplitudes never leave shared memory, so the bound is the shared-memory
+    pipe: every pass (one per two-qubit gate after the host folds the one-qubit gates in, plus the measurement
+    rotations) reads and writes 2^w complex128 once (peak = 148 SMs x 128 B/clk x sm_max_mhz)."""
+    torch, tqc, dev = ctx["torch"], ctx["tqc"], ctx["dev"]
+    w, d, u = 12, 3, 3
+    rng = np.random.default_rng(250203445 + 4)
+    gates = []
+    for layer in range(3):
+        for q in range(w):
+            gates.append(("ry", (float(rng.random() * 2 * np.pi),), (q,)))
+            gates.append(("rz", (float(rng.random() * 2 * np.pi),), (q,)))
+        if layer < 2:
+            gates += [("cx", (), (q, q + 1)) for q in range(w - 1)]
+    desc = dict(w=w, gates=gates, D_wires=[0, 1, 2], U_wires=[9, 10, 11], O_wires=list(range(9)),
+                bond_pos=[0, 1, 2, 3, 4, 5])
+    out = torch.empty((4 ** (d + u), 2 ** (w - u)), dtype=torch.float32, device=dev)
+    ws = torch.empty(tqc.tqc_simulate_workspace_bytes(**desc), dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    for _ in range(warmup):
+        tqc.tqc_simulate_subcircuit_tensor(**desc, out=out, workspace=ws, stream=stream)
+    torch.cuda.synchronize()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for a, b in evs:
+        flush.zero_()
+        a.record(stream)
+        tqc.tqc_simulate_subcircuit_tensor(**desc, out=out, workspace=ws, stream=stream)
+        b.record(stream)
+    torch.cuda.synchronize()
+    ms = sum(a.elapsed_time(b) for a, b in evs) / steps
+    variants = 4 ** d * 3 ** u
+    peaks = measured_peaks()
+    # one read + one write of every amplitude per pass; passes = 22 two-qubit gates (the one-qubit gates are folded into
+    # them on the host) + on average 2/3 * u measurement rotations
+    passes = sum(1 for g in gates if len(g[2]) == 2) + 2
+    smem_bytes = variants * passes * 2 * 16 * 2 ** w
+    peak = 148 * 128 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e9
+    gbs = smem_bytes / (ms * 1e-3) / 1e9
+    assert abs(float(out[0].sum()) - 2 ** d) < 1e-3                # sum_x T[I...I, x] = 2^{d_s} (reading G16)
+    return {"workload": f"variants: {w}-wire subcircuit, d = u = 3, {len(gates)} gates, {variants} variants -> T_s "
+                        f"[4^6][2^9] (tqc_simulate_subcircuit_tensor)",
+            "value": variants / (ms * 1e-3), "unit": "subcircuit variants simulated/s", "ms_per_step": ms, "steps": steps,
+            "gpu_launches": 2 + d,
+            "roofline": {"bound": "smem", "kernel": "sim_variant_kernel (whole call timed: + 3 sim_kappa_axis_kernel + "
+                                                    "sim_permute_cast_kernel)",
+                         "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak, "traffic": None,
+                         "peak_source": "derived: 148 SMs x 32 banks x 4 B x sm_max_mhz",
+                         "algorithmic_bytes_per_launch": smem_bytes}}
 
 
 def measure_hss_contract(ctx, steps: int, warmup: int) -> dict:

@@ -238,7 +238,9 @@ typedef struct {
 typedef struct {
     int32_t w, n_gates;
     const tqc_gate *gates;
-    int32_t d, u, o, reserved;
+    int32_t d, u, o;
+    int32_t fuse_gates; /* 1: one-qubit gates are multiplied into the neighbouring two-qubit gate on their wire (one pass per
+                           two-qubit gate; same unitary up to fp64 rounding); 0: one pass per listed gate */
     const int32_t *D_wires, *U_wires, *O_wires, *bond_pos;
 } tqc_subcircuit_desc;
 size_t tqc_simulate_workspace_bytes(const tqc_subcircuit_desc *sub);

@@ -63,7 +63,7 @@ class _Gate(ctypes.Structure):
 
 class _SubcircuitDesc(ctypes.Structure):
     _fields_ = [("w", c_int32), ("n_gates", c_int32), ("gates", POINTER(_Gate)),
-                ("d", c_int32), ("u", c_int32), ("o", c_int32), ("reserved", c_int32),
+                ("d", c_int32), ("u", c_int32), ("o", c_int32), ("fuse_gates", c_int32),
                 ("D_wires", POINTER(c_int32)), ("U_wires", POINTER(c_int32)), ("O_wires", POINTER(c_int32)),
                 ("bond_pos", POINTER(c_int32))]
 
@@ -409,7 +409,7 @@ def tqc_hss_contract(plan: Plan, x, out=None, workspace=None, stream=None, devic
     return out
 
 
-def _subcircuit_desc(w, gates, D_wires, U_wires, O_wires, bond_pos):
+def _subcircuit_desc(w, gates, D_wires, U_wires, O_wires, bond_pos, fuse_gates=True):
     garr = (_Gate * max(1, len(gates)))()
     for t, (name, params, wires) in enumerate(gates):
         if name not in GATE_KINDS:
@@ -419,7 +419,7 @@ def _subcircuit_desc(w, gates, D_wires, U_wires, O_wires, bond_pos):
         garr[t].wire1 = int(wires[1]) if len(wires) > 1 else 0
         garr[t].param = float(params[0]) if len(params) else 0.0
     keep = [garr] + [_i32(v) for v in (D_wires, U_wires, O_wires, bond_pos)]
-    desc = _SubcircuitDesc(int(w), len(gates), garr, len(D_wires), len(U_wires), len(O_wires), 0,
+    desc = _SubcircuitDesc(int(w), len(gates), garr, len(D_wires), len(U_wires), len(O_wires), 1 if fuse_gates else 0,
                            *[ptr for (_arr, ptr) in keep[1:]])
     return desc, keep
 
@@ -430,12 +430,12 @@ def tqc_simulate_workspace_bytes(w, gates, D_wires, U_wires, O_wires, bond_pos) 
 
 
 def tqc_simulate_subcircuit_tensor(w, gates, D_wires, U_wires, O_wires, bond_pos, out=None, workspace=None, stream=None,
-                                   device="cuda"):
+                                   device="cuda", fuse_gates=True):
     """T_s of one subcircuit from a device simulation of its 4^d 3^u variants (section 2.1): CUDA fp32
     [4^{d+u}, 2^o] in the layout tqc_load_subcircuit_tensors takes.  gates: (name, params, local wires) in order;
     bond_pos[j]: digit position (0 = most significant) of bond j (D_wires, then U_wires) in the row index."""
     import torch
-    desc, _keep = _subcircuit_desc(w, gates, D_wires, U_wires, O_wires, bond_pos)
+    desc, _keep = _subcircuit_desc(w, gates, D_wires, U_wires, O_wires, bond_pos, fuse_gates)
     c, o = len(D_wires) + len(U_wires), len(O_wires)
     if out is None:
         out = torch.empty((4 ** c, 2 ** o), dtype=torch.float32, device=device)

@@ -1735,6 +1735,73 @@ bool sim_gate_matrix(int kind, double t, tqc::SimGate &g) {
     return true;
 }
 size_t sim_align(size_t b) { return (b + 255) & ~size_t(255); }
+
+double2 sim_cmul(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+// c = a * b for dim x dim row-major complex matrices
+void sim_matmul(const double2 *a, const double2 *b, double2 *c, int dim) {
+    double2 t[16];
+    for (int r = 0; r < dim; ++r)
+        for (int col = 0; col < dim; ++col) {
+            double2 acc = make_double2(0.0, 0.0);
+            for (int k = 0; k < dim; ++k) {
+                const double2 p = sim_cmul(a[r * dim + k], b[k * dim + col]);
+                acc.x += p.x; acc.y += p.y;
+            }
+            t[r * dim + col] = acc;
+        }
+    std::copy(t, t + dim * dim, c);
+}
+// 4x4 of a one-qubit matrix acting on the first (slot 0) or second (slot 1) operand of a two-qubit op
+void sim_lift(const double2 *m, int slot, double2 *out) {
+    for (int r = 0; r < 4; ++r)
+        for (int c = 0; c < 4; ++c) {
+            const int r0 = r >> 1, r1 = r & 1, c0 = c >> 1, c1 = c & 1;
+            const bool same = slot == 0 ? r1 == c1 : r0 == c0;
+            out[r * 4 + c] = same ? (slot == 0 ? m[r0 * 2 + c0] : m[r1 * 2 + c1]) : make_double2(0.0, 0.0);
+        }
+}
+// Gate fusion (host, exact up to fp64 rounding): every pass over the amplitudes costs the same shared-memory traffic
+// whatever the gate, so one-qubit gates are multiplied into the two-qubit op that precedes them on their wire (nothing
+// between the two touches that wire), or, before the wire's first two-qubit gate, into the one that follows.  What is
+// left is one pass per two-qubit gate plus one per wire that has only one-qubit gates.
+std::vector<tqc::SimGate> sim_fuse(const std::vector<tqc::SimGate> &in, int n_in, int w) {
+    std::vector<tqc::SimGate> ops;
+    std::vector<int> last(w, -1);
+    std::vector<char> has_pend(w, 0);
+    std::vector<tqc::SimGate> pend(w);
+    for (int t = 0; t < n_in; ++t) {
+        const tqc::SimGate &g = in[t];
+        if (g.nq == 1) {
+            const int q = g.b0;
+            if (last[q] >= 0) {
+                tqc::SimGate &op = ops[last[q]];
+                double2 lifted[16];
+                sim_lift(g.m, op.b0 == q ? 0 : 1, lifted);
+                sim_matmul(lifted, op.m, op.m, 4);
+            } else if (has_pend[q]) {
+                sim_matmul(g.m, pend[q].m, pend[q].m, 2);
+            } else {
+                pend[q] = g;
+                has_pend[q] = 1;
+            }
+        } else {
+            tqc::SimGate op = g;
+            const int qs[2] = {g.b0, g.b1};
+            for (int slot = 0; slot < 2; ++slot)
+                if (has_pend[qs[slot]]) {
+                    double2 lifted[16];
+                    sim_lift(pend[qs[slot]].m, slot, lifted);
+                    sim_matmul(op.m, lifted, op.m, 4);
+                    has_pend[qs[slot]] = 0;
+                }
+            last[g.b0] = last[g.b1] = (int)ops.size();
+            ops.push_back(op);
+        }
+    }
+    for (int q = 0; q < w; ++q)
+        if (has_pend[q]) ops.push_back(pend[q]);
+    return ops;
+}
 }  // namespace
 
 size_t tqc_simulate_workspace_bytes(const tqc_subcircuit_desc *sub) {
@@ -1792,10 +1859,16 @@ int tqc_simulate_subcircuit_tensor(const tqc_subcircuit_desc *sub, float *out_de
         hg[t].b1 = hg[t].nq == 2 ? w - 1 - g.wire1 : 0;
         hg[t].pad = 0;
     }
+    const size_t gate_bytes = sim_align(sizeof(tqc::SimGate) * hg.size());     // the workspace is sized for the unfused list
+    if (sub->fuse_gates) {
+        hg = sim_fuse(hg, sub->n_gates, w);
+        a.n_gates = (int)hg.size();
+        if (hg.empty()) hg.resize(1);
+    }
     cudaStream_t st = (cudaStream_t)stream;
     tqc::SimGate *d_gates = (tqc::SimGate *)workspace_dev;
     a.gates = d_gates;
-    a.R = (double *)((char *)workspace_dev + sim_align(sizeof(tqc::SimGate) * hg.size()));
+    a.R = (double *)((char *)workspace_dev + gate_bytes);
     // pageable source: the runtime stages the bytes before the call returns, so hg may go out of scope
     TQC_CUDA(cudaMemcpyAsync(d_gates, hg.data(), sizeof(tqc::SimGate) * hg.size(), cudaMemcpyHostToDevice, st));
     const size_t smem = sizeof(double2) << w;

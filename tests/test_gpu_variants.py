@@ -24,14 +24,14 @@ def _args(net, sub):
                 O_wires=[w for (w, _q) in sub.O], bond_pos=[want.index(e) for e in have])
 
 
-def _gpu_tensors(net, subs):
-    out = [tqc.tqc_simulate_subcircuit_tensor(**_args(net, sub)) for sub in subs]
+def _gpu_tensors(net, subs, fuse=True):
+    out = [tqc.tqc_simulate_subcircuit_tensor(**_args(net, sub), fuse_gates=fuse) for sub in subs]
     torch.cuda.synchronize()
     return out
 
 
-def _check_against_oracle(net, subs, T64):
-    got = _gpu_tensors(net, subs)
+def _check_against_oracle(net, subs, T64, fuse=True):
+    got = _gpu_tensors(net, subs, fuse)
     for sub, g, t in zip(subs, got, T64):
         assert tuple(g.shape) == t.shape
         tol = 2.0 ** (len(sub.D) - 23)
@@ -70,7 +70,8 @@ def _cut_circuit(n, n2q, m, seed, kmax=6):
 def test_random_circuits_every_gate_kind(seed):
     circ = _cut_circuit(6 + seed % 4, 8 + seed, 2 + seed % 2, 1000 + seed)
     net, T64, subs = cutting.tensors_from_circuit(circ)
-    got = _check_against_oracle(net, subs, T64)
+    _check_against_oracle(net, subs, T64, fuse=False)           # one pass per listed gate
+    got = _check_against_oracle(net, subs, T64)                 # one-qubit gates folded into their two-qubit neighbours
     # the second construction (O5', no measurement rotations, no kappa table) agrees as well
     _net2, T64b, _ = cutting.tensors_from_circuit(circ, operator_form=True)
     for sub, g, t in zip(subs, got, T64b):
@@ -95,6 +96,7 @@ def test_cfg3_subcircuits_twelve_wires():
     circ = configs.cfg3_circuit()
     net, T64, subs = cutting.tensors_from_circuit(circ)
     assert max(sub.w for sub in subs) == 12
+    _check_against_oracle(net, subs, T64, fuse=False)
     _check_against_oracle(net, subs, T64)
 
 
