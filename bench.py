@@ -257,6 +257,12 @@ def run_ours(args) -> None:
     import paper_2502_03445_b200 as tqc      # fails loudly if libtqc.so is missing
 
     ctx = {"torch": torch, "dist": dist, "tqc": tqc, "world": world, "rank": rank, "local": local, "dev": dev}
+    if args.workload == "variants":
+        if rank == 0:
+            print(json.dumps(measure_variants(ctx, args.steps, args.warmup)), flush=True)
+        if world > 1:
+            dist.destroy_process_group()
+        return
     line = measure(ctx, args, args.workload, args.batch, args.steps, args.warmup)
     if rank == 0:
         if world == 1 and args.others:
@@ -663,7 +669,8 @@ def main() -> None:
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg4", choices=["cfg2", "cfg3", "cfg4", "cfg5"])
+    ap.add_argument("--workload", default="cfg4", choices=["cfg2", "cfg3", "cfg4", "cfg5", "variants"],
+                    help="variants: only the subcircuit-variant simulation row (secondary line, for profiling)")
     ap.add_argument("--batch", type=int, default=0, help="states per step per GPU (0: the config's own batch)")
     ap.add_argument("--restarts", type=int, default=0, help="planner restarts (0: deterministic greedy)")
     ap.add_argument("--plan-seed", type=int, default=1)
