@@ -242,6 +242,9 @@ typedef struct {
     int32_t fuse_gates; /* 1: one-qubit gates are multiplied into the neighbouring two-qubit gate on their wire (one pass per
                            two-qubit gate; same unitary up to fp64 rounding); 0: one pass per listed gate */
     const int32_t *D_wires, *U_wires, *O_wires, *bond_pos;
+    int32_t walk_settings; /* 1: a block simulates a preparation once and walks several measurement settings from that
+                              state (Gray-code order, one rotation pass per setting); 0: one block per variant */
+    int32_t reserved;
 } tqc_subcircuit_desc;
 size_t tqc_simulate_workspace_bytes(const tqc_subcircuit_desc *sub);
 int tqc_simulate_subcircuit_tensor(const tqc_subcircuit_desc *sub, float *out_dev, void *workspace_dev,

@@ -65,7 +65,7 @@ class _SubcircuitDesc(ctypes.Structure):
     _fields_ = [("w", c_int32), ("n_gates", c_int32), ("gates", POINTER(_Gate)),
                 ("d", c_int32), ("u", c_int32), ("o", c_int32), ("fuse_gates", c_int32),
                 ("D_wires", POINTER(c_int32)), ("U_wires", POINTER(c_int32)), ("O_wires", POINTER(c_int32)),
-                ("bond_pos", POINTER(c_int32))]
+                ("bond_pos", POINTER(c_int32)), ("walk_settings", c_int32), ("reserved", c_int32)]
 
 
 GATE_KINDS = {"h": 0, "x": 1, "s": 2, "sdg": 3, "sx": 4, "sy": 5, "sw": 6, "rx": 7, "ry": 8, "rz": 9, "cz": 10, "cx": 11,
@@ -409,7 +409,7 @@ def tqc_hss_contract(plan: Plan, x, out=None, workspace=None, stream=None, devic
     return out
 
 
-def _subcircuit_desc(w, gates, D_wires, U_wires, O_wires, bond_pos, fuse_gates=True):
+def _subcircuit_desc(w, gates, D_wires, U_wires, O_wires, bond_pos, fuse_gates=True, walk_settings=True):
     garr = (_Gate * max(1, len(gates)))()
     for t, (name, params, wires) in enumerate(gates):
         if name not in GATE_KINDS:
@@ -420,7 +420,7 @@ def _subcircuit_desc(w, gates, D_wires, U_wires, O_wires, bond_pos, fuse_gates=T
         garr[t].param = float(params[0]) if len(params) else 0.0
     keep = [garr] + [_i32(v) for v in (D_wires, U_wires, O_wires, bond_pos)]
     desc = _SubcircuitDesc(int(w), len(gates), garr, len(D_wires), len(U_wires), len(O_wires), 1 if fuse_gates else 0,
-                           *[ptr for (_arr, ptr) in keep[1:]])
+                           *[ptr for (_arr, ptr) in keep[1:]], 1 if walk_settings else 0, 0)
     return desc, keep
 
 
@@ -430,12 +430,12 @@ def tqc_simulate_workspace_bytes(w, gates, D_wires, U_wires, O_wires, bond_pos) 
 
 
 def tqc_simulate_subcircuit_tensor(w, gates, D_wires, U_wires, O_wires, bond_pos, out=None, workspace=None, stream=None,
-                                   device="cuda", fuse_gates=True):
+                                   device="cuda", fuse_gates=True, walk_settings=True):
     """T_s of one subcircuit from a device simulation of its 4^d 3^u variants (section 2.1): CUDA fp32
     [4^{d+u}, 2^o] in the layout tqc_load_subcircuit_tensors takes.  gates: (name, params, local wires) in order;
     bond_pos[j]: digit position (0 = most significant) of bond j (D_wires, then U_wires) in the row index."""
     import torch
-    desc, _keep = _subcircuit_desc(w, gates, D_wires, U_wires, O_wires, bond_pos, fuse_gates)
+    desc, _keep = _subcircuit_desc(w, gates, D_wires, U_wires, O_wires, bond_pos, fuse_gates, walk_settings)
     c, o = len(D_wires) + len(U_wires), len(O_wires)
     if out is None:
         out = torch.empty((4 ** c, 2 ** o), dtype=torch.float32, device=device)

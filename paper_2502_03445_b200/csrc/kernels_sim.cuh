@@ -3,11 +3,12 @@
 //
 // A subcircuit with d downstream cut wires and u upstream cut wires has 4^d * 3^u variants: every downstream wire is
 // initialised in one of |0>, |1>, |+>, |i> and every upstream wire is measured in Z, X or Y ("only 3 ... per upstream
-// cut": I and Z share the Z setting).  One thread block simulates one variant: the 2^w
-// complex128 amplitudes live in shared memory for the whole run (w <= 13: 128 KB), every gate is one pass over them,
-// the measurement rotation and |amp|^2 follow, a Walsh-Hadamard pass over the upstream wires forms the signed sums over
-// the measured bits for every basis at once, and the block scatters its 2^{#Z settings} * 2^o results into
-// R[a][k_u][x].  The downstream bases are then "constructed as a linear combination from the initialization states"
+// cut": I and Z share the Z setting).  The variants of one preparation differ only in the
+// measurement rotations, so a thread block simulates one preparation once - the 2^w complex128 amplitudes live in
+// shared memory for the whole run (w <= 13: 192 KB with the probabilities), every gate is one pass over them - and
+// then walks a share of the 3^u settings; per setting: the rotation, |amp|^2, a Walsh-Hadamard pass over the upstream
+// wires that forms the signed sums over the measured bits for every basis at once, and a scatter of the
+// 2^{#Z settings} * 2^o results into R[a][k_u][x].  The downstream bases are then "constructed as a linear combination from the initialization states"
 // (line 188; coefficients: DESIGN.md reading G3) one axis at a time, and the result is written in the caller's axis
 // order as fp32.  All arithmetic is fp64 (B200 has full-rate FP64 units; the work is tiny next to the contraction).
 #pragma once
@@ -25,6 +26,7 @@ struct SimGate {
 
 struct SimArgs {
     int32_t w, d, u, o, n_gates;
+    int32_t g;                                 // the first g upstream wires' settings come from blockIdx, the rest are walked
     int32_t D_bit[16], U_bit[16], O_bit[32];   // amplitude-index bit positions of the listed wires
     const SimGate *gates;
     double *R;                                 // [4^d][4^u][2^o]
@@ -73,16 +75,28 @@ __device__ __forceinline__ void sim_apply_2q(double2 *psi, int w, int b0, int b1
     __syncthreads();
 }
 
-// blockIdx.x = a * 3^u + beta; a in base 4 (first downstream wire = most significant digit, 0..3 = |0>,|1>,|+>,|i>),
-// beta in base 3 (first upstream wire most significant, 0..2 = Z, X, Y).
-__global__ void __launch_bounds__(256) sim_variant_kernel(SimArgs g) {
+// Reflected ternary Gray code: digit k (0 = least significant) of step t.  Consecutive steps differ in one digit by +-1.
+__device__ __forceinline__ int gray3_digit(uint32_t t, uint32_t pow3k) {
+    const uint32_t q = t / pow3k;
+    const int dgt = int(q % 3);
+    return ((q / 3) & 1u) ? 2 - dgt : dgt;
+}
+
+// blockIdx.x = a * 3^g + group.  a in base 4 (first downstream wire = most significant digit, 0..3 = |0>,|1>,|+>,|i>).
+// The block simulates preparation a ONCE and then walks 3^{u-g} measurement settings (0..2 = Z, X, Y): the settings of
+// the first g upstream wires are the base-3 digits of `group`, those of the other u-g wires run through a reflected
+// Gray code, so going from one setting to the next is ONE one-qubit pass (new rotation times the inverse of the old one).
+// Shared memory: 2^w complex128 amplitudes followed by 2^w float64 probabilities.
+__global__ void __launch_bounds__(512) sim_variant_kernel(SimArgs g) {
     extern __shared__ double2 psi[];
-    __shared__ double2 rot[2][4];
-    const int w = g.w;
+    __shared__ double2 rot[4][4];
+    const int w = g.w, u = g.u, ng = g.g;
     const uint32_t size = 1u << w;
-    uint32_t pow3 = 1;
-    for (int j = 0; j < g.u; ++j) pow3 *= 3;
-    const uint32_t a = blockIdx.x / pow3, beta = blockIdx.x % pow3;
+    double *q = reinterpret_cast<double *>(psi + size);
+    uint32_t pow3g = 1, n_walk = 1;
+    for (int j = 0; j < ng; ++j) pow3g *= 3;
+    for (int j = ng; j < u; ++j) n_walk *= 3;
+    const uint32_t a = blockIdx.x / pow3g, group = blockIdx.x % pow3g;
     const double r = 0.70710678118654752440;
 
     // initial product state: downstream wires prepared, every other wire in |0>
@@ -102,11 +116,17 @@ __global__ void __launch_bounds__(256) sim_variant_kernel(SimArgs g) {
         psi[idx] = amp;
     }
     if (threadIdx.x == 0) {
-        // X setting: H.  Y setting: H * Sdg = [[1, -i], [1, i]] / sqrt2 (rotate so that a Z measurement reads the basis).
+        // rotate so that a Z measurement reads the basis.  rot[0]: X setting, H (also Z -> X and X -> Z: H is its own
+        // inverse).  rot[1]: Y setting, H Sdg = [[1, -i], [1, i]] / sqrt2.  rot[2]: X -> Y, (H Sdg) H.  rot[3]: Y -> X,
+        // H (S H) = H (H Sdg)^-1.
         rot[0][0] = make_double2(r, 0.0); rot[0][1] = make_double2(r, 0.0);
         rot[0][2] = make_double2(r, 0.0); rot[0][3] = make_double2(-r, 0.0);
         rot[1][0] = make_double2(r, 0.0); rot[1][1] = make_double2(0.0, -r);
         rot[1][2] = make_double2(r, 0.0); rot[1][3] = make_double2(0.0, r);
+        rot[2][0] = make_double2(0.5, -0.5); rot[2][1] = make_double2(0.5, 0.5);
+        rot[2][2] = make_double2(0.5, 0.5); rot[2][3] = make_double2(0.5, -0.5);
+        rot[3][0] = make_double2(0.5, 0.5); rot[3][1] = make_double2(0.5, -0.5);
+        rot[3][2] = make_double2(0.5, -0.5); rot[3][3] = make_double2(0.5, 0.5);
     }
     __syncthreads();
 
@@ -116,48 +136,63 @@ __global__ void __launch_bounds__(256) sim_variant_kernel(SimArgs g) {
         else sim_apply_2q(psi, w, gt->b0, gt->b1, gt->m);
     }
 
-    // measurement rotations of this setting
+    // settings of the fixed wires (the walked wires start at Z: no rotation)
     {
-        uint32_t rem = beta;
-        for (int j = g.u - 1; j >= 0; --j) {
+        uint32_t rem = group;
+        for (int j = ng - 1; j >= 0; --j) {
             const int bj = rem % 3;
             rem /= 3;
             if (bj) sim_apply_1q(psi, w, g.U_bit[j], rot[bj - 1]);
         }
     }
-    // q[x_O, b_U] = |amp|^2, kept in the real part
-    for (uint32_t idx = threadIdx.x; idx < size; idx += blockDim.x) {
-        const double2 v = psi[idx];
-        psi[idx].x = v.x * v.x + v.y * v.y;
-    }
-    __syncthreads();
-    // signed sums over the measured bits: sigma(I, b) = +1, sigma(X|Y|Z, b) = (-1)^b.  After the pass, the entry whose
-    // upstream bit is 0 holds the I sum and the entry whose bit is 1 holds the signed sum.
-    for (int j = 0; j < g.u; ++j) {
-        const int bit = g.U_bit[j];
-        for (uint32_t p = threadIdx.x; p < (size >> 1); p += blockDim.x) {
-            const uint32_t i0 = insert_zero(p, bit), i1 = i0 | (1u << bit);
-            const double p0 = psi[i0].x, p1 = psi[i1].x;
-            psi[i0].x = p0 + p1;
-            psi[i1].x = p0 - p1;
+    for (uint32_t step = 0; step < n_walk; ++step) {
+        // q[x_O, b_U] = |amp|^2
+        for (uint32_t idx = threadIdx.x; idx < size; idx += blockDim.x) {
+            const double2 v = psi[idx];
+            q[idx] = v.x * v.x + v.y * v.y;
         }
         __syncthreads();
-    }
-    // scatter: a Z setting serves I (bit 0) and Z (bit 1); an X or Y setting serves only its own basis (bit 1)
-    for (uint32_t idx = threadIdx.x; idx < size; idx += blockDim.x) {
-        uint32_t ku = 0, rem = beta;
-        bool keep = true;
-        for (int j = g.u - 1; j >= 0; --j) {
-            const int bj = rem % 3, bit = (idx >> g.U_bit[j]) & 1;
-            rem /= 3;
-            const uint32_t digit = bj == 0 ? (bit ? 3u : 0u) : uint32_t(bj);
-            keep = keep && (bj == 0 || bit);
-            ku |= digit << (2 * (g.u - 1 - j));
+        // signed sums over the measured bits: sigma(I, b) = +1, sigma(X|Y|Z, b) = (-1)^b.  After the pass, the entry whose
+        // upstream bit is 0 holds the I sum and the entry whose bit is 1 holds the signed sum.
+        for (int j = 0; j < u; ++j) {
+            const int bit = g.U_bit[j];
+            for (uint32_t p = threadIdx.x; p < (size >> 1); p += blockDim.x) {
+                const uint32_t i0 = insert_zero(p, bit), i1 = i0 | (1u << bit);
+                const double p0 = q[i0], p1 = q[i1];
+                q[i0] = p0 + p1;
+                q[i1] = p0 - p1;
+            }
+            __syncthreads();
         }
-        if (!keep) continue;
-        uint32_t x = 0;
-        for (int j = 0; j < g.o; ++j) x = (x << 1) | ((idx >> g.O_bit[j]) & 1u);
-        g.R[((((size_t(a) << (2 * g.u)) + ku)) << g.o) + x] = psi[idx].x;
+        // scatter: a Z setting serves I (bit 0) and Z (bit 1); an X or Y setting serves only its own basis (bit 1)
+        for (uint32_t idx = threadIdx.x; idx < size; idx += blockDim.x) {
+            uint32_t ku = 0, rem = group, pw = 1;
+            bool keep = true;
+            for (int j = u - 1; j >= 0; --j) {
+                int bj;
+                if (j >= ng) { bj = gray3_digit(step, pw); pw *= 3; }
+                else { bj = rem % 3; rem /= 3; }
+                const int bit = (idx >> g.U_bit[j]) & 1;
+                const uint32_t digit = bj == 0 ? (bit ? 3u : 0u) : uint32_t(bj);
+                keep = keep && (bj == 0 || bit);
+                ku |= digit << (2 * (u - 1 - j));
+            }
+            if (!keep) continue;
+            uint32_t x = 0;
+            for (int j = 0; j < g.o; ++j) x = (x << 1) | ((idx >> g.O_bit[j]) & 1u);
+            g.R[((((size_t(a) << (2 * u)) + ku)) << g.o) + x] = q[idx];
+        }
+        // next setting: the one walked wire whose Gray digit changes
+        if (step + 1 < n_walk) {
+            uint32_t pw = 1;
+            for (int j = u - 1; j >= ng; --j, pw *= 3) {
+                const int from = gray3_digit(step, pw), to = gray3_digit(step + 1, pw);
+                if (from == to) continue;
+                // 0 <-> 1: H;  1 -> 2: (H Sdg) H;  2 -> 1: H (S H)
+                const int which = (from + to == 1) ? 0 : (to == 2 ? 2 : 3);
+                sim_apply_1q(psi, w, g.U_bit[j], rot[which]);     // ends with __syncthreads (also fences the scatter reads)
+            }
+        }
     }
 }
 

@@ -1871,16 +1871,21 @@ int tqc_simulate_subcircuit_tensor(const tqc_subcircuit_desc *sub, float *out_de
     a.R = (double *)((char *)workspace_dev + gate_bytes);
     // pageable source: the runtime stages the bytes before the call returns, so hg may go out of scope
     TQC_CUDA(cudaMemcpyAsync(d_gates, hg.data(), sizeof(tqc::SimGate) * hg.size(), cudaMemcpyHostToDevice, st));
-    const size_t smem = sizeof(double2) << w;
+    const size_t smem = (sizeof(double2) + sizeof(double)) << w;          // amplitudes + probabilities
     static bool attr_set = false;
     if (!attr_set) {
-        TQC_CUDA(cudaFuncSetAttribute(tqc::sim_variant_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 16 << 13));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::sim_variant_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 24 << 13));
         attr_set = true;
     }
-    unsigned variants = 1;
-    for (int i = 0; i < d; ++i) variants *= 4;
-    for (int j = 0; j < u; ++j) variants *= 3;
-    tqc::sim_variant_kernel<<<variants, 256, smem, st>>>(a);
+    // One block per (preparation, group of settings): the settings of the first g upstream wires come from the block id,
+    // the block walks the other 3^{u-g}.  g = the smallest split that gives every SM two blocks (integers only).
+    unsigned blocks_v = 1;
+    for (int i = 0; i < d; ++i) blocks_v *= 4;
+    int g_fixed = 0;
+    while (g_fixed < u && blocks_v < 2 * 148) { blocks_v *= 3; ++g_fixed; }
+    if (sub->walk_settings == 0) { for (; g_fixed < u; ++g_fixed) blocks_v *= 3; }     // one block per variant
+    a.g = g_fixed;
+    tqc::sim_variant_kernel<<<blocks_v, w >= 11 ? 512 : 256, smem, st>>>(a);
     TQC_CUDA(cudaGetLastError());
     const size_t total = size_t(1) << (2 * c + o);
     for (int i = 0; i < d; ++i) {

@@ -25,7 +25,8 @@ def _args(net, sub):
 
 
 def _gpu_tensors(net, subs, fuse=True):
-    out = [tqc.tqc_simulate_subcircuit_tensor(**_args(net, sub), fuse_gates=fuse) for sub in subs]
+    # fuse = False also turns the settings walk off: one pass per listed gate, one block per variant
+    out = [tqc.tqc_simulate_subcircuit_tensor(**_args(net, sub), fuse_gates=fuse, walk_settings=fuse) for sub in subs]
     torch.cuda.synchronize()
     return out
 
