@@ -454,8 +454,7 @@ def measure_variants(ctx, steps: int, warmup: int) -> dict:
     """NEXT row 4 (section 2.1): T_s of one subcircuit from a device simulation of its 4^d 3^u variants.  Synthetic
     subcircuit with the shape of cfg3's middle one (12 wires, d = u = 3, o = 9; three RY/RZ layers, two CX ladders, seeded
     angles): 1728 variants, one block each.  The amplitudes never leave shared memory, so the bound is the shared-memory
-    pipe: every pass (one per two-qubit gate after the host folds the one-qubit gates in, plus the measurement
-    rotations) reads and writes 2^w complex128 once (peak = 148 SMs x 128 B/clk x sm_max_mhz)."""
+    pipe: every pass reads and writes the 2^w amplitudes once (peak = 148 SMs x 128 B/clk x sm_max_mhz)."""
     torch, tqc, dev = ctx["torch"], ctx["tqc"], ctx["dev"]
     w, d, u = 12, 3, 3
     rng = np.random.default_rng(250203445 + 4)
@@ -485,10 +484,18 @@ def measure_variants(ctx, steps: int, warmup: int) -> dict:
     ms = sum(a.elapsed_time(b) for a, b in evs) / steps
     variants = 4 ** d * 3 ** u
     peaks = measured_peaks()
-    # one read + one write of every amplitude per pass; passes = 22 two-qubit gates (the one-qubit gates are folded into
-    # them on the host) + on average 2/3 * u measurement rotations
-    passes = sum(1 for g in gates if len(g[2]) == 2) + 2
-    smem_bytes = variants * passes * 2 * 16 * 2 ** w
+    # Algorithmic shared-memory bytes: per preparation one pass per two-qubit gate (the one-qubit gates are
+    # folded into them on the host), 32 B per amplitude (complex128 read + write); per setting one rotation pass (32 B),
+    # |amp|^2 (16 B read + 8 B write), u Walsh-Hadamard passes over float64 (16 B each) and the scatter read (8 B).
+    n2q = sum(1 for g in gates if len(g[2]) == 2)
+    smem_bytes = 4 ** d * 2 ** w * (n2q * 32 + 3 ** u * (32 + 24 + 16 * u + 8))
+    # what the launch issues: the library splits the 3^u settings of a preparation over 3^g blocks (g = 2 here: 576
+    # blocks, two per SM) and each of them repeats the preparation's gate passes
+    g_fixed, blocks = 0, 4 ** d
+    while g_fixed < u and blocks < 2 * 148:
+        blocks, g_fixed = blocks * 3, g_fixed + 1
+    issued_bytes = 2 ** w * (blocks * (n2q + 2.0 * g_fixed / 3.0) * 32 + 4 ** d * 3 ** u * (24 + 16 * u + 8)
+                             + (4 ** d * 3 ** u - blocks) * 32)
     peak = 148 * 128 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e9
     gbs = smem_bytes / (ms * 1e-3) / 1e9
     assert abs(float(out[0].sum()) - 2 ** d) < 1e-3                # sum_x T[I...I, x] = 2^{d_s} (reading G16)
@@ -500,7 +507,8 @@ def measure_variants(ctx, steps: int, warmup: int) -> dict:
                                                     "sim_permute_cast_kernel)",
                          "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak, "traffic": None,
                          "peak_source": "derived: 148 SMs x 32 banks x 4 B x sm_max_mhz",
-                         "algorithmic_bytes_per_launch": smem_bytes}}
+                         "algorithmic_bytes_per_launch": smem_bytes, "issued_bytes_per_launch": issued_bytes,
+                         "issued_gbs": issued_bytes / (ms * 1e-3) / 1e9}}
 
 
 def measure_hss_contract(ctx, steps: int, warmup: int) -> dict:
