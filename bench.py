@@ -259,7 +259,7 @@ def run_ours(args) -> None:
     ctx = {"torch": torch, "dist": dist, "tqc": tqc, "world": world, "rank": rank, "local": local, "dev": dev}
     if args.workload == "variants":
         if rank == 0:
-            print(json.dumps(measure_variants(ctx, args.steps, args.warmup)), flush=True)
+            print(json.dumps(measure_variants(ctx, args.steps, args.warmup, not args.no_cpu_baseline)), flush=True)
         if world > 1:
             dist.destroy_process_group()
         return
@@ -276,7 +276,7 @@ def run_ours(args) -> None:
                               {"workload": o["config"]["workload"], "e2e_value": o["e2e"]["value"]})
             others.append(measure_hss(ctx, 10, 3))
             others.append(measure_hss_contract(ctx, 10, 3))
-            others.append(measure_variants(ctx, 10, 3))
+            others.append(measure_variants(ctx, 10, 3, not args.no_cpu_baseline))
             line["other_workloads"] = others
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(make_workload(args.workload, args.batch), args.cpu_seconds)
@@ -450,23 +450,16 @@ def measure_hss(ctx, steps: int, warmup: int) -> dict:
                          "algorithmic_bytes_per_launch": nbytes // net.m}}
 
 
-def measure_variants(ctx, steps: int, warmup: int) -> dict:
+def measure_variants(ctx, steps: int, warmup: int, with_cpu: bool = True) -> dict:
     """NEXT row 4 (section 2.1): T_s of one subcircuit from a device simulation of its 4^d 3^u variants.  Synthetic
     subcircuit with the shape of cfg3's middle one (12 wires, d = u = 3, o = 9; three RY/RZ layers, two CX ladders, seeded
     angles): 1728 variants, one block each.  The amplitudes never leave shared memory, so the bound is the shared-memory
     pipe: every pass reads and writes the 2^w amplitudes once (peak = 148 SMs x 128 B/clk x sm_max_mhz)."""
     torch, tqc, dev = ctx["torch"], ctx["tqc"], ctx["dev"]
+    from tqc_inputs.circuits import hea_subcircuit
     w, d, u = 12, 3, 3
-    rng = np.random.default_rng(250203445 + 4)
-    gates = []
-    for layer in range(3):
-        for q in range(w):
-            gates.append(("ry", (float(rng.random() * 2 * np.pi),), (q,)))
-            gates.append(("rz", (float(rng.random() * 2 * np.pi),), (q,)))
-        if layer < 2:
-            gates += [("cx", (), (q, q + 1)) for q in range(w - 1)]
-    desc = dict(w=w, gates=gates, D_wires=[0, 1, 2], U_wires=[9, 10, 11], O_wires=list(range(9)),
-                bond_pos=[0, 1, 2, 3, 4, 5])
+    desc = hea_subcircuit(w, d, u)
+    gates = desc["gates"]
     out = torch.empty((4 ** (d + u), 2 ** (w - u)), dtype=torch.float32, device=dev)
     ws = torch.empty(tqc.tqc_simulate_workspace_bytes(**desc), dtype=torch.uint8, device=dev)
     stream = torch.cuda.current_stream()
@@ -499,6 +492,24 @@ def measure_variants(ctx, steps: int, warmup: int) -> dict:
     peak = 148 * 128 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e9
     gbs = smem_bytes / (ms * 1e-3) / 1e9
     assert abs(float(out[0].sum()) - 2 ** d) < 1e-3                # sum_x T[I...I, x] = 2^{d_s} (reading G16)
+    cpu = None
+    if with_cpu:
+        # the oracle as it stands (O4/O5, numpy float64, one thread) on the SAME subcircuit, whole tensor; also a parity
+        # check of the timed configuration: |dT| <= 2^d 2^-23
+        from oracle import cutting
+        from types import SimpleNamespace
+        sub = cutting.Subcircuit(0, w=w, gates=gates, D=[(q, i) for i, q in enumerate(desc["D_wires"])],
+                                 U=[(q, d + j) for j, q in enumerate(desc["U_wires"])],
+                                 O=[(q, q) for q in desc["O_wires"]])
+        net1 = SimpleNamespace(sub_cuts=[list(range(d + u))])     # build_tensor reads only the subcircuit's axis order
+        t0 = time.perf_counter()
+        want = cutting.build_tensor(net1, sub)
+        sec = time.perf_counter() - t0
+        err = float(np.abs(out.cpu().numpy().astype(np.float64) - want).max())
+        assert err <= 2.0 ** (d - 23), ("variants row against the oracle", err)
+        cpu = {"value": variants / sec, "unit": "subcircuit variants simulated/s", "cores": 1, "kind": "oracle",
+               "sample": f"oracle.cutting.build_tensor on the same subcircuit, all {variants} variants, {sec:.1f} s; "
+                         f"max |T_gpu - T_oracle| = {err:.2e}"}
     return {"workload": f"variants: {w}-wire subcircuit, d = u = 3, {len(gates)} gates, {variants} variants -> T_s "
                         f"[4^6][2^9] (tqc_simulate_subcircuit_tensor)",
             "value": variants / (ms * 1e-3), "unit": "subcircuit variants simulated/s", "ms_per_step": ms, "steps": steps,
@@ -508,7 +519,8 @@ def measure_variants(ctx, steps: int, warmup: int) -> dict:
                          "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak, "traffic": None,
                          "peak_source": "derived: 148 SMs x 32 banks x 4 B x sm_max_mhz",
                          "algorithmic_bytes_per_launch": smem_bytes, "issued_bytes_per_launch": issued_bytes,
-                         "issued_gbs": issued_bytes / (ms * 1e-3) / 1e9}}
+                         "issued_gbs": issued_bytes / (ms * 1e-3) / 1e9},
+            "cpu_baseline": cpu}
 
 
 def measure_hss_contract(ctx, steps: int, warmup: int) -> dict:

@@ -101,6 +101,24 @@ def test_cfg3_subcircuits_twelve_wires():
     _check_against_oracle(net, subs, T64)
 
 
+def test_bench_subcircuit_in_the_launch_configuration_bench_times():
+    # bench.py's `variants` row: 12 wires, d = u = 3, 576 blocks walking 3 settings each, whole tensor against O4/O5
+    from types import SimpleNamespace
+    desc = C.hea_subcircuit(12, 3, 3)
+    sub = cutting.Subcircuit(0, w=12, gates=desc["gates"], D=[(q, i) for i, q in enumerate(desc["D_wires"])],
+                             U=[(q, 3 + j) for j, q in enumerate(desc["U_wires"])], O=[(q, q) for q in desc["O_wires"]])
+    want = cutting.build_tensor(SimpleNamespace(sub_cuts=[list(range(6))]), sub)
+    for walk in (True, False):
+        got = tqc.tqc_simulate_subcircuit_tensor(**desc, walk_settings=walk).cpu().numpy().astype(np.float64)
+        assert np.abs(got - want).max() <= 2.0 ** (3 - 23)
+    assert abs(want[0].sum() - 8.0) < 1e-9                      # sum_x T[I...I, x] = 2^{d_s}   (reading G16)
+    # a permuted axis order is the same tensor with its base-4 digits permuted
+    perm = [2, 0, 1, 5, 3, 4]
+    got_p = tqc.tqc_simulate_subcircuit_tensor(**{**desc, "bond_pos": perm}).cpu().numpy().astype(np.float64)
+    want_p = np.transpose(want.reshape((4,) * 6 + (512,)), list(np.argsort(perm)) + [6]).reshape(4096, 512)
+    assert np.abs(got_p - want_p).max() <= 2.0 ** (3 - 23)
+
+
 def test_errors():
     with pytest.raises(tqc.TqcError) as e:
         tqc.tqc_simulate_subcircuit_tensor(14, [], [], [], list(range(14)), [])

@@ -250,3 +250,20 @@ def assign_parts_random(circ: Circuit, m: int, seed: int) -> None:
     home = rng.integers(0, m, size=circ.n)
     circ.parts = [int(home[qs[int(rng.integers(0, 2))]]) if len(qs) == 2 else None
                   for (_n, _p, qs) in circ.gates]
+
+
+def hea_subcircuit(w: int = 12, d: int = 3, u: int = 3, seed: int = 250203445 + 4) -> dict:
+    """Description of ONE synthetic subcircuit with the shape of cfg3's middle one (bench.py's `variants` row and its
+    full-size parity test): three RY/RZ layers with a CX ladder after the first two, seeded angles; the first d wires
+    begin at a downstream cut, the last u wires end at an upstream cut, the others at circuit outputs; bonds in
+    (downstream..., upstream...) order.  Gate names and angles only: no arithmetic of the method."""
+    rng = np.random.default_rng(seed)
+    gates = []
+    for layer in range(3):
+        for q in range(w):
+            gates.append(("ry", (float(rng.random() * 2 * np.pi),), (q,)))
+            gates.append(("rz", (float(rng.random() * 2 * np.pi),), (q,)))
+        if layer < 2:
+            gates += [("cx", (), (q, q + 1)) for q in range(w - 1)]
+    return dict(w=w, gates=gates, D_wires=list(range(d)), U_wires=list(range(w - u, w)), O_wires=list(range(w - u)),
+                bond_pos=list(range(d + u)))
