@@ -1875,6 +1875,7 @@ int tqc_simulate_subcircuit_tensor(const tqc_subcircuit_desc *sub, float *out_de
     static bool attr_set = false;
     if (!attr_set) {
         TQC_CUDA(cudaFuncSetAttribute(tqc::sim_variant_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 24 << 13));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::sim_variant_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
         attr_set = true;
     }
     // One block per (preparation, group of settings): the settings of the first g upstream wires come from the block id,
@@ -1885,7 +1886,9 @@ int tqc_simulate_subcircuit_tensor(const tqc_subcircuit_desc *sub, float *out_de
     while (g_fixed < u && blocks_v < 2 * 148) { blocks_v *= 3; ++g_fixed; }
     if (sub->walk_settings == 0) { for (; g_fixed < u; ++g_fixed) blocks_v *= 3; }     // one block per variant
     a.g = g_fixed;
-    tqc::sim_variant_kernel<<<blocks_v, w >= 11 ? 512 : 256, smem, st>>>(a);
+    // 124 registers per thread: two 256-thread blocks share an SM (the other issues while one waits at a barrier); when
+    // the grid cannot give every SM two blocks, one wider block per SM
+    tqc::sim_variant_kernel<<<blocks_v, (w >= 11 && blocks_v < 2 * 148) ? 512 : 256, smem, st>>>(a);
     TQC_CUDA(cudaGetLastError());
     const size_t total = size_t(1) << (2 * c + o);
     for (int i = 0; i < d; ++i) {
