@@ -93,6 +93,23 @@ def test_simulated_tensors_reconstruct_the_uncut_distribution(cfg, n):
     assert abs(p.sum() - 1.0) < 1e-4
 
 
+def test_ghz_closed_form_through_device_tensors():
+    # GHZ-10 (P:742-744 benchmark family; closed form S:61): H, CX ladder, three parts -> p(0...0) = p(1...1) = 1/2
+    n = 10
+    gates = [("h", (), (0,))] + [("cx", (), (q, q + 1)) for q in range(n - 1)]
+    circ = C.Circuit(n, gates, name="ghz10")
+    C.assign_parts_by_qubit_ranges(circ, [3, 7])
+    net, subs = cutting.extract(circ)
+    assert net.K >= 2
+    plan = tqc.tqc_plan(net, tqc.MODE_DISTRIBUTION)
+    for sub, t in zip(subs, _gpu_tensors(net, subs)):
+        tqc.tqc_load_subcircuit_tensors(plan, sub.sid, t)
+    p = tqc.tqc_contract_distribution(plan).cpu().numpy().astype(np.float64)
+    want = np.zeros(1 << n)
+    want[0] = want[-1] = 0.5
+    assert np.abs(p - want).max() <= 1e-6
+
+
 def test_cfg3_subcircuits_twelve_wires():
     circ = configs.cfg3_circuit()
     net, T64, subs = cutting.tensors_from_circuit(circ)
