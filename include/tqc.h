@@ -22,7 +22,15 @@
  * thread-local message.  No exception crosses the boundary.  Pointers are marked HOST or
  * DEVICE.  The library never synchronises the caller's stream inside the contract calls and
  * never allocates there: persistent device state (re-laid-out tensors) is allocated in
- * tqc_load_subcircuit_tensors, scratch comes from the caller's workspace.
+ * tqc_load_subcircuit_tensors; the plan's device tables, the plan-specialised chain kernel (an NVRTC
+ * compile) and the side streams of forked table steps are created by tqc_plan_finalize, which the
+ * load that completes the tensor set calls; scratch comes from the caller's workspace.  A contract
+ * call is therefore capturable in a CUDA graph from the first call on.  (Exception: with
+ * tqc_plan_profile_enable on, a contract call creates the CUDA events it records.)
+ * A plan is not re-entrant: at most one load / contract call per plan at a time, and consecutive
+ * calls on one plan must be ordered on the device (same stream, or the caller's own events);
+ * different plans are independent.  Attributes of the library's kernels are set per device.
+ * A release build of the library reads no environment variable.
  * There is no CPU fallback: without a CUDA device the compute calls fail with TQC_E_CUDA.
  */
 #ifndef TQC_H
@@ -93,7 +101,7 @@ typedef struct {
                                        smaller networks, planned once) and the results are summed.  HOST [n_slice_cuts] distinct
                                        cut ids.  Tensors are still loaded whole; every intermediate that carried a sliced cut is 4x
                                        smaller per cut.  Sliced plans run step by step (no fused chain); workspace sizes include
-                                       one partial-sum buffer (4 bytes per output; add it to tqc_plan_workspace_min_bytes). */
+                                       one partial-sum buffer (4 bytes per output of a chunk). */
     int32_t kmax_cap;               /* restarts > 0 only: among the randomised-greedy orders keep the cheapest one whose widest
                                        step K_max = max_t |E_a u E_b| is <= kmax_cap; while no order meets the
                                        cap the smaller K_max wins.  0 = no cap (total multiplication count only). */
@@ -149,6 +157,13 @@ size_t tqc_plan_workspace_min_bytes(const tqc_plan_t *plan);
  * the caller may free `data` once `stream` has completed.  Reloading replaces the tensor. */
 int tqc_load_subcircuit_tensors(tqc_plan_t *plan, int s, const float *data, size_t n_elems,
                                 int on_device, void *stream /* cudaStream_t */);
+
+/* Completes a plan whose tensors are all loaded: device copies of the key-slot tables, the fused chain's step table and its
+ * plan-specialised kernel (NVRTC; if libnvrtc is missing the generic chain kernel is kept and tqc_plan_chain_status says
+ * so), side streams / events, kernel attributes of the current device.  May allocate and synchronise.  Called implicitly by
+ * the tqc_load_subcircuit_tensors call that loads the last missing tensor; calling it again is a no-op.  TQC_E_STATE if a
+ * tensor is missing.  The contract calls return TQC_E_STATE on a plan that was never finalized. */
+int tqc_plan_finalize(tqc_plan_t *plan, void *stream /* cudaStream_t */);
 
 /* ---- a2-a5: states mode ------------------------------------------------------------------
  * out_dev[b] = p(x_b) for b < n_states.  states_dev: DEVICE [n_states][ceil(n/64)] uint64.

@@ -142,6 +142,52 @@ def bucket_elimination(net, tensors, bits: np.ndarray, order=None, chunk: int = 
     return out
 
 
+def pairwise_steps_from_elimination(net, order):
+    """The pairwise order an elimination order over cut ids induces when parallel cuts are merged: take the
+    cuts in `order`; a cut that is still open is held by exactly two current nodes, which are contracted over ALL the
+    cuts they share.  Returns (lhs, rhs) node ids, leaves 0..m-1, step t creates m+t; a disconnected network leaves
+    several nodes, multiplied at the end by the caller."""
+    groups = {s: set(net.sub_cuts[s]) for s in range(net.m)}
+    steps, nxt = [], net.m
+    for e in order:
+        holders = sorted(v for v, g in groups.items() if e in g)
+        if len(holders) != 2:
+            continue                                           # already summed together with a parallel cut
+        a, b = holders
+        steps.append((a, b))
+        groups[nxt] = groups[a] ^ groups[b]
+        del groups[a], groups[b]
+        nxt += 1
+    return steps
+
+
+def contract_states_tensordot(net, tensors, bits: np.ndarray, order=None, order_trials: int = 0) -> np.ndarray:
+    """O8' - the large-K tier that is fast enough for hundreds of cfg5 states: ONE STATE AT A TIME (no batch axis), the
+    network is contracted pairwise along the order induced by the oracle's own elimination order (_elimination_order:
+    greedy min-size with seeded noise, unrelated to the library's memory-score planner), each step a library
+    `np.tensordot` over all cuts the two nodes share (multiply and sum over the shared indices; P:318-319
+    parallel cuts are one bond).  Any order gives the same value.  float64 throughout."""
+    if order is None:
+        order = _elimination_order(net, trials=order_trials)
+    steps = pairwise_steps_from_elimination(net, order)
+    keys = keys_from_bits(net, bits)
+    T = [np.asarray(t, dtype=np.float64) for t in tensors]
+    out = np.zeros(bits.shape[0], dtype=np.float64)
+    for b in range(bits.shape[0]):
+        nodes = {s: (T[s][:, keys[b, s]].reshape((4,) * net.c(s)), list(net.sub_cuts[s])) for s in range(net.m)}
+        for t, (u, v) in enumerate(steps):
+            (va, la), (vb, lb) = nodes.pop(u), nodes.pop(v)
+            shared = [l for l in la if l in lb]
+            val = np.tensordot(va, vb, axes=([la.index(l) for l in shared], [lb.index(l) for l in shared]))
+            nodes[net.m + t] = (val, [l for l in la if l not in shared] + [l for l in lb if l not in shared])
+        p = 1.0
+        for (val, lab) in nodes.values():
+            assert lab == []
+            p *= float(val)
+        out[b] = p / (2.0 ** net.K)
+    return out
+
+
 def multiplication_counts(net, steps):
     """Per-step costs 4^{#inner + #outer} for a pairwise order given as
     (lhs, rhs) node ids (leaves 0..m-1, step t creates node m+t); returns (costs, K_max).

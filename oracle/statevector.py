@@ -27,6 +27,14 @@ def gate_matrix(name: str, params=()) -> np.ndarray:
         return np.array([[1, 1], [1, -1]], dtype=np.complex128) / np.sqrt(2.0)
     if name == "x":
         return _X.copy()
+    if name == "y":
+        return _Y.copy()
+    if name == "z":
+        return _Z.copy()
+    if name == "t":
+        return np.array([[1, 0], [0, np.exp(0.25j * np.pi)]], dtype=np.complex128)
+    if name == "tdg":
+        return np.array([[1, 0], [0, np.exp(-0.25j * np.pi)]], dtype=np.complex128)
     if name == "s":
         return np.array([[1, 0], [0, 1j]], dtype=np.complex128)
     if name == "sdg":
@@ -42,6 +50,9 @@ def gate_matrix(name: str, params=()) -> np.ndarray:
         return np.diag([1, 1, 1, -1]).astype(np.complex128)
     if name == "cx":
         return np.array([[1, 0, 0, 0], [0, 1, 0, 0], [0, 0, 0, 1], [0, 0, 1, 0]], dtype=np.complex128)
+    if name == "cp":                                           # controlled phase: |11> picks up e^{i lambda}
+        (lam,) = params
+        return np.diag([1, 1, 1, np.exp(1j * lam)]).astype(np.complex128)
     if name == "rzz":
         (gamma,) = params
         return np.diag(np.exp(-1j * gamma * np.array([1, -1, -1, 1]))).astype(np.complex128)

@@ -34,7 +34,7 @@ EXPORTED = ["tqc_plan", "tqc_plan_destroy", "tqc_plan_mode", "tqc_plan_num_qubit
             "tqc_plan_profile_enable", "tqc_plan_profile_read", "tqc_plan_chain_status", "tqc_hss_scores", "tqc_hss_select",
             "tqc_hss_expand", "tqc_plan_num_sliced_cuts", "tqc_choose_slice_cuts", "tqc_hss_prepare",
             "tqc_hss_workspace_bytes", "tqc_hss_contract", "tqc_simulate_workspace_bytes",
-            "tqc_simulate_subcircuit_tensor"]
+            "tqc_simulate_subcircuit_tensor", "tqc_plan_finalize"]
 
 
 class TqcError(RuntimeError):
@@ -101,6 +101,7 @@ def _load() -> ctypes.CDLL:
     lib.tqc_plan_workspace_min_bytes.argtypes = [c_void_p]
     lib.tqc_plan_workspace_min_bytes.restype = c_size_t
     lib.tqc_load_subcircuit_tensors.argtypes = [c_void_p, c_int, c_void_p, c_size_t, c_int, c_void_p]
+    lib.tqc_plan_finalize.argtypes = [c_void_p, c_void_p]
     lib.tqc_contract_states.argtypes = [c_void_p, c_void_p, c_size_t, c_void_p, c_void_p, c_size_t, c_void_p]
     lib.tqc_contract_distribution.argtypes = [c_void_p, c_uint64, c_int, c_void_p, c_void_p, c_size_t, c_void_p]
     lib.tqc_plan_launch_count.argtypes = [c_void_p]
@@ -222,6 +223,10 @@ class Plan:
 
     def workspace_bytes_host(self, n_states: int = 0, prefix_bits: int = 0) -> int:
         return int(_lib.tqc_plan_workspace_bytes_host(self._h, n_states, prefix_bits))
+
+    def finalize(self, stream=None) -> None:
+        """tqc_plan_finalize: device tables, specialised chain kernel, side streams (implicit at the last tensor load)."""
+        _check(_lib.tqc_plan_finalize(self._h, _stream_ptr(stream)))
 
     def chain_status(self):
         """(0 no fused chain | 1 generic chain kernel | 2 plan-specialised chain kernel, note)."""

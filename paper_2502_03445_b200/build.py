@@ -24,7 +24,8 @@ def _stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or _stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + \
+        develop = ["-DTQC_DEVELOP"] if os.environ.get("TQC_DEVELOP") else []     # measurement switches
+        cmd = [nvcc] + NVCC_FLAGS + develop + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + \
               [os.path.join(CSRC, s) for s in SOURCES]
         subprocess.check_call(cmd)
     return LIB

@@ -49,6 +49,13 @@ struct TcArgs {
     int debug;                      // development knobs (TQC_TC_DEBUG): 1 no global stores, 2 no store phase, 4 no split, 8 no drains
 };
 
+// development knobs (TcArgs.debug) exist only in -DTQC_DEVELOP builds; a release build compiles every test of them away
+#ifdef TQC_DEVELOP
+#define TQC_DBG(a, bit) (((a).debug & (bit)) != 0)
+#else
+#define TQC_DBG(a, bit) false
+#endif
+
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
 __device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
@@ -280,7 +287,7 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
                     const int s = (int)(it % S);
                     const uint32_t ph = (uint32_t)((it / S) & 1);
                     mbar_wait(&empty_bar[s], ph ^ 1u);
-                    if (a.debug & 16) { mbar_arrive(&full_bar[s]); continue; }
+                    if (TQC_DBG(a, 16)) { mbar_arrive(&full_bar[s]); continue; }
                     mbar_expect_tx(&full_bar[s], bytesA + bytesB);
                     tma_load_3d(&mapA, &full_bar[s], A_raw(s), kb * TC_BK, (int)(mt * TC_BM), rowA);
                     tma_load_3d(&mapB, &full_bar[s], B_raw(s), kb * TC_BK, (int)(nt * BN), rowB);
@@ -311,7 +318,7 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                     const uint64_t dah = umma_desc_sw128(smem_u32(A_raw(s))), dal = umma_desc_sw128(smem_u32(A_lo(s)));
                     const uint64_t dbh = umma_desc_sw128(smem_u32(B_raw(s))), dbl = umma_desc_sw128(smem_u32(B_lo(s)));
-                    const bool run = !(a.debug & 32) || (kb | kc) == 0;
+                    const bool run = !TQC_DBG(a, 32) || (kb | kc) == 0;
                     if (lane == 0 && run) {
 #pragma unroll
                         for (int k = 0; k < TC_BK / 8; ++k) {
@@ -358,7 +365,7 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
                 mbar_wait(&hi_full_bar[hb], hph);
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                 const uint32_t taddr = tmem_base + lane_base + hb * (uint32_t)BN + (uint32_t)col_base;
-                if (!(a.debug & 8))
+                if (!TQC_DBG(a, 8))
 #pragma unroll
                 for (int c0 = 0; c0 < EC; c0 += 32) {
                     uint32_t v[32];
@@ -390,7 +397,7 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
             __syncwarp();
             if (lane == 0) mbar_arrive(&lo_empty_bar[lb]);
             float *scr = scratch[warp - 2];
-            if (a.debug & 2) continue;
+            if (TQC_DBG(a, 2)) continue;
 #pragma unroll
             for (int c0 = 0; c0 < EC; c0 += CB) {
                 __syncwarp();
@@ -404,7 +411,7 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
 #pragma unroll
                     for (int p = 0; p < CB / 4; ++p) {
                         const float4 val = *reinterpret_cast<const float4 *>(scr + rd_ofs[p]);
-                        if (!(a.debug & 1) || val.x == 123.456f) *reinterpret_cast<float4 *>(cblk + st_ofs[p]) = val;
+                        if (!TQC_DBG(a, 1) || val.x == 123.456f) *reinterpret_cast<float4 *>(cblk + st_ofs[p]) = val;
                     }
                 } else if (perm_off[1] == 1u && perm_off[2] == 2u && perm_off[3] == 3u) {
                     // four consecutive elements of the ascending order are contiguous in C (the two lowest C bits lie inside
@@ -437,11 +444,11 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
                 mbar_wait(&full_bar[s], ph);
                 // per stage: [A_raw][A_lo][B_raw][B_lo]; element e of a raw tile and of its lo tile share the swizzled offset
                 const uint32_t sa = smem_u32(A_raw(s)) + (uint32_t)st * 16u;
-                if (!(a.debug & 4))
+                if (!TQC_DBG(a, 4))
                 split_tile<(int)(bytesA >> 4) / TC_SPLIT_THREADS>(sa, bytesA, mask_hi);
-                if (!(a.debug & 4))
+                if (!TQC_DBG(a, 4))
                 split_tile<(int)(bytesB >> 4) / TC_SPLIT_THREADS>(sa + 2u * bytesA, bytesB, mask_hi);
-                if (!(a.debug & 64)) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // generic-proxy writes -> visible to the MMA's async proxy
+                if (!TQC_DBG(a, 64)) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // generic-proxy writes -> visible to the MMA's async proxy
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&ready_bar[s]);
             }

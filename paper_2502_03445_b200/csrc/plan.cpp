@@ -159,48 +159,61 @@ double order_cost_log2(const HostPlan &p, const std::vector<std::vector<int>> &l
 
 }  // namespace
 
-int build_plan(int n, int m, int K, const int32_t *cut_up, const int32_t *cut_down,
-               const int32_t *sub_cut_ofs, const int32_t *sub_cuts, const int32_t *sub_qubit_ofs,
-               const int32_t *sub_qubits, const PlanOptions &opts, HostPlan &p, std::string &err) {
+int validate_network(int n, int m, int K, const int32_t *cut_up, const int32_t *cut_down, const int32_t *sub_cut_ofs,
+                     const int32_t *sub_cuts, const int32_t *sub_qubit_ofs, const int32_t *sub_qubits, std::string &err) {
     if (n < 0 || m < 1 || K < 0) { err = "n_qubits >= 0, m >= 1, K >= 0 required"; return E_ARG; }
-    if (opts.mode != 0 && opts.mode != 1) { err = "mode must be 0 (states) or 1 (distribution)"; return E_ARG; }
     if (!sub_cut_ofs || !sub_qubit_ofs || (K > 0 && (!cut_up || !cut_down || !sub_cuts)) || (n > 0 && !sub_qubits)) {
         err = "null array in network description"; return E_ARG;
     }
-    p = HostPlan();
-    p.mode = opts.mode; p.n = n; p.m = m; p.K = K;
-    p.cut_up.assign(cut_up, cut_up + K);
-    p.cut_down.assign(cut_down, cut_down + K);
     for (int e = 0; e < K; ++e) {
         if (cut_up[e] < 0 || cut_up[e] >= m || cut_down[e] < 0 || cut_down[e] >= m || cut_up[e] == cut_down[e]) {
             err = "cut " + std::to_string(e) + ": ends must be two distinct subcircuits"; return E_ARG;
         }
     }
-    p.sub_cuts.resize(m); p.sub_qubits.resize(m); p.d.assign(m, 0);
     std::vector<int> seen_cut(K, 0), seen_q(n, 0);
     for (int s = 0; s < m; ++s) {
         if (sub_cut_ofs[s + 1] < sub_cut_ofs[s] || sub_qubit_ofs[s + 1] < sub_qubit_ofs[s]) { err = "offsets must ascend"; return E_ARG; }
+        std::vector<int> mine;
         for (int j = sub_cut_ofs[s]; j < sub_cut_ofs[s + 1]; ++j) {
             const int e = sub_cuts[j];
             if (e < 0 || e >= K || (cut_up[e] != s && cut_down[e] != s)) {
                 err = "subcircuit " + std::to_string(s) + " lists cut " + std::to_string(e) + " it does not touch"; return E_ARG;
             }
-            if (std::find(p.sub_cuts[s].begin(), p.sub_cuts[s].end(), e) != p.sub_cuts[s].end()) { err = "duplicate cut in subcircuit"; return E_ARG; }
-            p.sub_cuts[s].push_back(e);
+            if (std::find(mine.begin(), mine.end(), e) != mine.end()) { err = "duplicate cut in subcircuit"; return E_ARG; }
+            mine.push_back(e);
             seen_cut[e]++;
-            if (cut_down[e] == s) p.d[s]++;
         }
         for (int j = sub_qubit_ofs[s]; j < sub_qubit_ofs[s + 1]; ++j) {
             const int q = sub_qubits[j];
             if (q < 0 || q >= n || seen_q[q]) { err = "output qubit " + std::to_string(q) + " out of range or listed twice"; return E_ARG; }
             seen_q[q] = 1;
-            p.sub_qubits[s].push_back(q);
         }
-        if (p.c(s) > 15) { err = "subcircuit with more than 15 incident cuts"; return E_TOO_LARGE; }
-        if (p.o(s) > 30) { err = "subcircuit with more than 30 output qubits"; return E_TOO_LARGE; }
+        if (sub_qubit_ofs[s + 1] - sub_qubit_ofs[s] > 30) { err = "subcircuit with more than 30 output qubits"; return E_TOO_LARGE; }
     }
     for (int e = 0; e < K; ++e) if (seen_cut[e] != 2) { err = "cut " + std::to_string(e) + " must be listed by exactly its two subcircuits"; return E_ARG; }
     for (int q = 0; q < n; ++q) if (!seen_q[q]) { err = "qubit " + std::to_string(q) + " is owned by no subcircuit"; return E_ARG; }
+    return 0;
+}
+
+int build_plan(int n, int m, int K, const int32_t *cut_up, const int32_t *cut_down,
+               const int32_t *sub_cut_ofs, const int32_t *sub_cuts, const int32_t *sub_qubit_ofs,
+               const int32_t *sub_qubits, const PlanOptions &opts, HostPlan &p, std::string &err) {
+    if (opts.mode != 0 && opts.mode != 1) { err = "mode must be 0 (states) or 1 (distribution)"; return E_ARG; }
+    if (const int vrc = validate_network(n, m, K, cut_up, cut_down, sub_cut_ofs, sub_cuts, sub_qubit_ofs, sub_qubits, err)) return vrc;
+    p = HostPlan();
+    p.mode = opts.mode; p.n = n; p.m = m; p.K = K;
+    p.cut_up.assign(cut_up, cut_up + K);
+    p.cut_down.assign(cut_down, cut_down + K);
+    p.sub_cuts.resize(m); p.sub_qubits.resize(m); p.d.assign(m, 0);
+    for (int s = 0; s < m; ++s) {
+        for (int j = sub_cut_ofs[s]; j < sub_cut_ofs[s + 1]; ++j) {
+            const int e = sub_cuts[j];
+            p.sub_cuts[s].push_back(e);
+            if (cut_down[e] == s) p.d[s]++;
+        }
+        for (int j = sub_qubit_ofs[s]; j < sub_qubit_ofs[s + 1]; ++j) p.sub_qubits[s].push_back(sub_qubits[j]);
+        if (p.c(s) > 15) { err = "subcircuit with more than 15 incident cuts"; return E_TOO_LARGE; }
+    }
 
     std::vector<std::vector<int>> leaf_open(m);
     for (int s = 0; s < m; ++s) { leaf_open[s] = p.sub_cuts[s]; std::sort(leaf_open[s].begin(), leaf_open[s].end()); }

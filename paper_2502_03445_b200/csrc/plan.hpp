@@ -111,6 +111,11 @@ struct PlanOptions {
     int table_log2_floats_max = 0;              // 0: default 24 (64 MB per table)
 };
 
+// Structural checks of a network description (ids in range, every cut listed by exactly its two subcircuits, every qubit
+// owned once).  Returns 0 or a negative tqc_status; fills err.
+int validate_network(int n, int m, int K, const int32_t *cut_up, const int32_t *cut_down, const int32_t *sub_cut_ofs,
+                     const int32_t *sub_cuts, const int32_t *sub_qubit_ofs, const int32_t *sub_qubits, std::string &err);
+
 // Returns 0 or a negative tqc_status; fills err.
 int build_plan(int n, int m, int K, const int32_t *cut_up, const int32_t *cut_down,
                const int32_t *sub_cut_ofs, const int32_t *sub_cuts, const int32_t *sub_qubit_ofs,

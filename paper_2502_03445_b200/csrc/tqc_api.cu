@@ -11,6 +11,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <functional>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -60,6 +61,18 @@ struct BitPairs {
     }
 };
 
+// Development switches (measurement variants of DESIGN.md 5.1).  A release build reads NO environment variable: the
+// lookups below exist only when the library is compiled with -DTQC_DEVELOP (python -m paper_2502_03445_b200.build with
+// TQC_DEVELOP=1 in the environment).
+const char *dev_env(const char *name) {
+#ifdef TQC_DEVELOP
+    return std::getenv(name);
+#else
+    (void)name;
+    return nullptr;
+#endif
+}
+
 int index_of(const std::vector<int> &v, int x) {
     for (size_t i = 0; i < v.size(); ++i) if (v[i] == x) return (int)i;
     return -1;
@@ -88,7 +101,8 @@ struct tqc_plan {
     float *d_staging = nullptr;
     size_t staging_elems = 0;
     uint64_t launches = 0;
-    bool attrs_set = false;
+    bool finalized = false;            // tqc_plan_finalize has run (device tables, specialised chain kernel, side streams)
+    int sm_count = 0;
     // optional per-launch timing (tqc_plan_profile_*): one event before each launch + one at the end
     bool profile = false;
     std::vector<cudaEvent_t> ev_pool;
@@ -99,7 +113,6 @@ struct tqc_plan {
     cudaStream_t lane[N_LANES] = {nullptr, nullptr, nullptr};
     cudaEvent_t ev_fork = nullptr, ev_join[N_LANES] = {nullptr, nullptr, nullptr};
     int tables_parallel = -1;          // -1 not decided; 0 serial; 1 fork/join
-    bool fork_recorded = false;        // the host-buffer entry point recorded ev_fork before its H2D copy
     // bond slicing: hp describes the network WITHOUT the sliced cuts; a leaf keeps one re-laid-out
     // sub-tensor per value of its sliced axes, the contract calls sum over all 4^{n_sliced} assignments
     int K_full = 0;
@@ -122,6 +135,7 @@ using tqc::Node;
 using tqc::Step;
 
 constexpr int kMaxDynSmem = 200 * 1024;
+constexpr int TQC_MAX_DEVICES = 64;
 
 // Tags of profiled launches: step index t >= 0, or one of these.
 enum { TAG_KEYS = -1, TAG_GATHER = -2, TAG_RELAYOUT = -3, TAG_CHAIN = -4, TAG_HSS = -5 };
@@ -148,13 +162,44 @@ int prof_begin(tqc_plan_t *pl) {
 }
 int prof_close(tqc_plan_t *pl, cudaStream_t st) { return pl->profile ? prof_event(pl, st) : 0; }
 
+// Opt-in shared-memory sizes of every kernel that needs more than 48 KB, set once per DEVICE (cudaFuncSetAttribute acts
+// on the current device's copy of the function; a per-process flag would leave a second device unset).  Called from the
+// load / finalize / simulate entry points, never from a contract call.  *sm_count (may be null) receives the SM count.
+int ensure_device_attrs(int *sm_count) {
+    static std::mutex mu;
+    static bool done[TQC_MAX_DEVICES] = {};
+    static int sms[TQC_MAX_DEVICES] = {};
+    int dev = 0;
+    TQC_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= TQC_MAX_DEVICES) return fail(TQC_E_TOO_LARGE, "device ordinal beyond the library's table");
+    std::lock_guard<std::mutex> lock(mu);
+    if (!done[dev]) {
+        TQC_CUDA(cudaDeviceGetAttribute(&sms[dev], cudaDevAttrMultiProcessorCount, dev));
+        const auto dyn = cudaFuncAttributeMaxDynamicSharedMemorySize;
+        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tile_kernel<4, 4>, dyn, kMaxDynSmem));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tile_kernel<4, 1>, dyn, kMaxDynSmem));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tile_kernel<1, 4>, dyn, kMaxDynSmem));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tile_kernel<1, 1>, dyn, kMaxDynSmem));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::cross_mma_kernel<3>, dyn, 100 * 1024));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::cross_mma_kernel<4>, dyn, 100 * 1024));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::cross_mma_kernel<5>, dyn, 100 * 1024));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::cross_mma_kernel<6>, dyn, 100 * 1024));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc_kernel<16>, dyn, 201 * 1024));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc_kernel<32>, dyn, 201 * 1024));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc_kernel<64>, dyn, 201 * 1024));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc_kernel<128>, dyn, 201 * 1024));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tcw_kernel, dyn, 194 * 1024));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::chain_kernel, dyn, 128 * 1024));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::sim_variant_kernel, dyn, 24 << 13));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::sim_variant_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+        done[dev] = true;
+    }
+    if (sm_count) *sm_count = sms[dev];
+    return 0;
+}
+
 template <int MI, int MJ>
 int launch_tile_t(const StepArgs &a, size_t smem, long long blocks, cudaStream_t st) {
-    static bool attr = false;
-    if (!attr) {
-        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tile_kernel<MI, MJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
-        attr = true;
-    }
     tqc::step_tile_kernel<MI, MJ><<<(unsigned)blocks, 256, smem, st>>>(a);
     TQC_CUDA(cudaGetLastError());
     return 0;
@@ -293,22 +338,14 @@ int launch_cross_step(tqc_plan_t *pl, const CrossCtx &cx, int t, cudaStream_t st
     if (!pa.build(a.outA) || !pb.build(a.outB)) return fail(TQC_E_TOO_LARGE, "bit map needs too many segments");
     // short bond, many rows on both sides: warp-level 3xTF32 tensor-core tiles (kernels_cross.cuh)
     if (pl->use_tcgen05 >= 0 && a.lgK >= 3 && a.lgK <= 6 && std::min(a.lgM, a.lgN) >= 6 && std::max(a.lgM, a.lgN) >= 7 &&
-        !getenv("TQC_NO_CROSS_MMA")) {
+        !dev_env("TQC_NO_CROSS_MMA")) {
         if (a.lgN < 7) { std::swap(a.A, a.B); std::swap(a.outA, a.outB); std::swap(a.lgM, a.lgN); }
         a.lgTilesI = a.lgM - 6; a.lgTilesJ = a.lgN - 7;
         a.vec_store = (a.outB.n >= 1 && a.outB.src[0] == 0 && a.outB.dst[0] == 0 && a.outB.len[0] >= 2) ? 1 : 0;
-        if (a.vec_store && !getenv("TQC_CROSS_STAGED")) a.vec_store = 2;          // 8-byte stores straight from the fragments
+        if (a.vec_store && !dev_env("TQC_CROSS_STAGED")) a.vec_store = 2;          // 8-byte stores straight from the fragments
         const long long blocks = 1ll << (a.lgTilesI + a.lgTilesJ);
         if (blocks > 0x7fffffffll) return fail(TQC_E_TOO_LARGE, "step needs more than 2^31 thread blocks");
         const size_t smem = tqc::cross_mma_smem(a.lgK, a.vec_store != 2);
-        static bool attr = false;
-        if (!attr) {
-            TQC_CUDA(cudaFuncSetAttribute(tqc::cross_mma_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
-            TQC_CUDA(cudaFuncSetAttribute(tqc::cross_mma_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
-            TQC_CUDA(cudaFuncSetAttribute(tqc::cross_mma_kernel<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
-            TQC_CUDA(cudaFuncSetAttribute(tqc::cross_mma_kernel<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
-            attr = true;
-        }
         if ((rc = note_launch(pl, t, st))) return rc;
         switch (a.lgK) {
             case 3: tqc::cross_mma_kernel<3><<<(unsigned)blocks, 256, smem, st>>>(a); break;
@@ -385,25 +422,13 @@ struct TcOperand { const float *base; const uint32_t *keys; long long n_outer; }
 
 int launch_tc_step(tqc_plan_t *pl, TcOperand A, TcOperand B, BitMap outA, BitMap outB, int lgM, int lgN, int lgK, float *C,
                    long long c_row_stride, int R, int tag, cudaStream_t st) {
-    static int sm_count = 0;
-    static bool attr = false;
-    if (!attr) {
-        int dev = 0;
-        TQC_CUDA(cudaGetDevice(&dev));
-        TQC_CUDA(cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev));
-        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 201 * 1024));
-        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 201 * 1024));
-        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, 201 * 1024));
-        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 201 * 1024));
-        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tcw_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 194 * 1024));
-        attr = true;
-    }
+    const int sm_count = pl->sm_count > 0 ? pl->sm_count : 148;
     auto has_bit0 = [](const BitMap &m) { for (int s = 0; s < m.n; ++s) if (m.dst[s] == 0) return true; return false; };
     // the M side needs >= 128 rows; with both sides large, the N side (vector stores run along it) takes C's lowest bits
     bool swap = lgM < 7;
     if (lgM >= 7 && lgN >= 7 && has_bit0(outA)) swap = true;
     // wide tiles (128 x 256) need N >= 256: when only one side reaches 256 it becomes N
-    static const bool no_wide = std::getenv("TQC_TC_NO_WIDE") != nullptr;
+    static const bool no_wide = dev_env("TQC_TC_NO_WIDE") != nullptr;
     if (lgM >= 7 && lgN >= 7 && !no_wide) {
         const int n_if_keep = lgN, n_if_swap = lgM;
         if (swap && n_if_swap < 8 && n_if_keep >= 8) swap = false;
@@ -424,11 +449,11 @@ int launch_tc_step(tqc_plan_t *pl, TcOperand A, TcOperand B, BitMap outA, BitMap
     a.outA = outA; a.outB = outB;
     a.lgM = lgM; a.lgN = lgN; a.lgK = lgK; a.R = R;
     a.BN = wide ? tqc::TCW_BN : (int)std::min<long long>(128, 1ll << lgN);
-    { const char *dbg = std::getenv("TQC_TC_DEBUG"); a.debug = dbg ? std::atoi(dbg) : 0; }
-    { const char *ck = std::getenv("TQC_TC_CHUNK"); a.chunk_kb = ck ? std::atoi(ck) : 0; }
+    { const char *dbg = dev_env("TQC_TC_DEBUG"); a.debug = dbg ? std::atoi(dbg) : 0; }
+    { const char *ck = dev_env("TQC_TC_CHUNK"); a.chunk_kb = ck ? std::atoi(ck) : 0; }
     // hi parts rounded to nearest (rewritten in shared memory): removes the systematic -2.4e-7 per step of the truncating
     // split (dropped lo*lo and truncated lo are then zero-mean).  TQC_TC_TRUNC=1 keeps the raw tile as hi (measurements).
-    a.mask_hi = std::getenv("TQC_TC_TRUNC") ? 0 : 1;
+    a.mask_hi = dev_env("TQC_TC_TRUNC") ? 0 : 1;
     const size_t stage_bytes = 2 * (size_t)tqc::TC_BM * tqc::TC_BK * 4 + 2 * (size_t)a.BN * tqc::TC_BK * 4;
     a.stages = (int)std::min<size_t>(4, (200 * 1024) / stage_bytes);     // + 24 KB static (epilogue scratch, tables)
     a.vec4 = (outB.n >= 1 && outB.src[0] == 0 && outB.dst[0] == 0 && outB.len[0] >= 2) ? 1 : 0;
@@ -438,7 +463,7 @@ int launch_tc_step(tqc_plan_t *pl, TcOperand A, TcOperand B, BitMap outA, BitMap
     if ((rc = make_operand_map(&mapB, B.base, lgK, lgN, B.n_outer, a.BN))) return rc;
     const long long total = (1ll << (lgM - 7)) * ((1ll << lgN) / a.BN) * (long long)R;
     const unsigned grid = (unsigned)std::min<long long>(total, sm_count);
-    if (std::getenv("TQC_TC_TRACE"))
+    if (dev_env("TQC_TC_TRACE"))
         fprintf(stderr, "tc step %d: lgM %d lgN %d lgK %d swap %d wide %d vec4 %d keyedA %d keyedB %d R %d outB.n %d outB[0]=(%d,%d,%d)\n", tag, lgM, lgN, lgK,
                 (int)swap, (int)wide, a.vec4, A.keys != nullptr, B.keys != nullptr, R, outB.n, outB.src[0], outB.dst[0], outB.len[0]);
     if ((rc = note_launch(pl, tag, st))) return rc;
@@ -682,7 +707,7 @@ std::string chain_source(const tqc_plan_t *pl) {
     src += "  }\n";
     // the staged operands of one state: for every 32-chunk slot the lane ranges of the gathers it covers, with the row
     // size, the padding and the destination as constants (the generic kernel reads the same from a shared-memory table)
-    if (getenv("TQC_CHAIN_TABLE_GATHER")) src += "  static constexpr bool kOwnGather = false;\n  static __device__ __forceinline__ void gather(const ChainArgs &, uint32_t, uint32_t, int) {}\n";
+    if (dev_env("TQC_CHAIN_TABLE_GATHER")) src += "  static constexpr bool kOwnGather = false;\n  static __device__ __forceinline__ void gather(const ChainArgs &, uint32_t, uint32_t, int) {}\n";
     else {
         src += "  static constexpr bool kOwnGather = true;\n"
                "  static __device__ __forceinline__ void gather(const ChainArgs &a, uint32_t key, uint32_t dst, int lane) {\n";
@@ -728,8 +753,8 @@ void chain_jit_build(tqc_plan_t *pl) {
     if (api.CreateProgram(&prog, src.c_str(), "chain_spec.cu", 0, nullptr, nullptr) != NVRTC_SUCCESS) { pl->jit_note = "nvrtcCreateProgram failed"; return; }
     const std::string inc = "-I" + dir;
     const char *opts[] = {"--gpu-architecture=sm_100a", "-std=c++17", inc.c_str(), "-lineinfo", "-DTQC_CHAIN_NO_MMA"};
-    if (getenv("TQC_MMA_MASK_LO")) opts[4] = "-DTQC_MMA_MASK_LO";
-    const nvrtcResult rc = api.CompileProgram(prog, getenv("TQC_CHAIN_NO_MMA") || getenv("TQC_MMA_MASK_LO") ? 5 : 4, opts);
+    if (dev_env("TQC_MMA_MASK_LO")) opts[4] = "-DTQC_MMA_MASK_LO";
+    const nvrtcResult rc = api.CompileProgram(prog, dev_env("TQC_CHAIN_NO_MMA") || dev_env("TQC_MMA_MASK_LO") ? 5 : 4, opts);
     if (rc != NVRTC_SUCCESS) {
         size_t n = 0;
         api.GetProgramLogSize(prog, &n);
@@ -766,7 +791,6 @@ int ensure_chain(tqc_plan_t *pl) {
     }
     TQC_CUDA(cudaMalloc(&pl->d_chain, tab.size() * sizeof(tqc::ChainStep)));
     TQC_CUDA(cudaMemcpy(pl->d_chain, tab.data(), tab.size() * sizeof(tqc::ChainStep), cudaMemcpyHostToDevice));
-    TQC_CUDA(cudaFuncSetAttribute(tqc::chain_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 128 * 1024));
     if (pl->chain_mode == 0) chain_jit_build(pl);
     return 0;
 }
@@ -788,6 +812,28 @@ int ensure_meta(tqc_plan_t *pl) {
 }
 
 size_t align256(size_t v) { return (v + 255) / 256 * 256; }
+// decides once whether the table steps of a states-mode plan fork onto side streams, and creates the streams / events
+int ensure_lanes(tqc_plan_t *pl) {
+    if (pl->tables_parallel >= 0) return 0;
+    const HostPlan &hp = pl->hp;
+    int n_tab = 0;
+    bool leaf_only = true;
+    for (int t = 0; t < hp.m - 1; ++t) {
+        if (hp.nodes[hp.m + t].kind != tqc::NODE_TABLE) continue;
+        ++n_tab;
+        if (hp.steps[t].lhs >= hp.m || hp.steps[t].rhs >= hp.m) leaf_only = false;
+    }
+    pl->tables_parallel = (hp.mode == TQC_MODE_STATES && n_tab >= 1 && leaf_only && !dev_env("TQC_NO_FORK")) ? 1 : 0;
+    if (pl->tables_parallel) {
+        TQC_CUDA(cudaEventCreateWithFlags(&pl->ev_fork, cudaEventDisableTiming));
+        for (int l = 0; l < tqc_plan::N_LANES; ++l) {
+            TQC_CUDA(cudaStreamCreateWithFlags(&pl->lane[l], cudaStreamNonBlocking));
+            TQC_CUDA(cudaEventCreateWithFlags(&pl->ev_join[l], cudaEventDisableTiming));
+        }
+    }
+    return 0;
+}
+
 
 // states-mode workspace: [tables][keys: n_slots x cap u32][batch: ws_floats_per_state x cap]
 size_t states_fixed_bytes(const HostPlan &hp) { return align256((size_t)hp.table_floats * 4); }
@@ -862,6 +908,12 @@ void plan_options_from(const tqc_plan_opts *opts, tqc::PlanOptions &po) {
 int tqc_choose_slice_cuts(const tqc_network_desc *net, const tqc_plan_opts *opts, int max_log2_input_floats,
                           int max_log2_intermediate_floats, int32_t *slice_cuts, int32_t *n_slice_cuts) {
     if (!net || !slice_cuts || !n_slice_cuts) return fail(TQC_E_ARG, "null argument");
+    {   // the whole description first: level 1 indexes the cut ends, reduce_network only looks at sub_cuts
+        std::string verr;
+        const int vrc = tqc::validate_network(net->n_qubits, net->m, net->K, net->cut_up, net->cut_down, net->sub_cut_ofs, net->sub_cuts,
+                                              net->sub_qubit_ofs, net->sub_qubits, verr);
+        if (vrc) return fail(vrc, verr);
+    }
     tqc::PlanOptions po;
     plan_options_from(opts, po);
     po.order.clear();                                   // an explicit order names nodes of one particular network
@@ -955,6 +1007,12 @@ int tqc_plan(const tqc_network_desc *net, const tqc_plan_opts *opts, tqc_plan_t 
         rc = tqc::build_plan(net->n_qubits, net->m, net->K, net->cut_up, net->cut_down, net->sub_cut_ofs,
                              net->sub_cuts, net->sub_qubit_ofs, net->sub_qubits, po, pl->hp, err);
     } else {
+        // the planner only sees the reduced network: check the caller's whole description here (ends of the sliced cuts,
+        // each cut listed by exactly its two subcircuits), else a malformed sliced cut would silently give a wrong sum
+        std::string verr;
+        const int vrc = tqc::validate_network(net->n_qubits, net->m, net->K, net->cut_up, net->cut_down, net->sub_cut_ofs, net->sub_cuts,
+                                              net->sub_qubit_ofs, net->sub_qubits, verr);
+        if (vrc) { delete pl; return fail(vrc, verr); }
         ReducedNet rn;
         std::string why;
         if (!reduce_network(net, opts->slice_cuts, ns, rn, why)) { delete pl; return fail(TQC_E_ARG, why); }
@@ -981,7 +1039,7 @@ int tqc_plan(const tqc_network_desc *net, const tqc_plan_opts *opts, tqc_plan_t 
     pl->chain = pl->chain_mode != -1 && build_chain(pl);
     if (pl->chain) pl->hp.ws_floats_per_state = 0;          // intermediates live in shared memory
     if (pl->chain) {
-        if (const char *dump = std::getenv("TQC_CHAIN_SRC_DUMP")) {      // development aid: the generated specialisation
+        if (const char *dump = dev_env("TQC_CHAIN_SRC_DUMP")) {      // development aid: the generated specialisation
             if (FILE *f = fopen(dump, "w")) { fputs(chain_source(pl).c_str(), f); fclose(f); }
         }
     }
@@ -1070,7 +1128,8 @@ int tqc_plan_serialize(const tqc_plan_t *pl, void *buf, size_t *len) {
 
 size_t tqc_plan_workspace_min_bytes(const tqc_plan_t *pl) {
     if (!pl) return 0;
-    if (pl->hp.mode == TQC_MODE_STATES) return states_fixed_bytes(pl->hp) + align256(states_bytes_per_state(pl->hp) * 64) + 256;
+    if (pl->hp.mode == TQC_MODE_STATES)
+        return states_fixed_bytes(pl->hp) + align256(states_bytes_per_state(pl->hp) * 64) + 256 + (pl->n_sliced() ? 1024 : 0);
     return tqc_plan_workspace_bytes(pl, 0, 0);
 }
 
@@ -1099,7 +1158,7 @@ int tqc_load_subcircuit_tensors(tqc_plan_t *pl, int s, const float *data, size_t
     const size_t need = (size_t)1 << (2 * cf + o);
     if (n_elems != need) return fail(TQC_E_SHAPE, "n_elems must be 4^c_s * 2^o_s = " + std::to_string(need));
     cudaStream_t st = (cudaStream_t)stream;
-    int rc = ensure_meta(pl);
+    int rc = ensure_device_attrs(&pl->sm_count);
     if (rc) return rc;
     float *&store = sliced ? pl->d_leaf_all[s] : pl->d_leaf[s];
     if (!store) TQC_CUDA(cudaMalloc(&store, need * sizeof(float)));
@@ -1150,6 +1209,26 @@ int tqc_load_subcircuit_tensors(tqc_plan_t *pl, int s, const float *data, size_t
     if (rc) return rc;
     TQC_CUDA(cudaGetLastError());
     pl->loaded[s] = 1;
+    // the load that completes the tensor set also prepares the plan for the contract calls (a reload keeps the same
+    // device allocation, so a finalized plan stays valid)
+    if (!pl->finalized && std::all_of(pl->loaded.begin(), pl->loaded.end(), [](char c) { return c != 0; })) return tqc_plan_finalize(pl, stream);
+    return 0;
+}
+
+// Everything a contract call needs beyond the tensors, done ONCE here so that the contract calls neither allocate nor
+// synchronise: kernel attributes of this device, the key-slot tables, the device step table of the fused chain and its
+// plan-specialised kernel (NVRTC compile + module load), the side streams and events of the forked table steps.
+int tqc_plan_finalize(tqc_plan_t *pl, void *stream) {
+    (void)stream;
+    if (!pl) return fail(TQC_E_ARG, "null plan");
+    for (int s = 0; s < pl->hp.m; ++s) if (!pl->loaded[s]) return fail(TQC_E_STATE, "tensor of subcircuit " + std::to_string(s) + " not loaded");
+    if (pl->finalized) return 0;
+    int rc;
+    if ((rc = ensure_device_attrs(&pl->sm_count))) return rc;
+    if ((rc = ensure_meta(pl))) return rc;
+    if ((rc = ensure_chain(pl))) return rc;
+    if ((rc = ensure_lanes(pl))) return rc;
+    pl->finalized = true;
     return 0;
 }
 
@@ -1165,7 +1244,7 @@ void select_slice(tqc_plan_t *pl, long long assign) {
     }
 }
 int contract_states_impl(tqc_plan_t *pl, const uint64_t *states_dev, size_t n_states, float *out_dev, void *workspace_dev,
-                         size_t workspace_bytes, void *stream);
+                         size_t workspace_bytes, void *stream, bool fork_recorded = false);
 int contract_distribution_impl(tqc_plan_t *pl, uint64_t prefix_value, int prefix_bits, float *out_dev, void *workspace_dev,
                                size_t workspace_bytes, void *stream);
 // sum over the 4^{n_sliced} sub-networks: the first lands in out, the others in a partial-sum buffer at the head of the
@@ -1197,10 +1276,22 @@ int tqc_contract_states(tqc_plan_t *pl, const uint64_t *states_dev, size_t n_sta
                         size_t workspace_bytes, void *stream) {
     if (!pl) return fail(TQC_E_ARG, "null plan");
     if (pl->n_sliced() == 0 || n_states == 0) return contract_states_impl(pl, states_dev, n_states, out_dev, workspace_dev, workspace_bytes, stream);
-    if (!out_dev) return fail(TQC_E_ARG, "null states/out pointer");
-    return sliced_sum(pl, out_dev, n_states, workspace_dev, workspace_bytes, stream, [&](float *dst, void *ws, size_t wb) {
-        return contract_states_impl(pl, states_dev, n_states, dst, ws, wb, stream);
-    });
+    if (!out_dev || !states_dev) return fail(TQC_E_ARG, "null states/out pointer");
+    // the partial-sum buffer (4 bytes per state) comes out of the workspace: when it does not fit for the whole batch next to
+    // the plan's own minimum, the batch is cut into pieces of `piece` states, each summed over all sub-networks
+    const size_t fixed = states_fixed_bytes(pl->hp), per = states_bytes_per_state(pl->hp) + 4;
+    if (workspace_bytes < fixed + 1024 + per * 64) return fail(TQC_E_WORKSPACE, "workspace smaller than tqc_plan_workspace_min_bytes");
+    size_t piece = (workspace_bytes - fixed - 1024) / per / 64 * 64;
+    piece = std::min(piece, (n_states + 63) / 64 * 64);
+    const size_t words = (size_t)(pl->hp.n + 63) / 64;
+    for (size_t lo = 0; lo < n_states; lo += piece) {
+        const size_t cnt = std::min(piece, n_states - lo);
+        const int rc = sliced_sum(pl, out_dev + lo, cnt, workspace_dev, workspace_bytes, stream, [&](float *dst, void *ws, size_t wb) {
+            return contract_states_impl(pl, states_dev + lo * words, cnt, dst, ws, wb, stream);
+        });
+        if (rc) return rc;
+    }
+    return 0;
 }
 
 int tqc_contract_distribution(tqc_plan_t *pl, uint64_t prefix_value, int prefix_bits, float *out_dev, void *workspace_dev,
@@ -1215,30 +1306,9 @@ int tqc_contract_distribution(tqc_plan_t *pl, uint64_t prefix_value, int prefix_
 }
 
 namespace {
-// decides once whether the table steps of a states-mode plan fork onto side streams, and creates the streams / events
-int ensure_lanes(tqc_plan_t *pl) {
-    if (pl->tables_parallel >= 0) return 0;
-    const HostPlan &hp = pl->hp;
-    int n_tab = 0;
-    bool leaf_only = true;
-    for (int t = 0; t < hp.m - 1; ++t) {
-        if (hp.nodes[hp.m + t].kind != tqc::NODE_TABLE) continue;
-        ++n_tab;
-        if (hp.steps[t].lhs >= hp.m || hp.steps[t].rhs >= hp.m) leaf_only = false;
-    }
-    pl->tables_parallel = (hp.mode == TQC_MODE_STATES && n_tab >= 1 && leaf_only && !getenv("TQC_NO_FORK")) ? 1 : 0;
-    if (pl->tables_parallel) {
-        TQC_CUDA(cudaEventCreateWithFlags(&pl->ev_fork, cudaEventDisableTiming));
-        for (int l = 0; l < tqc_plan::N_LANES; ++l) {
-            TQC_CUDA(cudaStreamCreateWithFlags(&pl->lane[l], cudaStreamNonBlocking));
-            TQC_CUDA(cudaEventCreateWithFlags(&pl->ev_join[l], cudaEventDisableTiming));
-        }
-    }
-    return 0;
-}
-
+// fork_recorded: the caller (host-buffer entry point) has already recorded ev_fork on the stream, before its H2D copy
 int contract_states_impl(tqc_plan_t *pl, const uint64_t *states_dev, size_t n_states, float *out_dev, void *workspace_dev,
-                        size_t workspace_bytes, void *stream) {
+                        size_t workspace_bytes, void *stream, bool fork_recorded) {
     if (!pl) return fail(TQC_E_ARG, "null plan");
     HostPlan &hp = pl->hp;
     if (hp.mode != TQC_MODE_STATES) return fail(TQC_E_STATE, "plan was built for distribution mode");
@@ -1264,19 +1334,17 @@ int contract_states_impl(tqc_plan_t *pl, const uint64_t *states_dev, size_t n_st
     float *batch = (float *)(ws + fixed + align256((size_t)hp.n_key_slots * 4 * (size_t)cap));
     // the alignment pad of the key region is covered by the +256 of tqc_plan_workspace_bytes
     int rc;
-    if ((rc = ensure_chain(pl))) return rc;
+    if (!pl->finalized) return fail(TQC_E_STATE, "plan not finalized (tqc_plan_finalize runs at the last tqc_load_subcircuit_tensors)");
     prof_begin(pl);
     // phase T: nodes evaluated once per key (tables), independent of the batch
     CrossCtx cx;
     cx.ws = tables;
     // Table steps whose operands are all leaves neither depend on one another nor share storage (plan.cpp releases a
     // table's block only when another table step consumes it): they go to side streams and overlap the key kernel.
-    if ((rc = ensure_lanes(pl))) return rc;
     const bool fork = pl->tables_parallel == 1 && !pl->profile;
     int lanes_used = 0;
     if (fork) {
-        if (!pl->fork_recorded) TQC_CUDA(cudaEventRecord(pl->ev_fork, st));
-        pl->fork_recorded = false;
+        if (!fork_recorded) TQC_CUDA(cudaEventRecord(pl->ev_fork, st));
         int next = 0;
         for (int t = 0; t < hp.m - 1; ++t) {
             if (hp.nodes[hp.m + t].kind != tqc::NODE_TABLE) continue;
@@ -1355,6 +1423,7 @@ int contract_distribution_impl(tqc_plan_t *pl, uint64_t prefix_value, int prefix
     HostPlan &hp = pl->hp;
     if (hp.mode != TQC_MODE_DISTRIBUTION) return fail(TQC_E_STATE, "plan was built for states mode");
     for (int s = 0; s < hp.m; ++s) if (!pl->loaded[s]) return fail(TQC_E_STATE, "tensor of subcircuit " + std::to_string(s) + " not loaded");
+    if (!pl->finalized) return fail(TQC_E_STATE, "plan not finalized (tqc_plan_finalize runs at the last tqc_load_subcircuit_tensors)");
     if (prefix_bits < 0 || prefix_bits > hp.n || prefix_bits > 64) return fail(TQC_E_ARG, "prefix_bits out of range");
     if (prefix_bits < 64 && (prefix_value >> prefix_bits) != 0) return fail(TQC_E_ARG, "prefix_value has more than prefix_bits bits");
     if (hp.n - prefix_bits > 34) return fail(TQC_E_TOO_LARGE, "more than 2^34 outputs; raise prefix_bits");
@@ -1433,14 +1502,14 @@ int tqc_contract_states_host(tqc_plan_t *pl, const uint64_t *states_host, size_t
     float *od = (float *)(ws + sb);
     // the table steps do not depend on the states: fork their side streams off BEFORE the host-to-device copy so that
     // they run under it (only for the plain path: a sliced plan loops over sub-networks, profile mode stays serial)
-    if (pl->hp.mode == TQC_MODE_STATES && pl->n_sliced() == 0 && !pl->profile) {
-        const int lrc = ensure_lanes(pl);
-        if (lrc) return lrc;
-        if (pl->tables_parallel == 1) { TQC_CUDA(cudaEventRecord(pl->ev_fork, st)); pl->fork_recorded = true; }
+    bool forked = false;
+    if (pl->hp.mode == TQC_MODE_STATES && pl->n_sliced() == 0 && !pl->profile && pl->finalized && pl->tables_parallel == 1) {
+        TQC_CUDA(cudaEventRecord(pl->ev_fork, st));
+        forked = true;
     }
     if (words > 0) TQC_CUDA(cudaMemcpyAsync(sd, states_host, n_states * words * 8, cudaMemcpyHostToDevice, st));
-    const int rc = tqc_contract_states(pl, sd, n_states, od, ws + sb + ob, workspace_bytes - sb - ob, stream);
-    pl->fork_recorded = false;
+    const int rc = forked ? contract_states_impl(pl, sd, n_states, od, ws + sb + ob, workspace_bytes - sb - ob, stream, true)
+                          : tqc_contract_states(pl, sd, n_states, od, ws + sb + ob, workspace_bytes - sb - ob, stream);
     if (rc) return rc;
     TQC_CUDA(cudaMemcpyAsync(out_host, od, n_states * 4, cudaMemcpyDeviceToHost, st));
     return 0;
@@ -1527,6 +1596,8 @@ int tqc_hss_select(const tqc_plan_t *pl, const float *const *scores_host, uint64
         const int n = 1 << hp.o(j);
         total_rows += (size_t)n;
         chosen[j].assign(n, 0);
+        for (int i = 0; i < n; ++i)
+            if (!std::isfinite(scores_host[j][i])) return fail(TQC_E_ARG, "non-finite score (subcircuit " + std::to_string(j) + ", state " + std::to_string(i) + ")");
         int best = 0;                                       // seed: the heaviest state of every subcircuit (ties: smaller i)
         for (int i = 1; i < n; ++i) if (scores_host[j][i] > scores_host[j][best]) best = i;
         chosen[j][best] = 1; cnt[j] = 1;
@@ -1644,7 +1715,7 @@ int tqc_hss_prepare(tqc_plan_t *pl, const int32_t *counts, const int32_t *keys_d
         kofs += (size_t)counts[j];
     }
     pl->hss_counts.assign(counts, counts + hp.m);
-    return 0;
+    return tqc_plan_finalize(sub, stream);
 }
 
 size_t tqc_hss_workspace_bytes(const tqc_plan_t *pl) {
@@ -1872,12 +1943,7 @@ int tqc_simulate_subcircuit_tensor(const tqc_subcircuit_desc *sub, float *out_de
     // pageable source: the runtime stages the bytes before the call returns, so hg may go out of scope
     TQC_CUDA(cudaMemcpyAsync(d_gates, hg.data(), sizeof(tqc::SimGate) * hg.size(), cudaMemcpyHostToDevice, st));
     const size_t smem = (sizeof(double2) + sizeof(double)) << w;          // amplitudes + probabilities
-    static bool attr_set = false;
-    if (!attr_set) {
-        TQC_CUDA(cudaFuncSetAttribute(tqc::sim_variant_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 24 << 13));
-        TQC_CUDA(cudaFuncSetAttribute(tqc::sim_variant_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
-        attr_set = true;
-    }
+    { const int arc = ensure_device_attrs(nullptr); if (arc) return arc; }
     // One block per (preparation, group of settings): the settings of the first g upstream wires come from the block id,
     // the block walks the other 3^{u-g}.  g = the smallest split that gives every SM two blocks (integers only).
     unsigned blocks_v = 1;

@@ -50,6 +50,18 @@ def test_fig5_costs_through_the_library():
     assert 2 ** g.cost_log2 <= net.m * 4 ** g.kmax                         # Eq. 2
 
 
+def test_library_planner_against_hand_worked_step_lists():
+    """The C++ planner against tests/golden/planner_steps.txt directly (not through the reference planner): operands,
+    bond widths and cost exponent of every step of the three hand-worked networks."""
+    from golden_planner import PLANNER_NETS, golden_planner_steps
+    gold = golden_planner_steps()
+    for name, make in PLANNER_NETS.items():
+        p = tqc.tqc_plan(make())
+        got = [(s["lhs"], s["rhs"], s["n_inner"], s["n_outer_lhs"], s["n_outer_rhs"], s["log2cost"]) for s in p.steps()]
+        want = [(g["lhs"], g["rhs"], len(g["inner"]), len(g["outer_lhs"]), len(g["outer_rhs"]), g["log2cost"]) for g in gold[name]]
+        assert got == want, name
+
+
 @pytest.mark.parametrize("mode", [tqc.MODE_STATES, tqc.MODE_DISTRIBUTION])
 def test_plan_is_bit_identical_to_reference_planner(mode):
     nets = [_fig5_network(), configs.cfg4_network()]

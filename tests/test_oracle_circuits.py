@@ -26,7 +26,7 @@ def _golden(name):
     return out
 
 
-ALL_GATES = [("h", ()), ("x", ()), ("s", ()), ("sdg", ()), ("sx", ()), ("sy", ()), ("sw", ()),
+ALL_GATES = [("y", ()), ("z", ()), ("t", ()), ("tdg", ()), ("cp", (0.9,)), ("h", ()), ("x", ()), ("s", ()), ("sdg", ()), ("sx", ()), ("sy", ()), ("sw", ()),
              ("rx", (0.7,)), ("ry", (1.3,)), ("rz", (2.1,)), ("cz", ()), ("cx", ()), ("rzz", (0.4,))]
 
 
@@ -50,6 +50,43 @@ def test_closed_forms_ghz_h():
     assert np.allclose(p, g["ghz3"], atol=1e-12)
     psi = sv.simulate(1, [("h", (), (0,))]).reshape(-1)
     assert np.allclose(psi, [1 / np.sqrt(2)] * 2, atol=1e-12)
+    # W-3 -> 1/3 on each one-hot bitstring; W-n and GHZ-n laws of the benchmark generators
+    assert np.allclose(sv.uncut_probabilities(3, C.wstate_circuit(3).gates), g["w3"], atol=1e-12)
+    for n in (2, 5, 8):
+        pw = sv.uncut_probabilities(n, C.wstate_circuit(n).gates)
+        hot = [1 << k for k in range(n)]
+        assert np.allclose(pw[hot], 1.0 / n, atol=1e-12) and abs(pw.sum() - 1.0) < 1e-12
+        pg = sv.uncut_probabilities(n, C.ghz_circuit(n).gates)
+        assert np.allclose(pg[[0, 2 ** n - 1]], 0.5, atol=1e-12)
+
+
+def test_new_gates_against_textbook_identities():
+    """y, z, t, tdg, cp are pinned by relations to the already-pinned gates: Y = iXZ, T^2 = S, T Tdg = 1, Z = S^2,
+    cp(pi) = cz, cp(l) = phase gates and two cx (the textbook decomposition)."""
+    X, S, T = (sv.gate_matrix(nm) for nm in ("x", "s", "t"))
+    assert np.allclose(sv.gate_matrix("z"), S @ S) and np.allclose(sv.gate_matrix("y"), 1j * X @ sv.gate_matrix("z"))
+    assert np.allclose(T @ T, S) and np.allclose(T @ sv.gate_matrix("tdg"), np.eye(2))
+    assert np.allclose(sv.gate_matrix("cp", (np.pi,)), sv.gate_matrix("cz"))
+    lam = 0.73
+    ph = lambda a: np.diag([1.0, np.exp(1j * a)])
+    cx = sv.gate_matrix("cx")
+    dec = np.kron(ph(lam / 2), np.eye(2)) @ cx @ np.kron(np.eye(2), ph(-lam / 2)) @ cx @ np.kron(np.eye(2), ph(lam / 2))
+    assert np.allclose(dec, sv.gate_matrix("cp", (lam,)), atol=1e-12)
+
+
+def test_aqft_full_degree_is_the_dft():
+    """aqft with no truncation is the quantum Fourier transform without the final swaps: on basis state |x> the output
+    amplitudes are those of numpy's DFT read in bit-reversed order (a library routine as the pin)."""
+    n = 4
+    circ = C.aqft_circuit(n, degree=n)
+    for x in (1, 6, 11):
+        psi0 = np.zeros((2,) * n, dtype=np.complex128)
+        psi0[tuple((x >> (n - 1 - q)) & 1 for q in range(n))] = 1.0
+        got = sv.simulate(n, circ.gates, psi0).reshape(-1)
+        e = np.zeros(2 ** n); e[x] = 1.0
+        want = np.fft.ifft(e) * np.sqrt(2.0 ** n)             # amplitudes exp(+2 pi i x y / N) / sqrt(N)
+        rev = [int(format(y, f"0{n}b")[::-1], 2) for y in range(2 ** n)]
+        assert np.allclose(got, want[rev], atol=1e-12)
 
 
 def _brute_force_apply(psi_flat, n, mat, qubits):

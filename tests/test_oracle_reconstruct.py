@@ -13,6 +13,7 @@ from oracle import planner_ref as P, reconstruct as R
 from oracle.direct_sum_c import direct_sum_c
 from tqc_inputs import configs, random_states, random_tensors, rank_one_tensors
 from tqc_inputs.network import Network
+from golden_planner import PLANNER_NETS, golden_planner_steps
 
 GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
 
@@ -184,6 +185,54 @@ def test_reference_planner_fixtures():
     # determinism and serialisation
     assert P.serialize(P.plan(net)) == P.serialize(P.plan(net))
     assert P.serialize(p)[:4] == b"TQCP"
+
+
+@pytest.mark.parametrize("name", sorted(PLANNER_NETS))
+def test_reference_planner_hand_worked_step_lists(name):
+    """planner_ref.plan against step lists worked by hand under rules P1-P6 (tests/golden/planner_steps.txt): pins the
+    memory score, its precedence over the cost exponent, both id tie-breaks, lhs = smaller id and merged parallel bonds."""
+    net = PLANNER_NETS[name]()
+    net.validate()
+    assert P.plan(net)["steps"] == golden_planner_steps()[name]
+
+
+@pytest.mark.parametrize("seed", range(6))
+def test_tensordot_tier_and_order_search_against_direct_sum(seed):
+    """O8' (contract_states_tensordot) and the seeded order search of O8 (order_trials > 0: the form the cfg5 GPU tests use)
+    against the literal sum Pi-4 on tiny networks, parallel cuts and disconnected pieces included."""
+    m = 3 + seed % 4
+    net = configs.random_network(m, (m - 1) + seed % 4, 500 + seed, o_lo=0, o_hi=2, connected=(seed % 3 != 2))
+    if net.n_qubits == 0:
+        net = configs.random_network(m, m, 500 + seed, o_lo=1, o_hi=2)
+    T = [t * (1 if seed % 2 else -1) ** np.arange(t.shape[1])[None, :] for t in random_tensors(net, 510 + seed)]   # signed
+    bits = random_states(net.n_qubits, 12, 520 + seed)
+    want = R.direct_sum(net, T, bits)
+    scale = np.abs(want).max()
+    assert np.abs(R.contract_states_tensordot(net, T, bits) - want).max() <= 1e-12 * scale
+    assert np.abs(R.contract_states_tensordot(net, T, bits, order_trials=64) - want).max() <= 1e-12 * scale
+    assert np.abs(R.bucket_elimination(net, T, bits, order_trials=64) - want).max() <= 1e-12 * scale
+    order = R._elimination_order(net, trials=64)
+    assert sorted(order) == list(range(net.K))                             # a permutation of the cut ids
+    steps = R.pairwise_steps_from_elimination(net, order)
+    assert np.abs(R.pairwise_contract(net, T, bits, steps + _join_rest(net, steps)) - want).max() <= 1e-12 * scale
+
+
+def _join_rest(net, steps):
+    """pairwise_contract multiplies leftover nodes itself; nothing to add (kept for clarity of the call above)."""
+    return []
+
+
+def test_tensordot_tier_at_cfg5_size_against_the_closed_form():
+    """O8' at full cfg5 size (m = 52, K = 152) against Pi-1, the only exact pin there; distinct a_{s,e} per edge make any
+    bond mix-up visible.  Also against O8 (bucket elimination) on a 22-cut network where both finish quickly."""
+    net = configs.cfg5_network()
+    T, g, a = rank_one_tensors(net, 55)
+    bits = random_states(196, 3, 56)
+    assert np.allclose(R.contract_states_tensordot(net, T, bits, order_trials=8), R.rank_one_closed_form(net, g, a, bits), rtol=1e-11)
+    big = configs.random_network(12, 22, 181, o_lo=1, o_hi=2)
+    Tb = random_tensors(big, 191)
+    bb = random_states(big.n_qubits, 6, 196)
+    assert np.allclose(R.contract_states_tensordot(big, Tb, bb), R.bucket_elimination(big, Tb, bb), rtol=1e-12)
 
 
 def test_cfg5_network_shape_and_rank_one():

@@ -8,7 +8,7 @@ lines 590-593).
 
 Gate names: h, rx, ry, rz (one angle), sx/sy/sw = exp(-i pi/4 P) for
 P = X, Y, W=(X+Y)/sqrt2 (sqrt(X), sqrt(Y), sqrt(W) up to phase, reading G11),
-cz, cx, rzz(gamma) = exp(-i gamma Z(x)Z).
+cz, cx, rzz(gamma) = exp(-i gamma Z(x)Z); y, z, t, tdg; cp(lambda) = diag(1, 1, 1, e^{i lambda}).
 """
 from __future__ import annotations
 
@@ -267,3 +267,42 @@ def hea_subcircuit(w: int = 12, d: int = 3, u: int = 3, seed: int = 250203445 + 
             gates += [("cx", (), (q, q + 1)) for q in range(w - 1)]
     return dict(w=w, gates=gates, D_wires=list(range(d)), U_wires=list(range(w - u, w)), O_wires=list(range(w - u)),
                 bond_pos=list(range(d + u)))
+
+
+# ---- the paper's other benchmark families (section 7.2): gate lists only -----------------------
+def ghz_circuit(n: int) -> Circuit:
+    """GHZ-n: h 0; cx 0 1; cx 1 2; ... ("two dominating states").  Output law: 1/2 on 0..0 and on 1..1."""
+    gates = [("h", (), (0,))] + [("cx", (), (q, q + 1)) for q in range(n - 1)]
+    return Circuit(n, gates, name=f"ghz{n}")
+
+
+def wstate_circuit(n: int) -> Circuit:
+    """W-n ("n dominating states for a n-qubit benchmark"): x on qubit 0, then for k = 0..n-2 a rotation of qubit
+    k+1 controlled on qubit k, RY(theta_k) with cos(theta_k / 2) = sqrt(1 / (n - k)), followed by cx(k+1, k).  The
+    controlled RY is written with this package's gate names as ry(theta/2) t; cx c t; ry(-theta/2) t; cx c t.
+    Output law: 1/n on each of the n one-hot bitstrings."""
+    gates = [("x", (), (0,))]
+    for k in range(n - 1):
+        theta = 2.0 * float(np.arccos(np.sqrt(1.0 / (n - k))))
+        c, t = k, k + 1
+        gates += [("ry", (theta / 2.0,), (t,)), ("cx", (), (c, t)), ("ry", (-theta / 2.0,), (t,)), ("cx", (), (c, t)),
+                  ("cx", (), (t, c))]
+    return Circuit(n, gates, name=f"w{n}")
+
+
+def aqft_circuit(n: int, degree: int | None = None, seed: int | None = None) -> Circuit:
+    """Approximate QFT: for every target qubit j an h, then controlled phases cp(pi / 2^k) from qubit j + k,
+    dropped when k > degree (default ceil(log2 n) + 2, the truncation the paper does not state).  No final swaps.
+    With a seed the register first gets one ry(U[0, pi)) per qubit so that the output is not the flat distribution."""
+    if degree is None:
+        degree = int(np.ceil(np.log2(max(n, 2)))) + 2
+    gates = []
+    if seed is not None:
+        rng = np.random.default_rng(seed)
+        gates += [("ry", (float(rng.random() * np.pi),), (q,)) for q in range(n)]
+    for j in range(n):
+        gates.append(("h", (), (j,)))
+        for k in range(1, n - j):
+            if k <= degree:
+                gates.append(("cp", (float(np.pi / 2 ** k),), (j + k, j)))
+    return Circuit(n, gates, name=f"aqft{n}")
