@@ -10,7 +10,7 @@ the states and D2H of the probabilities inside the timed region).  Multi-GPU (to
 path shards over independent states; every rank holds the tensors and
 contracts its own seeded batch, no collective on the data path ("scaling": "weak").
 
-`--impl reference` times the CPU oracle (oracle/, float64 direct sum / bucket elimination) on a
+`--impl reference` times the CPU oracle (oracle/, float64 direct sum / per-state tensordot contraction) on a
 bounded sample of the same workload; the `cpu_baseline` leg of the default arm does the same
 once.  These two legs are the only places this file touches oracle/.
 """
@@ -35,6 +35,7 @@ UNIT = "states/s"
 SM_COUNT = 148                  # B200 (B200_PROFILING.md)
 FP32_LANES_PER_SM = 128
 NOMINAL_TF32_OVER_BF16 = 1.1 / 2.25   # nominal dense peaks (B200_PROFILING.md table)
+TC_KERNEL_NAMES = "step_tc_kernel<BN> / step_tcw_kernel"
 
 
 def measured_peaks() -> dict:
@@ -46,6 +47,34 @@ def measured_peaks() -> dict:
         return p
     return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "sm_max_mhz": 1965.0,
             "source": "fallback"}
+
+
+def roof_peaks() -> dict:
+    """Every roofline denominator with its source.  HBM and bf16 come from MEASURED_PEAKS.json (driver-written); TF32
+    matmul, FP32 FFMA, shared-memory LDS.128 and L2 read rates from profiles/peaks_r02.json, written on a B200 of this
+    pool by `python -m paper_2502_03445_b200.measure_peaks` (measured by the build).  Where that file
+    is missing the value is DERIVED from unit counts x sm_max_mhz (FFMA, LDS) or from bf16 x the nominal ratio (TF32)
+    and labelled so."""
+    p = measured_peaks()
+    own_path = os.path.join(ROOT, "profiles", "peaks_r02.json")
+    own = {}
+    if os.path.exists(own_path):
+        with open(own_path) as f:
+            own = json.load(f)
+    mhz = p.get("sm_max_mhz", 1965.0)
+    out = dict(p)
+    def pick(key, derived, how):
+        if key in own:
+            out[key], out[key + "_source"] = float(own[key]), "measured (profiles/peaks_r02.json)"
+        else:
+            out[key], out[key + "_source"] = derived, "derived: " + how
+    pick("tf32_tflops", p["bf16_tflops"] * NOMINAL_TF32_OVER_BF16, "bf16 x nominal tf32/bf16 ratio 1.1/2.25")
+    pick("tf32_tflops_sustained", p.get("bf16_tflops_sustained", p["bf16_tflops"]) * NOMINAL_TF32_OVER_BF16,
+         "sustained bf16 x nominal tf32/bf16 ratio")
+    pick("ffma_tflops", SM_COUNT * FP32_LANES_PER_SM * 2 * mhz * 1e6 / 1e12, "148 SMs x 128 lanes x 2 x sm_max_mhz")
+    pick("lds_gbs", SM_COUNT * 128 * mhz * 1e6 / 1e9, "148 SMs x 128 B/clk x sm_max_mhz")
+    pick("l2_read_gbs", None, "not measured")
+    return out
 
 
 # ---------------------------------------------------------------------------------------------
@@ -79,6 +108,11 @@ def make_workload(name: str, batch: int | None = None):
     tensors = random_tensors(net, seed_for(cfg, STREAM_TENSORS))
     return {"name": name, "cfg": cfg, "net": net, "tensors": tensors, "mode": configs.MODE[cfg], "B": int(B),
             "full_B": configs.BATCH[cfg]}
+
+
+def pack_states_of(wl, rank: int) -> np.ndarray:
+    from tqc_inputs import pack_states
+    return pack_states(workload_states(wl, rank)).view(np.int64)
 
 
 def workload_states(wl, rank: int) -> np.ndarray:
@@ -163,7 +197,7 @@ def step_work(plan, t: int, B: int, mode_states: bool):
     return flop, nbytes
 
 
-def roofline_for(plan, tag: int, avg_ms: float, B: int, mode_states: bool, peaks: dict, traffic):
+def roofline_for(plan, tag: int, avg_ms: float, B: int, mode_states: bool, peaks: dict, traffic, long_step: bool = False):
     """Roofline object for the dominant launch (tag = plan step index)."""
     if tag == -4 and avg_ms > 0:
         # fused chain kernel: every per-state step of the plan in one launch
@@ -179,7 +213,7 @@ def roofline_for(plan, tag: int, avg_ms: float, B: int, mode_states: bool, peaks
                 if nd["kind"] != NODE_BATCH and v not in seen:          # gathered operand: distinct slices once + its keys
                     seen.add(v)
                     nbytes += 4.0 * min(B, 1 << nd["n_bits"]) * (4.0 ** nd["n_open"]) + 4.0 * B
-        alu_peak = SM_COUNT * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+        alu_peak = peaks["ffma_tflops"]
         sec = avg_ms * 1e-3
         t_alu, t_hbm = flop / (alu_peak * 1e12), nbytes / (peaks["hbm_gbs"] * 1e9)
         if t_hbm > t_alu:
@@ -189,17 +223,18 @@ def roofline_for(plan, tag: int, avg_ms: float, B: int, mode_states: bool, peaks
         return {"bound": bound, "achieved": achieved, "peak": peak, "unit": unit, "frac": achieved / peak,
                 "traffic": traffic, "kernel": "chain_spec_kernel / chain_kernel (fused per-state chain: fp32 FFMA steps + 3xTF32 mma.sync blocks for 16x16x16-class steps; specialised per plan when NVRTC is present; the FP32-ALU peak is the reference for its algorithmic flops)", "plan_step": "all per-state steps",
                 "algorithmic_flop": flop, "algorithmic_bytes": nbytes, "avg_launch_ms": avg_ms,
-                "peak_source": peaks["source"] + (" hbm copy" if bound == "hbm" else " sm_max_mhz x 148 SMs x 128 lanes x 2")}
+                "peak_source": (peaks["source"] + " hbm copy") if bound == "hbm" else ("FP32 FFMA rate, " + peaks["ffma_tflops_source"])}
     if tag < 0 or avg_ms <= 0:
         return {"bound": "hbm", "achieved": None, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": None,
                 "traffic": traffic, "kernel": {-1: "key_kernel", -2: "gather_kernel"}.get(tag, "?")}
     flop, nbytes = step_work(plan, tag, B, mode_states)
     kclass = plan.step(tag)["kernel_class"]
-    alu_peak = SM_COUNT * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12        # TFLOP/s fp32 FFMA
-    tf32_peak = peaks["bf16_tflops"] * NOMINAL_TF32_OVER_BF16
+    alu_peak = peaks["ffma_tflops"]                    # TFLOP/s fp32 FFMA
+    # a tensor-pipe launch inside a seconds-long cfg5 step runs under the power cap: the sustained matmul figure
+    tf32_peak = peaks["tf32_tflops_sustained"] if long_step else peaks["tf32_tflops"]
     t_hbm = nbytes / (peaks["hbm_gbs"] * 1e9)
     sec = avg_ms * 1e-3
-    name = {0: "step_tile_kernel (fp32 FFMA)", 1: "dot_kernel", 2: "step_tc_kernel (3xTF32 tcgen05)"}.get(kclass, "?")
+    name = {0: "step_tile_kernel (fp32 FFMA)", 1: "dot_kernel", 2: "tensor-pipe step kernel (3xTF32 tcgen05: " + TC_KERNEL_NAMES + ")"}.get(kclass, "?")
     st_ = plan.step(tag)
     if kclass == 0 and (not mode_states or plan.node(plan.m + tag)["kind"] == 1):
         # cross-mode step: the launcher's integer rule for the warp-level tensor-core tile kernel
@@ -216,11 +251,17 @@ def roofline_for(plan, tag: int, avg_ms: float, B: int, mode_states: bool, peaks
         achieved = flop / sec / 1e12
     if t_hbm > t_cmp:
         bound, peak, unit, achieved = "hbm", peaks["hbm_gbs"], "GB/s", nbytes / sec / 1e9
-    return {"bound": bound, "achieved": achieved, "peak": peak, "unit": unit, "frac": achieved / peak,
+    src = (peaks["source"] + " hbm copy") if bound == "hbm" else ("FP32 FFMA rate, " + peaks["ffma_tflops_source"]) if bound == "alu" \
+        else (("sustained " if long_step else "burst ") + "TF32 matmul, " + peaks["tf32_tflops_source"])
+    roof = {"bound": bound, "achieved": achieved, "peak": peak, "unit": unit, "frac": achieved / peak,
             "traffic": traffic, "kernel": name, "plan_step": tag, "algorithmic_flop": flop, "algorithmic_bytes": nbytes,
-            "avg_launch_ms": avg_ms, "peak_source": peaks["source"] +
-            (" hbm copy" if bound == "hbm" else " sm_max_mhz x 148 SMs x 128 lanes x 2" if bound == "alu"
-             else " bf16 x nominal tf32/bf16 ratio")}
+            "avg_launch_ms": avg_ms, "peak_source": src}
+    if bound == "tensor":
+        # both denominators SURVEY H1 asks for: issued 3xTF32 flops against the TF32 peak (frac), and the fp32-equivalent
+        # rate against TF32 / 3
+        roof["fp32_equivalent_tflops"] = flop / sec / 1e12
+        roof["frac_of_tf32_over_3"] = (flop / sec / 1e12) / (tf32_peak / 3.0)
+    return roof
 
 
 def committed_traffic(workload: str, tag: int, states_per_launch: float):
@@ -263,23 +304,26 @@ def run_ours(args) -> None:
         if world > 1:
             dist.destroy_process_group()
         return
-    line = measure(ctx, args, args.workload, args.batch, args.steps, args.warmup)
+    # cfg5 without --batch: the 8d-5 prefix rule (batch = -1); --batch N times the first N states; --batch 1000000 the full batch
+    head_batch = args.batch if args.batch > 0 else (-1 if args.workload == "cfg5" else 0)
+    line = measure(ctx, args, args.workload, head_batch, args.steps, args.warmup)
     if rank == 0:
         if world == 1 and args.others:
             # the other BASELINE configs, shorter runs, same protocol (cfg5: a labelled prefix of its 10^6-state batch)
             others = []
-            for name, batch, steps in (("cfg5", 1024, 2), ("cfg3", 0, 10), ("cfg2", 0, 10)):
+            for name, batch, steps in (("cfg5", -1, 3), ("cfg4", 0, 20), ("cfg3", 0, 10), ("cfg2", 0, 10)):
                 if name == args.workload:
                     continue
                 o = measure(ctx, args, name, batch, steps, 3)
                 others.append({k: o[k] for k in ("value", "unit", "ms_per_step", "steps", "gpu_launches", "roofline")} |
-                              {"workload": o["config"]["workload"], "e2e_value": o["e2e"]["value"]})
+                              {"workload": o["config"]["workload"], "e2e_value": o["e2e"]["value"],
+                               "chain_status": o["config"]["chain_status"], "kernel_classes": o["config"]["kernel_classes"]})
             others.append(measure_hss(ctx, 10, 3))
             others.append(measure_hss_contract(ctx, 10, 3))
             others.append(measure_variants(ctx, 10, 3, not args.no_cpu_baseline))
             line["other_workloads"] = others
         if world == 1 and not args.no_cpu_baseline:
-            line["cpu_baseline"] = cpu_baseline(make_workload(args.workload, args.batch), args.cpu_seconds)
+            line["cpu_baseline"] = cpu_baseline(make_workload(args.workload, args.batch if args.batch > 0 else None), args.cpu_seconds)
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -289,20 +333,47 @@ def measure(ctx, args, workload: str, batch: int, steps: int, warmup: int):
     """One workload through the full protocol; returns the JSON line as a dict (rank 0) or None."""
     torch, dist, tqc = ctx["torch"], ctx["dist"], ctx["tqc"]
     world, rank, local, dev = ctx["world"], ctx["rank"], ctx["local"], ctx["dev"]
-    peaks = measured_peaks()
-    wl = make_workload(workload, batch)
-    net, B = wl["net"], wl["B"]
+    peaks = roof_peaks()
+    wl = make_workload(workload, batch if batch > 0 else None)
+    net = wl["net"]
     states_mode = wl["mode"] == "states"
     restarts = max(args.restarts, 0)
-    plan = tqc.tqc_plan(net, tqc.MODE_STATES if states_mode else tqc.MODE_DISTRIBUTION, batch_hint=B,
+    # batch_hint = the config's FULL batch: a prefix run keeps the plan (tables, kernel classes) of the real workload
+    plan = tqc.tqc_plan(net, tqc.MODE_STATES if states_mode else tqc.MODE_DISTRIBUTION, batch_hint=wl["full_B"],
                         restarts=restarts, seed=args.plan_seed)
     for s, t in enumerate(wl["tensors"]):
         tqc.tqc_load_subcircuit_tensors(plan, s, t)
+    prefix_note = None
+    if batch < 0:
+        # SURVEY 8d-5: the full batch does not fit a bench step; time a power-of-two PREFIX of the same seeded batch, the
+        # smallest one whose step runs >= 1 s, found from a calibration run of 2^10 states (all ranks agree on it)
+        n_cal = 1 << 10
+        wl["B"] = n_cal
+        cal_states = torch.from_numpy(pack_states_of(wl, rank)).to(dev)
+        cal_ws = torch.empty(min(plan.workspace_bytes(n_cal), args.max_workspace_gb << 30), dtype=torch.uint8, device=dev)
+        cal_out = torch.empty(n_cal, dtype=torch.float32, device=dev)
+        for _ in range(2):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            tqc.tqc_contract_states(plan, cal_states, out=cal_out, workspace=cal_ws)
+            e1.record()
+            torch.cuda.synchronize()
+        t_cal = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(t_cal, op=dist.ReduceOp.MAX)
+        lg = 10
+        while (1 << lg) < wl["full_B"] and float(t_cal.item()) * (1 << (lg - 10)) < 1000.0:
+            lg += 1
+        wl["B"] = min(1 << lg, wl["full_B"])
+        prefix_note = (f"calibration: 2^10 states in {float(t_cal.item()):.1f} ms -> smallest power-of-two prefix with a step >= 1 s "
+                       f"is 2^{lg}")
+        del cal_states, cal_ws, cal_out
+        torch.cuda.empty_cache()
+    B = wl["B"]
     n_out = B if states_mode else (1 << net.n_qubits)
 
-    from tqc_inputs import pack_states
     if states_mode:
-        packed = pack_states(workload_states(wl, rank)).view(np.int64)
+        packed = pack_states_of(wl, rank)
         states_host = torch.from_numpy(packed).pin_memory()
         states_dev = states_host.to(dev)
         ws_bytes = min(plan.workspace_bytes_host(B), max(args.max_workspace_gb << 30,
@@ -358,7 +429,8 @@ def measure(ctx, args, workload: str, batch: int, steps: int, warmup: int):
     # per-launch times of the same step, CUDA events on the launching stream inside the library
     plan.profile_enable(True)
     per_tag: dict = {}
-    for _ in range(steps):
+    prof_steps = steps if ms_hint_short(total_ms, steps) else min(steps, 2)
+    for _ in range(prof_steps):
         flush.zero_()
         step_device()
         for tag, ms in plan.profile_read():
@@ -369,6 +441,7 @@ def measure(ctx, args, workload: str, batch: int, steps: int, warmup: int):
     torch.cuda.synchronize()
     clocks = sampler.stop() if sampler else None
 
+    chain_rc, chain_note = plan.chain_status()
     ms_per_step = total_ms / steps
     value = world * n_out / (ms_per_step * 1e-3)
     e2e_value = world * n_out / (e2e_ms / steps * 1e-3)
@@ -377,14 +450,31 @@ def measure(ctx, args, workload: str, batch: int, steps: int, warmup: int):
 
     dom = max(per_tag.items(), key=lambda kv: kv[1][0])
     dom_tag, (dom_total, dom_n) = dom
-    launches_per_step = dom_n / steps
+    launches_per_step = dom_n / prof_steps
     rows_B = B / launches_per_step if states_mode else B          # a chunked batch runs the step once per chunk
     roof = roofline_for(plan, dom_tag, dom_total / dom_n, int(rows_B), states_mode, peaks,
-                        committed_traffic(wl["name"], dom_tag, rows_B))
-    step_ms_sum = sum(v[0] for v in per_tag.values()) / steps
-    roof["share_of_step"] = (dom_total / steps) / step_ms_sum if step_ms_sum > 0 else None
-    kernels = {str(tag): {"ms_per_step": v[0] / steps, "launches_per_step": v[1] / steps}
-               for tag, v in sorted(per_tag.items())}
+                        committed_traffic(wl["name"], dom_tag, rows_B), long_step=ms_per_step > 200.0)
+    step_ms_sum = sum(v[0] for v in per_tag.values()) / prof_steps
+    roof["share_of_step"] = (dom_total / prof_steps) / step_ms_sum if step_ms_sum > 0 else None
+    kclass_name = {0: "simt_tile", 1: "dot", 2: "tcgen05", 3: "chain"}
+    kernels = {}
+    for tag, v in sorted(per_tag.items()):
+        ent = {"ms_per_step": v[0] / prof_steps, "launches_per_step": v[1] / prof_steps}
+        if tag >= 0:
+            st_ = plan.step(tag)
+            ent["kernel_class"] = kclass_name.get(st_["kernel_class"], "?")
+            ent["log2_mults_per_row"] = st_["log2cost"]
+        else:
+            ent["kernel_class"] = {-1: "key_kernel", -2: "gather_kernel", -4: "fused chain"}.get(tag, "?")
+        kernels[str(tag)] = ent
+    # whole-step tensor-pipe accounting (cfg5): algorithmic flops of every tcgen05 step over their summed launch time
+    tc_flop = sum(2.0 * 2.0 ** plan.step(t)["log2cost"] * B for t in range(plan.num_steps) if plan.step(t)["kernel_class"] == 2)
+    tc_ms = sum(v[0] / prof_steps for tag, v in per_tag.items() if tag >= 0 and plan.step(tag)["kernel_class"] == 2)
+    if tc_ms > 0:
+        tfs = tc_flop / (tc_ms * 1e-3) / 1e12
+        pk = peaks["tf32_tflops_sustained"] if ms_per_step > 200.0 else peaks["tf32_tflops"]
+        roof["all_tensor_steps"] = {"fp32_equivalent_tflops": tfs, "ms_per_step": tc_ms, "frac_of_tf32_over_3": tfs / (pk / 3.0),
+                                    "frac_of_tf32_issued": 3.0 * tfs / pk}
 
     words = (net.n_qubits + 63) // 64
     line = {
@@ -394,7 +484,10 @@ def measure(ctx, args, workload: str, batch: int, steps: int, warmup: int):
         "config": {"workload": workload_description(wl, plan), "states_per_step_per_gpu": n_out,
                    "parallelism": f"states sharded over {world} GPU(s), tensors replicated, no collective",
                    "l2": "flushed between timed iterations (256 MB write)", "plan_cost_log2_per_state": plan.cost_log2, "planner_restarts": restarts,
-                   "kmax": plan.kmax, "workspace_gb": ws_bytes / 2 ** 30},
+                   "kmax": plan.kmax, "workspace_gb": ws_bytes / 2 ** 30, "prefix_rule": prefix_note,
+                   "library": tqc.version(), "chain_status": chain_rc, "chain_note": chain_note,
+                   "kernel_classes": {kclass_name[k]: sum(1 for t in range(plan.num_steps) if plan.step(t)["kernel_class"] == k)
+                                      for k in kclass_name}},
         "e2e": {"value": e2e_value, "unit": UNIT,
                 "h2d_bytes_per_step": int(B * words * 8) if states_mode else 0, "d2h_bytes_per_step": int(n_out * 4)},
         "gpu_launches": int(launches),
@@ -406,6 +499,11 @@ def measure(ctx, args, workload: str, batch: int, steps: int, warmup: int):
     del workspace, flush, out_dev
     torch.cuda.empty_cache()
     return line
+
+
+def ms_hint_short(total_ms: float, steps: int) -> bool:
+    """True when a step is short enough to repeat the per-launch profiling pass `steps` times."""
+    return total_ms / max(steps, 1) < 50.0
 
 
 def measure_hss(ctx, steps: int, warmup: int) -> dict:
@@ -588,10 +686,10 @@ def workload_description(wl, plan) -> str:
 # ---------------------------------------------------------------------------------------------
 # the CPU oracle legs (the only code here that touches oracle/)
 # ---------------------------------------------------------------------------------------------
-def oracle_sample_rate(wl, seconds: float, rank: int = 0):
+def oracle_sample_rate(wl, seconds: float, rank: int = 0, threads: int = 0):
     """Times the oracle AS IT STANDS on a bounded sample of the workload's states: the float64 direct sum over all
-    4^K cut assignments (oracle/direct_sum.c, OpenMP over states) while 4^K is feasible, else the float64 bucket
-    elimination (oracle/reconstruct.py, numpy).  Returns (states/s, cores, sample description)."""
+    4^K cut assignments (oracle/direct_sum.c, OpenMP over states) while 4^K is feasible, else the float64 per-state
+    tensordot contraction O8' (oracle/reconstruct.py, numpy).  Returns (states/s, cores, sample description)."""
     from oracle import reconstruct as R
     from oracle.direct_sum_c import direct_sum_c
     net = wl["net"]
@@ -603,28 +701,42 @@ def oracle_sample_rate(wl, seconds: float, rank: int = 0):
         bits_all = ((idx[:, None] >> (net.n_qubits - 1 - np.arange(net.n_qubits))[None, :]) & 1).astype(np.uint8)
     T = wl["tensors"]
     if net.K <= 16:
-        probe = min(len(bits_all), max(cores, 8))
+        probe = min(len(bits_all), max(cores if threads == 0 else threads, 8 if threads == 0 else 1))
         t0 = time.perf_counter()
-        _, used = direct_sum_c(net, T, bits_all[:probe])
+        _, used = direct_sum_c(net, T, bits_all[:probe], num_threads=threads)
         dt = max(time.perf_counter() - t0, 1e-6)
         n = int(min(len(bits_all), max(probe, probe * seconds / dt)))
         t0 = time.perf_counter()
-        _, used = direct_sum_c(net, T, bits_all[:n])
+        _, used = direct_sum_c(net, T, bits_all[:n], num_threads=threads)
         dt = time.perf_counter() - t0
         return n / dt, used, f"direct sum over 4^{net.K} cut assignments (C, OpenMP), first {n} states of the batch, {dt:.1f} s"
+    # 4^K infeasible (cfg5, K = 152): the oracle's large-K tier O8' as it stands, per-state pairwise np.tensordot along
+    # the oracle's own elimination order, numpy float64 (BLAS threads = host cores)
     order = R._elimination_order(net, trials=16)
     n, t0 = 0, time.perf_counter()
     while n < len(bits_all) and (n == 0 or time.perf_counter() - t0 < seconds):
-        R.bucket_elimination(net, T, bits_all[n:n + 1], order=order, chunk=1)
+        R.contract_states_tensordot(net, T, bits_all[n:n + 1], order=order)
         n += 1
     dt = time.perf_counter() - t0
-    return n / dt, cores, (f"bucket elimination (numpy float64, 4^K infeasible at K={net.K}), first {n} state(s) of the "
-                           f"batch, {dt:.1f} s; cores = host threads available to numpy")
+    return n / dt, cores, (f"O8' per-state tensordot contraction (numpy float64; 4^K infeasible at K={net.K}), first {n} state(s) of "
+                           f"the batch, {dt:.1f} s; cores = host threads available to BLAS")
+
+
+def single_core_rate(wl, seconds: float):
+    """The same oracle leg limited to one thread (BASELINE.md section 3 asks for both figures); None if it cannot be limited."""
+    try:
+        from threadpoolctl import threadpool_limits
+    except ImportError:
+        return None
+    with threadpool_limits(limits=1):                      # numpy's BLAS; the C direct sum takes num_threads = 1
+        rate, _cores, sample = oracle_sample_rate(wl, seconds, threads=1)
+    return {"value": rate, "unit": UNIT, "cores": 1, "sample": sample}
 
 
 def cpu_baseline(wl, seconds: float) -> dict:
     rate, cores, sample = oracle_sample_rate(wl, seconds)
-    return {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+    return {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+            "single_core": single_core_rate(wl, max(3.0, seconds / 3.0))}
 
 
 def oracle_run(wl, bits, order=None):
@@ -635,7 +747,7 @@ def oracle_run(wl, bits, order=None):
     if wl["net"].K <= 16:
         _, used = direct_sum_c(wl["net"], wl["tensors"], bits)
     else:
-        R.bucket_elimination(wl["net"], wl["tensors"], bits, order=order, chunk=1)
+        R.contract_states_tensordot(wl["net"], wl["tensors"], bits, order=order)
         used = os.cpu_count() or 1
     return time.perf_counter() - t0, used
 
@@ -668,7 +780,7 @@ def run_reference(args) -> None:
             done += n
     value = done / total
     kind = ("direct sum over 4^%d cut assignments (C, OpenMP)" % net.K) if net.K <= 16 else \
-           ("bucket elimination (numpy float64; 4^K infeasible at K=%d)" % net.K)
+           ("O8' per-state tensordot contraction (numpy float64; 4^K infeasible at K=%d)" % net.K)
     sample = f"{kind}; {args.steps} timed steps of {n} states each from the seeded batch, {total:.1f} s"
     n_out = wl["B"] if wl["mode"] == "states" else (1 << net.n_qubits)
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT,
@@ -686,12 +798,13 @@ def run_reference(args) -> None:
 def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg4", choices=["cfg2", "cfg3", "cfg4", "cfg5", "variants"],
+    ap.add_argument("--workload", default="cfg5", choices=["cfg2", "cfg3", "cfg4", "cfg5", "variants"],
                     help="variants: only the subcircuit-variant simulation row (secondary line, for profiling)")
-    ap.add_argument("--batch", type=int, default=0, help="states per step per GPU (0: the config's own batch)")
+    ap.add_argument("--batch", type=int, default=0, help="states per step per GPU (0: the config's own batch; for cfg5 "
+                    "the SURVEY 8d-5 prefix: the smallest power of two whose step runs >= 1 s; 1000000 = the full cfg5 batch)")
     ap.add_argument("--restarts", type=int, default=0, help="planner restarts (0: deterministic greedy)")
     ap.add_argument("--plan-seed", type=int, default=1)
     ap.add_argument("--max-workspace-gb", type=int, default=64)

@@ -235,8 +235,8 @@ int tqc_hss_contract(tqc_plan_t *plan, float *out_dev, void *workspace_dev, size
  *   w wires; wire 0 is the most significant bit of the amplitude index (G4); all wires start in |0> unless listed in D.
  *     w = 0 (a subcircuit no gate was assigned to) gives the 1 x 1 tensor [1].
  *   gates[n_gates] applied in order; kind = TQC_GATE_*, wire0 (and wire1 for two-qubit gates; CX controls on wire0),
- *     param = angle of RX/RY/RZ (exp(-i param P / 2)) and RZZ (exp(-i param Z(x)Z)); SX/SY/SW = exp(-i pi/4 P) for
- *     P = X, Y, (X+Y)/sqrt2.
+ *     param = angle of RX/RY/RZ (exp(-i param P / 2)), of RZZ (exp(-i param Z(x)Z): the FULL angle, not param / 2) and of
+ *     CP (phase e^{i param} on |11>); SX/SY/SW = exp(-i pi/4 P) for P = X, Y, (X+Y)/sqrt2; T / TDG = diag(1, e^{+-i pi/4}).
  *   D_wires[d]: wires that begin at a downstream cut end;  U_wires[u]: wires that end at an upstream cut end;
  *   O_wires[o]: wires that end at a circuit output, in the order of x_s (first = MSB).  u + o = w.
  *   bond_pos[d + u]: bond j (D_wires in order, then U_wires in order) is digit bond_pos[j] of the row index of T_s
@@ -245,7 +245,9 @@ int tqc_hss_contract(tqc_plan_t *plan, float *out_dev, void *workspace_dev, size
  * description is out of range).  Asynchronous on `stream`, no allocation.  Errors: TQC_E_ARG (inconsistent lists, unknown
  * gate), TQC_E_TOO_LARGE (w > 13 or 4^{d+u} 2^o > 2^31), TQC_E_WORKSPACE, TQC_E_CUDA. */
 enum { TQC_GATE_H = 0, TQC_GATE_X = 1, TQC_GATE_S = 2, TQC_GATE_SDG = 3, TQC_GATE_SX = 4, TQC_GATE_SY = 5, TQC_GATE_SW = 6,
-       TQC_GATE_RX = 7, TQC_GATE_RY = 8, TQC_GATE_RZ = 9, TQC_GATE_CZ = 10, TQC_GATE_CX = 11, TQC_GATE_RZZ = 12 };
+       TQC_GATE_RX = 7, TQC_GATE_RY = 8, TQC_GATE_RZ = 9, TQC_GATE_CZ = 10, TQC_GATE_CX = 11, TQC_GATE_RZZ = 12,
+       TQC_GATE_Y = 13, TQC_GATE_Z = 14, TQC_GATE_T = 15, TQC_GATE_TDG = 16,
+       TQC_GATE_CP = 17 /* controlled phase diag(1, 1, 1, e^{i param}) */ };
 typedef struct {
     int32_t kind, wire0, wire1, reserved;
     double param;
@@ -264,6 +266,62 @@ typedef struct {
 size_t tqc_simulate_workspace_bytes(const tqc_subcircuit_desc *sub);
 int tqc_simulate_subcircuit_tensor(const tqc_subcircuit_desc *sub, float *out_dev, void *workspace_dev,
                                    size_t workspace_bytes, void *stream);
+
+/* ---- Front half: circuit -> DAG -> partition -> cuts -> network -> plan (section 6) ---------------
+ * The circuit is cut by partitioning its two-qubit gates (lines 578-594: the DAG keeps only two-qubit gates, a one-qubit
+ * gate follows its adjacent two-qubit gate, input / output terminals are never cut) with Greedy Graph Growing (Alg. 2,
+ * lines 624-641): starting from one partition per two-qubit gate, repeatedly merge the pair of neighbouring partitions with
+ * the smallest merging cost Q_e <= Q_max (ties: the pair with the smaller partition ids), where Alg. 3 / Table 1 (lines
+ * 643-675) give Q_e = w_trial / w_max + s_trial / s_max + (K_trial / K_t if K_trial <= K_t else 4^{K_trial - K_t} + 1);
+ * w_trial = wires of the merged partition (one per maximal run of its gates along a qubit), s_trial = its two-qubit gates,
+ * K_trial = max over its neighbours c of the cut edges a pairwise contraction with c would carry (inner + outer); a merge
+ * with w_trial > w_max or s_trial > s_max is not allowed (lines 596-617).  Every wire segment between two partitions is
+ * a cut, upstream end in the earlier partition (lines 183-187).  Numbering conventions: csrc/partition.cpp.
+ * Deterministic: the same circuit and options give the same partition.
+ *
+ * tqc_plan_from_circuit: circuit_text HOST, NUL-terminated: "qubits <n>" then one gate per line, <name>[(<angle>)] <q0> [<q1>]
+ *   with names h x y z s sdg t tdg sx sy sw rx ry rz cz cx cp rzz, '#' comments.  TQC_E_PARSE names the offending line.
+ * tqc_plan_from_gates: the same from a gate list (wire0 / wire1 = circuit qubits).
+ * cut: w_max, s_max required (> 0); K_t = 0 -> 10, Q_max = 0 -> 1e4 (line 726).  TQC_E_INFEASIBLE when a single gate breaks
+ *   the caps.  opts as for tqc_plan (order / slice_cuts must be empty: the network does not exist yet).
+ * The plan owns the cut description; the queries below expose it (pointers stay valid until tqc_plan_destroy):
+ *   tqc_plan_cut_network     the tqc_network_desc the plan was built from;
+ *   tqc_plan_cut_subcircuit  subcircuit s as a tqc_subcircuit_desc ready for tqc_simulate_subcircuit_tensor (fuse_gates = 1,
+ *                            walk_settings = 1), its two-qubit gate count and its depth t_s (ASAP layers, line 531);
+ *   tqc_plan_cut_assignment  per gate of the circuit, the subcircuit it went to (HOST [n_gates]). */
+typedef struct {
+    int32_t w_max, s_max;   /* caps: qubits (wires) and two-qubit gates per subcircuit */
+    int32_t K_t;            /* 0 = 10 */
+    int32_t reserved;
+    double Q_max;           /* 0 = 1e4 */
+} tqc_cut_opts;
+int tqc_plan_from_circuit(const char *circuit_text, const tqc_cut_opts *cut, const tqc_plan_opts *opts, tqc_plan_t **out);
+int tqc_plan_from_gates(int n_qubits, const tqc_gate *gates, int n_gates, const tqc_cut_opts *cut, const tqc_plan_opts *opts,
+                        tqc_plan_t **out);
+int tqc_plan_cut_network(const tqc_plan_t *plan, tqc_network_desc *net);
+int tqc_plan_cut_subcircuit(const tqc_plan_t *plan, int s, tqc_subcircuit_desc *sub, int32_t *n_two_qubit_gates, int32_t *depth);
+int tqc_plan_cut_assignment(const tqc_plan_t *plan, int32_t *part_of_gate, size_t n_gates);
+/* Table 1 alone (host): the merging cost of a trial partition, or a negative value when a cap is broken ("Not allowed"). */
+double tqc_cut_merging_cost(int w_trial, int w_max, int s_trial, int s_max, int K_trial, int K_t);
+
+/* ---- Hybrid cost model (section 5, Eqs. 4-6) -------------------------------------------------------
+ * T_QPU = sum_i 3^{u_i} 4^{d_i} shots_i (t_i t_g + t_m) / n_qpus,  shots_i = 2^{w_i} kept within [2^shots_log2_min,
+ * 2^shots_log2_max] ("the number of shots equal to the number of quantum states per subcircuit, with limits ranging from
+ * 2^10 to 2^20", lines 523-524);  T_classical = C_TN / flops with C_TN = 2 x the plan's multiplication count (x n_states in
+ * states mode);  T = T_QPU + T_classical (Eq. 6).  Zero fields take the paper's values: t_g = 1e-7 s, t_m = 1e-6 s (lines
+ * 520-521), n_qpus = 10 (line 724), shots limits 10 and 20; flops must be given.  depth HOST [m] = t_i per subcircuit, or
+ * NULL for a plan made by tqc_plan_from_circuit / _gates (its own depths; any other plan then fails with TQC_E_ARG). */
+typedef struct {
+    double t_g, t_m, flops;
+    int32_t n_qpus, shots_log2_min, shots_log2_max, reserved;
+} tqc_cost_model;
+typedef struct {
+    double t_qpu, t_classical, t_total;   /* seconds */
+    double c_tn_flop;                     /* C_TN */
+    double qpu_variants;                  /* sum_i 3^{u_i} 4^{d_i}: subcircuit variants to run */
+} tqc_cost_report;
+int tqc_plan_cost_report(const tqc_plan_t *plan, const tqc_cost_model *model, const int32_t *depth, double n_states,
+                         tqc_cost_report *out);
 
 /* ---- measurement hooks (bench.py) --------------------------------------------------------------
  * tqc_plan_launch_count: kernels launched so far on behalf of this plan.

@@ -34,7 +34,9 @@ EXPORTED = ["tqc_plan", "tqc_plan_destroy", "tqc_plan_mode", "tqc_plan_num_qubit
             "tqc_plan_profile_enable", "tqc_plan_profile_read", "tqc_plan_chain_status", "tqc_hss_scores", "tqc_hss_select",
             "tqc_hss_expand", "tqc_plan_num_sliced_cuts", "tqc_choose_slice_cuts", "tqc_hss_prepare",
             "tqc_hss_workspace_bytes", "tqc_hss_contract", "tqc_simulate_workspace_bytes",
-            "tqc_simulate_subcircuit_tensor", "tqc_plan_finalize"]
+            "tqc_simulate_subcircuit_tensor", "tqc_plan_finalize", "tqc_plan_from_circuit", "tqc_plan_from_gates",
+            "tqc_plan_cut_network", "tqc_plan_cut_subcircuit", "tqc_plan_cut_assignment", "tqc_cut_merging_cost",
+            "tqc_plan_cost_report"]
 
 
 class TqcError(RuntimeError):
@@ -68,8 +70,23 @@ class _SubcircuitDesc(ctypes.Structure):
                 ("bond_pos", POINTER(c_int32)), ("walk_settings", c_int32), ("reserved", c_int32)]
 
 
+class _CutOpts(ctypes.Structure):
+    _fields_ = [("w_max", c_int32), ("s_max", c_int32), ("K_t", c_int32), ("reserved", c_int32), ("Q_max", c_double)]
+
+
+class _CostModel(ctypes.Structure):
+    _fields_ = [("t_g", c_double), ("t_m", c_double), ("flops", c_double), ("n_qpus", c_int32),
+                ("shots_log2_min", c_int32), ("shots_log2_max", c_int32), ("reserved", c_int32)]
+
+
+class _CostReport(ctypes.Structure):
+    _fields_ = [("t_qpu", c_double), ("t_classical", c_double), ("t_total", c_double), ("c_tn_flop", c_double),
+                ("qpu_variants", c_double)]
+
+
 GATE_KINDS = {"h": 0, "x": 1, "s": 2, "sdg": 3, "sx": 4, "sy": 5, "sw": 6, "rx": 7, "ry": 8, "rz": 9, "cz": 10, "cx": 11,
-              "rzz": 12}
+              "rzz": 12, "y": 13, "z": 14, "t": 15, "tdg": 16, "cp": 17}
+GATE_NAMES = {v: k for k, v in GATE_KINDS.items()}
 
 
 def lib_path() -> str:
@@ -123,6 +140,14 @@ def _load() -> ctypes.CDLL:
     lib.tqc_simulate_workspace_bytes.argtypes = [POINTER(_SubcircuitDesc)]
     lib.tqc_simulate_workspace_bytes.restype = c_size_t
     lib.tqc_simulate_subcircuit_tensor.argtypes = [POINTER(_SubcircuitDesc), c_void_p, c_void_p, c_size_t, c_void_p]
+    lib.tqc_plan_from_circuit.argtypes = [c_char_p, POINTER(_CutOpts), POINTER(_PlanOpts), POINTER(c_void_p)]
+    lib.tqc_plan_from_gates.argtypes = [c_int, POINTER(_Gate), c_int, POINTER(_CutOpts), POINTER(_PlanOpts), POINTER(c_void_p)]
+    lib.tqc_plan_cut_network.argtypes = [c_void_p, POINTER(_NetworkDesc)]
+    lib.tqc_plan_cut_subcircuit.argtypes = [c_void_p, c_int, POINTER(_SubcircuitDesc), POINTER(c_int32), POINTER(c_int32)]
+    lib.tqc_plan_cut_assignment.argtypes = [c_void_p, c_void_p, c_size_t]
+    lib.tqc_cut_merging_cost.argtypes = [c_int] * 6
+    lib.tqc_cut_merging_cost.restype = c_double
+    lib.tqc_plan_cost_report.argtypes = [c_void_p, POINTER(_CostModel), c_void_p, c_double, POINTER(_CostReport)]
     return lib
 
 
@@ -224,6 +249,51 @@ class Plan:
     def workspace_bytes_host(self, n_states: int = 0, prefix_bits: int = 0) -> int:
         return int(_lib.tqc_plan_workspace_bytes_host(self._h, n_states, prefix_bits))
 
+    # ---- plans made from a circuit (tqc_plan_from_circuit / tqc_plan_from_gates) ----------------
+    def cut_network(self):
+        """The cut network the partitioner produced: an object with n_qubits, cuts [(up, down)], sub_cuts, sub_qubits
+        (the attributes tqc_plan reads), plus m and K."""
+        from types import SimpleNamespace
+        d = _NetworkDesc()
+        _check(_lib.tqc_plan_cut_network(self._h, byref(d)))
+        cuts = [(int(d.cut_up[e]), int(d.cut_down[e])) for e in range(d.K)]
+        sub_cuts = [[int(d.sub_cuts[j]) for j in range(d.sub_cut_ofs[s], d.sub_cut_ofs[s + 1])] for s in range(d.m)]
+        sub_qubits = [[int(d.sub_qubits[j]) for j in range(d.sub_qubit_ofs[s], d.sub_qubit_ofs[s + 1])] for s in range(d.m)]
+        return SimpleNamespace(n_qubits=int(d.n_qubits), m=int(d.m), K=int(d.K), cuts=cuts, sub_cuts=sub_cuts,
+                               sub_qubits=sub_qubits)
+
+    def cut_subcircuit(self, s: int) -> dict:
+        """Subcircuit s in the argument form of tqc_simulate_subcircuit_tensor (w, gates, D_wires, U_wires, O_wires,
+        bond_pos) plus n2q (two-qubit gates) and depth (t_s)."""
+        d = _SubcircuitDesc()
+        n2q, depth = c_int32(), c_int32()
+        _check(_lib.tqc_plan_cut_subcircuit(self._h, s, byref(d), byref(n2q), byref(depth)))
+        gates = []
+        for t in range(d.n_gates):
+            g = d.gates[t]
+            name = GATE_NAMES[int(g.kind)]
+            two = name in ("cz", "cx", "rzz", "cp")
+            has_param = name in ("rx", "ry", "rz", "rzz", "cp")
+            gates.append((name, (float(g.param),) if has_param else (), (int(g.wire0), int(g.wire1)) if two else (int(g.wire0),)))
+        return dict(w=int(d.w), gates=gates, D_wires=[int(d.D_wires[i]) for i in range(d.d)],
+                    U_wires=[int(d.U_wires[i]) for i in range(d.u)], O_wires=[int(d.O_wires[i]) for i in range(d.o)],
+                    bond_pos=[int(d.bond_pos[i]) for i in range(d.d + d.u)], n2q=int(n2q.value), depth=int(depth.value))
+
+    def cut_assignment(self, n_gates: int):
+        out = np.zeros(max(1, n_gates), dtype=np.int32)
+        _check(_lib.tqc_plan_cut_assignment(self._h, out.ctypes.data, n_gates))
+        return [int(x) for x in out[:n_gates]]
+
+    def cost_report(self, flops: float, n_states: float = 1.0, depth=None, t_g: float = 0.0, t_m: float = 0.0,
+                    n_qpus: int = 0, shots_log2_min: int = 0, shots_log2_max: int = 0) -> dict:
+        """Eqs. 4-6 of the paper for this plan (include/tqc.h)."""
+        model = _CostModel(t_g, t_m, flops, n_qpus, shots_log2_min, shots_log2_max, 0)
+        rep = _CostReport()
+        darr = None if depth is None else np.ascontiguousarray(np.asarray(depth, dtype=np.int32))
+        _check(_lib.tqc_plan_cost_report(self._h, byref(model), None if darr is None else darr.ctypes.data, float(n_states),
+                                         byref(rep)))
+        return {k: float(getattr(rep, k)) for k in ("t_qpu", "t_classical", "t_total", "c_tn_flop", "qpu_variants")}
+
     def finalize(self, stream=None) -> None:
         """tqc_plan_finalize: device tables, specialised chain kernel, side streams (implicit at the last tensor load)."""
         _check(_lib.tqc_plan_finalize(self._h, _stream_ptr(stream)))
@@ -271,6 +341,59 @@ def tqc_plan(net, mode: int = MODE_STATES, order=None, restarts: int = 0, seed: 
     h = c_void_p()
     _check(_lib.tqc_plan(byref(desc), byref(opts), byref(h)))
     return Plan(h.value)
+
+
+def _gate_array(gates):
+    garr = (_Gate * max(1, len(gates)))()
+    for t, (name, params, wires) in enumerate(gates):
+        if name not in GATE_KINDS:
+            raise TqcError(-1, f"unknown gate {name}")
+        garr[t].kind = GATE_KINDS[name]
+        garr[t].wire0 = int(wires[0])
+        garr[t].wire1 = int(wires[1]) if len(wires) > 1 else 0
+        garr[t].param = float(params[0]) if len(params) else 0.0
+    return garr
+
+
+def circuit_text(n_qubits: int, gates) -> str:
+    """The circuit text tqc_plan_from_circuit parses: `qubits n`, then `<name>[(<angle>)] q0 [q1]` per gate."""
+    lines = [f"qubits {n_qubits}"]
+    for (name, params, wires) in gates:
+        arg = f"({float(params[0])!r})" if len(params) else ""
+        lines.append(f"{name}{arg} " + " ".join(str(int(q)) for q in wires))
+    return "\n".join(lines) + "\n"
+
+
+def _plan_opts_simple(mode, restarts, seed, batch_hint, table_log2_floats_max, use_tcgen05, use_chain, kmax_cap):
+    return _PlanOpts(mode, 0, None, restarts, seed, batch_hint, table_log2_floats_max, use_tcgen05, use_chain, 0, None, kmax_cap)
+
+
+def tqc_plan_from_circuit(text: str, w_max: int, s_max: int, K_t: int = 0, Q_max: float = 0.0, mode: int = MODE_STATES,
+                          restarts: int = 0, seed: int = 0, batch_hint: int = 0, table_log2_floats_max: int = 0,
+                          use_tcgen05: int = 0, use_chain: int = 0, kmax_cap: int = 0) -> Plan:
+    """Circuit text -> DAG -> Greedy Graph Growing partition under (w_max, s_max) -> cut network -> plan (section 6)."""
+    cut = _CutOpts(w_max, s_max, K_t, 0, Q_max)
+    opts = _plan_opts_simple(mode, restarts, seed, batch_hint, table_log2_floats_max, use_tcgen05, use_chain, kmax_cap)
+    h = c_void_p()
+    _check(_lib.tqc_plan_from_circuit(text.encode(), byref(cut), byref(opts), byref(h)))
+    return Plan(h.value)
+
+
+def tqc_plan_from_gates(n_qubits: int, gates, w_max: int, s_max: int, K_t: int = 0, Q_max: float = 0.0,
+                        mode: int = MODE_STATES, restarts: int = 0, seed: int = 0, batch_hint: int = 0,
+                        table_log2_floats_max: int = 0, use_tcgen05: int = 0, use_chain: int = 0, kmax_cap: int = 0) -> Plan:
+    """The same from a gate list [(name, params, qubits)]."""
+    garr = _gate_array(gates)
+    cut = _CutOpts(w_max, s_max, K_t, 0, Q_max)
+    opts = _plan_opts_simple(mode, restarts, seed, batch_hint, table_log2_floats_max, use_tcgen05, use_chain, kmax_cap)
+    h = c_void_p()
+    _check(_lib.tqc_plan_from_gates(n_qubits, garr, len(gates), byref(cut), byref(opts), byref(h)))
+    return Plan(h.value)
+
+
+def tqc_cut_merging_cost(w_trial: int, w_max: int, s_trial: int, s_max: int, K_trial: int, K_t: int) -> float:
+    """Table 1 of the paper; negative = not allowed."""
+    return float(_lib.tqc_cut_merging_cost(w_trial, w_max, s_trial, s_max, K_trial, K_t))
 
 
 def tqc_choose_slice_cuts(net, mode: int = MODE_STATES, max_log2_input_floats: int = 62,
@@ -415,14 +538,7 @@ def tqc_hss_contract(plan: Plan, x, out=None, workspace=None, stream=None, devic
 
 
 def _subcircuit_desc(w, gates, D_wires, U_wires, O_wires, bond_pos, fuse_gates=True, walk_settings=True):
-    garr = (_Gate * max(1, len(gates)))()
-    for t, (name, params, wires) in enumerate(gates):
-        if name not in GATE_KINDS:
-            raise TqcError(-1, f"unknown gate {name}")
-        garr[t].kind = GATE_KINDS[name]
-        garr[t].wire0 = int(wires[0])
-        garr[t].wire1 = int(wires[1]) if len(wires) > 1 else 0
-        garr[t].param = float(params[0]) if len(params) else 0.0
+    garr = _gate_array(gates)
     keep = [garr] + [_i32(v) for v in (D_wires, U_wires, O_wires, bond_pos)]
     desc = _SubcircuitDesc(int(w), len(gates), garr, len(D_wires), len(U_wires), len(O_wires), 1 if fuse_gates else 0,
                            *[ptr for (_arr, ptr) in keep[1:]], 1 if walk_settings else 0, 0)

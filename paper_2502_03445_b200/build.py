@@ -7,7 +7,7 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libtqc.so")
-SOURCES = ["tqc_api.cu", "plan.cpp"]
+SOURCES = ["tqc_api.cu", "plan.cpp", "partition.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-ldl"]
 
@@ -21,7 +21,21 @@ def _stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
+PEAKS_LIB = os.path.join(_HERE, "libtqc_peaks.so")
+
+
+def build_peaks(force: bool = False) -> str:
+    """The measurement micro-benchmarks (csrc/peaks.cu -> libtqc_peaks.so); not loaded by the product path."""
+    src = os.path.join(CSRC, "peaks.cu")
+    if force or not os.path.exists(PEAKS_LIB) or os.path.getmtime(src) > os.path.getmtime(PEAKS_LIB):
+        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+        subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
+                               "-Xcompiler", "-fPIC", "-shared", "-o", PEAKS_LIB, src])
+    return PEAKS_LIB
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
+    build_peaks(force)
     if force or _stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
         develop = ["-DTQC_DEVELOP"] if os.environ.get("TQC_DEVELOP") else []     # measurement switches (DESIGN.md 5.1)

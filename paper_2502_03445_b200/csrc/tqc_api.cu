@@ -23,6 +23,7 @@
 #include "kernels_cross.cuh"
 #include "kernels_sim.cuh"
 #include "plan.hpp"
+#include "partition.hpp"
 
 namespace {
 
@@ -126,6 +127,8 @@ struct tqc_plan {
     // carries ceil(log2 |x_j|) virtual output bits (tqc_hss_prepare / tqc_hss_contract)
     tqc_plan *hss_sub = nullptr;
     std::vector<int32_t> hss_counts;
+    // plans made by tqc_plan_from_circuit / _gates keep the cut description (partition, network, subcircuits)
+    tqc::CutResult *cut = nullptr;
 };
 
 namespace {
@@ -1063,6 +1066,7 @@ void tqc_plan_destroy(tqc_plan_t *pl) {
     if (pl->jit_module && jit_api().ok) jit_api().ModuleUnload((CUmodule)pl->jit_module);
     for (cudaEvent_t e : pl->ev_pool) cudaEventDestroy(e);
     if (pl->hss_sub) tqc_plan_destroy(pl->hss_sub);
+    delete pl->cut;
     if (pl->ev_fork) cudaEventDestroy(pl->ev_fork);
     for (int l = 0; l < tqc_plan::N_LANES; ++l) {
         if (pl->ev_join[l]) cudaEventDestroy(pl->ev_join[l]);
@@ -1776,6 +1780,10 @@ bool sim_gate_matrix(int kind, double t, tqc::SimGate &g) {
     switch (kind) {
     case TQC_GATE_H: m = {{r, 0}, {r, 0}, {r, 0}, {-r, 0}}; break;
     case TQC_GATE_X: m = {{0, 0}, {1, 0}, {1, 0}, {0, 0}}; break;
+    case TQC_GATE_Y: m = {{0, 0}, {0, -1}, {0, 1}, {0, 0}}; break;
+    case TQC_GATE_Z: m = {{1, 0}, {0, 0}, {0, 0}, {-1, 0}}; break;
+    case TQC_GATE_T: m = {{1, 0}, {0, 0}, {0, 0}, {r, r}}; break;             // e^{i pi/4}
+    case TQC_GATE_TDG: m = {{1, 0}, {0, 0}, {0, 0}, {r, -r}}; break;
     case TQC_GATE_S: m = {{1, 0}, {0, 0}, {0, 0}, {0, 1}}; break;
     case TQC_GATE_SDG: m = {{1, 0}, {0, 0}, {0, 0}, {0, -1}}; break;
     // exp(-i pi/4 P) = (I - iP)/sqrt2 for P = X, Y, W = (X + Y)/sqrt2 (reading G11)
@@ -1792,6 +1800,10 @@ bool sim_gate_matrix(int kind, double t, tqc::SimGate &g) {
     case TQC_GATE_CX:                                                   // control = first operand
         m.assign(16, cplx(0, 0));
         m[0] = m[5] = m[11] = m[14] = cplx(1, 0);
+        break;
+    case TQC_GATE_CP:                                                   // controlled phase: |11> picks up e^{it}
+        m.assign(16, cplx(0, 0));
+        m[0] = m[5] = m[10] = cplx(1, 0); m[15] = cplx(std::cos(t), std::sin(t));
         break;
     case TQC_GATE_RZZ: {                                                // exp(-i t Z(x)Z): diag e^{-it}, e^{it}, e^{it}, e^{-it}
         m.assign(16, cplx(0, 0));
@@ -1965,6 +1977,141 @@ int tqc_simulate_subcircuit_tensor(const tqc_subcircuit_desc *sub, float *out_de
     const unsigned blocks = (unsigned)std::min<size_t>((total + 255) / 256, 148 * 16);
     tqc::sim_permute_cast_kernel<<<blocks, 256, 0, st>>>(a.R, out_dev, pa, total);
     TQC_CUDA(cudaGetLastError());
+    return 0;
+}
+
+// ---- front half: circuit -> partition -> cuts -> network -> plan (section 6) ----------------------------------------
+namespace {
+int plan_from_gate_list(int n_qubits, const std::vector<tqc::CircuitGate> &gates, const tqc_cut_opts *cut, const tqc_plan_opts *opts,
+                        tqc_plan_t **out) {
+    if (!cut || !out) return fail(TQC_E_ARG, "null argument");
+    if (n_qubits < 1) return fail(TQC_E_ARG, "n_qubits must be positive");
+    if (opts && (opts->n_order_steps > 0 || opts->n_slice_cuts > 0))
+        return fail(TQC_E_ARG, "order / slice_cuts name nodes and cuts of a network that does not exist yet: leave them empty");
+    tqc::CutOptions co;
+    co.w_max = cut->w_max; co.s_max = cut->s_max;
+    co.K_t = cut->K_t > 0 ? cut->K_t : 10;
+    co.Q_max = cut->Q_max > 0 ? cut->Q_max : 1e4;
+    std::string err;
+    std::vector<int> part;
+    int merges = 0;
+    int rc = tqc::greedy_graph_growing(n_qubits, gates, co, part, &merges, err);
+    if (rc) return fail(rc, err);
+    tqc::CutResult *cr = new tqc::CutResult();
+    rc = tqc::extract_subcircuits(n_qubits, gates, part, *cr, err);
+    if (rc) { delete cr; return fail(rc, err); }
+    cr->merges = merges;
+    tqc_network_desc net;
+    net.n_qubits = cr->n; net.m = cr->m; net.K = cr->K;
+    net.cut_up = cr->cut_up.data(); net.cut_down = cr->cut_down.data();
+    net.sub_cut_ofs = cr->sub_cut_ofs.data(); net.sub_cuts = cr->sub_cuts.data();
+    net.sub_qubit_ofs = cr->sub_qubit_ofs.data(); net.sub_qubits = cr->sub_qubits.data();
+    tqc_plan_t *pl = nullptr;
+    rc = tqc_plan(&net, opts, &pl);
+    if (rc) { delete cr; return rc; }
+    pl->cut = cr;
+    *out = pl;
+    return 0;
+}
+}  // namespace
+
+int tqc_plan_from_circuit(const char *circuit_text, const tqc_cut_opts *cut, const tqc_plan_opts *opts, tqc_plan_t **out) {
+    int n = 0;
+    std::vector<tqc::CircuitGate> gates;
+    std::string err;
+    const int rc = tqc::parse_circuit_text(circuit_text, n, gates, err);
+    if (rc) return fail(rc, err);
+    return plan_from_gate_list(n, gates, cut, opts, out);
+}
+
+int tqc_plan_from_gates(int n_qubits, const tqc_gate *gates, int n_gates, const tqc_cut_opts *cut, const tqc_plan_opts *opts,
+                        tqc_plan_t **out) {
+    if (n_gates < 0 || (n_gates > 0 && !gates)) return fail(TQC_E_ARG, "null gate list");
+    std::vector<tqc::CircuitGate> gl((size_t)n_gates);
+    for (int i = 0; i < n_gates; ++i) {
+        const tqc_gate &g = gates[i];
+        if (std::string(tqc::gate_name(g.kind)) == "?") return fail(TQC_E_ARG, "gate " + std::to_string(i) + ": unknown kind " + std::to_string(g.kind));
+        gl[i].kind = g.kind; gl[i].param = g.param; gl[i].two = tqc::gate_is_two_qubit(g.kind);
+        gl[i].q0 = g.wire0; gl[i].q1 = gl[i].two ? g.wire1 : 0;
+        if (g.wire0 < 0 || g.wire0 >= n_qubits || (gl[i].two && (g.wire1 < 0 || g.wire1 >= n_qubits || g.wire1 == g.wire0)))
+            return fail(TQC_E_ARG, "gate " + std::to_string(i) + ": qubit out of range or duplicate operand");
+    }
+    return plan_from_gate_list(n_qubits, gl, cut, opts, out);
+}
+
+int tqc_plan_cut_network(const tqc_plan_t *pl, tqc_network_desc *net) {
+    if (!pl || !net) return fail(TQC_E_ARG, "null argument");
+    if (!pl->cut) return fail(TQC_E_STATE, "plan was not made from a circuit");
+    const tqc::CutResult &cr = *pl->cut;
+    net->n_qubits = cr.n; net->m = cr.m; net->K = cr.K;
+    net->cut_up = cr.cut_up.data(); net->cut_down = cr.cut_down.data();
+    net->sub_cut_ofs = cr.sub_cut_ofs.data(); net->sub_cuts = cr.sub_cuts.data();
+    net->sub_qubit_ofs = cr.sub_qubit_ofs.data(); net->sub_qubits = cr.sub_qubits.data();
+    return 0;
+}
+
+int tqc_plan_cut_subcircuit(const tqc_plan_t *pl, int s, tqc_subcircuit_desc *sub, int32_t *n2q, int32_t *depth) {
+    if (!pl || !sub) return fail(TQC_E_ARG, "null argument");
+    if (!pl->cut) return fail(TQC_E_STATE, "plan was not made from a circuit");
+    if (s < 0 || s >= pl->cut->m) return fail(TQC_E_ARG, "subcircuit id out of range");
+    const tqc::SubcircuitOut &so = pl->cut->subs[s];
+    memset(sub, 0, sizeof(*sub));
+    sub->w = so.w; sub->n_gates = (int32_t)so.gates.size(); sub->gates = so.gates.data();
+    sub->d = (int32_t)so.D_wires.size(); sub->u = (int32_t)so.U_wires.size(); sub->o = (int32_t)so.O_wires.size();
+    sub->fuse_gates = 1; sub->walk_settings = 1;
+    sub->D_wires = so.D_wires.data(); sub->U_wires = so.U_wires.data(); sub->O_wires = so.O_wires.data();
+    sub->bond_pos = so.bond_pos.data();
+    if (n2q) *n2q = so.n2q;
+    if (depth) *depth = so.depth;
+    return 0;
+}
+
+int tqc_plan_cut_assignment(const tqc_plan_t *pl, int32_t *part_of_gate, size_t n_gates) {
+    if (!pl || (!part_of_gate && n_gates)) return fail(TQC_E_ARG, "null argument");
+    if (!pl->cut) return fail(TQC_E_STATE, "plan was not made from a circuit");
+    if (n_gates != pl->cut->part_of_gate.size()) return fail(TQC_E_ARG, "n_gates must be " + std::to_string(pl->cut->part_of_gate.size()));
+    std::copy(pl->cut->part_of_gate.begin(), pl->cut->part_of_gate.end(), part_of_gate);
+    return 0;
+}
+
+double tqc_cut_merging_cost(int w_trial, int w_max, int s_trial, int s_max, int K_trial, int K_t) {
+    if (w_max < 1 || s_max < 1 || K_t < 1) return -1.0;
+    return tqc::merging_cost(w_trial, w_max, s_trial, s_max, K_trial, K_t);
+}
+
+// ---- hybrid cost model (section 5, Eqs. 4-6) --------------------------------------------------------------------
+int tqc_plan_cost_report(const tqc_plan_t *pl, const tqc_cost_model *model, const int32_t *depth, double n_states, tqc_cost_report *out) {
+    if (!pl || !model || !out) return fail(TQC_E_ARG, "null argument");
+    if (!(model->flops > 0)) return fail(TQC_E_ARG, "model.flops (floating point operations per second of the classical backend) must be given");
+    if (!depth && !pl->cut) return fail(TQC_E_ARG, "depth is needed for a plan that was not made from a circuit");
+    const double t_g = model->t_g > 0 ? model->t_g : 1e-7, t_m = model->t_m > 0 ? model->t_m : 1e-6;
+    const int n_qpus = model->n_qpus > 0 ? model->n_qpus : 10;
+    const int lo = model->shots_log2_min > 0 ? model->shots_log2_min : 10, hi = model->shots_log2_max > 0 ? model->shots_log2_max : 20;
+    if (lo > hi) return fail(TQC_E_ARG, "shots_log2_min > shots_log2_max");
+    const HostPlan &hp = pl->hp;
+    std::vector<int> dn(hp.m, 0), up(hp.m, 0);                      // over the caller's network, sliced cuts included
+    for (int s = 0; s < hp.m; ++s) dn[s] = hp.d[s] + (pl->n_sliced() ? pl->d_extra[s] : 0);
+    for (int s = 0; s < hp.m; ++s) up[s] = (pl->n_sliced() ? pl->c_full[s] : hp.c(s)) - dn[s];
+    double t_qpu = 0, variants = 0;
+    for (int s = 0; s < hp.m; ++s) {
+        const int w = up[s] + hp.o(s);                               // every wire ends at an upstream cut or at an output
+        const int t_i = depth ? depth[s] : pl->cut->subs[s].depth;
+        if (t_i < 0) return fail(TQC_E_ARG, "negative depth");
+        const double v = std::pow(3.0, up[s]) * std::pow(4.0, dn[s]);
+        const double shots = std::ldexp(1.0, std::min(std::max(w, lo), hi));
+        variants += v;
+        t_qpu += v * shots * ((double)t_i * t_g + t_m);
+    }
+    t_qpu /= (double)n_qpus;
+    double mults = 0;
+    for (const Step &st : hp.steps) mults += std::ldexp(1.0, st.log2cost);
+    mults *= std::ldexp(1.0, 2 * pl->n_sliced());                    // every sub-network of a sliced plan is contracted
+    if (hp.mode == TQC_MODE_STATES) mults *= n_states > 0 ? n_states : 1.0;
+    out->c_tn_flop = 2.0 * mults;
+    out->t_qpu = t_qpu;
+    out->t_classical = out->c_tn_flop / model->flops;
+    out->t_total = out->t_qpu + out->t_classical;
+    out->qpu_variants = variants;
     return 0;
 }
 

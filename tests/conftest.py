@@ -14,6 +14,11 @@ def pytest_configure(config):
 
 
 def pytest_collection_modifyitems(config, items):
+    if "slow" not in (config.getoption("-m") or ""):
+        skip_slow = pytest.mark.skip(reason="opt-in: select with -m 'gpu and slow' (or -m slow)")
+        for item in items:
+            if "slow" in item.keywords:
+                item.add_marker(skip_slow)
     try:
         import torch
         has_gpu = torch.cuda.is_available()

@@ -85,22 +85,41 @@ def random_tensors(net: Network, seed: int) -> list:
 _DYADIC = np.array([0.5, 0.75, 1.0, 1.5], dtype=np.float64)
 
 
-def rank_one_tensors(net: Network, seed: int):
+def rank_one_tensors(net: Network, seed: int, signed: bool = False):
     """Factor vectors for the rank-one closed-form pin.
 
     Returns (tensors, g, a): g[s] is a length-2^{o_s} vector, a[(s, e)] a
     length-4 vector, all entries drawn from {0.5, 0.75, 1, 1.5} (two significant
     bits) so that T_s[k, x] = g_s[x] * prod_e a_{s,e}[k_e] is EXACT in fp32 for
     c_s <= 10.  The tensors are the plain outer products; the closed form that
-    uses g and a lives with the oracle.
+    uses g and a lives with the oracle.  signed = True: every factor vector and
+    every g entry gets a random overall sign (results of both signs, no
+    cancellation), and on every eighth cut ONE entry of the downstream vector is
+    flipped - the one with the smallest product - so that those bond sums cancel
+    partially with a bounded condition number (sum |terms| / |sum| <= 2).  Fully
+    random entry signs would make the value 10^60 times smaller than its terms at
+    cfg5 size: any fp32 evaluation, FFMA or tensor pipe alike, then loses three
+    more digits, which is a property of the data, not of a kernel.
     """
     rng = np.random.default_rng(seed)
-    g, a, tensors = [], {}, []
+    g, a = [], {}
     for s in range(net.m):
         g.append(_DYADIC[rng.integers(0, 4, size=2 ** net.o(s))])
+        for e in net.sub_cuts[s]:
+            a[(s, e)] = _DYADIC[rng.integers(0, 4, size=4)]
+    if signed:
+        for s in range(net.m):
+            g[s] = g[s] * rng.choice([-1.0, 1.0], size=g[s].shape)
+            for e in net.sub_cuts[s]:
+                a[(s, e)] = a[(s, e)] * float(rng.choice([-1.0, 1.0]))
+        for e, (up, down) in enumerate(net.cuts):
+            if e % 8 == 0:
+                k = int(np.argmin(np.abs(a[(up, e)] * a[(down, e)])))
+                a[(down, e)][k] = -a[(down, e)][k]
+    tensors = []
+    for s in range(net.m):
         row = np.ones(1, dtype=np.float64)
         for e in net.sub_cuts[s]:          # first listed cut = most significant digit
-            a[(s, e)] = _DYADIC[rng.integers(0, 4, size=4)]
             row = np.multiply.outer(row, a[(s, e)]).reshape(-1)
         t = np.multiply.outer(row, g[s])
         t32 = t.astype(np.float32)
