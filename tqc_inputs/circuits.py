@@ -306,3 +306,21 @@ def aqft_circuit(n: int, degree: int | None = None, seed: int | None = None) -> 
             if k <= degree:
                 gates.append(("cp", (float(np.pi / 2 ** k),), (j + k, j)))
     return Circuit(n, gates, name=f"aqft{n}")
+
+
+def qaoa_graph_circuit(n: int, kind: str, seed: int) -> Circuit:
+    """The paper's Regular / Erdos benchmarks: one QAOA layer on a seeded random 3-regular graph ("regular") or
+    G(n, 1/2) graph ("erdos"): h on all, rzz(gamma) per edge in ascending (min, max) order, rx(2 beta) on all; gamma, beta
+    seeded in [0, pi) (reading G13)."""
+    rng = np.random.default_rng(seed)
+    if kind == "regular":
+        edges = random_regular_graph(n, 3, rng)
+    elif kind == "erdos":
+        edges = [(a, b) for a in range(n) for b in range(a + 1, n) if rng.random() < 0.5]
+    else:
+        raise ValueError(kind)
+    gamma, beta = (float(x) for x in rng.random(2) * np.pi)
+    gates = [("h", (), (q,)) for q in range(n)]
+    gates += [("rzz", (gamma,), (a, b)) for (a, b) in sorted(edges)]
+    gates += [("rx", (2.0 * beta,), (q,)) for q in range(n)]
+    return Circuit(n, gates, name=f"qaoa-{kind}{n}", meta={"edges": sorted(edges)})
