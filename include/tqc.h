@@ -64,6 +64,8 @@ enum { TQC_MODE_STATES = 0, TQC_MODE_DISTRIBUTION = 1 };
  * CHAIN      the step is part of the fused small-bond chain: all per-state steps of the plan run in one kernel, one
  *            warp per state, intermediates in shared memory, bond sums finished by warp shuffles. */
 enum { TQC_KERNEL_SIMT_TILE = 0, TQC_KERNEL_DOT = 1, TQC_KERNEL_TCGEN05 = 2, TQC_KERNEL_CHAIN = 3 };
+/* TCGEN05 steps with both outer dimensions >= 256 run step_tc2_kernel: 256 x 256 tiles over CTA pairs (cta_group::2), which
+ * halve the operand bytes per flop; the others run the one-CTA kernels step_tc_kernel<BN> / step_tcw_kernel. */
 /* How a node of the contraction tree is evaluated. */
 enum { TQC_NODE_LEAF = 0, TQC_NODE_TABLE = 1, TQC_NODE_BATCH = 2 };
 
@@ -331,6 +333,8 @@ int tqc_plan_cost_report(const tqc_plan_t *plan, const tqc_cost_model *model, co
  * order, its tag (plan step index t >= 0; -1 key extraction; -2 root gather) and the time to the
  * next event in ms.  Call with tags = NULL to get the count in *n.  HOST arrays. */
 uint64_t tqc_plan_launch_count(const tqc_plan_t *plan);
+/* of those, launches of step_tc2_kernel (tcgen05 cta_group::2 tiles over CTA pairs, csrc/kernels_tc2.cuh) */
+uint64_t tqc_plan_pair_launch_count(const tqc_plan_t *plan);
 /* 0: the plan does not use the fused chain kernel; 1: it runs the generic (table-driven) chain kernel; 2: it runs the chain
  * kernel specialised for this plan (the library generates the plan's steps as straight-line CUDA from its own templates
  * in csrc/kernels_chain.cuh and compiles them with NVRTC at the first contract call; if NVRTC is not available the

@@ -36,7 +36,7 @@ EXPORTED = ["tqc_plan", "tqc_plan_destroy", "tqc_plan_mode", "tqc_plan_num_qubit
             "tqc_hss_workspace_bytes", "tqc_hss_contract", "tqc_simulate_workspace_bytes",
             "tqc_simulate_subcircuit_tensor", "tqc_plan_finalize", "tqc_plan_from_circuit", "tqc_plan_from_gates",
             "tqc_plan_cut_network", "tqc_plan_cut_subcircuit", "tqc_plan_cut_assignment", "tqc_cut_merging_cost",
-            "tqc_plan_cost_report"]
+            "tqc_plan_cost_report", "tqc_plan_pair_launch_count"]
 
 
 class TqcError(RuntimeError):
@@ -123,6 +123,8 @@ def _load() -> ctypes.CDLL:
     lib.tqc_contract_distribution.argtypes = [c_void_p, c_uint64, c_int, c_void_p, c_void_p, c_size_t, c_void_p]
     lib.tqc_plan_launch_count.argtypes = [c_void_p]
     lib.tqc_plan_launch_count.restype = c_uint64
+    lib.tqc_plan_pair_launch_count.argtypes = [c_void_p]
+    lib.tqc_plan_pair_launch_count.restype = c_uint64
     lib.tqc_plan_workspace_bytes_host.argtypes = [c_void_p, c_size_t, c_int]
     lib.tqc_plan_workspace_bytes_host.restype = c_size_t
     lib.tqc_contract_states_host.argtypes = [c_void_p, c_void_p, c_size_t, c_void_p, c_void_p, c_size_t, c_void_p]
@@ -213,6 +215,8 @@ class Plan:
     def cost_log2(self) -> float: return _lib.tqc_plan_cost_log2(self._h)
     @property
     def launch_count(self) -> int: return int(_lib.tqc_plan_launch_count(self._h))
+    @property
+    def pair_launch_count(self) -> int: return int(_lib.tqc_plan_pair_launch_count(self._h))
 
     def tensor_shape(self, s: int):
         c, o = c_int(), c_int()

@@ -46,6 +46,7 @@ struct TcArgs {
     int mask_hi;                    // hi = TF32 value nearest to x, written back in place (else: x itself, truncated by the MMA)
     int vec4;                       // 4 consecutive j are contiguous in C
     int chunk_kb;                   // k-blocks per hi*hi drain (0: TC_CHUNK_KB)
+    unsigned long long *trace;      // develop builds: clock64 stamps of the first k-blocks of cluster 0 (kernels_tc2.cuh)
     int debug;                      // development knobs (TQC_TC_DEBUG): 1 no global stores, 2 no store phase, 4 no split, 8 no drains
 };
 
@@ -559,7 +560,8 @@ step_tcw_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
                 const uint32_t d_tmem = tmem_base + db * (uint32_t)TCW_BN;
                 const uint64_t dah = umma_desc_sw128(smem_u32(A_raw(s))), dal = umma_desc_sw128(smem_u32(A_lo(s)));
                 const uint64_t dbh = umma_desc_sw128(smem_u32(B_raw(s))), dbl = umma_desc_sw128(smem_u32(B_lo(s)));
-                if (lane == 0) {
+                if (lane == 0 && TQC_DBG(a, 32)) { umma_commit(&empty_bar[s]); umma_commit(&d_full_bar[db]); }
+                else if (lane == 0) {
                     // the small terms first: while the accumulator holds only lo products (2^-11 of the final value) its
                     // round-toward-zero steps are 2^-11 smaller too; only the four hi*hi accumulations see a full-size sum
 #pragma unroll
@@ -584,10 +586,12 @@ step_tcw_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
                 const uint32_t ph = (uint32_t)((it / TCW_STAGES) & 1);
                 mbar_wait(&full_bar[s], ph);
                 const uint32_t sa = smem_u32(A_raw(s)) + (uint32_t)st * 16u;
+                if (!TQC_DBG(a, 4)) {
 #pragma unroll
                 for (int c = 0; c < (int)(bytesA >> 4) / 64 / 8; ++c) split_tile_n<8, 64>(sa + (uint32_t)c * 8u * 64u * 16u, bytesA, a.mask_hi != 0);
 #pragma unroll
                 for (int c = 0; c < (int)(bytesB >> 4) / 64 / 8; ++c) split_tile_n<8, 64>(sa + 2u * bytesA + (uint32_t)c * 8u * 64u * 16u, bytesB, a.mask_hi != 0);
+                }
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&ready_bar[s]);
@@ -607,6 +611,7 @@ step_tcw_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
                 mbar_wait(&d_full_bar[db], dph);
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                 const uint32_t taddr = tmem_base + lane_base + db * (uint32_t)TCW_BN;
+                if (!TQC_DBG(a, 8))
 #pragma unroll
                 for (int c0 = 0; c0 < 64; c0 += 8) {
                     uint32_t v[8];
@@ -620,6 +625,7 @@ step_tcw_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
                 if (lane == 0) mbar_arrive(&d_empty_bar[db]);
             }
             float *crow = a.C + r * a.c_row_stride + (oa_mt[mt] | oa_q[w4] | ob_nt[nt]) + bitmap_apply_small(a.outA, (unsigned)lane);
+            if (TQC_DBG(a, 2)) continue;
             if (a.vec4) {
 #pragma unroll
                 for (int q = 0; q < 64; q += 4)

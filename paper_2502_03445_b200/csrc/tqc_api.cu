@@ -19,6 +19,7 @@
 #include "device_args.h"
 #include "kernels_simt.cuh"
 #include "kernels_tc.cuh"
+#include "kernels_tc2.cuh"
 #include "kernels_chain.cuh"
 #include "kernels_cross.cuh"
 #include "kernels_sim.cuh"
@@ -101,7 +102,7 @@ struct tqc_plan {
     int32_t *d_slot_ofs = nullptr, *d_slot_qubits = nullptr;
     float *d_staging = nullptr;
     size_t staging_elems = 0;
-    uint64_t launches = 0;
+    uint64_t launches = 0, pair_launches = 0;      // all kernels / step_tc2_kernel (CTA-pair tensor-pipe steps)
     bool finalized = false;            // tqc_plan_finalize has run (device tables, specialised chain kernel, side streams)
     int sm_count = 0;
     // optional per-launch timing (tqc_plan_profile_*): one event before each launch + one at the end
@@ -192,6 +193,7 @@ int ensure_device_attrs(int *sm_count) {
         TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc_kernel<64>, dyn, 201 * 1024));
         TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc_kernel<128>, dyn, 201 * 1024));
         TQC_CUDA(cudaFuncSetAttribute(tqc::step_tcw_kernel, dyn, 194 * 1024));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc2_kernel<256>, dyn, 194 * 1024));
         TQC_CUDA(cudaFuncSetAttribute(tqc::chain_kernel, dyn, 128 * 1024));
         TQC_CUDA(cudaFuncSetAttribute(tqc::sim_variant_kernel, dyn, 24 << 13));
         TQC_CUDA(cudaFuncSetAttribute(tqc::sim_variant_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
@@ -427,6 +429,47 @@ int launch_tc_step(tqc_plan_t *pl, TcOperand A, TcOperand B, BitMap outA, BitMap
                    long long c_row_stride, int R, int tag, cudaStream_t st) {
     const int sm_count = pl->sm_count > 0 ? pl->sm_count : 148;
     auto has_bit0 = [](const BitMap &m) { for (int s = 0; s < m.n; ++s) if (m.dst[s] == 0) return true; return false; };
+    // CTA-pair kernel (kernels_tc2.cuh): 256 x BN tiles over two SMs.  The M side needs >= 256 rows, the N side >= 128; with
+    // both orientations possible the N side is the operand that owns C's lowest offset bit (8-byte stores from registers).
+    static const bool no_pair = dev_env("TQC_TC_NO_PAIR") != nullptr;
+    {
+        // (64-column pair tiles were tried: a k-block then holds 384 cycles of MMAs against about 1800 cycles of fixed pipeline
+        // hand-shake per k-block, no gain over step_tc_kernel<64>; those steps are bound by streaming their 16 MB operand)
+        const bool keep_ok = lgM >= 8 && lgN >= 8, swap_ok = keep_ok;          // outer dimensions are powers of four
+        if (!no_pair && lgK >= 5 && (keep_ok || swap_ok)) {
+            bool sw = !keep_ok;
+            if (keep_ok && swap_ok) sw = has_bit0(outA);
+            if (sw) { std::swap(A, B); std::swap(outA, outB); std::swap(lgM, lgN); }
+            tqc::TcArgs a;
+            memset(&a, 0, sizeof(a));
+            a.keysA = A.keys; a.keysB = B.keys;
+            a.C = C; a.c_row_stride = c_row_stride;
+            a.outA = outA; a.outB = outB;
+            a.lgM = lgM; a.lgN = lgN; a.lgK = lgK; a.R = R;
+            a.BN = 256;
+            { const char *dbg = dev_env("TQC_TC_DEBUG"); a.debug = dbg ? std::atoi(dbg) : 0; }
+            a.mask_hi = 1;
+            if (const char *tp = dev_env("TQC_TC_TRACE_PTR")) a.trace = (unsigned long long *)std::strtoull(tp, nullptr, 0);
+            a.vec4 = (outB.n >= 1 && outB.src[0] == 0 && outB.dst[0] == 0) ? 1 : 0;      // columns j, j + 1 adjacent in C
+            const size_t stage_bytes = 2 * (size_t)128 * tqc::TC_BK * 4 + 2 * (size_t)(a.BN / 2) * tqc::TC_BK * 4;
+            a.stages = (int)std::min<size_t>(6, (192 * 1024) / stage_bytes);
+            if (const char *sv = dev_env("TQC_TC_STAGES")) a.stages = std::max(2, std::min(a.stages, std::atoi(sv)));
+            CUtensorMap mapA, mapB;
+            int rc;
+            if ((rc = make_operand_map(&mapA, A.base, lgK, lgM, A.n_outer, 128))) return rc;
+            if ((rc = make_operand_map(&mapB, B.base, lgK, lgN, B.n_outer, a.BN / 2))) return rc;
+            const long long total = (1ll << (lgM - 8)) * ((1ll << lgN) / a.BN) * (long long)R;
+            const unsigned grid = 2u * (unsigned)std::min<long long>(total, sm_count / 2);
+            if (dev_env("TQC_TC_TRACE"))
+                fprintf(stderr, "tc2 step %d: lgM %d lgN %d lgK %d swap %d BN %d vec2 %d R %d stages %d\n", tag, lgM, lgN, lgK, (int)sw, a.BN, a.vec4, R, a.stages);
+            if ((rc = note_launch(pl, tag, st))) return rc;
+            const size_t smem = a.stages * stage_bytes + 1024;
+            pl->pair_launches++;
+            tqc::step_tc2_kernel<256><<<grid, tqc::tc2_threads(256), smem, st>>>(mapA, mapB, a);
+            TQC_CUDA(cudaGetLastError());
+            return 0;
+        }
+    }
     // the M side needs >= 128 rows; with both sides large, the N side (vector stores run along it) takes C's lowest bits
     bool swap = lgM < 7;
     if (lgM >= 7 && lgN >= 7 && has_bit0(outA)) swap = true;
@@ -1757,6 +1800,7 @@ int tqc_hss_contract(tqc_plan_t *pl, float *out_dev, void *workspace_dev, size_t
 }
 
 uint64_t tqc_plan_launch_count(const tqc_plan_t *pl) { return pl ? pl->launches : 0; }
+uint64_t tqc_plan_pair_launch_count(const tqc_plan_t *pl) { return pl ? pl->pair_launches : 0; }
 
 int tqc_plan_chain_status(const tqc_plan_t *pl, char *note, size_t note_len) {
     if (!pl) return fail(TQC_E_ARG, "null plan");

@@ -63,6 +63,42 @@ def test_tc_step_leaf_times_leaf(na, nb, ni, B):
     assert np.abs(got - ffma).max() / want.max() <= 3e-6
 
 
+def _owned(pattern, ni, oa=1, ob=1, od=1):
+    """A-B share ni cuts (the bond); the cuts to D are owned by A ('a') or B ('b') in ascending id order, which is the digit
+    order of the result (last = lowest): the pattern decides which operand owns C's lowest offset bits."""
+    cuts = [(0, 1)] * ni + [((0, 2) if ch == "a" else (1, 2)) for ch in pattern]
+    ida = [ni + i for i, ch in enumerate(pattern) if ch == "a"]
+    idb = [ni + i for i, ch in enumerate(pattern) if ch == "b"]
+    net = Network(oa + ob + od, cuts, [list(range(ni)) + ida, list(range(ni)) + idb, ida + idb],
+                  [list(range(oa)), list(range(oa, oa + ob)), list(range(oa + ob, oa + ob + od))], name="owned-" + pattern)
+    net.validate()
+    return net
+
+
+@pytest.mark.parametrize("pattern,ni,B,signed", [("aaaabbbb", 3, 37, False),      # B owns the low digits: 8-byte stores
+                                                 ("bbbbaaaa", 3, 21, True),       # A owns them: operands swapped by the launcher
+                                                 ("abababab", 4, 18, True),       # interleaved digits
+                                                 ("aaaaabbbb", 3, 5, False),      # M = 1024: several pair tiles per state
+                                                 ("aaaabbbbb", 5, 3, False)])     # N = 1024, K = 1024 (32 k-blocks per tile)
+def test_pair_kernel_cta_group_2(pattern, ni, B, signed):
+    """step_tc2_kernel (tcgen05 cta_group::2, 256 x 256 tiles over two SMs): both outer dimensions >= 256.  Ragged tile
+    counts against the 74 clusters, both store orientations, signed values; against the float64 per-state contraction O8'
+    and against the same plan on the FFMA kernels."""
+    from oracle import reconstruct as R
+    net = _owned(pattern, ni)
+    rng = np.random.default_rng(len(pattern) * 10 + ni)
+    T = [(rng.random(net.tensor_shape(s)) * (2 if signed else 1) - (1 if signed else 0)).astype(np.float32) for s in range(net.m)]
+    bits = random_states(net.n_qubits, B, 11)
+    got, plan = _run(net, T, bits, order=[(0, 1), (3, 2)], batch_hint=4)
+    assert plan.step(0)["kernel_class"] == KERNEL_TCGEN05 and plan.pair_launch_count >= 1
+    want = R.contract_states_tensordot(net, T, bits)
+    scale = np.abs(want).max()
+    assert np.abs(got - want).max() <= TOL * scale, np.abs(got - want).max() / scale
+    ffma, plan2 = _run(net, T, bits, order=[(0, 1), (3, 2)], batch_hint=4, use_tcgen05=-1)
+    assert plan2.pair_launch_count == 0
+    assert np.abs(got - ffma).max() <= TOL * scale
+
+
 def test_tc_step_with_batch_operand_and_signed_values():
     """4 subcircuits: (A,B) first (FFMA, small), then (AB, C) as a tensor-pipe step whose lhs is a per-state
     intermediate; signed values exercise the hi/lo split with cancellation."""
