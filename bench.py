@@ -337,10 +337,12 @@ def measure(ctx, args, workload: str, batch: int, steps: int, warmup: int):
     wl = make_workload(workload, batch if batch > 0 else None)
     net = wl["net"]
     states_mode = wl["mode"] == "states"
-    restarts = max(args.restarts, 0)
+    # cfg5: the order search with the run-time objective (seeded restarts + tree rotations, about 15 s of host time, outside
+    # every timed region); the other configs keep the deterministic greedy plan (their plans are a handful of steps)
+    restarts = args.restarts if args.restarts >= 0 else (1024 if wl_name_is_cfg5(workload) else 0)
     # batch_hint = the config's FULL batch: a prefix run keeps the plan (tables, kernel classes) of the real workload
     plan = tqc.tqc_plan(net, tqc.MODE_STATES if states_mode else tqc.MODE_DISTRIBUTION, batch_hint=wl["full_B"],
-                        restarts=restarts, seed=args.plan_seed)
+                        restarts=restarts, seed=args.plan_seed, objective=1 if (restarts > 0 and states_mode) else 0)
     for s, t in enumerate(wl["tensors"]):
         tqc.tqc_load_subcircuit_tensors(plan, s, t)
     prefix_note = None
@@ -484,6 +486,8 @@ def measure(ctx, args, workload: str, batch: int, steps: int, warmup: int):
         "config": {"workload": workload_description(wl, plan), "states_per_step_per_gpu": n_out,
                    "parallelism": f"states sharded over {world} GPU(s), tensors replicated, no collective",
                    "l2": "flushed between timed iterations (256 MB write)", "plan_cost_log2_per_state": plan.cost_log2, "planner_restarts": restarts,
+                   "planner_objective": "modelled run time (tqc_plan_opts.objective = 1)" if (restarts > 0 and states_mode) else "deterministic greedy",
+                   "planner_modelled_us_per_state": plan.modelled_seconds_per_state * 1e6 if states_mode else None,
                    "kmax": plan.kmax, "workspace_gb": ws_bytes / 2 ** 30, "prefix_rule": prefix_note,
                    "library": tqc.version(), "chain_status": chain_rc, "chain_note": chain_note,
                    "kernel_classes": {kclass_name[k]: sum(1 for t in range(plan.num_steps) if plan.step(t)["kernel_class"] == k)
@@ -499,6 +503,10 @@ def measure(ctx, args, workload: str, batch: int, steps: int, warmup: int):
     del workspace, flush, out_dev
     torch.cuda.empty_cache()
     return line
+
+
+def wl_name_is_cfg5(name: str) -> bool:
+    return name == "cfg5"
 
 
 def ms_hint_short(total_ms: float, steps: int) -> bool:
@@ -805,7 +813,8 @@ def main() -> None:
                     help="variants: only the subcircuit-variant simulation row (secondary line, for profiling)")
     ap.add_argument("--batch", type=int, default=0, help="states per step per GPU (0: the config's own batch; for cfg5 "
                     "the SURVEY 8d-5 prefix: the smallest power of two whose step runs >= 1 s; 1000000 = the full cfg5 batch)")
-    ap.add_argument("--restarts", type=int, default=0, help="planner restarts (0: deterministic greedy)")
+    ap.add_argument("--restarts", type=int, default=-1, help="planner restarts with the run-time objective (0: deterministic "
+                    "greedy; default: 1024 for cfg5, 0 otherwise)")
     ap.add_argument("--plan-seed", type=int, default=1)
     ap.add_argument("--max-workspace-gb", type=int, default=64)
     ap.add_argument("--cpu-seconds", type=float, default=15.0)

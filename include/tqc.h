@@ -107,6 +107,11 @@ typedef struct {
     int32_t kmax_cap;               /* restarts > 0 only: among the randomised-greedy orders keep the cheapest one whose widest
                                        step K_max = max_t |E_a u E_b| is <= kmax_cap; while no order meets the
                                        cap the smaller K_max wins.  0 = no cap (total multiplication count only). */
+    int32_t objective;              /* restarts > 0 only: 0 = keep the order with the fewest multiplications; 1 (states mode) = keep
+                                       the order with the smallest MODELLED RUN TIME: per step, flops over the measured rate of the
+                                       kernel class the step would get (CTA-pair tensor pipe / one-CTA tensor pipe / FFMA) plus the
+                                       HBM bytes of per-state results and operands; integers only, deterministic per seed
+                                       (csrc/plan.cpp order_time_fs; tqc_plan_modelled_seconds_per_state reports it) */
 } tqc_plan_opts;
 
 /* ---- planning (host only; no CUDA call) -------------------------------------------------
@@ -143,6 +148,8 @@ int tqc_plan_step(const tqc_plan_t *plan, int i, int *lhs, int *rhs, int *n_inne
 int tqc_plan_node(const tqc_plan_t *plan, int v, int *kind, int *n_bits, int *n_open);
 /* log2 of the total multiplication count sum_t 2^{log2cost_t} (per state in states mode) */
 double tqc_plan_cost_log2(const tqc_plan_t *plan);
+/* the run-time model of tqc_plan_opts.objective = 1 evaluated on this plan (states mode; negative otherwise) */
+double tqc_plan_modelled_seconds_per_state(const tqc_plan_t *plan);
 /* Serialised plan (little-endian int32 words, format in DESIGN.md "Plan blob"): the object
  * compared byte-for-byte with the reference planner.  Call with buf = NULL to get *len. */
 int tqc_plan_serialize(const tqc_plan_t *plan, void *buf /*HOST*/, size_t *len);
@@ -245,7 +252,9 @@ int tqc_hss_contract(tqc_plan_t *plan, float *out_dev, void *workspace_dev, size
  *     (0 = most significant = the subcircuit's first listed incident cut).
  * out_dev DEVICE [4^{d+u}][2^o] fp32.  workspace DEVICE, 256-byte aligned, >= tqc_simulate_workspace_bytes(sub) (0 if the
  * description is out of range).  Asynchronous on `stream`, no allocation.  Errors: TQC_E_ARG (inconsistent lists, unknown
- * gate), TQC_E_TOO_LARGE (w > 13 or 4^{d+u} 2^o > 2^31), TQC_E_WORKSPACE, TQC_E_CUDA. */
+ * gate), TQC_E_TOO_LARGE (w > 15 or 4^{d+u} 2^o > 2^31), TQC_E_WORKSPACE, TQC_E_CUDA.
+ * Up to 13 wires the 2^w complex128 amplitudes of a variant stay in one block's shared memory; 14- and 15-wire subcircuits (the
+ * paper's cap) keep them in the workspace, which then also holds 24 * 2^w bytes per thread block. */
 enum { TQC_GATE_H = 0, TQC_GATE_X = 1, TQC_GATE_S = 2, TQC_GATE_SDG = 3, TQC_GATE_SX = 4, TQC_GATE_SY = 5, TQC_GATE_SW = 6,
        TQC_GATE_RX = 7, TQC_GATE_RY = 8, TQC_GATE_RZ = 9, TQC_GATE_CZ = 10, TQC_GATE_CX = 11, TQC_GATE_RZZ = 12,
        TQC_GATE_Y = 13, TQC_GATE_Z = 14, TQC_GATE_T = 15, TQC_GATE_TDG = 16,

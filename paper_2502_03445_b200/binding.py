@@ -36,7 +36,7 @@ EXPORTED = ["tqc_plan", "tqc_plan_destroy", "tqc_plan_mode", "tqc_plan_num_qubit
             "tqc_hss_workspace_bytes", "tqc_hss_contract", "tqc_simulate_workspace_bytes",
             "tqc_simulate_subcircuit_tensor", "tqc_plan_finalize", "tqc_plan_from_circuit", "tqc_plan_from_gates",
             "tqc_plan_cut_network", "tqc_plan_cut_subcircuit", "tqc_plan_cut_assignment", "tqc_cut_merging_cost",
-            "tqc_plan_cost_report", "tqc_plan_pair_launch_count"]
+            "tqc_plan_cost_report", "tqc_plan_pair_launch_count", "tqc_plan_modelled_seconds_per_state"]
 
 
 class TqcError(RuntimeError):
@@ -56,7 +56,7 @@ class _PlanOpts(ctypes.Structure):
     _fields_ = [("mode", c_int32), ("n_order_steps", c_int32), ("order", POINTER(c_int32)),
                 ("restarts", c_int32), ("seed", c_uint64), ("batch_hint", c_int64),
                 ("table_log2_floats_max", c_int32), ("use_tcgen05", c_int32), ("use_chain", c_int32),
-                ("n_slice_cuts", c_int32), ("slice_cuts", POINTER(c_int32)), ("kmax_cap", c_int32)]
+                ("n_slice_cuts", c_int32), ("slice_cuts", POINTER(c_int32)), ("kmax_cap", c_int32), ("objective", c_int32)]
 
 
 class _Gate(ctypes.Structure):
@@ -112,6 +112,8 @@ def _load() -> ctypes.CDLL:
     lib.tqc_plan_node.argtypes = [c_void_p, c_int] + [POINTER(c_int)] * 3
     lib.tqc_plan_cost_log2.argtypes = [c_void_p]
     lib.tqc_plan_cost_log2.restype = c_double
+    lib.tqc_plan_modelled_seconds_per_state.argtypes = [c_void_p]
+    lib.tqc_plan_modelled_seconds_per_state.restype = c_double
     lib.tqc_plan_serialize.argtypes = [c_void_p, c_void_p, POINTER(c_size_t)]
     lib.tqc_plan_workspace_bytes.argtypes = [c_void_p, c_size_t, c_int]
     lib.tqc_plan_workspace_bytes.restype = c_size_t
@@ -213,6 +215,8 @@ class Plan:
     def kmax(self) -> int: return _lib.tqc_plan_kmax(self._h)
     @property
     def cost_log2(self) -> float: return _lib.tqc_plan_cost_log2(self._h)
+    @property
+    def modelled_seconds_per_state(self) -> float: return _lib.tqc_plan_modelled_seconds_per_state(self._h)
     @property
     def launch_count(self) -> int: return int(_lib.tqc_plan_launch_count(self._h))
     @property
@@ -332,7 +336,7 @@ def _network_desc(net):
 
 def tqc_plan(net, mode: int = MODE_STATES, order=None, restarts: int = 0, seed: int = 0, batch_hint: int = 0,
              table_log2_floats_max: int = 0, use_tcgen05: int = 0, use_chain: int = 0, slice_cuts=None,
-             kmax_cap: int = 0) -> Plan:
+             kmax_cap: int = 0, objective: int = 0) -> Plan:
     """net: any object with n_qubits, cuts [(up, down)], sub_cuts [[cut ids]], sub_qubits [[qubit ids]]
     (e.g. tqc_inputs.Network).  order: optional list of m-1 (lhs, rhs) node-id pairs.  slice_cuts: cut ids evaluated by
     index slicing (summed over their 4 bases) instead of being contracted as bonds."""
@@ -341,7 +345,7 @@ def tqc_plan(net, mode: int = MODE_STATES, order=None, restarts: int = 0, seed: 
     sflat, sflat_p = _i32(slice_cuts or [])
     opts = _PlanOpts(mode, len(order) if order else 0, oflat_p, restarts, seed, batch_hint,
                      table_log2_floats_max, use_tcgen05, use_chain, len(slice_cuts) if slice_cuts else 0, sflat_p,
-                     kmax_cap)
+                     kmax_cap, objective)
     h = c_void_p()
     _check(_lib.tqc_plan(byref(desc), byref(opts), byref(h)))
     return Plan(h.value)
@@ -369,7 +373,7 @@ def circuit_text(n_qubits: int, gates) -> str:
 
 
 def _plan_opts_simple(mode, restarts, seed, batch_hint, table_log2_floats_max, use_tcgen05, use_chain, kmax_cap):
-    return _PlanOpts(mode, 0, None, restarts, seed, batch_hint, table_log2_floats_max, use_tcgen05, use_chain, 0, None, kmax_cap)
+    return _PlanOpts(mode, 0, None, restarts, seed, batch_hint, table_log2_floats_max, use_tcgen05, use_chain, 0, None, kmax_cap, 0)
 
 
 def tqc_plan_from_circuit(text: str, w_max: int, s_max: int, K_t: int = 0, Q_max: float = 0.0, mode: int = MODE_STATES,
@@ -404,7 +408,7 @@ def tqc_choose_slice_cuts(net, mode: int = MODE_STATES, max_log2_input_floats: i
                           max_log2_intermediate_floats: int = 62, batch_hint: int = 0):
     """The paper's two-level slicing choice (include/tqc.h): list of cut ids in pick order."""
     desc, _keep = _network_desc(net)
-    opts = _PlanOpts(mode, 0, None, 0, 0, batch_hint, 0, 0, 0, 0, None, 0)
+    opts = _PlanOpts(mode, 0, None, 0, 0, batch_hint, 0, 0, 0, 0, None, 0, 0)
     out = np.zeros(max(1, len(net.cuts)), dtype=np.int32)
     n = c_int32(0)
     _check(_lib.tqc_choose_slice_cuts(byref(desc), byref(opts), max_log2_input_floats, max_log2_intermediate_floats,

@@ -30,6 +30,7 @@ struct SimArgs {
     int32_t D_bit[16], U_bit[16], O_bit[32];   // amplitude-index bit positions of the listed wires
     const SimGate *gates;
     double *R;                                 // [4^d][4^u][2^o]
+    double2 *scratch;                          // w >= 14 only: per block 2^w complex128 amplitudes + 2^w float64 probabilities
 };
 
 __device__ __forceinline__ double2 cfma(double2 a, double2 b, double2 acc) {
@@ -86,12 +87,16 @@ __device__ __forceinline__ int gray3_digit(uint32_t t, uint32_t pow3k) {
 // The block simulates preparation a ONCE and then walks 3^{u-g} measurement settings (0..2 = Z, X, Y): the settings of
 // the first g upstream wires are the base-3 digits of `group`, those of the other u-g wires run through a reflected
 // Gray code, so going from one setting to the next is ONE one-qubit pass (new rotation times the inverse of the old one).
-// Shared memory: 2^w complex128 amplitudes followed by 2^w float64 probabilities.
+// Shared memory: 2^w complex128 amplitudes followed by 2^w float64 probabilities (w <= 13: 192 KB).  IN_GLOBAL: subcircuits of
+// 14 and 15 wires (the paper's cap) keep the same 24 * 2^w bytes per block in the caller's workspace,
+// where they stay L2-resident (at most 2 * 148 blocks x 768 KB); the passes are the same code on a global pointer.
+template <bool IN_GLOBAL>
 __global__ void __launch_bounds__(512) sim_variant_kernel(SimArgs g) {
-    extern __shared__ double2 psi[];
+    extern __shared__ double2 psi_smem[];
     __shared__ double2 rot[4][4];
     const int w = g.w, u = g.u, ng = g.g;
     const uint32_t size = 1u << w;
+    double2 *psi = IN_GLOBAL ? g.scratch + (size_t)blockIdx.x * (size + size / 2) : psi_smem;
     double *q = reinterpret_cast<double *>(psi + size);
     uint32_t pow3g = 1, n_walk = 1;
     for (int j = 0; j < ng; ++j) pow3g *= 3;

@@ -149,7 +149,8 @@ step_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
     auto B_raw = [&](int s) { return tiles + (size_t)s * stage_bytes + 2 * bytesA; };
     auto B_lo = [&](int s) { return tiles + (size_t)s * stage_bytes + 2 * bytesA + bytesB; };
 
-    const int n_kb = 1 << (a.lgK - 5);
+    // K = 16 (lgK = 4) runs as ONE k-block: the TMA box is 32 floats wide, the 16 beyond the tensor's K extent arrive as zeros
+    const int n_kb = a.lgK >= 5 ? 1 << (a.lgK - 5) : 1;
     const int lg_tm = a.lgM - 8;
     const long long tiles_m = 1ll << lg_tm, tiles_n = (1ll << a.lgN) / BN;
     const long long total = tiles_m * tiles_n * a.R;

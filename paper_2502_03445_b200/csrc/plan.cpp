@@ -157,6 +157,135 @@ double order_cost_log2(const HostPlan &p, const std::vector<std::vector<int>> &l
     return es.empty() ? 0.0 : maxe + std::log2(total);
 }
 
+// Modelled run time of an order in states mode, femtoseconds per state (integers only, so the choice is reproducible).
+// Rates measured on a B200 in round 2 (profiles/r02_tc2_kernel.md, profiles/peaks_r02.md), per fp32-equivalent flop
+// (2 per multiplication of PAPER.md lines 407-412):
+//   CTA-pair tensor-pipe kernel (both outer dimensions >= 256, K >= 16)   235 TFLOP/s  ->  4.26 fs / flop
+//   one-CTA tensor-pipe kernels (larger side >= 128, smaller >= 16, K >= 32)  100 TFLOP/s  ->  10 fs / flop
+//   fp32 FFMA tile kernel                                                  25 TFLOP/s  ->  40 fs / flop
+// plus the bytes of a per-state result that goes through HBM (0.65 / 3.9 TB/s = 167 fs / byte: the stores of a tile overlap
+// its successor's MMAs only in part) and of per-state operands read back (200 fs / byte).  A node that carries few output
+// bits is a table, evaluated once per key: its cost is spread over the expected batch.
+int64_t order_time_fs(const HostPlan &p, const std::vector<std::vector<int>> &leaf_open,
+                      const std::vector<std::pair<int, int>> &order, const PlanOptions &opts) {
+    const int m = p.m;
+    int64_t hint = opts.batch_hint > 0 ? opts.batch_hint : ((int64_t)1 << 20);
+    int lg = 0;
+    while (((int64_t)2 << lg) <= hint) ++lg;
+    const int table_bits_max = std::max(0, lg - 2);
+    const int table_log2_floats_max = opts.table_log2_floats_max > 0 ? opts.table_log2_floats_max : 24;
+    std::map<int, std::vector<int>> open;
+    std::map<int, int> bits, kind;                                  // kind: 0 leaf, 1 table, 2 batch
+    for (int s = 0; s < m; ++s) { open[s] = leaf_open[s]; bits[s] = p.o(s); kind[s] = 0; }
+    __int128 total = 0;
+    int t = 0;
+    for (const auto &ab : order) {
+        const std::vector<int> &A = open[ab.first], &B = open[ab.second];
+        const int shared = count_and(A, B);
+        const int lgK = 2 * shared, lgM = 2 * ((int)A.size() - shared), lgN = 2 * ((int)B.size() - shared);
+        const int cbits = bits[ab.first] + bits[ab.second], copen = (int)A.size() + (int)B.size() - 2 * shared;
+        const bool kids = kind[ab.first] != 2 && kind[ab.second] != 2;
+        const bool table = kids && cbits <= table_bits_max && cbits + 2 * copen <= table_log2_floats_max;
+        const int e = std::min(lgM + lgN + lgK + 1, 100);            // log2 flops of one row
+        __int128 fs;
+        if (table) {
+            fs = (((__int128)40 << e) << cbits) / hint;              // FFMA / warp-MMA tables, once per key
+        } else {
+            int fs_per_flop_x100;
+            const int hi = std::max(lgM, lgN), lo = std::min(lgM, lgN);
+            if (lo >= 8 && lgK >= 4) fs_per_flop_x100 = 426;
+            else if (hi >= 7 && lo >= 4 && lgK >= 5) fs_per_flop_x100 = 1000;
+            else fs_per_flop_x100 = 4000;
+            fs = ((__int128)fs_per_flop_x100 << e) / 100;
+            fs += (__int128)167 * 4 << std::min(2 * copen, 100);     // result bytes
+            if (kind[ab.first] == 2) fs += (__int128)200 * 4 << std::min(2 * (int)A.size(), 100);
+            if (kind[ab.second] == 2) fs += (__int128)200 * 4 << std::min(2 * (int)B.size(), 100);
+        }
+        total += fs;
+        std::vector<int> merged = set_xor(A, B);
+        open.erase(ab.first); open.erase(ab.second);
+        bits.erase(ab.first); bits.erase(ab.second);
+        open[m + t] = merged; bits[m + t] = cbits; kind[m + t] = table ? 1 : 2;
+        ++t;
+    }
+    const __int128 cap = ((__int128)1 << 62);
+    return (int64_t)std::min(total, cap);
+}
+
+// Local search on the contraction TREE (the "subtree reconfiguration" of the order-search library the paper used, PAPER.md
+// line 449): a move rewrites X = (P . Q) . Z into (P . Z) . Q or (Q . Z) . P at a random internal node, i.e. it changes which
+// pair under X is contracted first; every order is reachable by such rotations.  Simulated annealing on the objective of the
+// restarts (multiplication count or modelled run time), seeded, integers and one deterministic generator: the same seed
+// gives the same plan.  Returns the best order seen (never worse than the input).
+std::vector<std::pair<int, int>> improve_by_rotations(const HostPlan &p, const std::vector<std::vector<int>> &leaf_open,
+                                                      std::vector<std::pair<int, int>> order, const PlanOptions &opts,
+                                                      int iters, SplitMix64 &rng, int kmax_cap) {
+    const int m = p.m, n_nodes = 2 * m - 1;
+    if (m < 4 || iters <= 0) return order;
+    std::vector<int> left(n_nodes, -1), right(n_nodes, -1), parent(n_nodes, -1);
+    for (int t = 0; t < m - 1; ++t) {
+        left[m + t] = order[t].first; right[m + t] = order[t].second;
+        parent[order[t].first] = m + t; parent[order[t].second] = m + t;
+    }
+    const int root = n_nodes - 1;
+    const bool by_time = opts.objective == 1 && p.mode == 0;
+    auto emit = [&](std::vector<std::pair<int, int>> &out) {          // post-order renumbering: children before parents
+        out.clear();
+        std::vector<int> id(n_nodes, -1), stack = {root}, state(n_nodes, 0);
+        for (int s = 0; s < m; ++s) id[s] = s;
+        int next = m;
+        while (!stack.empty()) {
+            const int v = stack.back();
+            if (v < m) { stack.pop_back(); continue; }
+            if (state[v] == 0) { state[v] = 1; stack.push_back(right[v]); stack.push_back(left[v]); }
+            else {
+                stack.pop_back();
+                if (id[v] >= 0) continue;
+                id[v] = next++;
+                const int a = id[left[v]], b = id[right[v]];
+                out.emplace_back(std::min(a, b), std::max(a, b));
+            }
+        }
+    };
+    auto score = [&](const std::vector<std::pair<int, int>> &o, int *kmax) -> double {
+        const double c = order_cost_log2(p, leaf_open, o, kmax);
+        return by_time ? (double)order_time_fs(p, leaf_open, o, opts) : c;
+    };
+    std::vector<std::pair<int, int>> cur, best = order, cand;
+    emit(cur);
+    int k = 0;
+    double cur_s = score(cur, &k), best_s = cur_s;
+    std::vector<int> internal;
+    for (int it = 0; it < iters; ++it) {
+        // X: internal node with at least one internal child
+        const int X = m + (int)(rng.next() % (uint64_t)(m - 1));
+        const bool take_left = (rng.next() & 1) != 0;
+        int Y = take_left ? left[X] : right[X], Z = take_left ? right[X] : left[X];
+        if (Y < m) { std::swap(Y, Z); if (Y < m) continue; }
+        const bool keep_p = (rng.next() & 1) != 0;
+        const int P = left[Y], Q = right[Y];
+        // new Y = (keep_p ? Q : P) . Z ; new X = Y . (keep_p ? P : Q)
+        const int stay = keep_p ? P : Q, join = keep_p ? Q : P;
+        left[Y] = join; right[Y] = Z; parent[Z] = Y;
+        left[X] = Y; right[X] = stay; parent[stay] = X;
+        emit(cand);
+        int kc = 0;
+        const double s2 = score(cand, &kc);
+        const double temp = 0.02 * (double)(iters - it) / (double)iters;             // relative uphill tolerance, cooling to 0
+        const double u = rng.uniform();
+        const bool cap_ok = kmax_cap <= 0 || kc <= kmax_cap || kc <= k;
+        const double cur_cmp = by_time ? cur_s * (1.0 + temp * u) : cur_s + temp * 10.0 * u;
+        if (cap_ok && s2 <= cur_cmp) {
+            cur_s = s2; k = kc; cur.swap(cand);
+            if (s2 < best_s) { best_s = s2; best = cur; }
+        } else {                                                                     // undo
+            left[Y] = P; right[Y] = Q; parent[Z] = X; parent[stay] = Y;
+            if (take_left) { left[X] = Y; right[X] = Z; } else { left[X] = Z; right[X] = Y; }
+        }
+    }
+    return best;
+}
+
 }  // namespace
 
 int validate_network(int n, int m, int K, const int32_t *cut_up, const int32_t *cut_down, const int32_t *sub_cut_ofs,
@@ -237,8 +366,11 @@ int build_plan(int n, int m, int K, const int32_t *cut_up, const int32_t *cut_do
         if (opts.restarts > 0) {
             // objective: total multiplication count, among the orders whose K_max (the widest step)
             // stays within kmax_cap; while no order meets the cap the smaller K_max wins
+            // (objective = 1, states mode: the modelled run time order_time_fs instead of the multiplication count)
+            const bool by_time = opts.objective == 1 && p.mode == 0;
             int best_k = 0;
             double best = order_cost_log2(p, leaf_open, order, &best_k);
+            if (by_time) best = (double)order_time_fs(p, leaf_open, order, opts);
             const int cap = opts.kmax_cap > 0 ? opts.kmax_cap : 1 << 30;
             SplitMix64 rng(opts.seed);
             for (int r = 0; r < opts.restarts; ++r) {
@@ -246,11 +378,14 @@ int build_plan(int n, int m, int K, const int32_t *cut_up, const int32_t *cut_do
                 auto cand = greedy_order(p, leaf_open, noise, &rng, &too_large);
                 if (too_large) { too_large = false; continue; }
                 int k = 0;
-                const double c = order_cost_log2(p, leaf_open, cand, &k);
+                double c = order_cost_log2(p, leaf_open, cand, &k);
+                if (by_time) c = (double)order_time_fs(p, leaf_open, cand, opts);      // exact: the value is an integer < 2^53 in practice
                 const bool ok = k <= cap, best_ok = best_k <= cap;
-                const bool better = (ok && !best_ok) || (ok == best_ok && (ok ? c < best - 1e-12 : (k < best_k || (k == best_k && c < best - 1e-12))));
+                const bool better = (ok && !best_ok) || (ok == best_ok && (ok ? c < best - (by_time ? 0.5 : 1e-12) : (k < best_k || (k == best_k && c < best - (by_time ? 0.5 : 1e-12)))));
                 if (better) { best = c; best_k = k; order = cand; }
             }
+            // then tree rotations from the best restart (200 moves per restart asked for)
+            order = improve_by_rotations(p, leaf_open, order, opts, std::min(opts.restarts, 1 << 16) * 200, rng, opts.kmax_cap);
         }
     }
 
@@ -366,6 +501,14 @@ int64_t distribution_layout(const HostPlan &p, int prefix_bits, std::vector<int>
             if (op >= m) al.release(offsets[op], size_of(op));
     }
     return al.top;
+}
+
+int64_t plan_time_fs(const HostPlan &p, const PlanOptions &opts) {
+    std::vector<std::vector<int>> leaf_open(p.m);
+    for (int s = 0; s < p.m; ++s) { leaf_open[s] = p.sub_cuts[s]; std::sort(leaf_open[s].begin(), leaf_open[s].end()); }
+    std::vector<std::pair<int, int>> order;
+    for (const Step &st : p.steps) order.emplace_back(st.lhs, st.rhs);
+    return order_time_fs(p, leaf_open, order, opts);
 }
 
 std::vector<int32_t> serialize_words(const HostPlan &p) {

@@ -109,6 +109,7 @@ struct PlanOptions {
     int kmax_cap = 0;                           // restarts only: prefer orders with K_max <= cap (0: no cap)
     int64_t batch_hint = 0;                     // expected states per call (0: 2^20); sets table_bits_max
     int table_log2_floats_max = 0;              // 0: default 24 (64 MB per table)
+    int objective = 0;                          // restarts only: 0 = multiplication count, 1 = modelled run time (states mode)
 };
 
 // Structural checks of a network description (ids in range, every cut listed by exactly its two subcircuits, every qubit
@@ -121,6 +122,8 @@ int build_plan(int n, int m, int K, const int32_t *cut_up, const int32_t *cut_do
                const int32_t *sub_cut_ofs, const int32_t *sub_cuts, const int32_t *sub_qubit_ofs,
                const int32_t *sub_qubits, const PlanOptions &opts, HostPlan &out, std::string &err);
 
+// modelled run time of the plan's order, femtoseconds per state (states mode; the objective of `objective = 1`)
+int64_t plan_time_fs(const HostPlan &p, const PlanOptions &opts);
 std::vector<int32_t> serialize_words(const HostPlan &p);
 double cost_log2(const HostPlan &p);
 

@@ -84,6 +84,7 @@ int index_of(const std::vector<int> &v, int x) {
 
 struct tqc_plan {
     tqc::HostPlan hp;
+    tqc::PlanOptions plan_opts;
     int use_tcgen05 = 0;
     // fused small-bond chain (kernels_chain.cuh): the per-state steps as one device step table
     bool chain = false;
@@ -195,8 +196,8 @@ int ensure_device_attrs(int *sm_count) {
         TQC_CUDA(cudaFuncSetAttribute(tqc::step_tcw_kernel, dyn, 194 * 1024));
         TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc2_kernel<256>, dyn, 194 * 1024));
         TQC_CUDA(cudaFuncSetAttribute(tqc::chain_kernel, dyn, 128 * 1024));
-        TQC_CUDA(cudaFuncSetAttribute(tqc::sim_variant_kernel, dyn, 24 << 13));
-        TQC_CUDA(cudaFuncSetAttribute(tqc::sim_variant_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::sim_variant_kernel<false>, dyn, 24 << 13));
+        TQC_CUDA(cudaFuncSetAttribute(tqc::sim_variant_kernel<false>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
         done[dev] = true;
     }
     if (sm_count) *sm_count = sms[dev];
@@ -420,6 +421,7 @@ int make_operand_map(CUtensorMap *map, const float *base, int lgK, int lgRows, l
 
 bool tc_eligible(int lgM, int lgN, int lgK) {
     if (std::max(lgM, lgN) > 14) return false;                  // at most 256 tiles per side (C-offset tables of the kernel)
+    if (lgK == 4 && lgM >= 8 && lgN >= 8) return dev_env("TQC_TC_NO_PAIR") == nullptr && dev_env("TQC_TC_NO_K16") == nullptr;   // K = 16 on the CTA-pair kernel (half of each k-block is zero fill)
     return lgK >= 5 && std::max(lgM, lgN) >= 7 && std::min(lgM, lgN) >= 4;
 }
 
@@ -436,7 +438,7 @@ int launch_tc_step(tqc_plan_t *pl, TcOperand A, TcOperand B, BitMap outA, BitMap
         // (64-column pair tiles were tried: a k-block then holds 384 cycles of MMAs against about 1800 cycles of fixed pipeline
         // hand-shake per k-block, no gain over step_tc_kernel<64>; those steps are bound by streaming their 16 MB operand)
         const bool keep_ok = lgM >= 8 && lgN >= 8, swap_ok = keep_ok;          // outer dimensions are powers of four
-        if (!no_pair && lgK >= 5 && (keep_ok || swap_ok)) {
+        if (!no_pair && lgK >= 4 && (keep_ok || swap_ok)) {
             bool sw = !keep_ok;
             if (keep_ok && swap_ok) sw = has_bit0(outA);
             if (sw) { std::swap(A, B); std::swap(outA, outB); std::swap(lgM, lgN); }
@@ -470,6 +472,7 @@ int launch_tc_step(tqc_plan_t *pl, TcOperand A, TcOperand B, BitMap outA, BitMap
             return 0;
         }
     }
+    if (lgK < 5) return fail(TQC_E_TOO_LARGE, "internal: a K = 16 tensor-pipe step needs the CTA-pair kernel");
     // the M side needs >= 128 rows; with both sides large, the N side (vector stores run along it) takes C's lowest bits
     bool swap = lgM < 7;
     if (lgM >= 7 && lgN >= 7 && has_bit0(outA)) swap = true;
@@ -941,6 +944,7 @@ void plan_options_from(const tqc_plan_opts *opts, tqc::PlanOptions &po) {
     po.batch_hint = opts->batch_hint;
     po.table_log2_floats_max = opts->table_log2_floats_max;
     po.kmax_cap = opts->kmax_cap;
+    po.objective = opts->objective;
     for (int i = 0; i < opts->n_order_steps && opts->order; ++i) po.order.emplace_back(opts->order[2 * i], opts->order[2 * i + 1]);
 }
 }  // namespace
@@ -1036,6 +1040,7 @@ int tqc_plan(const tqc_network_desc *net, const tqc_plan_opts *opts, tqc_plan_t 
         po.batch_hint = opts->batch_hint;
         po.table_log2_floats_max = opts->table_log2_floats_max;
         po.kmax_cap = opts->kmax_cap;
+        po.objective = opts->objective;
         use_tc = opts->use_tcgen05;
         if (opts->n_order_steps > 0) {
             if (!opts->order) return fail(TQC_E_ARG, "n_order_steps > 0 but order is null");
@@ -1070,6 +1075,7 @@ int tqc_plan(const tqc_network_desc *net, const tqc_plan_opts *opts, tqc_plan_t 
     }
     if (rc != 0) { delete pl; return fail(rc, err); }
     pl->use_tcgen05 = use_tc;
+    pl->plan_opts = po;
     pl->d_leaf_all.assign(pl->hp.m, nullptr);
     pl->d_leaf.assign(pl->hp.m, nullptr);
     pl->loaded.assign(pl->hp.m, 0);
@@ -1157,6 +1163,10 @@ int tqc_plan_node(const tqc_plan_t *pl, int v, int *kind, int *n_bits, int *n_op
 }
 
 double tqc_plan_cost_log2(const tqc_plan_t *pl) { return pl ? tqc::cost_log2(pl->hp) : -1.0; }
+double tqc_plan_modelled_seconds_per_state(const tqc_plan_t *pl) {
+    if (!pl || pl->hp.mode != TQC_MODE_STATES) return -1.0;
+    return (double)tqc::plan_time_fs(pl->hp, pl->plan_opts) * 1e-15 * std::ldexp(1.0, 2 * pl->n_sliced());
+}
 
 int tqc_plan_serialize(const tqc_plan_t *pl, void *buf, size_t *len) {
     if (!pl || !len) return fail(TQC_E_ARG, "null argument");
@@ -1931,11 +1941,30 @@ std::vector<tqc::SimGate> sim_fuse(const std::vector<tqc::SimGate> &in, int n_in
 }
 }  // namespace
 
+namespace {
+// grid of sim_variant_kernel: 4^d preparations x 3^g setting groups, g = the smallest split that gives every SM two blocks
+// (integers only); w >= 14 keeps at most 2 * 148 blocks so that the per-block amplitudes in the workspace stay L2-resident
+void sim_grid(const tqc_subcircuit_desc *sub, unsigned *blocks, int *g_fixed) {
+    unsigned b = 1;
+    for (int i = 0; i < sub->d && b < (1u << 30); ++i) b *= 4;
+    int g = 0;
+    while (g < sub->u && b < 2 * 148) { b *= 3; ++g; }
+    if (sub->walk_settings == 0 && sub->w <= 13) { for (; g < sub->u && b < (1u << 30); ++g) b *= 3; }     // one block per variant
+    *blocks = b; *g_fixed = g;
+}
+size_t sim_scratch_bytes(const tqc_subcircuit_desc *sub) {
+    if (sub->w <= 13) return 0;
+    unsigned blocks; int g;
+    sim_grid(sub, &blocks, &g);
+    return sim_align((size_t)blocks * ((size_t)24 << sub->w));
+}
+}  // namespace
+
 size_t tqc_simulate_workspace_bytes(const tqc_subcircuit_desc *sub) {
-    if (!sub || sub->d < 0 || sub->u < 0 || sub->o < 0 || sub->n_gates < 0) return 0;
+    if (!sub || sub->d < 0 || sub->u < 0 || sub->o < 0 || sub->n_gates < 0 || sub->w < 0 || sub->w > 15 || sub->d > 15 || sub->u > 15) return 0;
     const int lg = 2 * (sub->d + sub->u) + sub->o;
     if (lg > 31) return 0;
-    return sim_align(sizeof(tqc::SimGate) * (size_t)std::max(sub->n_gates, 1)) + sim_align(sizeof(double) << lg);
+    return sim_align(sizeof(tqc::SimGate) * (size_t)std::max(sub->n_gates, 1)) + sim_align(sizeof(double) << lg) + sim_scratch_bytes(sub);
 }
 
 int tqc_simulate_subcircuit_tensor(const tqc_subcircuit_desc *sub, float *out_dev, void *workspace_dev,
@@ -1945,7 +1974,7 @@ int tqc_simulate_subcircuit_tensor(const tqc_subcircuit_desc *sub, float *out_de
     if (w < 0 || d < 0 || u < 0 || o < 0 || sub->n_gates < 0) return fail(TQC_E_ARG, "negative size");
     if (u + o != w) return fail(TQC_E_ARG, "every wire ends in an upstream cut or an output: u + o must equal w");
     if (d > w) return fail(TQC_E_ARG, "more downstream wires than wires");
-    if (w > 13) return fail(TQC_E_TOO_LARGE, "w > 13: 2^w complex128 amplitudes do not fit one block's shared memory");
+    if (w > 15) return fail(TQC_E_TOO_LARGE, "w > 15 wires (the paper's subcircuit cap, PAPER.md lines 12-14)");
     if (d > 15 || u > 15 || 2 * c + o > 31) return fail(TQC_E_TOO_LARGE, "4^c 2^o exceeds 2^31 entries");
     if ((d && !sub->D_wires) || (u && !sub->U_wires) || (o && !sub->O_wires) || (c && !sub->bond_pos) ||
         (sub->n_gates && !sub->gates))
@@ -1996,6 +2025,7 @@ int tqc_simulate_subcircuit_tensor(const tqc_subcircuit_desc *sub, float *out_de
     tqc::SimGate *d_gates = (tqc::SimGate *)workspace_dev;
     a.gates = d_gates;
     a.R = (double *)((char *)workspace_dev + gate_bytes);
+    a.scratch = (double2 *)((char *)a.R + sim_align(sizeof(double) << (2 * c + o)));
     // pageable source: the runtime stages the bytes before the call returns, so hg may go out of scope
     TQC_CUDA(cudaMemcpyAsync(d_gates, hg.data(), sizeof(tqc::SimGate) * hg.size(), cudaMemcpyHostToDevice, st));
     const size_t smem = (sizeof(double2) + sizeof(double)) << w;          // amplitudes + probabilities
@@ -2003,14 +2033,16 @@ int tqc_simulate_subcircuit_tensor(const tqc_subcircuit_desc *sub, float *out_de
     // One block per (preparation, group of settings): the settings of the first g upstream wires come from the block id,
     // the block walks the other 3^{u-g}.  g = the smallest split that gives every SM two blocks (integers only).
     unsigned blocks_v = 1;
-    for (int i = 0; i < d; ++i) blocks_v *= 4;
     int g_fixed = 0;
-    while (g_fixed < u && blocks_v < 2 * 148) { blocks_v *= 3; ++g_fixed; }
-    if (sub->walk_settings == 0) { for (; g_fixed < u; ++g_fixed) blocks_v *= 3; }     // one block per variant
+    sim_grid(sub, &blocks_v, &g_fixed);
     a.g = g_fixed;
-    // 124 registers per thread: two 256-thread blocks share an SM (the other issues while one waits at a barrier); when
-    // the grid cannot give every SM two blocks, one wider block per SM
-    tqc::sim_variant_kernel<<<blocks_v, (w >= 11 && blocks_v < 2 * 148) ? 512 : 256, smem, st>>>(a);
+    if (w <= 13) {
+        // 124 registers per thread: two 256-thread blocks share an SM (the other issues while one waits at a barrier); when
+        // the grid cannot give every SM two blocks, one wider block per SM
+        tqc::sim_variant_kernel<false><<<blocks_v, (w >= 11 && blocks_v < 2 * 148) ? 512 : 256, smem, st>>>(a);
+    } else {
+        tqc::sim_variant_kernel<true><<<blocks_v, 512, 0, st>>>(a);        // amplitudes in the workspace (L2), 14-15 wires
+    }
     TQC_CUDA(cudaGetLastError());
     const size_t total = size_t(1) << (2 * c + o);
     for (int i = 0; i < d; ++i) {

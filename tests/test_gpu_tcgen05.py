@@ -79,7 +79,8 @@ def _owned(pattern, ni, oa=1, ob=1, od=1):
                                                  ("bbbbaaaa", 3, 21, True),       # A owns them: operands swapped by the launcher
                                                  ("abababab", 4, 18, True),       # interleaved digits
                                                  ("aaaaabbbb", 3, 5, False),      # M = 1024: several pair tiles per state
-                                                 ("aaaabbbbb", 5, 3, False)])     # N = 1024, K = 1024 (32 k-blocks per tile)
+                                                 ("aaaabbbbb", 5, 3, False),      # N = 1024, K = 1024 (32 k-blocks per tile)
+                                                 ("aaaabbbbb", 2, 29, True)])     # K = 16: one k-block, half of it zero fill
 def test_pair_kernel_cta_group_2(pattern, ni, B, signed):
     """step_tc2_kernel (tcgen05 cta_group::2, 256 x 256 tiles over two SMs): both outer dimensions >= 256.  Ragged tile
     counts against the 74 clusters, both store orientations, signed values; against the float64 per-state contraction O8'

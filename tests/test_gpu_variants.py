@@ -12,7 +12,10 @@ import torch
 
 import paper_2502_03445_b200 as tqc
 from oracle import cutting, statevector as sv
+from types import SimpleNamespace
+
 from tqc_inputs import circuits as C, configs
+from tqc_inputs.circuits import hea_subcircuit
 
 pytestmark = pytest.mark.gpu
 
@@ -136,9 +139,23 @@ def test_bench_subcircuit_in_the_launch_configuration_bench_times():
     assert np.abs(got_p - want_p).max() <= 2.0 ** (3 - 23)
 
 
+@pytest.mark.parametrize("w,d,u", [(14, 2, 2), (15, 1, 2)])
+def test_subcircuits_of_14_and_15_wires(w, d, u):
+    """The paper caps subcircuits at 15 qubits.  Above 13 wires the amplitudes of a variant live in the workspace
+    instead of shared memory (same passes): a seeded HEA-shaped subcircuit against the oracle's O4/O5, whole tensor."""
+    desc = hea_subcircuit(w, d, u, seed=1400 + w)
+    got = tqc.tqc_simulate_subcircuit_tensor(**desc).cpu().numpy().astype(np.float64)
+    sub = cutting.Subcircuit(0, w=w, gates=desc["gates"], D=[(q, i) for i, q in enumerate(desc["D_wires"])],
+                             U=[(q, d + j) for j, q in enumerate(desc["U_wires"])], O=[(q, q) for q in desc["O_wires"]])
+    want = cutting.build_tensor(SimpleNamespace(sub_cuts=[list(range(d + u))]), sub)
+    assert got.shape == want.shape == (4 ** (d + u), 2 ** (w - u))
+    assert np.abs(got - want).max() <= 2.0 ** (d - 23)
+    assert abs(want[0].sum() - 2.0 ** d) < 1e-9                 # sum_x T[I...I, x] = 2^{d_s}
+
+
 def test_errors():
     with pytest.raises(tqc.TqcError) as e:
-        tqc.tqc_simulate_subcircuit_tensor(14, [], [], [], list(range(14)), [])
+        tqc.tqc_simulate_subcircuit_tensor(16, [], [], [], list(range(16)), [])
     assert e.value.code == -6
     with pytest.raises(tqc.TqcError) as e:                       # wire 1 has no end
         tqc.tqc_simulate_subcircuit_tensor(2, [], [], [0], [], [0])

@@ -205,7 +205,7 @@ def test_simulate_description_checks_run_without_a_gpu():
     fake = ctypes.c_void_p(256)
     for bad, code in (((2, gates, [0], [0], [], [1, 0]), -1),           # u + o != w
                       ((2, [("h", (), (5,))], [], [], [0, 1], []), -1),  # gate wire out of range
-                      ((14, [], [], [], list(range(14)), []), -6)):      # too wide for one block
+                      ((16, [], [], [], list(range(16)), []), -6)):      # more than 15 wires
         desc, _keep = _subcircuit_desc(*bad)
         assert _lib.tqc_simulate_subcircuit_tensor(ctypes.byref(desc), fake, fake, 1 << 30, None) == code
     with pytest.raises(binding.TqcError):
