@@ -110,17 +110,21 @@ def make_workload(name: str, batch: int | None = None):
             "full_B": configs.BATCH[cfg]}
 
 
-def pack_states_of(wl, rank: int) -> np.ndarray:
+def pack_states_of(wl, rank: int, world: int = 1) -> np.ndarray:
     from tqc_inputs import pack_states
-    return pack_states(workload_states(wl, rank)).view(np.int64)
+    return pack_states(workload_states(wl, rank, world)).view(np.int64)
 
 
-def workload_states(wl, rank: int) -> np.ndarray:
-    """(B, n) bits, uniform over {0,1}^n, seeded per rank (rank 0 = the config's own seed)."""
+def workload_states(wl, rank: int, world: int = 1) -> np.ndarray:
+    """(B, n) bits of THIS rank: the job's batch is the first world x B states of the config's seeded batch (uniform over
+    {0,1}^n), cut into contiguous per-rank ranges by paper_2502_03445_b200.sharding.shard_states (states
+    shard across ranks, tensors are replicated, no collective on the data path).  Weak scaling: B states per GPU."""
+    from paper_2502_03445_b200.sharding import shard_states
     from tqc_inputs import random_states, seed_for
     from tqc_inputs.seeds import STREAM_STATES
-    full = random_states(wl["net"].n_qubits, wl["B"], seed_for(wl["cfg"], STREAM_STATES, bump=rank))
-    return full
+    full = random_states(wl["net"].n_qubits, wl["B"] * world, seed_for(wl["cfg"], STREAM_STATES))
+    lo, hi = shard_states(wl["B"] * world, rank, world)
+    return full[lo:hi]
 
 
 class ClockSampler:
@@ -351,7 +355,7 @@ def measure(ctx, args, workload: str, batch: int, steps: int, warmup: int):
         # smallest one whose step runs >= 1 s, found from a calibration run of 2^10 states (all ranks agree on it)
         n_cal = 1 << 10
         wl["B"] = n_cal
-        cal_states = torch.from_numpy(pack_states_of(wl, rank)).to(dev)
+        cal_states = torch.from_numpy(pack_states_of(wl, rank, world)).to(dev)
         cal_ws = torch.empty(min(plan.workspace_bytes(n_cal), args.max_workspace_gb << 30), dtype=torch.uint8, device=dev)
         cal_out = torch.empty(n_cal, dtype=torch.float32, device=dev)
         for _ in range(2):
@@ -375,7 +379,7 @@ def measure(ctx, args, workload: str, batch: int, steps: int, warmup: int):
     n_out = B if states_mode else (1 << net.n_qubits)
 
     if states_mode:
-        packed = pack_states_of(wl, rank)
+        packed = pack_states_of(wl, rank, world)
         states_host = torch.from_numpy(packed).pin_memory()
         states_dev = states_host.to(dev)
         ws_bytes = min(plan.workspace_bytes_host(B), max(args.max_workspace_gb << 30,

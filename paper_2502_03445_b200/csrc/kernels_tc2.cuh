@@ -7,15 +7,15 @@
 // and ITS half of the B tile, both tensor cores read both halves of B, and each CTA accumulates 128 x BN outputs: half
 // the operand bytes per flop in L2 traffic, in TMA writes, in splitter traffic and in MMA operand reads.
 //
-// One CTA = 22 warps:
+// One CTA = 20 warps:
 //   warp 0       TMA producer (one lane): its CTA's A rows and B-half rows of every k-block (32 fp32 = one 128-byte swizzle
 //                row), 3-D maps {K, rows, state-or-key} as in kernels_tc.cuh
 //   warp 1       MMA issuer, LEADER CTA only (one lane): per k-block 8 lo MMAs then 4 hi*hi MMAs into one of two TMEM
 //                accumulators (BN columns each), tcgen05.commit multicast to both CTAs
-//   warps 2-5    splitters: the landed stage A -> hi = TF32 nearest (in place) and lo (second tile); B is used as it is for hi
+//   warps 2-3    splitters: the landed stage A -> hi = TF32 nearest (in place) and lo (second tile); B is used as it is for hi
 //                (the MMA reads the top 19 bits: a truncation) and gets a lo tile, every lo rounded to TF32 so that what the
 //                MMA drops is zero-mean; with the A residual signed and zero-mean the dropped lo*lo term has no bias either
-//   warps 6-21   accumulate + store: drain the accumulator of every k-block (tcgen05.ld 16x256b) and add it to registers in
+//   warps 4-19   accumulate + store: drain the accumulator of every k-block (tcgen05.ld 16x256b) and add it to registers in
 //                round-to-nearest -- the tensor pipe's fp32 accumulator rounds toward zero, so at most the
 //                four hi*hi accumulations of one k-block see a full-size sum; then store the finished 32 x BN/4 block straight
 //                from registers: in the 16x256b layout a quad of lanes holds 8 consecutive columns of one row, so a warp store
@@ -253,6 +253,7 @@ step_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
                 constexpr int NA = (int)(bytesA >> 4) / TC2_SPLIT, NB = (int)(bytesB >> 4) / TC2_SPLIT;   // vectors per thread
                 constexpr int CHA = NA < 16 ? NA : 16, CHB = NB < 16 ? NB : 16;     // all loads of a batch are in flight before the first use
                 static_assert(NA % CHA == 0 && NB % CHB == 0, "tile must divide over the splitter threads");
+#pragma unroll
 #pragma unroll
                 for (int c = 0; c < NA / CHA; ++c) split_tile_pair<CHA, TC2_SPLIT>(sa + (uint32_t)c * CHA * TC2_SPLIT * 16u, bytesA, ROUND_A);
 #pragma unroll
