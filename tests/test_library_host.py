@@ -193,6 +193,24 @@ def test_restarts_respect_kmax_cap_and_are_deterministic():
     assert impossible.kmax <= greedy.kmax
 
 
+def test_order_search_with_the_run_time_objective():
+    """tqc_plan_opts.objective = 1 (host only): the search keeps the order with the smallest MODELLED run time; never worse
+    than the greedy plan under that model, deterministic per seed, a valid plan (same network, m - 1 steps, root closed)."""
+    net = configs.cfg5_network()
+    B = configs.BATCH[5]
+    greedy = tqc.tqc_plan(net, tqc.MODE_STATES, batch_hint=B)
+    a = tqc.tqc_plan(net, tqc.MODE_STATES, batch_hint=B, restarts=16, seed=7, objective=1)
+    b = tqc.tqc_plan(net, tqc.MODE_STATES, batch_hint=B, restarts=16, seed=7, objective=1)
+    assert a.serialize() == b.serialize()
+    assert 0 < a.modelled_seconds_per_state <= greedy.modelled_seconds_per_state
+    assert a.num_steps == net.m - 1 and a.node(2 * net.m - 2)["n_open"] == 0
+    assert tqc.tqc_plan(_fig5_network(), tqc.MODE_DISTRIBUTION).modelled_seconds_per_state < 0      # states mode only
+    # finalize before the tensors are there is a state error, with no CUDA call involved
+    with pytest.raises(tqc.TqcError) as ei:
+        binding._check(binding._lib.tqc_plan_finalize(a._h, None))
+    assert ei.value.code == -3
+
+
 def test_simulate_description_checks_run_without_a_gpu():
     # tqc_simulate_subcircuit_tensor validates its description on the host before any CUDA call (include/tqc.h)
     import ctypes
