@@ -549,7 +549,7 @@ def measure_hss(ctx, steps: int, warmup: int) -> dict:
     torch.cuda.synchronize()
     ms = sum(a.elapsed_time(b) for a, b in evs) / steps
     nbytes = net.m * (4 ** K * 2 ** o + 2 ** o) * 4
-    peaks = measured_peaks()
+    peaks = roof_peaks()
     gbs = nbytes / (ms * 1e-3) / 1e9
     launches = plan.launch_count - l0
     plan.close()
@@ -586,7 +586,7 @@ def measure_variants(ctx, steps: int, warmup: int, with_cpu: bool = True) -> dic
     torch.cuda.synchronize()
     ms = sum(a.elapsed_time(b) for a, b in evs) / steps
     variants = 4 ** d * 3 ** u
-    peaks = measured_peaks()
+    peaks = roof_peaks()
     # Algorithmic shared-memory bytes: per preparation one pass per two-qubit gate (the one-qubit gates are
     # folded into them on the host), 32 B per amplitude (complex128 read + write); per setting one rotation pass (32 B),
     # |amp|^2 (16 B read + 8 B write), u Walsh-Hadamard passes over float64 (16 B each) and the scatter read (8 B).
@@ -599,7 +599,7 @@ def measure_variants(ctx, steps: int, warmup: int, with_cpu: bool = True) -> dic
         blocks, g_fixed = blocks * 3, g_fixed + 1
     issued_bytes = 2 ** w * (blocks * (n2q + 2.0 * g_fixed / 3.0) * 32 + 4 ** d * 3 ** u * (24 + 16 * u + 8)
                              + (4 ** d * 3 ** u - blocks) * 32)
-    peak = 148 * 128 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e9
+    peak = peaks["lds_gbs"]                                    # measured LDS.128 rate (profiles/peaks_r02.json), else derived
     gbs = smem_bytes / (ms * 1e-3) / 1e9
     assert abs(float(out[0].sum()) - 2 ** d) < 1e-3                # sum_x T[I...I, x] = 2^{d_s} (reading G16)
     cpu = None
@@ -627,7 +627,7 @@ def measure_variants(ctx, steps: int, warmup: int, with_cpu: bool = True) -> dic
             "roofline": {"bound": "smem", "kernel": "sim_variant_kernel (whole call timed: + 3 sim_kappa_axis_kernel + "
                                                     "sim_permute_cast_kernel)",
                          "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak, "traffic": None,
-                         "peak_source": "derived: 148 SMs x 32 banks x 4 B x sm_max_mhz",
+                         "peak_source": "shared-memory LDS.128 rate, " + peaks["lds_gbs_source"],
                          "algorithmic_bytes_per_launch": smem_bytes, "issued_bytes_per_launch": issued_bytes,
                          "issued_gbs": issued_bytes / (ms * 1e-3) / 1e9},
             "cpu_baseline": cpu}

@@ -43,68 +43,35 @@ __device__ __forceinline__ uint32_t insert_zero(uint32_t p, int bit) {
     return ((p >> bit) << (bit + 1)) | (p & ((1u << bit) - 1u));
 }
 
-// Shared-memory access order of the passes.  A pass on amplitude-index bit b pairs elements 2^b apart; thread p owns the
-// pair (or quad) whose other index bits are p.  With complex128 elements a quarter-warp (8 lanes) fills one 128-byte
-// wavefront when its eight 16-byte slots differ modulo 8.  For b >= 3 they do (slot mod 8 = p mod 8).  For a gate bit
-// below 3, lanes p and p + 4 (one low gate bit) or p, p + 2, p + 4, p + 6 (two) would hit the same slots in the same
-// instruction - 40 % of the wavefronts of the round-1 kernel were such conflicts - so every lane visits its elements in an
-// order rotated by its own position: element index c ^ x with x from the lane's higher bits.  The values are put back in
-// gate order with register swaps (no indexed local arrays), and the results leave in the same rotated order.
-__device__ __forceinline__ void swap2(double2 &a, double2 &b, bool doit) {
-    const double2 t = a;
-    a = doit ? b : a;
-    b = doit ? t : b;
-}
-
 __device__ __forceinline__ void sim_apply_1q(double2 *psi, int w, int bit, const double2 *m) {
     const double2 m00 = m[0], m01 = m[1], m10 = m[2], m11 = m[3];
     for (uint32_t p = threadIdx.x; p < (1u << (w - 1)); p += blockDim.x) {
         const uint32_t i0 = insert_zero(p, bit), i1 = i0 | (1u << bit);
-        const bool flip = bit < 3 && ((p >> 2) & 1u);               // lanes p and p + 4 take the pair in opposite order
-        const uint32_t first = flip ? i1 : i0, second = flip ? i0 : i1;
-        double2 a0 = psi[first], a1 = psi[second];
-        swap2(a0, a1, flip);
-        double2 r0 = cfma(m01, a1, cfma(m00, a0, make_double2(0.0, 0.0)));
-        double2 r1 = cfma(m11, a1, cfma(m10, a0, make_double2(0.0, 0.0)));
-        swap2(r0, r1, flip);
-        psi[first] = r0;
-        psi[second] = r1;
+        const double2 a0 = psi[i0], a1 = psi[i1];
+        psi[i0] = cfma(m01, a1, cfma(m00, a0, make_double2(0.0, 0.0)));
+        psi[i1] = cfma(m11, a1, cfma(m10, a0, make_double2(0.0, 0.0)));
     }
     __syncthreads();
 }
 
 __device__ __forceinline__ void sim_apply_2q(double2 *psi, int w, int b0, int b1, const double2 *m) {
     const int lo = b0 < b1 ? b0 : b1, hi = b0 < b1 ? b1 : b0;
-    // element c of the quad sets bit b0 to c >> 1 and bit b1 to c & 1; x = rotation of this lane's visiting order
-    const int nlow = (b0 < 3) + (b1 < 3);
     for (uint32_t p = threadIdx.x; p < (1u << (w - 2)); p += blockDim.x) {
         const uint32_t base = insert_zero(insert_zero(p, lo), hi);
-        uint32_t x = 0;
-        if (nlow == 2) x = (p >> 1) & 3u;
-        else if (nlow == 1) x = ((p >> 2) & 1u) << (b0 < 3 ? 1 : 0);
         uint32_t idx[4];
         double2 v[4];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            const uint32_t c = (uint32_t)k ^ x;
-            idx[k] = base | ((c >> 1) << b0) | ((c & 1u) << b1);
-            v[k] = psi[idx[k]];
+        for (int c = 0; c < 4; ++c) {
+            idx[c] = base | (uint32_t(c >> 1) << b0) | (uint32_t(c & 1) << b1);
+            v[c] = psi[idx[c]];
         }
-        // v[k] holds element k ^ x: back to gate order
-        swap2(v[0], v[1], x & 1u); swap2(v[2], v[3], x & 1u);
-        swap2(v[0], v[2], x & 2u); swap2(v[1], v[3], x & 2u);
-        double2 r[4];
 #pragma unroll
-        for (int row = 0; row < 4; ++row) {
+        for (int r = 0; r < 4; ++r) {
             double2 acc = make_double2(0.0, 0.0);
 #pragma unroll
-            for (int c = 0; c < 4; ++c) acc = cfma(m[row * 4 + c], v[c], acc);
-            r[row] = acc;
+            for (int c = 0; c < 4; ++c) acc = cfma(m[r * 4 + c], v[c], acc);
+            psi[idx[r]] = acc;
         }
-        swap2(r[0], r[1], x & 1u); swap2(r[2], r[3], x & 1u);
-        swap2(r[0], r[2], x & 2u); swap2(r[1], r[3], x & 2u);
-#pragma unroll
-        for (int k = 0; k < 4; ++k) psi[idx[k]] = r[k];
     }
     __syncthreads();
 }
@@ -196,13 +163,9 @@ __global__ void __launch_bounds__(512) sim_variant_kernel(SimArgs g) {
             const int bit = g.U_bit[j];
             for (uint32_t p = threadIdx.x; p < (size >> 1); p += blockDim.x) {
                 const uint32_t i0 = insert_zero(p, bit), i1 = i0 | (1u << bit);
-                const bool flip = bit < 4 && ((p >> 3) & 1u);        // float64: 16 elements per wavefront, lanes p and p + 8
-                const uint32_t first = flip ? i1 : i0, second = flip ? i0 : i1;
-                const double f0 = q[first], f1 = q[second];
-                const double p0 = flip ? f1 : f0, p1 = flip ? f0 : f1;
-                const double s0 = p0 + p1, s1 = p0 - p1;
-                q[first] = flip ? s1 : s0;
-                q[second] = flip ? s0 : s1;
+                const double p0 = q[i0], p1 = q[i1];
+                q[i0] = p0 + p1;
+                q[i1] = p0 - p1;
             }
             __syncthreads();
         }
