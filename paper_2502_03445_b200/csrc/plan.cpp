@@ -161,7 +161,9 @@ double order_cost_log2(const HostPlan &p, const std::vector<std::vector<int>> &l
 // Rates measured on a B200 in round 2 (profiles/r02_tc2_kernel.md, profiles/peaks_r02.md), per fp32-equivalent flop
 // (2 per multiplication of PAPER.md lines 407-412):
 //   CTA-pair tensor-pipe kernel (both outer dimensions >= 256, K >= 16)   235 TFLOP/s  ->  4.26 fs / flop
-//   one-CTA tensor-pipe kernels (larger side >= 128, smaller >= 16, K >= 32)  100 TFLOP/s  ->  10 fs / flop
+//   one-CTA tensor-pipe kernels (larger side >= 128, smaller >= 16, K >= 32)  70 TFLOP/s with a 64-wide narrow side, 20 with a
+//                                                                          16-wide one  ->  14 / 50 fs / flop; their per-state
+//                                                                          operands stream at 2.4 TB/s (415 fs / byte)
 //   fp32 FFMA tile kernel                                                  25 TFLOP/s  ->  40 fs / flop
 // plus the bytes of a per-state result that goes through HBM (0.65 / 3.9 TB/s = 167 fs / byte: the stores of a tile overlap
 // its successor's MMAs only in part) and of per-state operands read back (200 fs / byte).  A node that carries few output
@@ -191,15 +193,20 @@ int64_t order_time_fs(const HostPlan &p, const std::vector<std::vector<int>> &le
         if (table) {
             fs = (((__int128)40 << e) << cbits) / hint;              // FFMA / warp-MMA tables, once per key
         } else {
-            int fs_per_flop_x100;
+            int fs_per_flop_x100, fs_per_operand_byte = 200;
             const int hi = std::max(lgM, lgN), lo = std::min(lgM, lgN);
-            if (lo >= 8 && lgK >= 4) fs_per_flop_x100 = 426;
-            else if (hi >= 7 && lo >= 4 && lgK >= 5) fs_per_flop_x100 = 1000;
-            else fs_per_flop_x100 = 4000;
+            if (lo >= 8 && lgK >= 4) fs_per_flop_x100 = 426;                                   // CTA pairs
+            else if (hi >= 7 && lo >= 4 && lgK >= 5) {                                         // one-CTA tensor kernels: the narrow
+                fs_per_flop_x100 = lo >= 6 ? 1400 : 5000;                                      // side sets the tile (70 / 20 TFLOP/s)
+                fs_per_operand_byte = 415;                                                     // and they stream operands at 2.4 TB/s
+            } else fs_per_flop_x100 = 4000;
             fs = ((__int128)fs_per_flop_x100 << e) / 100;
+            __int128 rd = 0;
+            if (kind[ab.first] == 2) rd += (__int128)fs_per_operand_byte * 4 << std::min(2 * (int)A.size(), 100);
+            if (kind[ab.second] == 2) rd += (__int128)fs_per_operand_byte * 4 << std::min(2 * (int)B.size(), 100);
+            if (fs_per_operand_byte == 415) fs = std::max(fs, rd);   // narrow tiles: MMAs and the operand stream overlap, the slower one counts
+            else fs += rd;
             fs += (__int128)167 * 4 << std::min(2 * copen, 100);     // result bytes
-            if (kind[ab.first] == 2) fs += (__int128)200 * 4 << std::min(2 * (int)A.size(), 100);
-            if (kind[ab.second] == 2) fs += (__int128)200 * 4 << std::min(2 * (int)B.size(), 100);
         }
         total += fs;
         std::vector<int> merged = set_xor(A, B);
