@@ -35,7 +35,7 @@ UNIT = "states/s"
 SM_COUNT = 148                  # B200 (B200_PROFILING.md)
 FP32_LANES_PER_SM = 128
 NOMINAL_TF32_OVER_BF16 = 1.1 / 2.25   # nominal dense peaks (B200_PROFILING.md table)
-TC_KERNEL_NAMES = "step_tc_kernel<BN> / step_tcw_kernel"
+TC_KERNEL_NAMES = "step_tc2_kernel on CTA pairs, step_tc_kernel<BN> on one CTA"
 
 
 def measured_peaks() -> dict:

@@ -65,7 +65,7 @@ enum { TQC_MODE_STATES = 0, TQC_MODE_DISTRIBUTION = 1 };
  *            warp per state, intermediates in shared memory, bond sums finished by warp shuffles. */
 enum { TQC_KERNEL_SIMT_TILE = 0, TQC_KERNEL_DOT = 1, TQC_KERNEL_TCGEN05 = 2, TQC_KERNEL_CHAIN = 3 };
 /* TCGEN05 steps with both outer dimensions >= 256 run step_tc2_kernel: 256 x 256 tiles over CTA pairs (cta_group::2), which
- * halve the operand bytes per flop; the others run the one-CTA kernels step_tc_kernel<BN> / step_tcw_kernel. */
+ * halve the operand bytes per flop; the others run the one-CTA kernel step_tc_kernel<BN>. */
 /* How a node of the contraction tree is evaluated. */
 enum { TQC_NODE_LEAF = 0, TQC_NODE_TABLE = 1, TQC_NODE_BATCH = 2 };
 

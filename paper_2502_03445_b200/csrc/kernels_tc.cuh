@@ -129,27 +129,6 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[32]) {  
 }
 
 
-// hi/lo split of NV 16-byte vectors per thread (stride TC_SPLIT_THREADS vectors), raw tile at `addr`, lo tile `lo_ofs` bytes
-// further: lo = x - (x & 0xFFFFE000) is exact in fp32; explicit shared-space accesses, all loads issued before the math
-// same as split_tile for a splitter of NT threads, raw tile kept as it is (the MMA ignores the low mantissa bits)
-template <int NV, int NT>
-__device__ __forceinline__ void split_tile_n(uint32_t addr, uint32_t lo_ofs, bool round_hi) {
-    uint4 x[NV];
-#pragma unroll
-    for (int v = 0; v < NV; ++v)
-        asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(x[v].x), "=r"(x[v].y), "=r"(x[v].z), "=r"(x[v].w)
-                     : "r"(addr + (uint32_t)v * (NT * 16u)));
-#pragma unroll
-    for (int v = 0; v < NV; ++v) {
-        const uint32_t rnd = round_hi ? 0x1000u : 0u;
-        const uint4 h = make_uint4((x[v].x + rnd) & 0xFFFFE000u, (x[v].y + rnd) & 0xFFFFE000u, (x[v].z + rnd) & 0xFFFFE000u, (x[v].w + rnd) & 0xFFFFE000u);
-        const float l0 = __uint_as_float(x[v].x) - __uint_as_float(h.x), l1 = __uint_as_float(x[v].y) - __uint_as_float(h.y);
-        const float l2 = __uint_as_float(x[v].z) - __uint_as_float(h.z), l3 = __uint_as_float(x[v].w) - __uint_as_float(h.w);
-        asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr + (uint32_t)v * (NT * 16u) + lo_ofs), "f"(l0), "f"(l1), "f"(l2), "f"(l3) : "memory");
-        if (round_hi) asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr + (uint32_t)v * (NT * 16u)), "r"(h.x), "r"(h.y), "r"(h.z), "r"(h.w) : "memory");
-    }
-}
-
 // bit map applied to a small index (a lane id or a column within a vector): same as bitmap_apply
 __device__ __forceinline__ unsigned long long bitmap_apply_small(const BitMap &m, unsigned x) { return bitmap_apply(m, (unsigned long long)x); }
 
@@ -462,186 +441,6 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
     if (warp == 1) {
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(tmem_cols) : "memory");
-    }
-}
-
-// ---------------------------------------------------------------------------------------------------------------------
-// Wide-tile variant for steps with N >= 256: 128 x 256 tiles halve the shared-memory operand bytes per MMA flop (the limit
-// of the 128 x 128 kernel above).  TMEM then holds only two 256-column accumulators, so all three MMAs of a k-block go
-// to ONE accumulator, the eight lo MMAs first (while the sum is still 2^-11 of its final size their round-toward-zero
-// steps do not matter) and the four hi*hi MMAs last; the accumulator is drained and added to registers in
-// round-to-nearest after EVERY k-block (two accumulators alternate): four full-size accumulations per drain, as in the
-// 128 x 128 kernel.  20 warps: TMA, MMA, 2 splitter warps, 16 accumulate/epilogue warps (4 column groups of 64 x
-// 4 TMEM lane quadrants); two stages of 96 KB.  Results go straight from registers to C as 16-byte vectors (with operand
-// digits ordered by the result's layout a thread's 64 columns form contiguous runs of C).
-// ---------------------------------------------------------------------------------------------------------------------
-constexpr int TCW_BN = 256;
-constexpr int TCW_THREADS = 640;
-constexpr int TCW_STAGES = 2;
-
-__device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t (&v)[8]) {
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
-                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]) : "r"(taddr));
-}
-
-__global__ void __launch_bounds__(TCW_THREADS, 1)
-step_tcw_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB, const TcArgs a) {
-    extern __shared__ unsigned char tc_smem_raw[];
-    __shared__ __align__(8) uint64_t full_bar[TCW_STAGES], ready_bar[TCW_STAGES], empty_bar[TCW_STAGES], d_full_bar[2], d_empty_bar[2];
-    __shared__ uint32_t tmem_base_slot;
-    __shared__ uint32_t oa_mt[256], oa_q[4], ob_nt[256], ob_c4[TCW_BN / 4];      // C-offset tables: m-tile, quadrant, n-tile, column / 4
-
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    constexpr uint32_t bytesA = TC_BM * TC_BK * 4, bytesB = (uint32_t)TCW_BN * TC_BK * 4;
-    constexpr uint32_t stage_bytes = 2 * bytesA + 2 * bytesB;
-    unsigned char *tiles = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(tc_smem_raw) + 1023) & ~(uintptr_t)1023);
-    auto A_raw = [&](int s) { return tiles + (size_t)s * stage_bytes; };
-    auto A_lo = [&](int s) { return tiles + (size_t)s * stage_bytes + bytesA; };
-    auto B_raw = [&](int s) { return tiles + (size_t)s * stage_bytes + 2 * bytesA; };
-    auto B_lo = [&](int s) { return tiles + (size_t)s * stage_bytes + 2 * bytesA + bytesB; };
-
-    const int n_kb = 1 << (a.lgK - 5);
-    const long long tiles_m = 1ll << (a.lgM - 7), tiles_n = 1ll << (a.lgN - 8);
-    const int lg_tn = a.lgN - 8, lg_tm = a.lgM - 7;
-    const long long total = tiles_m * tiles_n * a.R;
-
-    for (int x = threadIdx.x; x < 256; x += TCW_THREADS) {
-        oa_mt[x] = x < tiles_m ? (uint32_t)bitmap_apply(a.outA, (unsigned long long)x * TC_BM) : 0u;
-        ob_nt[x] = x < tiles_n ? (uint32_t)bitmap_apply(a.outB, (unsigned long long)x * TCW_BN) : 0u;
-        if (x < 4) oa_q[x] = (uint32_t)bitmap_apply(a.outA, (unsigned long long)x * 32);
-        if (x < TCW_BN / 4) ob_c4[x] = (uint32_t)bitmap_apply(a.outB, (unsigned long long)x * 4);
-    }
-    if (threadIdx.x == 0) {
-        for (int s = 0; s < TCW_STAGES; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&ready_bar[s], 2); mbar_init(&empty_bar[s], 1); }
-        for (int s = 0; s < 2; ++s) { mbar_init(&d_full_bar[s], 1); mbar_init(&d_empty_bar[s], 16); }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    if (warp == 0 && lane == 0) {
-        asm volatile("prefetch.tensormap [%0];" ::"l"(&mapA) : "memory");
-        asm volatile("prefetch.tensormap [%0];" ::"l"(&mapB) : "memory");
-    }
-    if (warp == 1) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_slot)), "r"(512u) : "memory");
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-    }
-    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-    __syncthreads();
-    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-    const uint32_t tmem_base = tmem_base_slot;
-
-    if (warp == 0) {
-        if (lane == 0) {                                     // ===== TMA producer =====
-            long long it = 0;
-            for (long long t = blockIdx.x; t < total; t += gridDim.x) {
-                const long long nt = t & (tiles_n - 1), mt = (t >> lg_tn) & (tiles_m - 1), r = t >> (lg_tn + lg_tm);
-                const int rowA = a.keysA ? (int)a.keysA[r] : (int)r;
-                const int rowB = a.keysB ? (int)a.keysB[r] : (int)r;
-                for (int kb = 0; kb < n_kb; ++kb, ++it) {
-                    const int s = (int)(it % TCW_STAGES);
-                    const uint32_t ph = (uint32_t)((it / TCW_STAGES) & 1);
-                    mbar_wait(&empty_bar[s], ph ^ 1u);
-                    mbar_expect_tx(&full_bar[s], bytesA + bytesB);
-                    tma_load_3d(&mapA, &full_bar[s], A_raw(s), kb * TC_BK, (int)(mt * TC_BM), rowA);
-                    tma_load_3d(&mapB, &full_bar[s], B_raw(s), kb * TC_BK, (int)(nt * TCW_BN), rowB);
-                }
-            }
-        }
-    } else if (warp == 1) {                                  // ===== MMA issuer =====
-        constexpr uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(TCW_BN >> 3) << 17) | ((uint32_t)(TC_BM >> 4) << 24);
-        long long it = 0;
-        for (long long t = blockIdx.x; t < total; t += gridDim.x) {
-            for (int kb = 0; kb < n_kb; ++kb, ++it) {
-                const int s = (int)(it % TCW_STAGES);
-                const uint32_t ph = (uint32_t)((it / TCW_STAGES) & 1);
-                const uint32_t db = (uint32_t)(it & 1), dph = (uint32_t)((it >> 1) & 1);
-                mbar_wait(&d_empty_bar[db], dph ^ 1u);
-                mbar_wait(&ready_bar[s], ph);
-                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                const uint32_t d_tmem = tmem_base + db * (uint32_t)TCW_BN;
-                const uint64_t dah = umma_desc_sw128(smem_u32(A_raw(s))), dal = umma_desc_sw128(smem_u32(A_lo(s)));
-                const uint64_t dbh = umma_desc_sw128(smem_u32(B_raw(s))), dbl = umma_desc_sw128(smem_u32(B_lo(s)));
-                if (lane == 0 && TQC_DBG(a, 32)) { umma_commit(&empty_bar[s]); umma_commit(&d_full_bar[db]); }
-                else if (lane == 0) {
-                    // the small terms first: while the accumulator holds only lo products (2^-11 of the final value) its
-                    // round-toward-zero steps are 2^-11 smaller too; only the four hi*hi accumulations see a full-size sum
-#pragma unroll
-                    for (int k = 0; k < TC_BK / 8; ++k) {
-                        umma_tf32(d_tmem, dal + (uint64_t)(2 * k), dbh + (uint64_t)(2 * k), idesc, k ? 1u : 0u);
-                        umma_tf32(d_tmem, dah + (uint64_t)(2 * k), dbl + (uint64_t)(2 * k), idesc, 1u);
-                    }
-#pragma unroll
-                    for (int k = 0; k < TC_BK / 8; ++k) umma_tf32(d_tmem, dah + (uint64_t)(2 * k), dbh + (uint64_t)(2 * k), idesc, 1u);
-                    umma_commit(&empty_bar[s]);
-                    umma_commit(&d_full_bar[db]);
-                }
-                __syncwarp();
-            }
-        }
-    } else if (warp < 4) {                                   // ===== splitter: 64 threads =====
-        const int st = threadIdx.x - 64;
-        long long it = 0;
-        for (long long t = blockIdx.x; t < total; t += gridDim.x) {
-            for (int kb = 0; kb < n_kb; ++kb, ++it) {
-                const int s = (int)(it % TCW_STAGES);
-                const uint32_t ph = (uint32_t)((it / TCW_STAGES) & 1);
-                mbar_wait(&full_bar[s], ph);
-                const uint32_t sa = smem_u32(A_raw(s)) + (uint32_t)st * 16u;
-                if (!TQC_DBG(a, 4)) {
-#pragma unroll
-                for (int c = 0; c < (int)(bytesA >> 4) / 64 / 8; ++c) split_tile_n<8, 64>(sa + (uint32_t)c * 8u * 64u * 16u, bytesA, a.mask_hi != 0);
-#pragma unroll
-                for (int c = 0; c < (int)(bytesB >> 4) / 64 / 8; ++c) split_tile_n<8, 64>(sa + 2u * bytesA + (uint32_t)c * 8u * 64u * 16u, bytesB, a.mask_hi != 0);
-                }
-                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&ready_bar[s]);
-            }
-        }
-    } else {                                                 // ===== accumulate + epilogue: 16 warps =====
-        const int w4 = warp & 3, grp = (warp - 4) >> 2;
-        const uint32_t lane_base = ((uint32_t)(32 * w4) << 16) + (uint32_t)(64 * grp);
-        long long it = 0;
-        for (long long t = blockIdx.x; t < total; t += gridDim.x) {
-            const long long nt = t & (tiles_n - 1), mt = (t >> lg_tn) & (tiles_m - 1), r = t >> (lg_tn + lg_tm);
-            float acc[64];
-#pragma unroll
-            for (int q = 0; q < 64; ++q) acc[q] = 0.f;
-            for (int kb = 0; kb < n_kb; ++kb, ++it) {
-                const uint32_t db = (uint32_t)(it & 1), dph = (uint32_t)((it >> 1) & 1);
-                mbar_wait(&d_full_bar[db], dph);
-                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                const uint32_t taddr = tmem_base + lane_base + db * (uint32_t)TCW_BN;
-                if (!TQC_DBG(a, 8))
-#pragma unroll
-                for (int c0 = 0; c0 < 64; c0 += 8) {
-                    uint32_t v[8];
-                    tmem_ld8(taddr + c0, v);
-                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-                    for (int q = 0; q < 8; ++q) acc[c0 + q] += __uint_as_float(v[q]);
-                }
-                asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&d_empty_bar[db]);
-            }
-            float *crow = a.C + r * a.c_row_stride + (oa_mt[mt] | oa_q[w4] | ob_nt[nt]) + bitmap_apply_small(a.outA, (unsigned)lane);
-            if (TQC_DBG(a, 2)) continue;
-            if (a.vec4) {
-#pragma unroll
-                for (int q = 0; q < 64; q += 4)
-                    *reinterpret_cast<float4 *>(crow + ob_c4[16 * grp + q / 4]) = make_float4(acc[q], acc[q + 1], acc[q + 2], acc[q + 3]);
-            } else {
-#pragma unroll
-                for (int q = 0; q < 64; ++q) crow[ob_c4[16 * grp + q / 4] + (uint32_t)bitmap_apply_small(a.outB, (unsigned)(q & 3))] = acc[q];
-            }
-        }
-    }
-
-    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-    __syncthreads();
-    if (warp == 1) {
-        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512u) : "memory");
     }
 }
 

@@ -193,7 +193,6 @@ int ensure_device_attrs(int *sm_count) {
         TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc_kernel<32>, dyn, 201 * 1024));
         TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc_kernel<64>, dyn, 201 * 1024));
         TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc_kernel<128>, dyn, 201 * 1024));
-        TQC_CUDA(cudaFuncSetAttribute(tqc::step_tcw_kernel, dyn, 194 * 1024));
         TQC_CUDA(cudaFuncSetAttribute(tqc::step_tc2_kernel<256>, dyn, 194 * 1024));
         TQC_CUDA(cudaFuncSetAttribute(tqc::chain_kernel, dyn, 128 * 1024));
         TQC_CUDA(cudaFuncSetAttribute(tqc::sim_variant_kernel<false>, dyn, 24 << 13));
@@ -476,28 +475,14 @@ int launch_tc_step(tqc_plan_t *pl, TcOperand A, TcOperand B, BitMap outA, BitMap
     // the M side needs >= 128 rows; with both sides large, the N side (vector stores run along it) takes C's lowest bits
     bool swap = lgM < 7;
     if (lgM >= 7 && lgN >= 7 && has_bit0(outA)) swap = true;
-    // wide tiles (128 x 256) need N >= 256: when only one side reaches 256 it becomes N
-    static const bool no_wide = dev_env("TQC_TC_NO_WIDE") != nullptr;
-    if (lgM >= 7 && lgN >= 7 && !no_wide) {
-        const int n_if_keep = lgN, n_if_swap = lgM;
-        if (swap && n_if_swap < 8 && n_if_keep >= 8) swap = false;
-        else if (!swap && n_if_keep < 8 && n_if_swap >= 8) swap = true;
-    }
     if (swap) { std::swap(A, B); std::swap(outA, outB); std::swap(lgM, lgN); }
-    // The wide kernel stores results straight from registers (a lane owns one row and 64 consecutive columns).  That is
-    // efficient when the bond loop is long (K >= 256 amortises the unstaged epilogue) and the N side's contiguous run in
-    // C is short (<= 16 floats), so that the 16-byte stores of adjacent lanes fall next to each other; with long runs
-    // adjacent lanes are KBs apart and the staged, permuted epilogue of the 128 x 128 kernel wins (measured per step on
-    // cfg5, profiles/r01c notes).
-    const int run_len = (outB.n >= 1 && outB.src[0] == 0 && outB.dst[0] == 0) ? outB.len[0] : 0;
-    const bool wide = lgN >= 8 && lgM >= 7 && lgK >= 8 && run_len >= 2 && run_len <= 4 && !no_wide;
     tqc::TcArgs a;
     memset(&a, 0, sizeof(a));
     a.keysA = A.keys; a.keysB = B.keys;
     a.C = C; a.c_row_stride = c_row_stride;
     a.outA = outA; a.outB = outB;
     a.lgM = lgM; a.lgN = lgN; a.lgK = lgK; a.R = R;
-    a.BN = wide ? tqc::TCW_BN : (int)std::min<long long>(128, 1ll << lgN);
+    a.BN = (int)std::min<long long>(128, 1ll << lgN);
     { const char *dbg = dev_env("TQC_TC_DEBUG"); a.debug = dbg ? std::atoi(dbg) : 0; }
     { const char *ck = dev_env("TQC_TC_CHUNK"); a.chunk_kb = ck ? std::atoi(ck) : 0; }
     // hi parts rounded to nearest (rewritten in shared memory): removes the systematic -2.4e-7 per step of the truncating
@@ -513,14 +498,9 @@ int launch_tc_step(tqc_plan_t *pl, TcOperand A, TcOperand B, BitMap outA, BitMap
     const long long total = (1ll << (lgM - 7)) * ((1ll << lgN) / a.BN) * (long long)R;
     const unsigned grid = (unsigned)std::min<long long>(total, sm_count);
     if (dev_env("TQC_TC_TRACE"))
-        fprintf(stderr, "tc step %d: lgM %d lgN %d lgK %d swap %d wide %d vec4 %d keyedA %d keyedB %d R %d outB.n %d outB[0]=(%d,%d,%d)\n", tag, lgM, lgN, lgK,
-                (int)swap, (int)wide, a.vec4, A.keys != nullptr, B.keys != nullptr, R, outB.n, outB.src[0], outB.dst[0], outB.len[0]);
+        fprintf(stderr, "tc step %d: lgM %d lgN %d lgK %d swap %d vec4 %d keyedA %d keyedB %d R %d outB.n %d outB[0]=(%d,%d,%d)\n", tag, lgM, lgN, lgK,
+                (int)swap, a.vec4, A.keys != nullptr, B.keys != nullptr, R, outB.n, outB.src[0], outB.dst[0], outB.len[0]);
     if ((rc = note_launch(pl, tag, st))) return rc;
-    if (wide) {
-        tqc::step_tcw_kernel<<<grid, tqc::TCW_THREADS, tqc::TCW_STAGES * stage_bytes + 1024, st>>>(mapA, mapB, a);
-        TQC_CUDA(cudaGetLastError());
-        return 0;
-    }
     const size_t smem = a.stages * stage_bytes + 1024;
     switch (a.BN) {
         case 16: tqc::step_tc_kernel<16><<<grid, tqc::TC_THREADS, smem, st>>>(mapA, mapB, a); break;

@@ -46,6 +46,9 @@ def test_sliced_states_match_oracle(seed, slice_cuts):
     # a workspace that forces several chunks (partial-sum buffer + minimum + a little)
     small = torch.empty(plan.workspace_min_bytes() + 4 * 777 + 256 + 150 * 64, dtype=torch.uint8, device="cuda")
     assert np.array_equal(_states(plan, bits, workspace=small), got)
+    # the advertised minimum is enough (include/tqc.h): the batch is then cut into pieces, each summed over all sub-networks
+    tiny = torch.empty(plan.workspace_min_bytes(), dtype=torch.uint8, device="cuda")
+    assert np.array_equal(_states(plan, bits, workspace=tiny), got)
     # reloading a tensor replaces every slice of it
     T2 = [t.copy() for t in T]
     T2[0] = T2[0][::-1].copy()
