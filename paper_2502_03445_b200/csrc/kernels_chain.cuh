@@ -134,7 +134,10 @@ __device__ __forceinline__ void mma_tf32_16x8x8(float (&d)[4], const uint32_t (&
 // one state is an M x N x K product small enough for mma.sync fragments, far too small for a tcgen05 tile.  3xTF32
 // (lo*hi + hi*lo + hi*hi, fp32 accumulate); each lane loads 4 A and 2 B scalars per 16x8x8 block from the K-major rows
 // (conflict-free with the 4-float row pad) and splits them once per k-step.
-template <int LGM, int LGN, int LGK, int PA, int PB, class Emit>
+// SLICE_SUM: see the comment at the MMAs.  The table steps (kernels_cross.cuh) feed one another - cfg5 runs 24 in a row -
+// and take the slice sums; a chain's one product per state keeps the running accumulator (cfg4: mean error -5e-8 of max p,
+// and the extra adds cost 1.5 % of the chain kernel).
+template <int LGM, int LGN, int LGK, int PA, int PB, bool SLICE_SUM = false, class Emit>
 __device__ __forceinline__ void chain_step_mma(const float *pa, const float *pb, int lane, Emit emit) {
     constexpr int MT = (1 << LGM) / 16, NT = (1 << LGN) / 8, K = 1 << LGK;
     const int g = lane >> 2, t = lane & 3;
@@ -166,9 +169,21 @@ __device__ __forceinline__ void chain_step_mma(const float *pa, const float *pb,
         for (int mi = 0; mi < MT; ++mi)
 #pragma unroll
             for (int nj = 0; nj < NT; ++nj) {
-                mma_tf32_16x8x8(acc[mi][nj], al[mi], bh[nj]);       // small terms first
-                mma_tf32_16x8x8(acc[mi][nj], ah[mi], bl[nj]);
-                mma_tf32_16x8x8(acc[mi][nj], ah[mi], bh[nj]);
+                // the tensor pipe truncates its accumulator (measured: DESIGN.md 5.3), so a running sum kept there drifts
+                // by about -0.5 ulp per MMA.  With SLICE_SUM each bond slice is summed from zero (small terms first: one
+                // truncation at the slice's own magnitude) and joins the running sum in registers, rounded to nearest.
+                if constexpr (SLICE_SUM) {
+                    float d[4] = {0.f, 0.f, 0.f, 0.f};
+                    mma_tf32_16x8x8(d, al[mi], bh[nj]);
+                    mma_tf32_16x8x8(d, ah[mi], bl[nj]);
+                    mma_tf32_16x8x8(d, ah[mi], bh[nj]);
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) acc[mi][nj][e] += d[e];
+                } else {
+                    mma_tf32_16x8x8(acc[mi][nj], al[mi], bh[nj]);       // small terms first
+                    mma_tf32_16x8x8(acc[mi][nj], ah[mi], bl[nj]);
+                    mma_tf32_16x8x8(acc[mi][nj], ah[mi], bh[nj]);
+                }
             }
     }
 #pragma unroll

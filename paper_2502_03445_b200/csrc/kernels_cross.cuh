@@ -2,7 +2,9 @@
 //     C[outA(i') | outB(j')] = sum_k A[rowA(i'), k] * B[rowB(j'), k]
 // is one M' x N' x K product per step (PAPER.md lines 318-330 merged bond).  With K this
 // short the fp32 FFMA kernel is bound by instruction issue, not by the result write, so the products run on the tensor
-// pipe as warp-level 3xTF32 mma.sync blocks (kernels_chain.cuh: chain_step_mma), 64 x 128 outputs per 256-thread block.
+// pipe as warp-level 3xTF32 mma.sync blocks (kernels_chain.cuh: chain_step_mma, one bond slice of 8 per accumulator and the
+// slices added in registers: table steps feed one another and the pipe's truncating accumulator would drift), 64 x 128
+// outputs per 256-thread block.
 // Where j' and j' + 1 are neighbours in C (the usual case: the result layout keeps the operand's digit order) the results
 // leave straight from the fragments as 8-byte stores, four lanes per 32-byte sector; otherwise the tile goes through
 // shared memory and leaves row by row.
@@ -56,7 +58,7 @@ __global__ void __launch_bounds__(256, 4) cross_mma_kernel(const StepArgs a) {
         // lanes fill a 32-byte sector, no trip through shared memory
         const int wi = warp >> 2, wj = warp & 3;
         float keep = 0.f;
-        chain_step_mma<5, 5, LGK, P, P>(As + 32 * wi * P, Bs + 32 * wj * P, lane, [&](int i, int j, float v) {
+        chain_step_mma<5, 5, LGK, P, P, true>(As + 32 * wi * P, Bs + 32 * wj * P, lane, [&](int i, int j, float v) {
             if ((j & 1) == 0) keep = v;
             else *reinterpret_cast<float2 *>(a.C + (offA[32 * wi + i] | offB[32 * wj + j - 1])) = make_float2(keep, v);
         });
@@ -65,7 +67,7 @@ __global__ void __launch_bounds__(256, 4) cross_mma_kernel(const StepArgs a) {
     {   // warp grid 2 x 4 over the 64 x 128 tile: 32 x 32 outputs per warp
         const int wi = warp >> 2, wj = warp & 3;
         float *cw = Cs + (32 * wi) * CROSS_CP + 32 * wj;
-        chain_step_mma<5, 5, LGK, P, P>(As + 32 * wi * P, Bs + 32 * wj * P, lane, [&](int i, int j, float v) { cw[i * CROSS_CP + j] = v; });
+        chain_step_mma<5, 5, LGK, P, P, true>(As + 32 * wi * P, Bs + 32 * wj * P, lane, [&](int i, int j, float v) { cw[i * CROSS_CP + j] = v; });
     }
     __syncthreads();
     for (int e = tid; e < CROSS_TI * (CROSS_TJ / 4); e += 256) {
