@@ -278,6 +278,24 @@ size_t tqc_simulate_workspace_bytes(const tqc_subcircuit_desc *sub);
 int tqc_simulate_subcircuit_tensor(const tqc_subcircuit_desc *sub, float *out_dev, void *workspace_dev,
                                    size_t workspace_bytes, void *stream);
 
+/* ---- Callers that cannot allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc) -------------------
+ * tqc_simulate_subcircuit_tensor_static is tqc_simulate_subcircuit_tensor (same section of the paper, lines 182-192; same
+ * kernels, same results) with NO workspace argument: the scratch of the simulation kernel - the device copy of the gate list
+ * and the fp64 array R [4^{d+u}][2^o] the variants are accumulated in - lives in one array of TQC_STATIC_SCRATCH_BYTES (8 MiB)
+ * that is part of the library image: every GPU that loads the library holds those 8 MiB until the process exits, and the call
+ * itself calls no cudaMalloc, cudaFree or allocating library routine (host side: a std::vector of the gate list).
+ *   sub, out_dev, stream: as for tqc_simulate_subcircuit_tensor (sub HOST, out_dev DEVICE [4^{d+u}][2^o] fp32, caller-owned).
+ *   Limit: tqc_simulate_workspace_bytes(sub) <= tqc_static_scratch_bytes() = 8 MiB, i.e. w <= 13 wires and roughly
+ *   4^{d+u} 2^o <= 2^19 entries with a few thousand gates; anything larger returns TQC_E_TOO_LARGE (the message names both
+ *   sizes) and launches nothing - use the workspace entry point for it.  Other errors as tqc_simulate_subcircuit_tensor.
+ *   The device must be current when the call is made (the array's address is looked up once per device).
+ *   The array is SHARED by every call on a device and keeps the last call's contents: the part a call reads is cleared or
+ *   overwritten by that call first, so calls that follow one another on one stream (or are ordered by events) are
+ *   independent; two calls that may OVERLAP on the GPU (different streams, different host threads) race on it - order them. */
+#define TQC_STATIC_SCRATCH_BYTES (8u << 20)
+size_t tqc_static_scratch_bytes(void);
+int tqc_simulate_subcircuit_tensor_static(const tqc_subcircuit_desc *sub, float *out_dev, void *stream);
+
 /* ---- Front half: circuit -> DAG -> partition -> cuts -> network -> plan (section 6) ---------------
  * The circuit is cut by partitioning its two-qubit gates (lines 578-594: the DAG keeps only two-qubit gates, a one-qubit
  * gate follows its adjacent two-qubit gate, input / output terminals are never cut) with Greedy Graph Growing (Alg. 2,

@@ -34,7 +34,8 @@ EXPORTED = ["tqc_plan", "tqc_plan_destroy", "tqc_plan_mode", "tqc_plan_num_qubit
             "tqc_plan_profile_enable", "tqc_plan_profile_read", "tqc_plan_chain_status", "tqc_hss_scores", "tqc_hss_select",
             "tqc_hss_expand", "tqc_plan_num_sliced_cuts", "tqc_choose_slice_cuts", "tqc_hss_prepare",
             "tqc_hss_workspace_bytes", "tqc_hss_contract", "tqc_simulate_workspace_bytes",
-            "tqc_simulate_subcircuit_tensor", "tqc_plan_finalize", "tqc_plan_from_circuit", "tqc_plan_from_gates",
+            "tqc_simulate_subcircuit_tensor", "tqc_simulate_subcircuit_tensor_static", "tqc_static_scratch_bytes",
+            "tqc_plan_finalize", "tqc_plan_from_circuit", "tqc_plan_from_gates",
             "tqc_plan_cut_network", "tqc_plan_cut_subcircuit", "tqc_plan_cut_assignment", "tqc_cut_merging_cost",
             "tqc_plan_cost_report", "tqc_plan_pair_launch_count", "tqc_plan_modelled_seconds_per_state"]
 
@@ -144,6 +145,9 @@ def _load() -> ctypes.CDLL:
     lib.tqc_simulate_workspace_bytes.argtypes = [POINTER(_SubcircuitDesc)]
     lib.tqc_simulate_workspace_bytes.restype = c_size_t
     lib.tqc_simulate_subcircuit_tensor.argtypes = [POINTER(_SubcircuitDesc), c_void_p, c_void_p, c_size_t, c_void_p]
+    lib.tqc_simulate_subcircuit_tensor_static.argtypes = [POINTER(_SubcircuitDesc), c_void_p, c_void_p]
+    lib.tqc_static_scratch_bytes.argtypes = []
+    lib.tqc_static_scratch_bytes.restype = c_size_t
     lib.tqc_plan_from_circuit.argtypes = [c_char_p, POINTER(_CutOpts), POINTER(_PlanOpts), POINTER(c_void_p)]
     lib.tqc_plan_from_gates.argtypes = [c_int, POINTER(_Gate), c_int, POINTER(_CutOpts), POINTER(_PlanOpts), POINTER(c_void_p)]
     lib.tqc_plan_cut_network.argtypes = [c_void_p, POINTER(_NetworkDesc)]
@@ -542,6 +546,20 @@ def tqc_hss_contract(plan: Plan, x, out=None, workspace=None, stream=None, devic
     if workspace is None:
         workspace = torch.empty(max(256, int(_lib.tqc_hss_workspace_bytes(plan._h))), dtype=torch.uint8, device=device)
     _check(_lib.tqc_hss_contract(plan._h, out.data_ptr(), workspace.data_ptr(), workspace.numel(), _stream_ptr(stream)))
+    return out
+
+
+def tqc_static_scratch_bytes() -> int:
+    return int(_lib.tqc_static_scratch_bytes())
+
+
+def tqc_simulate_subcircuit_tensor_static(w, gates, D_wires, U_wires, O_wires, bond_pos, out, stream=None, fuse_gates=True,
+                                          walk_settings=True):
+    """tqc_simulate_subcircuit_tensor without a workspace and without any device allocation (tqc.h: "Callers that cannot
+    allocate"): `out` is the caller's CUDA fp32 [4^{d+u}, 2^o] tensor, the kernel's scratch is the library's static 8 MiB
+    array.  TqcError(TQC_E_TOO_LARGE) when the subcircuit needs more scratch than that."""
+    desc, _keep = _subcircuit_desc(w, gates, D_wires, U_wires, O_wires, bond_pos, fuse_gates, walk_settings)
+    _check(_lib.tqc_simulate_subcircuit_tensor_static(byref(desc), out.data_ptr(), _stream_ptr(stream)))
     return out
 
 

@@ -2036,6 +2036,53 @@ int tqc_simulate_subcircuit_tensor(const tqc_subcircuit_desc *sub, float *out_de
     return 0;
 }
 
+// ---- allocation-free variant of tqc_simulate_subcircuit_tensor (tqc.h: "Callers that cannot allocate") ---------------------
+// The gate list and the fp64 result array R of sim_variant_kernel live in ONE file-scope device array instead of a caller's
+// workspace.  In host code `tqc_static_scratch` is only the host-side stand-in of the symbol: its device address is looked
+// up once per device, with that device current, and that pointer is what the kernels get.
+namespace {
+static __device__ __align__(256) unsigned char tqc_static_scratch[TQC_STATIC_SCRATCH_BYTES];
+
+int static_scratch_ptr(void **out) {
+    static std::mutex mu;
+    static void *ptrs[TQC_MAX_DEVICES] = {};
+    int dev = 0;
+    TQC_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= TQC_MAX_DEVICES) return fail(TQC_E_TOO_LARGE, "device ordinal beyond the library's table");
+    std::lock_guard<std::mutex> lock(mu);
+    if (!ptrs[dev]) {
+        void *p = nullptr;
+        TQC_CUDA(cudaGetSymbolAddress(&p, tqc_static_scratch));      // the address on the CURRENT device
+        if (!p || ((uintptr_t)p & 255)) return fail(TQC_E_CUDA, "static scratch array has no usable device address");
+        ptrs[dev] = p;
+    }
+    *out = ptrs[dev];
+    return 0;
+}
+}  // namespace
+
+size_t tqc_static_scratch_bytes(void) { return (size_t)TQC_STATIC_SCRATCH_BYTES; }
+
+int tqc_simulate_subcircuit_tensor_static(const tqc_subcircuit_desc *sub, float *out_dev, void *stream) {
+    if (!sub || !out_dev) return fail(TQC_E_ARG, "null argument");
+    const size_t need = tqc_simulate_workspace_bytes(sub);
+    if (need == 0) return fail(TQC_E_ARG, "subcircuit description out of range (tqc_simulate_workspace_bytes = 0)");
+    if (need > (size_t)TQC_STATIC_SCRATCH_BYTES)
+        return fail(TQC_E_TOO_LARGE, "this subcircuit needs " + std::to_string(need) + " bytes of scratch, the static array holds " +
+                                         std::to_string((size_t)TQC_STATIC_SCRATCH_BYTES) +
+                                         " (tqc_static_scratch_bytes): use tqc_simulate_subcircuit_tensor with a workspace");
+    void *scratch = nullptr;
+    const int rc = static_scratch_ptr(&scratch);
+    if (rc) return rc;
+    // the array keeps the last call's contents.  The gate list is overwritten by this call's copy and every entry of R that
+    // the later passes read is written by sim_variant_kernel first; R is cleared all the same, so that no value of an
+    // earlier call can reach out_dev whatever the description
+    const size_t gate_bytes = sim_align(sizeof(tqc::SimGate) * (size_t)std::max(sub->n_gates, 1));
+    const size_t r_bytes = sizeof(double) << (2 * (sub->d + sub->u) + sub->o);
+    TQC_CUDA(cudaMemsetAsync((char *)scratch + gate_bytes, 0, r_bytes, (cudaStream_t)stream));
+    return tqc_simulate_subcircuit_tensor(sub, out_dev, scratch, (size_t)TQC_STATIC_SCRATCH_BYTES, stream);
+}
+
 // ---- front half: circuit -> partition -> cuts -> network -> plan (section 6) ----------------------------------------
 namespace {
 int plan_from_gate_list(int n_qubits, const std::vector<tqc::CircuitGate> &gates, const tqc_cut_opts *cut, const tqc_plan_opts *opts,
