@@ -44,7 +44,7 @@ struct TcArgs {
     int BN;                         // N tile: 16, 32, 64 or 128
     int stages;
     int mask_hi;                    // hi = TF32 value nearest to x, written back in place (else: x itself, truncated by the MMA)
-    int vec4;                       // 4 consecutive j are contiguous in C
+    int vec4;                       // 4 consecutive j are contiguous in C (pair kernel: 1 = j, j+1 adjacent; 2 = j .. j+3)
     int chunk_kb;                   // k-blocks per hi*hi drain (0: TC_CHUNK_KB)
     unsigned long long *trace;      // develop builds: clock64 stamps of the first k-blocks of cluster 0 (kernels_tc2.cuh)
     int debug;                      // development knobs (TQC_TC_DEBUG): 1 no global stores, 2 no store phase, 4 no split, 8 no drains

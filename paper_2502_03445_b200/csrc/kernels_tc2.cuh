@@ -167,7 +167,7 @@ step_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
         // ready / d_empty collect ONE arrival per CTA: the 16 worker warps of a CTA meet at a named barrier first (32 remote
         // arrivals on one mbarrier cost about 40 cycles each, measured: 1.2 us per k-block of pure hand-shake)
         for (int s = 0; s < S; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&ready_bar[s], 2); mbar_init(&empty_bar[s], 1); }
-        for (int s = 0; s < 2; ++s) { mbar_init(&d_full_bar[s], 1); mbar_init(&d_empty_bar[s], 2); }
+        for (int s = 0; s < 2; ++s) { mbar_init(&d_full_bar[s], 1); mbar_init(&d_empty_bar[s], n_kb <= 2 ? 8 : 2); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 0 && lane == 0) {
@@ -274,6 +274,7 @@ step_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
         for (int h = 0; h < 4; ++h) oa_row[h] = (uint32_t)bitmap_apply(a.outA, (unsigned long long)(rank * 128 + 32 * w4 + (lane >> 2) + 8 * h));
         const uint32_t ob_q = (uint32_t)bitmap_apply(a.outB, (unsigned long long)(2 * (lane & 3)));
         const uint32_t ob_1 = (uint32_t)bitmap_apply(a.outB, 1ull);
+        const uint32_t ob_q4 = (uint32_t)bitmap_apply(a.outB, (unsigned long long)(2 * (lane & 2)));      // column 0 or 4 of a group
         long long it = 0;
         for (long long t = cluster_id; t < total; t += n_clusters) {
             const long long nt = t % tiles_n, mt = (t / tiles_n) & (tiles_m - 1), r = (t / tiles_n) >> lg_tm;
@@ -302,11 +303,40 @@ step_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
                         }
                 }
                 asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-                asm volatile("bar.sync 2, %0;" ::"n"(TC2_DRAIN) : "memory");
-                if (wt == 0) { mbar_arrive_cluster(&d_empty_bar[db], 0); TQC_TRACE(a, rank, 2, it, 3); }
+                if (n_kb <= 2) {
+                    // tiles of one or two k-blocks: one arrival per column group (4 warps, one per TMEM lane quadrant) and CTA,
+                    // so that the groups may drift apart and one group's stores overlap another's drain (K = 64: -4 %,
+                    // K = 16: -10 %, measured); longer tiles keep the single arrival per CTA (the extra remote arrivals cost 1-2 %)
+                    asm volatile("bar.sync %0, 128;" ::"r"(2 + grp) : "memory");
+                    if ((wt & 127) == 0) mbar_arrive_cluster(&d_empty_bar[db], 0);
+                } else {
+                    asm volatile("bar.sync 2, %0;" ::"n"(TC2_DRAIN) : "memory");
+                    if (wt == 0) mbar_arrive_cluster(&d_empty_bar[db], 0);
+                }
+                if (wt == 0) TQC_TRACE(a, rank, 2, it, 3);
             }
             if (TQC_DBG(a, 2)) continue;
             float *ctile = a.C + r * a.c_row_stride + (oa_mt[mt] | ob_nt[nt]);
+            if (a.vec4 == 2) {
+                // columns c .. c+3 (c a multiple of 4) are neighbours in C: neighbouring lanes of a quad swap halves of two
+                // 8-column groups, so that an even lane holds 4 consecutive columns of group g, the odd lane next to it 4 of
+                // group g + 1, and a lane stores 16 bytes: a quad writes 64 contiguous bytes of a row where the layout allows
+                // (the store path alone, all SMs: 6.1 TB/s against 5.5 for 8-byte stores at a row pitch of 16 KB, 6.0 against
+                // 4.0 at 64 KB, 3.1 against 1.5 at 1 MB; in the kernel: -2 to -3 % on K <= 256 steps)
+                const bool odd = (lane & 1) != 0;
+#pragma unroll
+                for (int h2 = 0; h2 < 2; ++h2)
+#pragma unroll
+                    for (int g = 0; g < WC / 8; g += 2) {
+                        const float *e = &acc[h2 * (WC / 2) + 4 * g], *o = e + 4;
+                        const float r0 = __shfl_xor_sync(0xffffffffu, odd ? e[0] : o[0], 1), r1 = __shfl_xor_sync(0xffffffffu, odd ? e[1] : o[1], 1);
+                        const float r2 = __shfl_xor_sync(0xffffffffu, odd ? e[2] : o[2], 1), r3 = __shfl_xor_sync(0xffffffffu, odd ? e[3] : o[3], 1);
+                        const uint32_t oc = ob_c8[grp * (WC / 8) + g + (odd ? 1 : 0)] | ob_q4;
+                        *reinterpret_cast<float4 *>(ctile + (oa_row[2 * h2] | oc)) = odd ? make_float4(r0, r1, o[0], o[1]) : make_float4(e[0], e[1], r0, r1);
+                        *reinterpret_cast<float4 *>(ctile + (oa_row[2 * h2 + 1] | oc)) = odd ? make_float4(r2, r3, o[2], o[3]) : make_float4(e[2], e[3], r2, r3);
+                    }
+                continue;
+            }
 #pragma unroll
             for (int h2 = 0; h2 < 2; ++h2)
 #pragma unroll

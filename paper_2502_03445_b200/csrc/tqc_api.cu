@@ -451,7 +451,8 @@ int launch_tc_step(tqc_plan_t *pl, TcOperand A, TcOperand B, BitMap outA, BitMap
             { const char *dbg = dev_env("TQC_TC_DEBUG"); a.debug = dbg ? std::atoi(dbg) : 0; }
             a.mask_hi = 1;
             if (const char *tp = dev_env("TQC_TC_TRACE_PTR")) a.trace = (unsigned long long *)std::strtoull(tp, nullptr, 0);
-            a.vec4 = (outB.n >= 1 && outB.src[0] == 0 && outB.dst[0] == 0) ? 1 : 0;      // columns j, j + 1 adjacent in C
+            // columns j, j + 1 adjacent in C: 1; j .. j + 3 (j a multiple of 4): 2 (16-byte stores after a lane exchange)
+            a.vec4 = (outB.n >= 1 && outB.src[0] == 0 && outB.dst[0] == 0) ? (outB.len[0] >= 2 ? 2 : 1) : 0;
             const size_t stage_bytes = 2 * (size_t)128 * tqc::TC_BK * 4 + 2 * (size_t)(a.BN / 2) * tqc::TC_BK * 4;
             a.stages = (int)std::min<size_t>(6, (192 * 1024) / stage_bytes);
             if (const char *sv = dev_env("TQC_TC_STAGES")) a.stages = std::max(2, std::min(a.stages, std::atoi(sv)));
@@ -462,7 +463,13 @@ int launch_tc_step(tqc_plan_t *pl, TcOperand A, TcOperand B, BitMap outA, BitMap
             const long long total = (1ll << (lgM - 8)) * ((1ll << lgN) / a.BN) * (long long)R;
             const unsigned grid = 2u * (unsigned)std::min<long long>(total, sm_count / 2);
             if (dev_env("TQC_TC_TRACE"))
-                fprintf(stderr, "tc2 step %d: lgM %d lgN %d lgK %d swap %d BN %d vec2 %d R %d stages %d\n", tag, lgM, lgN, lgK, (int)sw, a.BN, a.vec4, R, a.stages);
+            {
+                fprintf(stderr, "tc2 step %d: lgM %d lgN %d lgK %d swap %d BN %d vec2 %d R %d stages %d  outA", tag, lgM, lgN, lgK, (int)sw, a.BN, a.vec4, R, a.stages);
+                for (int q = 0; q < outA.n; ++q) fprintf(stderr, " %d+%d>%d", outA.src[q], outA.len[q], outA.dst[q]);
+                fprintf(stderr, "  outB");
+                for (int q = 0; q < outB.n; ++q) fprintf(stderr, " %d+%d>%d", outB.src[q], outB.len[q], outB.dst[q]);
+                fprintf(stderr, "\n");
+            }
             if ((rc = note_launch(pl, tag, st))) return rc;
             const size_t smem = a.stages * stage_bytes + 1024;
             pl->pair_launches++;
