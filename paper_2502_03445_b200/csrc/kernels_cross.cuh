@@ -17,7 +17,7 @@ namespace tqc {
 constexpr int CROSS_TI = 64, CROSS_TJ = 128, CROSS_CP = CROSS_TJ + 8;      // C tile pitch (floats)
 
 template <int LGK>
-__global__ void __launch_bounds__(256, 4) cross_mma_kernel(const StepArgs a) {
+__global__ void __launch_bounds__(256, LGK >= 5 ? 3 : 4) cross_mma_kernel(const StepArgs a) {     // K >= 32: 64 registers spill (slice sums)
     constexpr int K = 1 << LGK, P = K + 4;                                // row pitch: fragment loads hit 32 distinct banks
     extern __shared__ __align__(16) unsigned char cross_smem_raw[];
     unsigned long long *rowA = reinterpret_cast<unsigned long long *>(cross_smem_raw);   // [TI] operand row offsets (floats)
