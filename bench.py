@@ -673,12 +673,26 @@ def measure_hss_contract(ctx, steps: int, warmup: int) -> dict:
     ms_states = timed(lambda: tqc.tqc_contract_states(plan, states, out=out2, workspace=ws, stream=stream))
     torch.cuda.synchronize()
     agree = float((out - out2).abs().max() / out2.abs().max())
+    # algorithmic work of the pruned contraction: 2 x the multiplication count of its plan (tqc_hss_cost_log2) against the
+    # measured FFMA rate; bytes = the pruned tensors read once + the result written once
+    peaks = roof_peaks()
+    flop = 2.0 * 2.0 ** plan.hss_cost_log2
+    nbytes = 4.0 * (sum(len(v) * 4.0 ** len(net.sub_cuts[j]) for j, v in enumerate(x)) + n)
+    sec = ms_product * 1e-3
+    t_alu, t_hbm = flop / (peaks["ffma_tflops"] * 1e12), nbytes / (peaks["hbm_gbs"] * 1e9)
+    if t_alu >= t_hbm:
+        roof = {"bound": "alu", "achieved": flop / sec / 1e12, "peak": peaks["ffma_tflops"], "unit": "TFLOP/s",
+                "peak_source": "FP32 FFMA rate, " + peaks["ffma_tflops_source"]}
+    else:
+        roof = {"bound": "hbm", "achieved": nbytes / sec / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                "peak_source": peaks["source"] + " hbm copy"}
+    roof.update({"frac": roof["achieved"] / roof["peak"], "traffic": None, "algorithmic_flop": flop, "algorithmic_bytes": nbytes,
+                 "kernel": "whole call: hss_rows_kernel (pruned tensors) + distribution-mode steps (step_tile / cross_mma) + hss_compact_kernel"})
     plan.close()
     return {"workload": f"hss-contract: cfg3-shaped network, |x_j| = {[len(v) for v in x]}, {n} composite states",
             "value": n / (ms_product * 1e-3), "unit": UNIT, "ms_per_step": ms_product, "steps": steps,
             "gpu_launches": int(launches), "per_state_path_ms": ms_states, "max_rel_diff_vs_per_state_path": agree,
-            "roofline": {"bound": "hbm", "kernel": "pruned distribution-mode contraction (step_tile / cross_mma) + hss_compact_kernel",
-                         "achieved": None, "peak": None, "unit": "GB/s", "frac": None, "traffic": None}}
+            "roofline": roof}
 
 
 def workload_description(wl, plan) -> str:

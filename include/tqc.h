@@ -230,6 +230,9 @@ int tqc_hss_expand(const tqc_plan_t *plan, const int32_t *counts, const int32_t 
  *   workspace >= tqc_hss_workspace_bytes(plan), 256-byte aligned; asynchronous on `stream`, no allocation. */
 int tqc_hss_prepare(tqc_plan_t *plan, const int32_t *counts, const int32_t *keys_dev, void *stream);
 size_t tqc_hss_workspace_bytes(const tqc_plan_t *plan);
+/* log2 of the multiplication count of the pruned contraction tqc_hss_prepare planned (all padded composite states
+ * together, the count of tqc_plan_cost_log2 in distribution mode); negative before tqc_hss_prepare.  Host only. */
+double tqc_hss_cost_log2(const tqc_plan_t *plan);
 int tqc_hss_contract(tqc_plan_t *plan, float *out_dev, void *workspace_dev, size_t workspace_bytes, void *stream);
 
 /* ---- Subcircuit variants on the device (section 2.1) -- fourth row of SURVEY 8(f) ---------------

@@ -33,7 +33,7 @@ EXPORTED = ["tqc_plan", "tqc_plan_destroy", "tqc_plan_mode", "tqc_plan_num_qubit
             "tqc_plan_workspace_bytes_host", "tqc_contract_states_host", "tqc_contract_distribution_host",
             "tqc_plan_profile_enable", "tqc_plan_profile_read", "tqc_plan_chain_status", "tqc_hss_scores", "tqc_hss_select",
             "tqc_hss_expand", "tqc_plan_num_sliced_cuts", "tqc_choose_slice_cuts", "tqc_hss_prepare",
-            "tqc_hss_workspace_bytes", "tqc_hss_contract", "tqc_simulate_workspace_bytes",
+            "tqc_hss_workspace_bytes", "tqc_hss_cost_log2", "tqc_hss_contract", "tqc_simulate_workspace_bytes",
             "tqc_simulate_subcircuit_tensor", "tqc_simulate_subcircuit_tensor_static", "tqc_static_scratch_bytes",
             "tqc_plan_finalize", "tqc_plan_from_circuit", "tqc_plan_from_gates",
             "tqc_plan_cut_network", "tqc_plan_cut_subcircuit", "tqc_plan_cut_assignment", "tqc_cut_merging_cost",
@@ -141,6 +141,8 @@ def _load() -> ctypes.CDLL:
     lib.tqc_hss_prepare.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p]
     lib.tqc_hss_workspace_bytes.argtypes = [c_void_p]
     lib.tqc_hss_workspace_bytes.restype = c_size_t
+    lib.tqc_hss_cost_log2.argtypes = [c_void_p]
+    lib.tqc_hss_cost_log2.restype = c_double
     lib.tqc_hss_contract.argtypes = [c_void_p, c_void_p, c_void_p, c_size_t, c_void_p]
     lib.tqc_simulate_workspace_bytes.argtypes = [POINTER(_SubcircuitDesc)]
     lib.tqc_simulate_workspace_bytes.restype = c_size_t
@@ -315,6 +317,11 @@ class Plan:
         buf = ctypes.create_string_buffer(4096)
         rc = _lib.tqc_plan_chain_status(self._h, buf, 4096)
         return rc, buf.value.decode(errors="replace")
+
+    @property
+    def hss_cost_log2(self) -> float:
+        """log2 multiplications of the pruned contraction planned by the last tqc_hss_prepare / tqc_hss_contract (< 0: none)."""
+        return float(_lib.tqc_hss_cost_log2(self._h))
 
     def profile_enable(self, on: bool = True) -> None:
         _check(_lib.tqc_plan_profile_enable(self._h, 1 if on else 0))

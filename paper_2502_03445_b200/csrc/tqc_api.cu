@@ -1762,6 +1762,10 @@ int tqc_hss_prepare(tqc_plan_t *pl, const int32_t *counts, const int32_t *keys_d
     return tqc_plan_finalize(sub, stream);
 }
 
+double tqc_hss_cost_log2(const tqc_plan_t *pl) {
+    return (pl && pl->hss_sub) ? tqc::cost_log2(pl->hss_sub->hp) : -1.0;
+}
+
 size_t tqc_hss_workspace_bytes(const tqc_plan_t *pl) {
     if (!pl || !pl->hss_sub) return 0;
     return align256(((size_t)4) << pl->hss_sub->hp.n) + tqc_plan_workspace_bytes(pl->hss_sub, 0, 0);

@@ -105,9 +105,13 @@ def test_product_structured_contraction(seed, s_max):
     tensors = [np.asarray(t, dtype=np.float32) for t in random_tensors(net, 710 + seed)]
     plan = _loaded(net, tensors)
     x = tqc.tqc_hss_select(plan, _gpu_scores(plan), s_max)
+    assert plan.hss_cost_log2 < 0                                # nothing prepared yet
     got = tqc.tqc_hss_contract(plan, x)
     torch.cuda.synchronize()
     got = got.cpu().numpy().astype(np.float64)
+    # the pruned plan's multiplication count: at least one multiplication per (padded) composite state and contraction step
+    n_pad = np.prod([1 << int(np.ceil(np.log2(max(len(v), 1)))) for v in x], dtype=np.float64)
+    assert plan.hss_cost_log2 >= np.log2(n_pad) - 1e-9
     bits = H.expand(net, [v.tolist() for v in x])
     assert got.shape == (bits.shape[0],)
     sample = np.arange(bits.shape[0]) if bits.shape[0] <= 4096 else np.random.default_rng(1).choice(bits.shape[0], 4096, replace=False)
