@@ -9,16 +9,19 @@
 //   warp 0      TMA producer: cp.async.bulk.tensor 3-D tiles {32 k, 128 or BN rows, 1 state} with 128-byte swizzle;
 //               the state coordinate of a LEAF/TABLE operand is the state's key (a3 gather = a TMA coordinate)
 //   warp 1      MMA issuer: one elected lane, 12 tcgen05.mma.kind::tf32 per k-block, tcgen05.commit frees the stage
-//   warps 2-9   accumulate + epilogue: tcgen05.ld -> fp32 round-to-nearest adds in registers -> scatter to C; two groups of
-//               four warps (one per TMEM lane quadrant), each group owning half of the tile's columns when BN >= 64
-//   warps 10-11 splitter: fp32 tile -> hi (in place) and lo (second buffer), same swizzled byte offsets
-// Pipelines: full[s] (TMA -> splitter), ready[s] (splitter -> MMA), empty[s] (MMA -> TMA).
+//   warps 2-9   accumulate + epilogue: tcgen05.ld -> fp32 round-to-nearest adds in registers -> scatter to C; BN = 128: two
+//               groups of four warps (one per TMEM lane quadrant), each owning half of the tile's columns; BN <= 64: warps 2-5
+//   warps 6-9   BN <= 64 only: A splitter - a thread per tile row reads the landed raw row once, splits it in registers and
+//               writes hi and lo into TENSOR MEMORY (tcgen05.st), the MMAs take A from there (tcgen05.mma with a TMEM A operand)
+//   warps 10-11 splitter: fp32 tile -> hi (in place) and lo (second buffer), same swizzled byte offsets (BN <= 64: B only)
+// Pipelines: full[s] (TMA -> splitters), ready[s] (splitters -> MMA), empty[s] (MMA -> TMA, and -> A splitter: the TMEM A
+// buffer of k-block it - 2 is free).
 // The tensor pipe's fp32 accumulator rounds toward zero on every add (measured: -5e-8 relative per accumulation,
 // profiles/r01c notes), a bias that grows with the number of k-steps.  So (i) the hi*hi products of at most
 // TC_CHUNK_KB k-blocks (8 MMAs) accumulate in a TMEM buffer D_hi that the accumulate warps then drain and add to
 // registers in round-to-nearest, two D_hi buffers alternating so draining overlaps the next chunk's MMAs; (ii) the
 // hi*lo + lo*hi products, 2^-11 smaller, accumulate over the whole K in their own buffer D_lo (two of them,
-// alternating per tile), where the same bias is negligible.  TMEM columns: 4 x BN <= 512.
+// alternating per tile), where the same bias is negligible.  TMEM columns: 4 x BN <= 512 (BN <= 64: + 2 x 64 for A).
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -105,6 +108,22 @@ __device__ __forceinline__ void umma_tf32(uint32_t tmem_d, uint64_t da, uint64_t
         "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t"
         "}" ::"r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(accumulate) : "memory");
 }
+// A operand from TENSOR MEMORY (lane = row, one 32-bit column per K element), B from a shared-memory descriptor
+__device__ __forceinline__ void umma_tf32_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n\t"
+        "}" ::"r"(tmem_d), "r"(tmem_a), "l"(db), "r"(idesc), "r"(accumulate) : "memory");
+}
+// 16 consecutive columns of this lane's row
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&v)[16]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};"
+        ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]),
+          "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]) : "memory");
+}
 __device__ __forceinline__ void umma_commit(uint64_t *bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
@@ -174,7 +193,14 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
     __shared__ uint32_t tmem_base_slot;
     // epilogue: each warp stages 32 rows x CB columns in its own scratch and writes them out in ascending C-offset
     // order (perm tables), so a warp store covers the longest contiguous run the consumer's digit layout allows
-    constexpr int EG = BN >= 64 ? 2 : 1;             // epilogue warp groups
+    // Narrow tiles (BN <= 64) take the A operand of every MMA from TENSOR MEMORY: a k-block's A tile is read three times by the
+    // MMAs (hi twice, lo once) on top of the TMA write and the split, 112 KB of shared-memory traffic per k-block whatever BN,
+    // and the narrow steps ran at 0.7-0.8 of that shared-memory floor (measured: 1750 cycles per k-block for BN = 16 ... 64,
+    // operand in HBM or in L2 alike).  Warps 6-9 (one per TMEM lane quadrant, a thread per row) read the landed raw rows once,
+    // split them in registers and write hi and lo with tcgen05.st into one of two 64-column A buffers; the MMAs are the
+    // TMEM-A form.  The accumulate warps are one column group then (warps 2-5), B is split in shared memory as before.
+    constexpr bool A_TMEM = BN <= 64;
+    constexpr int EG = BN >= 128 ? 2 : 1;            // epilogue warp groups
     constexpr int EC = BN / EG;                       // columns each epilogue warp accumulates
     constexpr int CB = EG == 2 ? 16 : (BN < 32 ? BN : 32);   // columns per staged block
     constexpr int LB = CB == 32 ? 5 : 4;
@@ -201,7 +227,8 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
     const long long tiles_m = 1ll << (a.lgM - 7);
     const long long tiles_n = (1ll << a.lgN) / BN;
     const long long total = tiles_m * tiles_n * a.R;
-    constexpr uint32_t tmem_cols = 4 * BN < 32 ? 32 : 4 * BN;      // D_hi[0], D_hi[1], D_lo[0], D_lo[1]
+    // D_hi[0], D_hi[1], D_lo[0], D_lo[1]; with A_TMEM two A buffers of 64 columns (hi 32, lo 32) behind them
+    constexpr uint32_t tmem_cols = !A_TMEM ? (uint32_t)(4 * BN) : (4 * BN + 128 <= 256 ? 256u : 512u);
 
     // ---- one-time setup -------------------------------------------------------------------------
     for (int x = threadIdx.x; x < 256; x += TC_THREADS) {
@@ -235,7 +262,7 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
         }
     }
     if (threadIdx.x == 0) {
-        for (int s = 0; s < S; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&ready_bar[s], TC_SPLIT_THREADS / 32); mbar_init(&empty_bar[s], 1); }
+        for (int s = 0; s < S; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&ready_bar[s], TC_SPLIT_THREADS / 32 + (A_TMEM ? 4 : 0)); mbar_init(&empty_bar[s], 1); }
         for (int s = 0; s < 2; ++s) {
             mbar_init(&hi_full_bar[s], 1); mbar_init(&hi_empty_bar[s], 4 * EG);
             mbar_init(&lo_full_bar[s], 1); mbar_init(&lo_empty_bar[s], 4 * EG);
@@ -294,11 +321,35 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
                     // hi*hi reads only the raw tiles (TMA wrote them: no proxy fence needed), so it starts as soon as the
                     // load lands and overlaps the splitter; the lo terms wait for the splitter's ready barrier
                     // (with round-to-nearest hi parts the raw tiles are rewritten by the splitter: wait for it first)
-                    mbar_wait(a.mask_hi ? &ready_bar[s] : &full_bar[s], ph);
+                    mbar_wait((a.mask_hi || A_TMEM) ? &ready_bar[s] : &full_bar[s], ph);
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                     const uint64_t dah = umma_desc_sw128(smem_u32(A_raw(s))), dal = umma_desc_sw128(smem_u32(A_lo(s)));
                     const uint64_t dbh = umma_desc_sw128(smem_u32(B_raw(s))), dbl = umma_desc_sw128(smem_u32(B_lo(s)));
                     const bool run = !TQC_DBG(a, 32) || (kb | kc) == 0;
+                    if constexpr (A_TMEM) {
+                        // ready = A hi / lo of this k-block in TMEM buffer it & 1 and B split in shared memory
+                        const uint32_t a_hi = tmem_base + 4u * (uint32_t)BN + 64u * (uint32_t)(it & 1), a_lo = a_hi + 32u;
+                        if (lane == 0) {
+                            if (run) {
+#pragma unroll
+                                for (int k = 0; k < TC_BK / 8; ++k) {
+                                    const uint64_t adv = (uint64_t)(k * 8 * 4 >> 4);
+                                    umma_tf32_ts(d_lo, a_lo + 8u * k, dbh + adv, idesc, (kb | k) ? 1u : 0u);
+                                    umma_tf32_ts(d_lo, a_hi + 8u * k, dbl + adv, idesc, 1u);
+                                }
+#pragma unroll
+                                for (int k = 0; k < TC_BK / 8; ++k) {
+                                    const uint64_t adv = (uint64_t)(k * 8 * 4 >> 4);
+                                    umma_tf32_ts(d_hi, a_hi + 8u * k, dbh + adv, idesc, (kc | k) ? 1u : 0u);
+                                }
+                            }
+                            umma_commit(&empty_bar[s]);
+                            if (kc == chunk_kb - 1) umma_commit(&hi_full_bar[hb]);
+                            if (kb == n_kb - 1) umma_commit(&lo_full_bar[lb]);
+                        }
+                        __syncwarp();
+                        continue;
+                    }
                     if (lane == 0 && run) {
 #pragma unroll
                         for (int k = 0; k < TC_BK / 8; ++k) {
@@ -412,6 +463,44 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
                 }
             }
         }
+    } else if (A_TMEM && warp >= 6 && warp < 10) {
+        // ===== A splitter (narrow tiles): raw row -> registers -> hi / lo in tensor memory =====
+        const uint32_t row = (uint32_t)(32 * (warp & 3) + lane);          // TMEM lane = tile row; a warp owns its lane quadrant
+        const uint32_t lane_base = (uint32_t)(32 * (warp & 3)) << 16;
+        const bool mask_hi = a.mask_hi != 0;
+        const long long my_kb = ((long long)blockIdx.x < total ? (total - blockIdx.x + gridDim.x - 1) / gridDim.x : 0) * n_kb;
+        for (long long it = 0; it < my_kb; ++it) {
+            const int s = (int)(it % S);
+            if (it >= 2) {                                                // the MMAs that read this A buffer (k-block it - 2) have retired
+                const long long jt = it - 2;
+                mbar_wait(&empty_bar[(int)(jt % S)], (uint32_t)((jt / S) & 1));
+            }
+            mbar_wait(&full_bar[s], (uint32_t)((it / S) & 1));
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            const uint32_t src = smem_u32(A_raw(s)) + row * 128u;
+            const uint32_t a_hi = tmem_base + lane_base + 4u * (uint32_t)BN + 64u * (uint32_t)(it & 1), a_lo = a_hi + 32u;
+#pragma unroll
+            for (int half = 0; half < 2; ++half) {
+                uint32_t x[16], h[16], l[16];
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {                             // 16-byte chunk 4 half + c of the row sits at slot chunk ^ (row & 7)
+                    const uint32_t chunk = (uint32_t)(4 * half + c);
+                    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(x[4 * c]), "=r"(x[4 * c + 1]), "=r"(x[4 * c + 2]), "=r"(x[4 * c + 3])
+                                 : "r"(src + ((chunk ^ (row & 7u)) << 4)));
+                }
+#pragma unroll
+                for (int e = 0; e < 16; ++e) {
+                    h[e] = (x[e] + (mask_hi ? 0x1000u : 0u)) & 0xFFFFE000u;
+                    l[e] = __float_as_uint(__uint_as_float(x[e]) - __uint_as_float(h[e]));
+                }
+                tmem_st16(a_hi + 16u * half, h);
+                tmem_st16(a_lo + 16u * half, l);
+            }
+            asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&ready_bar[s]);
+        }
     } else if (warp >= (TC_THREADS - TC_SPLIT_THREADS) / 32) {
         // ===== splitter: fp32 -> hi (in place) + lo =====
         const int st = threadIdx.x - (TC_THREADS - TC_SPLIT_THREADS);
@@ -424,7 +513,7 @@ step_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
                 mbar_wait(&full_bar[s], ph);
                 // per stage: [A_raw][A_lo][B_raw][B_lo]; element e of a raw tile and of its lo tile share the swizzled offset
                 const uint32_t sa = smem_u32(A_raw(s)) + (uint32_t)st * 16u;
-                if (!TQC_DBG(a, 4))
+                if (!TQC_DBG(a, 4) && !A_TMEM)
                 split_tile<(int)(bytesA >> 4) / TC_SPLIT_THREADS>(sa, bytesA, mask_hi);
                 if (!TQC_DBG(a, 4))
                 split_tile<(int)(bytesB >> 4) / TC_SPLIT_THREADS>(sa + 2u * bytesA, bytesB, mask_hi);
