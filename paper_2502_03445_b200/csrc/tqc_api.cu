@@ -431,7 +431,7 @@ int launch_tc_step(tqc_plan_t *pl, TcOperand A, TcOperand B, BitMap outA, BitMap
     const int sm_count = pl->sm_count > 0 ? pl->sm_count : 148;
     auto has_bit0 = [](const BitMap &m) { for (int s = 0; s < m.n; ++s) if (m.dst[s] == 0) return true; return false; };
     // CTA-pair kernel (kernels_tc2.cuh): 256 x BN tiles over two SMs.  The M side needs >= 256 rows, the N side >= 128; with
-    // both orientations possible the N side is the operand that owns C's lowest offset bit (8-byte stores from registers).
+    // both orientations possible the N side is the operand that owns C's lowest offset bit (8- or 16-byte stores from registers).
     static const bool no_pair = dev_env("TQC_TC_NO_PAIR") != nullptr;
     {
         // (64-column pair tiles were tried: a k-block then holds 384 cycles of MMAs against about 1800 cycles of fixed pipeline
