@@ -137,11 +137,11 @@ __device__ __forceinline__ void mma_tf32_16x8x8(float (&d)[4], const uint32_t (&
 // SLICE_SUM: see the comment at the MMAs.  The table steps (kernels_cross.cuh) feed one another - cfg5 runs 24 in a row -
 // and take the slice sums; a chain's one product per state keeps the running accumulator (cfg4: mean error -5e-8 of max p,
 // and the extra adds cost 1.5 % of the chain kernel).
-template <int LGM, int LGN, int LGK, int PA, int PB, bool SLICE_SUM = false, class Emit>
-__device__ __forceinline__ void chain_step_mma(const float *pa, const float *pb, int lane, Emit emit) {
+// the accumulators only: acc[mi][nj] = {(row 16 mi + g, col 8 nj + 2 t), (same row, col + 1), (row + 8, col), (row + 8, col + 1)}
+template <int LGM, int LGN, int LGK, int PA, int PB, bool SLICE_SUM = false>
+__device__ __forceinline__ void chain_mma_acc(const float *pa, const float *pb, int lane, float (&acc)[(1 << LGM) / 16][(1 << LGN) / 8][4]) {
     constexpr int MT = (1 << LGM) / 16, NT = (1 << LGN) / 8, K = 1 << LGK;
     const int g = lane >> 2, t = lane & 3;
-    float acc[MT][NT][4];
 #pragma unroll
     for (int mi = 0; mi < MT; ++mi)
 #pragma unroll
@@ -186,6 +186,14 @@ __device__ __forceinline__ void chain_step_mma(const float *pa, const float *pb,
                 }
             }
     }
+}
+
+template <int LGM, int LGN, int LGK, int PA, int PB, bool SLICE_SUM = false, class Emit>
+__device__ __forceinline__ void chain_step_mma(const float *pa, const float *pb, int lane, Emit emit) {
+    constexpr int MT = (1 << LGM) / 16, NT = (1 << LGN) / 8;
+    const int g = lane >> 2, t = lane & 3;
+    float acc[MT][NT][4];
+    chain_mma_acc<LGM, LGN, LGK, PA, PB, SLICE_SUM>(pa, pb, lane, acc);
 #pragma unroll
     for (int mi = 0; mi < MT; ++mi)
 #pragma unroll

@@ -6,7 +6,7 @@
 // slices added in registers: table steps feed one another and the pipe's truncating accumulator would drift), 64 x 128
 // outputs per 256-thread block.
 // Where j' and j' + 1 are neighbours in C (the usual case: the result layout keeps the operand's digit order) the results
-// leave straight from the fragments as 8-byte stores, four lanes per 32-byte sector; otherwise the tile goes through
+// leave straight from the fragments as 16-byte stores after a lane exchange, 64 contiguous bytes per quad; otherwise the tile goes through
 // shared memory and leaves row by row.
 #pragma once
 #include "device_args.h"
@@ -54,14 +54,28 @@ __global__ void __launch_bounds__(256, LGK >= 5 ? 3 : 4) cross_mma_kernel(const 
     }
     __syncthreads();
     if (a.vec_store == 2) {
-        // j' and j' + 1 are neighbours in C: the two results a lane holds per fragment row leave as one 8-byte store, four
-        // lanes fill a 32-byte sector, no trip through shared memory
+        // results leave straight from the fragments, no trip through shared memory
+        // (columns j .. j + 3, j a multiple of 4, are neighbours in C: neighbouring lanes of a quad swap halves of two 8-column
+        // fragments, an even lane then holds 4 consecutive columns of fragment 2 n, the odd lane next to it 4 of fragment
+        // 2 n + 1, and a lane stores 16 bytes - a quad writes 64 contiguous bytes of a row: kernels_tc2.cuh, store-path numbers
+        // in DESIGN.md 5.2)
         const int wi = warp >> 2, wj = warp & 3;
-        float keep = 0.f;
-        chain_step_mma<5, 5, LGK, P, P, true>(As + 32 * wi * P, Bs + 32 * wj * P, lane, [&](int i, int j, float v) {
-            if ((j & 1) == 0) keep = v;
-            else *reinterpret_cast<float2 *>(a.C + (offA[32 * wi + i] | offB[32 * wj + j - 1])) = make_float2(keep, v);
-        });
+        const int g = lane >> 2, t = lane & 3;
+        const bool odd = (t & 1) != 0;
+        float acc[2][4][4];
+        chain_mma_acc<5, 5, LGK, P, P, true>(As + 32 * wi * P, Bs + 32 * wj * P, lane, acc);
+#pragma unroll
+        for (int mi = 0; mi < 2; ++mi)
+#pragma unroll
+            for (int np = 0; np < 2; ++np) {
+                const float *e = acc[mi][2 * np], *o = acc[mi][2 * np + 1];
+                const float r0 = __shfl_xor_sync(0xffffffffu, odd ? e[0] : o[0], 1), r1 = __shfl_xor_sync(0xffffffffu, odd ? e[1] : o[1], 1);
+                const float r2 = __shfl_xor_sync(0xffffffffu, odd ? e[2] : o[2], 1), r3 = __shfl_xor_sync(0xffffffffu, odd ? e[3] : o[3], 1);
+                const unsigned long long ob = offB[32 * wj + 8 * (2 * np + (odd ? 1 : 0)) + 2 * (t & 2)];
+                float *ctop = a.C + (offA[32 * wi + 16 * mi + g] | ob), *cbot = a.C + (offA[32 * wi + 16 * mi + g + 8] | ob);
+                *reinterpret_cast<float4 *>(ctop) = odd ? make_float4(r0, r1, o[0], o[1]) : make_float4(e[0], e[1], r0, r1);
+                *reinterpret_cast<float4 *>(cbot) = odd ? make_float4(r2, r3, o[2], o[3]) : make_float4(e[2], e[3], r2, r3);
+            }
         return;
     }
     {   // warp grid 2 x 4 over the 64 x 128 tile: 32 x 32 outputs per warp
