@@ -345,8 +345,10 @@ def measure(ctx, args, workload: str, batch: int, steps: int, warmup: int):
     # every timed region); the other configs keep the deterministic greedy plan (their plans are a handful of steps)
     restarts = args.restarts if args.restarts >= 0 else (1024 if wl_name_is_cfg5(workload) else 0)
     # batch_hint = the config's FULL batch: a prefix run keeps the plan (tables, kernel classes) of the real workload
+    table_log2 = args.table_log2 if args.table_log2 >= 0 else (30 if wl_name_is_cfg5(workload) else 0)
     plan = tqc.tqc_plan(net, tqc.MODE_STATES if states_mode else tqc.MODE_DISTRIBUTION, batch_hint=wl["full_B"],
-                        restarts=restarts, seed=args.plan_seed, objective=1 if (restarts > 0 and states_mode) else 0)
+                        restarts=restarts, seed=args.plan_seed, objective=1 if (restarts > 0 and states_mode) else 0,
+                        table_log2_floats_max=table_log2)
     for s, t in enumerate(wl["tensors"]):
         tqc.tqc_load_subcircuit_tensors(plan, s, t)
     prefix_note = None
@@ -489,7 +491,7 @@ def measure(ctx, args, workload: str, batch: int, steps: int, warmup: int):
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": workload_description(wl, plan), "states_per_step_per_gpu": n_out,
                    "parallelism": f"states sharded over {world} GPU(s), tensors replicated, no collective",
-                   "l2": "flushed between timed iterations (256 MB write)", "plan_cost_log2_per_state": plan.cost_log2, "planner_restarts": restarts,
+                   "l2": "flushed between timed iterations (256 MB write)", "plan_cost_log2_per_state": plan.cost_log2, "planner_restarts": restarts, "table_log2_floats_max": table_log2 or 24,
                    "planner_objective": "modelled run time (tqc_plan_opts.objective = 1)" if (restarts > 0 and states_mode) else "deterministic greedy",
                    "planner_modelled_us_per_state": plan.modelled_seconds_per_state * 1e6 if states_mode else None,
                    "kmax": plan.kmax, "workspace_gb": ws_bytes / 2 ** 30, "prefix_rule": prefix_note,
@@ -834,6 +836,8 @@ def main() -> None:
     ap.add_argument("--restarts", type=int, default=-1, help="planner restarts with the run-time objective (0: deterministic "
                     "greedy; default: 1024 for cfg5, 0 otherwise)")
     ap.add_argument("--plan-seed", type=int, default=1)
+    ap.add_argument("--table-log2", type=int, default=-1, help="cap on log2(entries) of a once-per-key table node (0: the library default, 24; "
+                    "default: 30 for cfg5 - 4 GB tables, built once per call - and the library default otherwise)")
     ap.add_argument("--max-workspace-gb", type=int, default=64)
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -227,10 +227,12 @@ def test_cfg5_order_invariance_between_two_gpu_plans():
     T = random_tensors(net, seed_for(5, STREAM_TENSORS))
     bits = random_states(196, configs.BATCH[5], seed_for(5, STREAM_STATES))[:128]
     plan_a = _loaded_plan(net, T, tqc.MODE_STATES, batch_hint=configs.BATCH[5])
-    plan_b = _loaded_plan(net, T, tqc.MODE_STATES, batch_hint=configs.BATCH[5], restarts=256, seed=1, objective=1)
+    # ... with once-per-key tables of up to 2^30 entries (bench.py's cfg5 setting: 4 GB tables are cheap in 180 GB of HBM)
+    plan_b = _loaded_plan(net, T, tqc.MODE_STATES, batch_hint=configs.BATCH[5], restarts=256, seed=1, objective=1,
+                          table_log2_floats_max=30)
     assert plan_a.serialize() != plan_b.serialize()
     assert plan_b.modelled_seconds_per_state < plan_a.modelled_seconds_per_state
-    again = tqc.tqc_plan(net, tqc.MODE_STATES, batch_hint=configs.BATCH[5], restarts=256, seed=1, objective=1)
+    again = tqc.tqc_plan(net, tqc.MODE_STATES, batch_hint=configs.BATCH[5], restarts=256, seed=1, objective=1, table_log2_floats_max=30)
     assert again.serialize() == plan_b.serialize()                                  # deterministic per seed
     got_a = _run_states(plan_a, bits, max_ws=32 << 30)
     got_b = _run_states(plan_b, bits, max_ws=32 << 30)
