@@ -165,6 +165,8 @@ def test_cfg4_full_batch_subset_vs_direct_sum():
     assert np.abs(got1 - want1).max() <= TOL * want1.max()
 
 
+# the plan bench.py times on cfg5 (its defaults: --restarts 1024 --plan-seed 1, run-time objective, --table-log2 30)
+BENCH_PLAN_CFG5 = dict(restarts=1024, seed=1, objective=1, table_log2_floats_max=30)
 CFG5_SUBSET = 256         # random-tensor states checked against O8' by default (0.15 s each on the box's 16 host cores); all 1000 behind -m slow
 
 
@@ -191,13 +193,15 @@ def test_cfg5_rank_one_and_oracle_subset():
     T = random_tensors(net, seed_for(5, STREAM_TENSORS))
     idx = np.random.default_rng(seed_for(5, STREAM_SUBSET)).choice(configs.BATCH[5], size=1000, replace=False)[:CFG5_SUBSET]
     sub = all_bits[idx]
-    plan = _loaded_plan(net, T, tqc.MODE_STATES, batch_hint=configs.BATCH[5])
-    got = _run_states(plan, sub, max_ws=8 << 30)
     want = R.contract_states_tensordot(net, T, sub, order_trials=64)
-    rel = (got - want) / want.max()
-    print(f"cfg5 random tensors: {len(sub)} states of the seeded 1000-state subset checked against O8': "
-          f"max |dp|/max p = {np.abs(rel).max():.2e}, mean {rel.mean():+.2e}")
-    assert np.abs(rel).max() <= TOL, np.abs(rel).max()
+    for label, kw in (("greedy plan", {}), ("the plan bench.py times", BENCH_PLAN_CFG5)):
+        plan = _loaded_plan(net, T, tqc.MODE_STATES, batch_hint=configs.BATCH[5], **kw)
+        got = _run_states(plan, sub, max_ws=32 << 30)
+        rel = (got - want) / want.max()
+        print(f"cfg5 random tensors, {label}: {len(sub)} states of the seeded 1000-state subset checked against O8': "
+              f"max |dp|/max p = {np.abs(rel).max():.2e}, mean {rel.mean():+.2e}")
+        assert np.abs(rel).max() <= TOL, np.abs(rel).max()
+        plan.close()
     want_be = R.bucket_elimination(net, T, sub[:1], chunk=1, order_trials=64)
     assert abs(got[0] - want_be[0]) <= TOL * want.max()
 
@@ -210,12 +214,14 @@ def test_cfg5_full_1k_subset_against_oracle():
     all_bits = random_states(196, configs.BATCH[5], seed_for(5, STREAM_STATES))
     idx = np.random.default_rng(seed_for(5, STREAM_SUBSET)).choice(configs.BATCH[5], size=1000, replace=False)
     T = random_tensors(net, seed_for(5, STREAM_TENSORS))
-    plan = _loaded_plan(net, T, tqc.MODE_STATES, batch_hint=configs.BATCH[5])
-    got = _run_states(plan, all_bits[idx], max_ws=32 << 30)
     want = R.contract_states_tensordot(net, T, all_bits[idx], order_trials=64)
-    rel = (got - want) / want.max()
-    print(f"cfg5 random tensors: 1000 states checked against O8': max {np.abs(rel).max():.2e}, mean {rel.mean():+.2e}")
-    assert np.abs(rel).max() <= TOL
+    for label, kw in (("greedy plan", {}), ("the plan bench.py times", BENCH_PLAN_CFG5)):
+        plan = _loaded_plan(net, T, tqc.MODE_STATES, batch_hint=configs.BATCH[5], **kw)
+        got = _run_states(plan, all_bits[idx], max_ws=48 << 30)
+        rel = (got - want) / want.max()
+        print(f"cfg5 random tensors, {label}: 1000 states checked against O8': max {np.abs(rel).max():.2e}, mean {rel.mean():+.2e}")
+        assert np.abs(rel).max() <= TOL
+        plan.close()
 
 
 def test_cfg5_order_invariance_between_two_gpu_plans():
