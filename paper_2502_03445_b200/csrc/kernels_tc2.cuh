@@ -321,8 +321,8 @@ step_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
                 // columns c .. c+3 (c a multiple of 4) are neighbours in C: neighbouring lanes of a quad swap halves of two
                 // 8-column groups, so that an even lane holds 4 consecutive columns of group g, the odd lane next to it 4 of
                 // group g + 1, and a lane stores 16 bytes: a quad writes 64 contiguous bytes of a row where the layout allows
-                // (the store path alone, all SMs: 6.1 TB/s against 5.5 for 8-byte stores at a row pitch of 16 KB, 6.0 against
-                // 4.0 at 64 KB, 3.1 against 1.5 at 1 MB; in the kernel: -2 to -3 % on K <= 256 steps)
+                // (the store path alone, all SMs, profiles/peaks_r02.md: 5.5 TB/s for both at a row pitch of 16 KB, 5.5 against
+                // 5.1 for 8-byte stores at 64 KB, 3.1 against 1.5 at 1 MB; in the kernel: -2 to -3 % on K <= 256 steps)
                 const bool odd = (lane & 1) != 0;
 #pragma unroll
                 for (int h2 = 0; h2 < 2; ++h2)

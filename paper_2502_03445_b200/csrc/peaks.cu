@@ -51,6 +51,47 @@ __global__ void __launch_bounds__(1024, 2) l2_kernel(const float4 *__restrict__ 
     if (acc.x + acc.y + acc.z + acc.w == 123.456f) out[blockIdx.x * blockDim.x + threadIdx.x] = acc.x;
 }
 
+// Store-path probe: one 512-thread block per SM writes 128 KB tiles (128 rows x 1024 B of a matrix with `pitch`
+// bytes per row, tiles in the pair kernel's order) in one of four warp-store patterns:
+//   1  st.v2, a quad of lanes = one 32-byte sector, 8 rows per instruction   (8-byte stores from the tcgen05.ld 16x256b layout)
+//   2  st.v4, 8 lanes = one 128-byte line, 4 rows per instruction
+//   4  st.v4, a warp writes 512 contiguous bytes of one row
+//   5  st.v4, a quad = 64 contiguous bytes of a row, 8 rows per instruction      (16-byte stores after the lane exchange)
+template <int PAT>
+__global__ void __launch_bounds__(512, 1) store_tiles_kernel(unsigned char *p, long long tiles, size_t pitch) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int w4 = warp & 3, grp = warp >> 2;
+    const long long per_row = (long long)(pitch / 1024);
+    for (long long t = blockIdx.x; t < tiles; t += gridDim.x) {
+        unsigned char *tile = p + (size_t)(t / per_row) * 128 * pitch + (size_t)(t % per_row) * 1024;
+        if (PAT == 1) {
+#pragma unroll
+            for (int h = 0; h < 4; ++h)
+#pragma unroll
+                for (int g = 0; g < 8; ++g)
+                    *reinterpret_cast<float2 *>(tile + (size_t)(32 * w4 + (lane >> 2) + 8 * h) * pitch + 256 * grp + 32 * g + 8 * (lane & 3)) = make_float2(1.f, 2.f);
+        } else if (PAT == 2) {
+#pragma unroll
+            for (int h = 0; h < 8; ++h)
+#pragma unroll
+                for (int g = 0; g < 2; ++g)
+                    *reinterpret_cast<float4 *>(tile + (size_t)(32 * w4 + (lane >> 3) + 4 * h) * pitch + 256 * grp + 128 * g + 16 * (lane & 7)) = make_float4(1.f, 2.f, 3.f, 4.f);
+        } else if (PAT == 5) {
+#pragma unroll
+            for (int h = 0; h < 4; ++h)
+#pragma unroll
+                for (int g = 0; g < 4; ++g)
+                    *reinterpret_cast<float4 *>(tile + (size_t)(32 * w4 + (lane >> 2) + 8 * h) * pitch + 256 * grp + 64 * g + 16 * (lane & 3)) = make_float4(1.f, 2.f, 3.f, 4.f);
+        } else {
+#pragma unroll
+            for (int h = 0; h < 8; ++h)
+#pragma unroll
+                for (int g = 0; g < 2; ++g)
+                    *reinterpret_cast<float4 *>(tile + (size_t)(8 * warp + h) * pitch + 512 * g + 16 * lane) = make_float4(1.f, 2.f, 3.f, 4.f);
+        }
+    }
+}
+
 template <typename F>
 int timed(F launch, float *ms) {
     cudaEvent_t a, b;
@@ -111,6 +152,27 @@ int tqc_peak_l2(size_t bytes, int reps, double *gbs, double *ms_out) {
     cudaFree(src); cudaFree(out);
     if (rc) return rc;
     *gbs = (double)bytes * reps / (ms * 1e-3) / 1e9;
+    *ms_out = ms;
+    return 0;
+}
+
+// store bandwidth in GB/s of `bytes` (a multiple of 128 x pitch) written once in pattern `pattern` (store_tiles_kernel) by
+// `blocks` blocks (0: one per SM); pitch = bytes per matrix row, a multiple of 1024
+int tqc_peak_store(int pattern, size_t bytes, size_t pitch, int blocks, double *gbs, double *ms_out) {
+    if (pitch < 1024 || pitch % 1024 || bytes % (128 * pitch)) return -1;
+    unsigned char *buf = nullptr;
+    if (cudaMalloc(&buf, bytes) != cudaSuccess) return -7;
+    const int nb = blocks > 0 ? blocks : sm_count();
+    const long long tiles = (long long)(bytes / (128 * 1024));
+    float ms = 0.f;
+    int rc = -1;
+    if (pattern == 1) rc = timed([&] { store_tiles_kernel<1><<<nb, 512>>>(buf, tiles, pitch); }, &ms);
+    else if (pattern == 2) rc = timed([&] { store_tiles_kernel<2><<<nb, 512>>>(buf, tiles, pitch); }, &ms);
+    else if (pattern == 4) rc = timed([&] { store_tiles_kernel<4><<<nb, 512>>>(buf, tiles, pitch); }, &ms);
+    else if (pattern == 5) rc = timed([&] { store_tiles_kernel<5><<<nb, 512>>>(buf, tiles, pitch); }, &ms);
+    cudaFree(buf);
+    if (rc) return rc;
+    *gbs = (double)bytes / (ms * 1e-3) / 1e9;
     *ms_out = ms;
     return 0;
 }

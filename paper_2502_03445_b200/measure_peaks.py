@@ -5,6 +5,7 @@ as JSON:  python -m paper_2502_03445_b200.measure_peaks [out.json]
   ffma_tflops                           register-resident FFMA loop on every SM (csrc/peaks.cu), >= 1 s
   lds_gbs                               conflict-free LDS.128 loop on every SM
   l2_read_gbs                           32 MB buffer read repeatedly (ld.global.cg)
+  store_gbs                             the store path by warp pattern and row pitch (the pair kernel's epilogue)
 bench.py reads the committed copy (profiles/peaks_r02.json) for the `peak` of its alu / tensor / smem rooflines.
 """
 from __future__ import annotations
@@ -55,6 +56,18 @@ def measure() -> dict:
     lib.tqc_peak_l2.argtypes = [ctypes.c_size_t, ctypes.c_int, ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
     assert lib.tqc_peak_l2(32 << 20, 2000, ctypes.byref(v), ctypes.byref(ms)) == 0
     out["l2_read_gbs"], out["l2_ms"] = v.value, ms.value
+    # store path by warp pattern and row pitch: 16 GB written once, one 512-thread block per SM, and one SM alone
+    lib.tqc_peak_store.argtypes = [ctypes.c_int, ctypes.c_size_t, ctypes.c_size_t, ctypes.c_int, ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
+    names = {1: "st.v2 quad = 32 B sector, 8 rows per instruction", 2: "st.v4 8 lanes = 128 B line, 4 rows",
+             4: "st.v4 warp = 512 B of one row", 5: "st.v4 quad = 64 B of a row, 8 rows"}
+    store = {}
+    for pat in (1, 2, 4, 5):
+        for pitch in (1024, 16384, 65536, 1 << 20):
+            assert lib.tqc_peak_store(pat, 16 << 30, pitch, 0, ctypes.byref(v), ctypes.byref(ms)) == 0
+            store[f"pattern {pat} ({names[pat]}), pitch {pitch}"] = round(v.value, 1)
+        assert lib.tqc_peak_store(pat, 1 << 30, 16384, 1, ctypes.byref(v), ctypes.byref(ms)) == 0
+        store[f"pattern {pat}, ONE block on one SM, pitch 16384"] = round(v.value, 1)
+    out["store_gbs"] = store
     out["how"] = ("tf32: torch.matmul fp32 8192^3, allow_tf32, best of 10 / back to back for 3 s; ffma: 8 FMA chains per "
                   "thread, 1024 threads per SM, all SMs; lds: conflict-free LDS.128, 1024 threads per SM; l2: 32 MB buffer, "
                   "ld.global.cg float4, 2048 threads per SM, 2000 passes (csrc/peaks.cu)")
